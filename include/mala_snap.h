@@ -1,0 +1,142 @@
+/*
+ * mala_snap.h -- C ABI of libmala_snap.so: SNAP bispectrum descriptors on a real-space grid,
+ * the data-parallel hot path of MALA inference (arXiv 2411.19617), hand-written CUDA for sm_100a.
+ *
+ * What is computed (PAPER.md = the paper text; SURVEY.md section 8 restates the mathematics):
+ *   - neighbor density around each grid point, with cutoff, element weight and self term:
+ *       Eq. (24)
+ *   - its expansion coefficients u_j in 4-D hyperspherical harmonics:  Eq. (25)
+ *   - the bispectrum B(r, j) = "scalar triple products of the expansion coefficients", real and
+ *     rotation invariant:  PAPER.md:261;  number of components, Eq. (26)
+ *   - evaluated at every point of the grid:
+ *   - hyperparameters twojmax / rcutfac as in PAPER.md:597-599; f_c, theta0 map, rfac0, rmin0, wself as
+ *     fixed by BASELINE.json north_star (DESIGN.md "Readings" #1-#6).
+ *
+ * Conventions
+ *   - every pointer argument says HOST or DEVICE.  Host inputs are copied before the call returns.
+ *   - angular momenta are DOUBLED integers (J = 2 j_true).
+ *   - the library never aborts, throws or prints; non-zero return codes are
+ *       MALA_SNAP_EINVAL  (-1)  invalid argument        (nothing was enqueued)
+ *       MALA_SNAP_ECUDA   (-2)  CUDA runtime error      (message names the call)
+ *       MALA_SNAP_ENOMEM  (-3)  host or device allocation failed
+ *     and mala_last_error() returns a thread-local description of the last failure.
+ *   - one handle must not be used by two host threads at once.  There is no CPU fallback: without a CUDA
+ *     device mala_snap_create fails with MALA_SNAP_ECUDA.
+ */
+#ifndef MALA_SNAP_H
+#define MALA_SNAP_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MALA_SNAP_OK 0
+#define MALA_SNAP_EINVAL (-1)
+#define MALA_SNAP_ECUDA (-2)
+#define MALA_SNAP_ENOMEM (-3)
+
+/* largest supported twojmax (32 grid points x all U levels must fit one SM's shared memory) */
+#define MALA_SNAP_MAX_TWOJMAX 10
+
+typedef struct mala_snap mala_snap_t; /* opaque; owns device tables and a lazily grown workspace */
+
+/*
+ * Create a descriptor calculator (descriptor_type "Bispectrum", twojmax, rcutfac).
+ *   handle   [out] HOST
+ *   twojmax  0..MALA_SNAP_MAX_TWOJMAX, even or odd (10 in the paper)
+ *   rcutfac  > 0; cutoff of type t is rcut_t = 2 * rcutfac * radelem[t]  (reading #10)
+ *   rfac0    in (0, 1]: theta0 = rfac0 * pi * (r - rmin0) / (rcut_t - rmin0)      (north_star: 0.99363)
+ *   rmin0    in [0, min rcut_t)                                                     (north_star: 0)
+ *   wself    weight of the self term delta(0) of Eq. (24)                           (north_star: 1)
+ *   ntypes   >= 1
+ *   radelem  HOST [ntypes], > 0     (0.5 makes rcut = rcutfac, the MALA usage)
+ *   wj       HOST [ntypes] element weights w_eta of Eq. (24)
+ * Builds the triple list, Clebsch-Gordan tables and index lists on the host, uploads them, and computes
+ * the constant zero-neighbor descriptor once.  Uses the current CUDA device.
+ */
+int mala_snap_create(mala_snap_t **handle, int twojmax, double rcutfac, double rfac0, double rmin0, double wself,
+                     int ntypes, const double *radelem, const double *wj);
+
+/* number of bispectrum components, Eq. (26) PAPER.md:263 (91 at twojmax = 10); < 0 on a NULL handle */
+int mala_snap_ncomp(const mala_snap_t *h);
+
+/* the (j1, j2, j) of every component, doubled, in output order (reading #7):
+ *   for j1 = 0..twojmax, j2 = 0..j1, j = j1-j2 .. min(twojmax, j1+j2) step 2, if j >= j1.
+ *   j1j2j  HOST [ncomp * 3] */
+int mala_snap_triples(const mala_snap_t *h, int *j1j2j);
+
+/*
+ * Bispectrum descriptors on the z-slab [z_begin, z_end) of an nx x ny x nz grid.
+ *   natoms   >= 0 (0 is valid: every point gets the self-term-only vector)
+ *   pos      HOST [natoms*3] Cartesian, need not be wrapped into the cell (reading #14)
+ *   types    HOST [natoms], 0-based, < ntypes
+ *   box      HOST [9]  rows a1, a2, a3 of a general triclinic cell (either handedness)
+ *   origin   HOST [3]  position of grid point (0,0,0); point (ix,iy,iz) sits at
+ *                      origin + ix/nx a1 + iy/ny a2 + iz/nz a3                        (reading #8)
+ *   pbc      HOST [3]  1 = periodic along a_i; all lattice images within the cutoff count, also an
+ *                      atom's own images when the cell is smaller than the cutoff    (reading #13)
+ *   ngrid    HOST [3]  nx, ny, nz > 0
+ *   z_begin, z_end     0 <= z_begin <= z_end <= nz
+ *   out      DEVICE [(z_end-z_begin)*ny*nx][ncomp] fp64, ix fastest, then iy, then iz; component k is
+ *            triple k of mala_snap_triples.  No B0 subtraction, no normalisation (reading #6).
+ *   cuda_stream  a cudaStream_t (NULL = default stream).  All device work is enqueued on it and the call
+ *            returns without synchronising; `out` must stay alive until the stream has drained.
+ * The slab is processed in internal chunks bounded by the workspace cap (see mala_snap_set_option).
+ */
+int mala_bispectrum_grid(mala_snap_t *h, int natoms, const double *pos, const int *types, const double box[9],
+                         const double origin[3], const int pbc[3], const int ngrid[3], int z_begin, int z_end,
+                         double *out, void *cuda_stream);
+
+/*
+ * Same, end to end with a HOST result: `out_host` is HOST memory [(z_end-z_begin)*ny*nx][ncomp]
+ * (pinned memory makes the copies asynchronous with respect to the kernels).  The slab is computed in
+ * z-chunks into two device staging buffers owned by the handle; the device->host copy of one chunk
+ * overlaps the kernels of the next.  The call returns after the last copy has completed.
+ */
+int mala_bispectrum_grid_host(mala_snap_t *h, int natoms, const double *pos, const int *types,
+                              const double box[9], const double origin[3], const int pbc[3], const int ngrid[3],
+                              int z_begin, int z_end, double *out_host, void *cuda_stream);
+
+/*
+ * Tuning / test knobs.  Unknown names give MALA_SNAP_EINVAL.
+ *   "zi_impl"          0 = automatic (specialised kernel when twojmax == 10), 1 = generic table-driven
+ *                      kernel, 2 = specialised kernel (EINVAL if twojmax != 10)
+ *   "workspace_mb"     cap, in MiB, of the U_tot + candidate workspace (default 4096)
+ *   "host_chunk_mb"    size, in MiB, of each of the two staging buffers of mala_bispectrum_grid_host
+ */
+int mala_snap_set_option(mala_snap_t *h, const char *name, long long value);
+
+/*
+ * Counters of the last mala_bispectrum_grid* call on this handle (HOST array of 8):
+ *   [0] kernels launched   [1] chunks   [2] tiles   [3] ghost atoms (atoms + periodic images kept)
+ *   [4] candidate capacity per tile   [5] workspace bytes in use   [6] points   [7] reserved
+ */
+int mala_snap_last_stats(const mala_snap_t *h, long long stats[8]);
+
+/*
+ * Test hook: the Clebsch-Gordan coefficient the library's own table generator produces (doubled arguments).
+ * Pure host arithmetic; lets the CPU-only test-suite check the tables without a GPU.
+ */
+double mala_snap_clebsch_gordan(int J1, int M1, int J2, int M2, int J, int M);
+
+/*
+ * Test hook: U_tot (Eq. (25) coefficients, summed over neighbors, self term included) at the grid points of
+ * one z-slab, in the library's internal half-column storage:
+ *   u_out  DEVICE [npoints][nelem][2] fp64 (re, im), nelem = sum_J (J+1)*(J/2+1); element (J, mb <= J/2, ma)
+ *          at index sum_{K<J}(K+1)*(K/2+1) + mb*(J+1) + ma.
+ * Returns nelem (>0) on success.  Synchronises the stream.
+ */
+int mala_snap_debug_utot(mala_snap_t *h, int natoms, const double *pos, const int *types, const double box[9],
+                         const double origin[3], const int pbc[3], const int ngrid[3], int z_begin, int z_end,
+                         double *u_out, void *cuda_stream);
+
+/* NULL-safe; frees tables, workspace and staging buffers */
+void mala_snap_destroy(mala_snap_t *h);
+
+/* thread-local message for the last non-zero return on this thread ("" if none) */
+const char *mala_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MALA_SNAP_H */

@@ -1,0 +1,714 @@
+// mala_snap.cu -- C ABI of libmala_snap.so and the host planner (include/mala_snap.h documents every call).
+//
+// Host side per call: validate, wrap atoms, enumerate the periodic images that can reach the slab ("ghosts"),
+// sort them into a Cartesian cell list, choose the tile shape and the chunking, then enqueue per chunk
+//     tile_bin_kernel -> compute_ui_kernel -> compute_zi_bi_*_kernel
+// on the caller's stream.  No step of the path runs on the CPU and there is no fallback.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/mala_snap.h"
+#include "snap_common.cuh"
+#include "snap_tables.h"
+#include "snap_ui.cuh"
+#include "snap_zi.cuh"
+#include "snap_zi_spec.cuh"
+
+using namespace mala;
+
+static thread_local std::string g_last_error;
+
+static int fail(int code, const std::string &msg) {
+    g_last_error = msg;
+    return code;
+}
+
+#define CUDA_TRY(call)                                                                              \
+    do {                                                                                            \
+        cudaError_t e_ = (call);                                                                    \
+        if (e_ != cudaSuccess) {                                                                    \
+            const int code_ = (e_ == cudaErrorMemoryAllocation) ? MALA_SNAP_ENOMEM : MALA_SNAP_ECUDA; \
+            return fail(code_, std::string(#call) + ": " + cudaGetErrorString(e_));                 \
+        }                                                                                           \
+    } while (0)
+
+namespace {
+
+template <typename T>
+struct DevBuf {
+    T *p = nullptr;
+    size_t cap = 0;  // elements
+    int reserve(size_t n) {
+        if (n <= cap) return 0;
+        if (p) cudaFree(p);
+        p = nullptr;
+        cap = 0;
+        size_t want = n + n / 4 + 16;
+        cudaError_t e = cudaMalloc((void **)&p, want * sizeof(T));
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            e = cudaMalloc((void **)&p, n * sizeof(T));
+            want = n;
+        }
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            p = nullptr;
+            return -1;
+        }
+        cap = want;
+        return 0;
+    }
+    void release() {
+        if (p) cudaFree(p);
+        p = nullptr;
+        cap = 0;
+    }
+};
+
+}  // namespace
+
+struct mala_snap {
+    // parameters
+    int twojmax = 0, ntypes = 0;
+    double rcutfac = 0, rfac0 = 0, rmin0 = 0, wself = 0;
+    std::vector<double> rcut, wj;
+    double rcutmax = 0;
+    SnapTables tab;
+    SnapConst sc{};
+    int device = 0, num_sms = 0;
+    // options
+    int zi_impl = 0;
+    long long workspace_mb = 4096;
+    long long host_chunk_mb = 512;
+    // device tables
+    DevBuf<int> d_triples, d_udiag, d_order;
+    DevBuf<double> d_cg, d_unorm, d_rcut, d_w, d_bconst;
+    // per-call buffers
+    // ghosts + cell list are double-buffered (set = call parity) and uploaded on a private stream, so that a
+    // call never waits on the host for the kernels of the previous call
+    DevBuf<Ghost> d_ghosts[2];
+    DevBuf<int> d_cell_start[2];
+    cudaStream_t upload_stream = nullptr;
+    cudaEvent_t ev_upload = nullptr, ev_call_done[2] = {nullptr, nullptr};
+    bool call_done_valid[2] = {false, false};
+    unsigned long long ncalls = 0;
+    int cur = 0;  // buffer set of the current call
+    std::vector<int> h_cell_start;
+    DevBuf<int> d_cand, d_ncand, d_active, d_counters;
+    DevBuf<double2> d_utot;
+    DevBuf<double> d_stage[2];
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_done[2] = {nullptr, nullptr}, ev_copied[2] = {nullptr, nullptr};
+    // plan of the current call
+    GridGeom geom{};
+    int cand_cap = 0;
+    long long stats[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+
+    DeviceTables tables() const {
+        DeviceTables t;
+        t.triples = d_triples.p; t.cg = d_cg.p; t.unorm = d_unorm.p; t.udiag = d_udiag.p; t.order = d_order.p;
+        t.type_rcut = d_rcut.p; t.type_w = d_w.p; t.bconst = d_bconst.p;
+        return t;
+    }
+    bool use_spec() const { return (zi_impl == 2) || (zi_impl == 0 && twojmax == kSpecTJ); }
+};
+
+namespace {
+
+constexpr int kSpecWarps = 8;
+
+template <typename T>
+int upload(DevBuf<T> &b, const std::vector<T> &v) {
+    if (b.reserve(std::max<size_t>(v.size(), 1))) return fail(MALA_SNAP_ENOMEM, "cudaMalloc (table) failed");
+    if (!v.empty()) CUDA_TRY(cudaMemcpy(b.p, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice));
+    return 0;
+}
+
+int set_kernel_attributes(mala_snap *h) {
+    const int ui_smem = (int)compute_ui_smem_bytes(kMaxTwoJ);
+    CUDA_TRY(cudaFuncSetAttribute(compute_ui_kernel<kMaxTwoJ, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, ui_smem));
+    CUDA_TRY(cudaFuncSetAttribute(compute_ui_kernel<kMaxTwoJ, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ui_smem));
+    const int zi_smem = (int)compute_zi_smem_bytes(uhalf_size(kMaxTwoJ), triple_count(kMaxTwoJ));
+    CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, zi_smem));
+    CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_spec_kernel<kSpecWarps>, cudaFuncAttributeMaxDynamicSharedMemorySize, zi_smem));
+    (void)h;
+    return 0;
+}
+
+// enqueue compute_zi_bi for one chunk
+int launch_zi(mala_snap *h, const ChunkBuffers &cb, double *out, cudaStream_t st) {
+    const int grid = std::max(1, std::min(h->num_sms, cb.ntiles));
+    const size_t smem = compute_zi_smem_bytes(h->sc.nelem, h->sc.ntriples);
+    if (h->use_spec())
+        compute_zi_bi_spec_kernel<kSpecWarps><<<grid, kSpecWarps * 32, smem, st>>>(h->geom, h->sc, h->tables(), cb, out);
+    else
+        compute_zi_bi_generic_kernel<<<grid, kZiWarps * 32, smem, st>>>(h->geom, h->sc, h->tables(), cb, out);
+    CUDA_TRY(cudaGetLastError());
+    h->stats[0]++;
+    return 0;
+}
+
+// B of a point without neighbors, computed by the same kernel that handles every other point
+int compute_bconst(mala_snap *h) {
+    const int nelem = h->sc.nelem, nt = h->sc.ntriples;
+    std::vector<double2> u((size_t)nelem * 32);
+    for (int e = 0; e < nelem; e++)
+        for (int l = 0; l < 32; l++) u[(size_t)e * 32 + l] = make_double2(h->tab.udiag[e] ? h->wself : 0.0, 0.0);
+    if (h->d_utot.reserve(u.size())) return fail(MALA_SNAP_ENOMEM, "cudaMalloc (utot) failed");
+    if (h->d_active.reserve(1) || h->d_counters.reserve(4) || h->d_bconst.reserve(nt)) return fail(MALA_SNAP_ENOMEM, "cudaMalloc failed");
+    DevBuf<double> tmp;
+    if (tmp.reserve((size_t)32 * nt)) return fail(MALA_SNAP_ENOMEM, "cudaMalloc failed");
+    CUDA_TRY(cudaMemcpy(h->d_utot.p, u.data(), u.size() * sizeof(double2), cudaMemcpyHostToDevice));
+    const int zero = 0;
+    const int counters[4] = {1, 0, 0, 0};
+    CUDA_TRY(cudaMemcpy(h->d_active.p, &zero, sizeof(int), cudaMemcpyHostToDevice));
+    CUDA_TRY(cudaMemcpy(h->d_counters.p, counters, sizeof(counters), cudaMemcpyHostToDevice));
+    GridGeom g{};
+    g.a1[0] = g.a2[1] = g.a3[2] = 1.0;
+    g.nx = 4; g.ny = 4; g.nz = 2; g.z0 = 0; g.z1 = 2; g.tx = 4; g.ty = 4; g.tz = 2; g.ntx = g.nty = g.ntz = 1;
+    const GridGeom saved = h->geom;
+    h->geom = g;
+    ChunkBuffers cb{};
+    cb.active = h->d_active.p; cb.counters = h->d_counters.p; cb.utot = h->d_utot.p; cb.tile_begin = 0; cb.ntiles = 1;
+    int rc = launch_zi(h, cb, tmp.p, nullptr);
+    h->geom = saved;
+    if (rc) { tmp.release(); return rc; }
+    cudaError_t e = cudaMemcpy(h->d_bconst.p, tmp.p, nt * sizeof(double), cudaMemcpyDeviceToDevice);
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    tmp.release();
+    if (e != cudaSuccess) return fail(MALA_SNAP_ECUDA, std::string("compute_bconst: ") + cudaGetErrorString(e));
+    return 0;
+}
+
+inline double dot3(const double *a, const double *b) { return a[0] * b[0] + a[1] * b[1] + a[2] * b[2]; }
+inline void cross3(const double *a, const double *b, double *c) {
+    c[0] = a[1] * b[2] - a[2] * b[1];
+    c[1] = a[2] * b[0] - a[0] * b[2];
+    c[2] = a[0] * b[1] - a[1] * b[0];
+}
+
+struct CallArgs {
+    int natoms;
+    const double *pos;
+    const int *types;
+    const double *box, *origin;
+    const int *pbc, *ngrid;
+    int z_begin, z_end;
+};
+
+int validate(const mala_snap *h, const CallArgs &a, bool need_out, const void *out) {
+    if (!h) return fail(MALA_SNAP_EINVAL, "handle is NULL");
+    if (a.natoms < 0) return fail(MALA_SNAP_EINVAL, "natoms < 0");
+    if (a.natoms > 0 && (!a.pos || !a.types)) return fail(MALA_SNAP_EINVAL, "pos/types is NULL");
+    if (!a.box || !a.origin || !a.pbc || !a.ngrid) return fail(MALA_SNAP_EINVAL, "box/origin/pbc/ngrid is NULL");
+    for (int i = 0; i < 3; i++)
+        if (a.ngrid[i] <= 0) return fail(MALA_SNAP_EINVAL, "ngrid must be positive");
+    if (a.z_begin < 0 || a.z_end > a.ngrid[2] || a.z_begin > a.z_end) return fail(MALA_SNAP_EINVAL, "z range outside [0, nz]");
+    if ((double)a.ngrid[0] * a.ngrid[1] * (double)(a.z_end - a.z_begin) * h->sc.ntriples > 9.0e15)
+        return fail(MALA_SNAP_EINVAL, "grid too large");
+    for (int i = 0; i < 9; i++)
+        if (!std::isfinite(a.box[i])) return fail(MALA_SNAP_EINVAL, "box is not finite");
+    for (int i = 0; i < 3; i++)
+        if (!std::isfinite(a.origin[i])) return fail(MALA_SNAP_EINVAL, "origin is not finite");
+    double c23[3];
+    cross3(a.box + 3, a.box + 6, c23);
+    const double det = dot3(a.box, c23);
+    const double scale = std::sqrt(dot3(a.box, a.box) * dot3(a.box + 3, a.box + 3) * dot3(a.box + 6, a.box + 6));
+    if (!(std::fabs(det) > 1e-12 * scale) || !(scale > 0)) return fail(MALA_SNAP_EINVAL, "box is singular");
+    for (int n = 0; n < a.natoms; n++) {
+        if (a.types[n] < 0 || a.types[n] >= h->ntypes) return fail(MALA_SNAP_EINVAL, "atom type out of range");
+        for (int k = 0; k < 3; k++)
+            if (!std::isfinite(a.pos[3 * n + k])) return fail(MALA_SNAP_EINVAL, "atom position is not finite");
+    }
+    if (need_out && !out && (a.z_end > a.z_begin)) return fail(MALA_SNAP_EINVAL, "out is NULL");
+    return 0;
+}
+
+// Ghost atoms + cell list for the slab [z_begin, z_end); fills h->geom (except the tile fields).
+int build_plan(mala_snap *h, const CallArgs &a, cudaStream_t st) {
+    GridGeom &g = h->geom;
+    h->cur = (int)(h->ncalls & 1ull);
+    h->ncalls++;
+    const int cur = h->cur;
+    std::memset(&g, 0, sizeof(g));
+    for (int k = 0; k < 3; k++) {
+        g.a1[k] = a.box[k]; g.a2[k] = a.box[3 + k]; g.a3[k] = a.box[6 + k]; g.origin[k] = a.origin[k];
+    }
+    g.nx = a.ngrid[0]; g.ny = a.ngrid[1]; g.nz = a.ngrid[2];
+    g.rcutmax = h->rcutmax;
+    // reciprocal rows and plane spacings
+    double c23[3], c31[3], c12[3];
+    cross3(g.a2, g.a3, c23); cross3(g.a3, g.a1, c31); cross3(g.a1, g.a2, c12);
+    const double det = dot3(g.a1, c23);
+    const double *rec[3] = {c23, c31, c12};
+    double hgt[3];
+    for (int i = 0; i < 3; i++) hgt[i] = std::fabs(det) / std::sqrt(dot3(rec[i], rec[i]));
+    // fractional extent of the grid points of the slab, widened by the cutoff
+    const int n3[3] = {g.nx, g.ny, g.nz};
+    double flo[3], fhi[3];
+    for (int i = 0; i < 3; i++) {
+        const double lo = (i == 2) ? (double)a.z_begin / n3[i] : 0.0;
+        const double hi = (i == 2) ? (double)(std::max(a.z_end - 1, a.z_begin)) / n3[i] : (double)(n3[i] - 1) / n3[i];
+        const double m = h->rcutmax / hgt[i] * (1.0 + 1e-12) + 1e-12;
+        flo[i] = lo - m;
+        fhi[i] = hi + m;
+    }
+    std::vector<Ghost> ghosts;
+    ghosts.reserve((size_t)a.natoms * 2 + 16);
+    const double *rows[3] = {g.a1, g.a2, g.a3};
+    for (int n = 0; n < a.natoms; n++) {
+        double x[3] = {a.pos[3 * n] - g.origin[0], a.pos[3 * n + 1] - g.origin[1], a.pos[3 * n + 2] - g.origin[2]};
+        double f[3];
+        int ilo[3], ihi[3];
+        bool keep = true;
+        for (int i = 0; i < 3; i++) {
+            f[i] = dot3(x, rec[i]) / det;
+            if (a.pbc[i]) {
+                f[i] -= std::floor(f[i]);  // wrap into [0,1)  (reading #14)
+                ilo[i] = (int)std::ceil(flo[i] - f[i]);
+                ihi[i] = (int)std::floor(fhi[i] - f[i]);
+                if (ilo[i] > ihi[i]) keep = false;
+            } else {
+                ilo[i] = ihi[i] = 0;
+                if (f[i] < flo[i] || f[i] > fhi[i]) keep = false;
+            }
+        }
+        if (!keep) continue;
+        for (int i1 = ilo[0]; i1 <= ihi[0]; i1++)
+            for (int i2 = ilo[1]; i2 <= ihi[1]; i2++)
+                for (int i3 = ilo[2]; i3 <= ihi[2]; i3++) {
+                    const double ff[3] = {f[0] + i1, f[1] + i2, f[2] + i3};
+                    Ghost gh;
+                    gh.x = g.origin[0] + ff[0] * rows[0][0] + ff[1] * rows[1][0] + ff[2] * rows[2][0];
+                    gh.y = g.origin[1] + ff[0] * rows[0][1] + ff[1] * rows[1][1] + ff[2] * rows[2][1];
+                    gh.z = g.origin[2] + ff[0] * rows[0][2] + ff[1] * rows[1][2] + ff[2] * rows[2][2];
+                    gh.type = a.types[n];
+                    gh.pad = 0;
+                    ghosts.push_back(gh);
+                    if (ghosts.size() > 400000000u) return fail(MALA_SNAP_ENOMEM, "too many periodic images");
+                }
+    }
+    const size_t ng = ghosts.size();
+    // Cartesian cell list
+    double lo[3] = {0, 0, 0}, hi[3] = {1, 1, 1};
+    if (ng > 0) {
+        lo[0] = hi[0] = ghosts[0].x; lo[1] = hi[1] = ghosts[0].y; lo[2] = hi[2] = ghosts[0].z;
+        for (const Ghost &gh : ghosts) {
+            lo[0] = std::min(lo[0], gh.x); hi[0] = std::max(hi[0], gh.x);
+            lo[1] = std::min(lo[1], gh.y); hi[1] = std::max(hi[1], gh.y);
+            lo[2] = std::min(lo[2], gh.z); hi[2] = std::max(hi[2], gh.z);
+        }
+    }
+    int nc[3];
+    double target = std::max(0.5 * h->rcutmax, 1e-6);
+    for (;;) {
+        double total = 1.0;
+        for (int d = 0; d < 3; d++) {
+            const double ext = hi[d] - lo[d];
+            nc[d] = (int)std::min(1024.0, std::max(1.0, std::floor(ext / target)));
+            total *= nc[d];
+        }
+        if (total <= 4.0e6) break;
+        target *= 1.26;
+    }
+    for (int d = 0; d < 3; d++) {
+        const double ext = std::max(hi[d] - lo[d], 1e-9);
+        g.cell_lo[d] = lo[d];
+        g.cell_inv[d] = nc[d] / ext;
+    }
+    g.ncx = nc[0]; g.ncy = nc[1]; g.ncz = nc[2];
+    const size_t ncell = (size_t)nc[0] * nc[1] * nc[2];
+    std::vector<int> cell_of(ng), start(ncell + 1, 0);
+    auto cidx = [&](double v, int d) {
+        int i = (int)std::floor((v - g.cell_lo[d]) * g.cell_inv[d]);
+        return std::min(std::max(i, 0), nc[d] - 1);
+    };
+    for (size_t i = 0; i < ng; i++) {
+        const int c = (cidx(ghosts[i].z, 2) * nc[1] + cidx(ghosts[i].y, 1)) * nc[0] + cidx(ghosts[i].x, 0);
+        cell_of[i] = c;
+        start[c + 1]++;
+    }
+    for (size_t c = 0; c < ncell; c++) start[c + 1] += start[c];
+    std::vector<Ghost> sorted(ng);
+    {
+        std::vector<int> fill(start.begin(), start.end() - 1);
+        for (size_t i = 0; i < ng; i++) sorted[fill[cell_of[i]]++] = ghosts[i];
+    }
+    // upload on the private stream once the call that last used this buffer set has drained
+    if (h->call_done_valid[cur]) CUDA_TRY(cudaStreamWaitEvent(h->upload_stream, h->ev_call_done[cur], 0));
+    if (h->d_ghosts[cur].reserve(std::max<size_t>(ng, 1)) || h->d_cell_start[cur].reserve(ncell + 1))
+        return fail(MALA_SNAP_ENOMEM, "cudaMalloc (ghosts) failed");
+    if (ng) CUDA_TRY(cudaMemcpyAsync(h->d_ghosts[cur].p, sorted.data(), ng * sizeof(Ghost), cudaMemcpyHostToDevice, h->upload_stream));
+    CUDA_TRY(cudaMemcpyAsync(h->d_cell_start[cur].p, start.data(), (ncell + 1) * sizeof(int), cudaMemcpyHostToDevice, h->upload_stream));
+    // (pageable sources: cudaMemcpyAsync returns only after they have been staged, so they may die with this scope)
+    CUDA_TRY(cudaEventRecord(h->ev_upload, h->upload_stream));
+    CUDA_TRY(cudaStreamWaitEvent(st, h->ev_upload, 0));
+    h->stats[3] = (long long)ng;
+    h->h_cell_start.swap(start);
+    return 0;
+}
+
+}  // namespace
+
+namespace {
+
+// tile shape: 32 points as a small brick; prefer the most compact brick among those that waste the fewest lanes
+void choose_tiles(mala_snap *h, int z0, int z1) {
+    GridGeom &g = h->geom;
+    static const int shapes[][3] = {{4, 4, 2}, {4, 2, 4}, {2, 4, 4}, {8, 2, 2}, {2, 8, 2}, {2, 2, 8}, {8, 4, 1}, {4, 8, 1},
+                                    {16, 2, 1}, {2, 16, 1}, {32, 1, 1}, {1, 32, 1}, {1, 1, 32}, {16, 1, 2}, {1, 16, 2},
+                                    {8, 1, 4}, {1, 8, 4}, {4, 1, 8}, {1, 4, 8}, {2, 1, 16}, {1, 2, 16}};
+    const int nzs = std::max(z1 - z0, 1);
+    double best_score = -1.0;
+    int best = 0;
+    for (int s = 0; s < (int)(sizeof(shapes) / sizeof(shapes[0])); s++) {
+        const int *t = shapes[s];
+        const double tiles = (double)((g.nx + t[0] - 1) / t[0]) * ((g.ny + t[1] - 1) / t[1]) * ((nzs + t[2] - 1) / t[2]);
+        const double util = (double)g.nx * g.ny * nzs / (tiles * 32.0);
+        // radius of the brick in units of the grid spacings (a proxy that does not need the metric)
+        double e[3][3];
+        for (int k = 0; k < 3; k++) {
+            e[0][k] = g.a1[k] * (t[0] - 1) / g.nx;
+            e[1][k] = g.a2[k] * (t[1] - 1) / g.ny;
+            e[2][k] = g.a3[k] * (t[2] - 1) / g.nz;
+        }
+        double r = 0.0;
+        for (int sg = 0; sg < 4; sg++) {
+            const double s1 = (sg & 1) ? -1.0 : 1.0, s2 = (sg & 2) ? -1.0 : 1.0;
+            double d[3];
+            for (int k = 0; k < 3; k++) d[k] = e[0][k] + s1 * e[1][k] + s2 * e[2][k];
+            r = std::max(r, 0.5 * std::sqrt(dot3(d, d)));
+        }
+        // fewer wasted lanes first; a larger radius costs candidate tests, roughly (1 + r/rcut)^3
+        const double reach = 1.0 + r / std::max(h->rcutmax, 1e-9);
+        const double score = util / (reach * reach * reach);
+        if (score > best_score * (1.0 + 1e-12)) {
+            best_score = score;
+            best = s;
+            g.tile_radius = r * (1.0 + 1e-9) + 1e-12;
+        }
+    }
+    g.tx = shapes[best][0]; g.ty = shapes[best][1]; g.tz = shapes[best][2];
+    g.z0 = z0; g.z1 = z1;
+    g.ntx = (g.nx + g.tx - 1) / g.tx;
+    g.nty = (g.ny + g.ty - 1) / g.ty;
+    g.ntz = (nzs + g.tz - 1) / g.tz;
+}
+
+// upper bound of the candidates tile_bin_kernel can collect for any tile: maximum ghost count over all windows
+// of cells it may scan (summed-area table over the cell counts)
+int candidate_bound(const mala_snap *h) {
+    const GridGeom &g = h->geom;
+    const int nc[3] = {g.ncx, g.ncy, g.ncz};
+    const double reach = g.tile_radius + g.rcutmax;
+    int w[3];
+    for (int d = 0; d < 3; d++) w[d] = std::min(nc[d], (int)std::floor(2.0 * reach * g.cell_inv[d]) + 2);
+    const size_t sx = nc[0] + 1, sy = nc[1] + 1, sz = nc[2] + 1;
+    std::vector<long long> S(sx * sy * sz, 0);
+    auto at = [&](int x, int y, int z) -> long long & { return S[((size_t)z * sy + y) * sx + x]; };
+    const std::vector<int> &st = h->h_cell_start;
+    for (int z = 1; z <= nc[2]; z++)
+        for (int y = 1; y <= nc[1]; y++)
+            for (int x = 1; x <= nc[0]; x++) {
+                const size_t c = ((size_t)(z - 1) * nc[1] + (y - 1)) * nc[0] + (x - 1);
+                const long long cnt = st[c + 1] - st[c];
+                at(x, y, z) = cnt + at(x - 1, y, z) + at(x, y - 1, z) + at(x, y, z - 1) - at(x - 1, y - 1, z) - at(x - 1, y, z - 1) -
+                              at(x, y - 1, z - 1) + at(x - 1, y - 1, z - 1);
+            }
+    long long best = 0;
+    for (int z = w[2]; z <= nc[2]; z++)
+        for (int y = w[1]; y <= nc[1]; y++)
+            for (int x = w[0]; x <= nc[0]; x++) {
+                const int x0 = x - w[0], y0 = y - w[1], z0 = z - w[2];
+                const long long v = at(x, y, z) - at(x0, y, z) - at(x, y0, z) - at(x, y, z0) + at(x0, y0, z) + at(x0, y, z0) +
+                                    at(x, y0, z0) - at(x0, y0, z0);
+                best = std::max(best, v);
+            }
+    best = std::max<long long>(best, 1);
+    best = (best + 31) / 32 * 32;
+    return (int)std::min<long long>(best, 1 << 24);
+}
+
+// enqueue the whole path for the slab [z0, z1) into out (DEVICE, relative to z0); out == nullptr: stop after compute_ui
+// and scatter U_tot into u_out (test hook)
+int run_slab(mala_snap *h, int z0, int z1, double *out, double2 *u_out, cudaStream_t st) {
+    if (z1 <= z0) return 0;
+    choose_tiles(h, z0, z1);
+    GridGeom &g = h->geom;
+    h->cand_cap = candidate_bound(h);
+    const long long total_tiles = (long long)g.ntx * g.nty * g.ntz;
+    if (total_tiles > 2000000000LL) return fail(MALA_SNAP_EINVAL, "slab has too many tiles; use smaller z-slabs");
+    const size_t per_tile = (size_t)h->sc.nelem * 32 * sizeof(double2) + (size_t)h->cand_cap * sizeof(int) + 2 * sizeof(int);
+    const size_t budget = (size_t)std::max<long long>(h->workspace_mb, 1) << 20;
+    long long chunk_tiles = (long long)std::max<size_t>(budget / per_tile, (size_t)h->num_sms);
+    chunk_tiles = std::min(chunk_tiles, total_tiles);
+    if (h->d_utot.reserve((size_t)chunk_tiles * h->sc.nelem * 32) || h->d_cand.reserve((size_t)chunk_tiles * h->cand_cap) ||
+        h->d_ncand.reserve(chunk_tiles) || h->d_active.reserve(chunk_tiles) || h->d_counters.reserve(4))
+        return fail(MALA_SNAP_ENOMEM, "cudaMalloc (workspace) failed");
+    h->stats[4] = h->cand_cap;
+    h->stats[5] = (long long)(per_tile * (size_t)chunk_tiles);
+    const DeviceTables tb = h->tables();
+    for (long long t0 = 0; t0 < total_tiles; t0 += chunk_tiles) {
+        ChunkBuffers cb{};
+        cb.ghosts = h->d_ghosts[h->cur].p; cb.cell_start = h->d_cell_start[h->cur].p;
+        cb.cand = h->d_cand.p; cb.ncand = h->d_ncand.p; cb.active = h->d_active.p; cb.counters = h->d_counters.p;
+        cb.utot = h->d_utot.p; cb.cand_cap = h->cand_cap;
+        cb.tile_begin = (int)t0;
+        cb.ntiles = (int)std::min(chunk_tiles, total_tiles - t0);
+        CUDA_TRY(cudaMemsetAsync(cb.counters, 0, 4 * sizeof(int), st));
+        const int bin_blocks = (cb.ntiles + 7) / 8;
+        tile_bin_kernel<<<bin_blocks, 256, 0, st>>>(g, h->sc, tb, cb, out);
+        CUDA_TRY(cudaGetLastError());
+        const int grid = std::max(1, std::min(h->num_sms, cb.ntiles));
+        if (h->twojmax == kMaxTwoJ)
+            compute_ui_kernel<kMaxTwoJ, true><<<grid, (kMaxTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kMaxTwoJ), st>>>(g, h->sc, tb, cb);
+        else  // smaller twojmax: same code with run-time guards on the levels
+            compute_ui_kernel<kMaxTwoJ, false><<<grid, (kMaxTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kMaxTwoJ), st>>>(g, h->sc, tb, cb);
+        CUDA_TRY(cudaGetLastError());
+        h->stats[0] += 2;
+        if (out) {
+            int rc = launch_zi(h, cb, out, st);
+            if (rc) return rc;
+        } else if (u_out) {
+            utot_scatter_kernel<<<bin_blocks, 256, 0, st>>>(g, h->sc, tb, cb, u_out);
+            CUDA_TRY(cudaGetLastError());
+            h->stats[0]++;
+        }
+        h->stats[1]++;
+    }
+    h->stats[2] += total_tiles;
+    h->stats[6] += (long long)g.nx * g.ny * (z1 - z0);
+    return 0;
+}
+
+int finish_call(mala_snap *h, cudaStream_t st) {
+    CUDA_TRY(cudaEventRecord(h->ev_call_done[h->cur], st));
+    h->call_done_valid[h->cur] = true;
+    return 0;
+}
+
+}  // namespace
+
+// =============================================================================================================
+// C ABI
+// =============================================================================================================
+extern "C" {
+
+const char *mala_last_error(void) { return g_last_error.c_str(); }
+
+double mala_snap_clebsch_gordan(int J1, int M1, int J2, int M2, int J, int M) { return clebsch_gordan(J1, M1, J2, M2, J, M); }
+
+int mala_snap_create(mala_snap_t **handle, int twojmax, double rcutfac, double rfac0, double rmin0, double wself, int ntypes,
+                     const double *radelem, const double *wj) {
+    if (!handle) return fail(MALA_SNAP_EINVAL, "handle is NULL");
+    *handle = nullptr;
+    if (twojmax < 0 || twojmax > MALA_SNAP_MAX_TWOJMAX) return fail(MALA_SNAP_EINVAL, "twojmax outside [0, 10]");
+    if (!(rcutfac > 0.0) || !std::isfinite(rcutfac)) return fail(MALA_SNAP_EINVAL, "rcutfac must be positive");
+    if (!(rfac0 > 0.0) || !(rfac0 <= 1.0)) return fail(MALA_SNAP_EINVAL, "rfac0 must lie in (0, 1]");
+    if (!std::isfinite(wself)) return fail(MALA_SNAP_EINVAL, "wself is not finite");
+    if (ntypes < 1 || !radelem || !wj) return fail(MALA_SNAP_EINVAL, "ntypes < 1 or radelem/wj is NULL");
+    mala_snap *h = new (std::nothrow) mala_snap();
+    if (!h) return fail(MALA_SNAP_ENOMEM, "out of host memory");
+    h->twojmax = twojmax; h->ntypes = ntypes; h->rcutfac = rcutfac; h->rfac0 = rfac0; h->rmin0 = rmin0; h->wself = wself;
+    double rcutmin = 1e300;
+    for (int t = 0; t < ntypes; t++) {
+        if (!(radelem[t] > 0.0) || !std::isfinite(radelem[t]) || !std::isfinite(wj[t])) {
+            delete h;
+            return fail(MALA_SNAP_EINVAL, "radelem must be positive and wj finite");
+        }
+        h->rcut.push_back(2.0 * rcutfac * radelem[t]);
+        h->wj.push_back(wj[t]);
+        h->rcutmax = std::max(h->rcutmax, h->rcut.back());
+        rcutmin = std::min(rcutmin, h->rcut.back());
+    }
+    if (!(rmin0 >= 0.0) || !(rmin0 < rcutmin)) {
+        delete h;
+        return fail(MALA_SNAP_EINVAL, "rmin0 must lie in [0, min rcut)");
+    }
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        delete h;
+        return fail(MALA_SNAP_ECUDA, "no CUDA device: this library has no CPU fallback");
+    }
+    int rc = 0;
+    auto body = [&]() -> int {
+        CUDA_TRY(cudaGetDevice(&h->device));
+        cudaDeviceProp prop;
+        CUDA_TRY(cudaGetDeviceProperties(&prop, h->device));
+        if (prop.major < 10) return fail(MALA_SNAP_ECUDA, "device is not sm_100 class (kernels are built for sm_100a only)");
+        h->num_sms = prop.multiProcessorCount;
+        h->tab = build_tables(twojmax);
+        h->sc.twojmax = twojmax; h->sc.ntriples = h->tab.ntriples; h->sc.nelem = h->tab.nelem; h->sc.ntypes = ntypes;
+        h->sc.rfac0 = rfac0; h->sc.rmin0 = rmin0; h->sc.wself = wself;
+        if ((rc = upload(h->d_triples, h->tab.triples))) return rc;
+        if ((rc = upload(h->d_cg, h->tab.cg))) return rc;
+        if ((rc = upload(h->d_unorm, h->tab.unorm))) return rc;
+        if ((rc = upload(h->d_udiag, h->tab.udiag))) return rc;
+        if ((rc = upload(h->d_order, h->tab.order))) return rc;
+        if ((rc = upload(h->d_rcut, h->rcut))) return rc;
+        if ((rc = upload(h->d_w, h->wj))) return rc;
+        if (twojmax == kSpecTJ) {
+            if ((int)h->tab.cg.size() != kSpecCG || h->tab.ntriples != kSpecNT) return fail(MALA_SNAP_ECUDA, "internal: table size mismatch");
+            CUDA_TRY(cudaMemcpyToSymbol(c_cg_spec, h->tab.cg.data(), sizeof(double) * kSpecCG));
+            CUDA_TRY(cudaMemcpyToSymbol(c_order_spec, h->tab.order.data(), sizeof(int) * kSpecNT));
+        }
+        if ((rc = set_kernel_attributes(h))) return rc;
+        CUDA_TRY(cudaStreamCreateWithFlags(&h->upload_stream, cudaStreamNonBlocking));
+        CUDA_TRY(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
+        CUDA_TRY(cudaEventCreateWithFlags(&h->ev_upload, cudaEventDisableTiming));
+        for (int i = 0; i < 2; i++) {
+            CUDA_TRY(cudaEventCreateWithFlags(&h->ev_call_done[i], cudaEventDisableTiming));
+            CUDA_TRY(cudaEventCreateWithFlags(&h->ev_done[i], cudaEventDisableTiming));
+            CUDA_TRY(cudaEventCreateWithFlags(&h->ev_copied[i], cudaEventDisableTiming));
+        }
+        return compute_bconst(h);
+    };
+    rc = body();
+    if (rc) {
+        const std::string keep = g_last_error;
+        mala_snap_destroy(h);
+        g_last_error = keep;
+        return rc;
+    }
+    *handle = h;
+    return MALA_SNAP_OK;
+}
+
+int mala_snap_ncomp(const mala_snap_t *h) {
+    if (!h) return fail(MALA_SNAP_EINVAL, "handle is NULL");
+    return h->sc.ntriples;
+}
+
+int mala_snap_triples(const mala_snap_t *h, int *j1j2j) {
+    if (!h || !j1j2j) return fail(MALA_SNAP_EINVAL, "handle or output is NULL");
+    for (int t = 0; t < h->tab.ntriples; t++)
+        for (int k = 0; k < 3; k++) j1j2j[3 * t + k] = h->tab.triples[4 * t + k];
+    return MALA_SNAP_OK;
+}
+
+int mala_snap_set_option(mala_snap_t *h, const char *name, long long value) {
+    if (!h || !name) return fail(MALA_SNAP_EINVAL, "handle or name is NULL");
+    const std::string n(name);
+    if (n == "zi_impl") {
+        if (value < 0 || value > 2) return fail(MALA_SNAP_EINVAL, "zi_impl must be 0, 1 or 2");
+        if (value == 2 && h->twojmax != kSpecTJ) return fail(MALA_SNAP_EINVAL, "the specialised kernel exists for twojmax = 10 only");
+        const bool before = h->use_spec();
+        h->zi_impl = (int)value;
+        if (before != h->use_spec()) return compute_bconst(h);
+        return MALA_SNAP_OK;
+    }
+    if (n == "workspace_mb") {
+        if (value < 1) return fail(MALA_SNAP_EINVAL, "workspace_mb must be >= 1");
+        h->workspace_mb = value;
+        return MALA_SNAP_OK;
+    }
+    if (n == "host_chunk_mb") {
+        if (value < 1) return fail(MALA_SNAP_EINVAL, "host_chunk_mb must be >= 1");
+        h->host_chunk_mb = value;
+        return MALA_SNAP_OK;
+    }
+    return fail(MALA_SNAP_EINVAL, "unknown option: " + n);
+}
+
+int mala_snap_last_stats(const mala_snap_t *h, long long stats[8]) {
+    if (!h || !stats) return fail(MALA_SNAP_EINVAL, "handle or stats is NULL");
+    for (int i = 0; i < 8; i++) stats[i] = h->stats[i];
+    return MALA_SNAP_OK;
+}
+
+int mala_bispectrum_grid(mala_snap_t *h, int natoms, const double *pos, const int *types, const double box[9],
+                         const double origin[3], const int pbc[3], const int ngrid[3], int z_begin, int z_end, double *out,
+                         void *cuda_stream) {
+    const CallArgs a{natoms, pos, types, box, origin, pbc, ngrid, z_begin, z_end};
+    int rc = validate(h, a, true, out);
+    if (rc) return rc;
+    std::fill(h->stats, h->stats + 8, 0LL);
+    if (z_end == z_begin) return MALA_SNAP_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if ((rc = build_plan(h, a, st))) return rc;
+    if ((rc = run_slab(h, z_begin, z_end, out, nullptr, st))) return rc;
+    return finish_call(h, st);
+}
+
+int mala_bispectrum_grid_host(mala_snap_t *h, int natoms, const double *pos, const int *types, const double box[9],
+                              const double origin[3], const int pbc[3], const int ngrid[3], int z_begin, int z_end,
+                              double *out_host, void *cuda_stream) {
+    const CallArgs a{natoms, pos, types, box, origin, pbc, ngrid, z_begin, z_end};
+    int rc = validate(h, a, true, out_host);
+    if (rc) return rc;
+    std::fill(h->stats, h->stats + 8, 0LL);
+    if (z_end == z_begin) return MALA_SNAP_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if ((rc = build_plan(h, a, st))) return rc;
+    const size_t plane = (size_t)ngrid[0] * ngrid[1] * h->sc.ntriples;  // doubles per z-plane
+    const size_t budget = ((size_t)h->host_chunk_mb << 20) / sizeof(double);
+    int planes = (int)std::max<size_t>(1, std::min<size_t>(budget / std::max<size_t>(plane, 1), (size_t)(z_end - z_begin)));
+    if (planes >= 8) planes = planes / 8 * 8;  // whole tiles for every tile shape
+    for (int b = 0; b < 2; b++)
+        if (h->d_stage[b].reserve(plane * planes)) return fail(MALA_SNAP_ENOMEM, "cudaMalloc (staging) failed");
+    bool used[2] = {false, false};
+    int i = 0;
+    for (int z = z_begin; z < z_end; z += planes, i++) {
+        const int b = i & 1;
+        const int ze = std::min(z + planes, z_end);
+        if (used[b]) CUDA_TRY(cudaStreamWaitEvent(st, h->ev_copied[b], 0));
+        if ((rc = run_slab(h, z, ze, h->d_stage[b].p, nullptr, st))) return rc;
+        CUDA_TRY(cudaEventRecord(h->ev_done[b], st));
+        CUDA_TRY(cudaStreamWaitEvent(h->copy_stream, h->ev_done[b], 0));
+        CUDA_TRY(cudaMemcpyAsync(out_host + (size_t)(z - z_begin) * plane, h->d_stage[b].p, (size_t)(ze - z) * plane * sizeof(double),
+                                 cudaMemcpyDeviceToHost, h->copy_stream));
+        CUDA_TRY(cudaEventRecord(h->ev_copied[b], h->copy_stream));
+        used[b] = true;
+    }
+    if ((rc = finish_call(h, st))) return rc;
+    CUDA_TRY(cudaStreamSynchronize(h->copy_stream));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return MALA_SNAP_OK;
+}
+
+int mala_snap_debug_utot(mala_snap_t *h, int natoms, const double *pos, const int *types, const double box[9],
+                         const double origin[3], const int pbc[3], const int ngrid[3], int z_begin, int z_end, double *u_out,
+                         void *cuda_stream) {
+    const CallArgs a{natoms, pos, types, box, origin, pbc, ngrid, z_begin, z_end};
+    int rc = validate(h, a, true, u_out);
+    if (rc) return rc;
+    std::fill(h->stats, h->stats + 8, 0LL);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (z_end > z_begin) {
+        if ((rc = build_plan(h, a, st))) return rc;
+        if ((rc = run_slab(h, z_begin, z_end, nullptr, reinterpret_cast<double2 *>(u_out), st))) return rc;
+        if ((rc = finish_call(h, st))) return rc;
+    }
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return h->sc.nelem;
+}
+
+void mala_snap_destroy(mala_snap_t *h) {
+    if (!h) return;
+    cudaDeviceSynchronize();
+    h->d_triples.release(); h->d_udiag.release(); h->d_order.release();
+    h->d_cg.release(); h->d_unorm.release(); h->d_rcut.release(); h->d_w.release(); h->d_bconst.release();
+    for (int i = 0; i < 2; i++) {
+        h->d_ghosts[i].release(); h->d_cell_start[i].release(); h->d_stage[i].release();
+        if (h->ev_call_done[i]) cudaEventDestroy(h->ev_call_done[i]);
+        if (h->ev_done[i]) cudaEventDestroy(h->ev_done[i]);
+        if (h->ev_copied[i]) cudaEventDestroy(h->ev_copied[i]);
+    }
+    h->d_cand.release(); h->d_ncand.release(); h->d_active.release(); h->d_counters.release(); h->d_utot.release();
+    if (h->ev_upload) cudaEventDestroy(h->ev_upload);
+    if (h->upload_stream) cudaStreamDestroy(h->upload_stream);
+    if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
+    cudaGetLastError();
+    delete h;
+}
+
+}  // extern "C"

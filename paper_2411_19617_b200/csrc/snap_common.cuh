@@ -1,0 +1,72 @@
+// snap_common.cuh -- structures shared by the host planner and the kernels.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+
+#include "snap_tables.h"
+
+namespace mala {
+
+constexpr int kTilePoints = 32;  // grid points per tile = lanes of a warp ("lanes as points")
+constexpr int kMaxTwoJ = 10;
+
+// Geometry of one slab call, passed by value to every kernel.
+struct GridGeom {
+    double a1[3], a2[3], a3[3], origin[3];  // cell rows and the position of grid point (0,0,0)
+    int nx, ny, nz;                          // grid
+    int z0, z1;                              // slab [z0, z1) handled by this launch sequence
+    int tx, ty, tz;                          // tile shape in points, tx*ty*tz == 32
+    int ntx, nty, ntz;                       // tiles per axis (ntz counts from z0)
+    double tile_radius;                      // bounding-sphere radius of one tile around its centre
+    // Cartesian cell list over the ghost atoms
+    double cell_lo[3], cell_inv[3];
+    int ncx, ncy, ncz;
+    double rcutmax;
+};
+
+struct SnapConst {
+    int twojmax, ntriples, nelem, ntypes;
+    double rfac0, rmin0, wself;
+};
+
+// one ghost atom (an atom or one of its periodic images): position and type, 32 bytes
+struct __align__(16) Ghost {
+    double x, y, z;
+    int type;
+    int pad;
+};
+
+// device pointers of one handle
+struct DeviceTables {
+    const int *triples;      // [ntriples*4] j1, j2, j, cg offset
+    const double *cg;        // dense CG blocks
+    const double *unorm;     // [nelem]
+    const int *udiag;        // [nelem]
+    const int *order;        // [ntriples] cost-sorted work order
+    const double *type_rcut; // [ntypes]
+    const double *type_w;    // [ntypes]
+    const double *bconst;    // [ntriples] zero-neighbor descriptor
+};
+
+// per-chunk work buffers
+struct ChunkBuffers {
+    const Ghost *ghosts;     // sorted by cell
+    const int *cell_start;   // [ncells+1]
+    int *cand;               // [chunk_tiles * cand_cap] ghost indices per tile
+    int *ncand;              // [chunk_tiles]
+    int *active;             // [chunk_tiles] compacted list of non-empty tiles (local tile ids)
+    int *counters;           // [0] number of active tiles, [1] ui work counter, [2] zi work counter
+    double2 *utot;           // [chunk_tiles][nelem][32]
+    int cand_cap;
+    int tile_begin;          // first global tile id of the chunk
+    int ntiles;              // tiles in the chunk
+};
+
+__host__ __device__ inline void tile_coords(const GridGeom &g, int tile, int &txi, int &tyi, int &tzi) {
+    txi = tile % g.ntx;
+    int r = tile / g.ntx;
+    tyi = r % g.nty;
+    tzi = r / g.nty;
+}
+
+}  // namespace mala

@@ -1,0 +1,343 @@
+// snap_ui.cuh -- tile binning (row a2) and the compute_ui kernel (rows a3 + a4 of SURVEY.md 8(a)).
+//
+// compute_ui accumulates, for the 32 grid points of a tile, U_tot^J = wself*I + sum_neighbors c * U^J(neighbor)
+// (Eq. (24)-(25)) in the half-column storage of snap_tables.h.
+//
+// Formulation used here (differs from the textbook root-weighted recursion):
+// with u^J[ma][mb] = sqrt(C(J,mb)/C(J,ma)) * q^J[ma][mb], column mb of level J is the coefficient list of the
+// polynomial  Q_{J,mb}(x) = (b + a x)^mb * (conj(a) - conj(b) x)^(J-mb),  a, b the Cayley-Klein parameters of the
+// neighbor.  So one column is advanced from level to level by multiplying with a linear factor -- no square
+// roots, no coupling between columns -- and the binomial weights are applied once per tile at the end.
+// Thread = (grid point, column): warp m owns column m of every level for the 32 points, so accumulation into
+// shared memory needs no atomics and is deterministic.  Two neighbors are advanced together to halve the
+// shared-memory read-modify-write traffic.
+#pragma once
+#include "snap_common.cuh"
+
+namespace mala {
+
+constexpr int kGeoCap = 48;     // neighbor entries per lane buffered between two accumulate passes
+constexpr int kCandBatch = 32;  // candidate atoms staged per batch
+
+__device__ __forceinline__ void lane_point(const GridGeom &g, int tile, int lane, int &ix, int &iy, int &iz, bool &valid) {
+    int txi, tyi, tzi;
+    tile_coords(g, tile, txi, tyi, tzi);
+    const int lx = lane % g.tx, ly = (lane / g.tx) % g.ty, lz = lane / (g.tx * g.ty);
+    ix = txi * g.tx + lx;
+    iy = tyi * g.ty + ly;
+    iz = g.z0 + tzi * g.tz + lz;
+    valid = (ix < g.nx) && (iy < g.ny) && (iz < g.z1);
+}
+
+__device__ __forceinline__ void point_position(const GridGeom &g, int ix, int iy, int iz, double &x, double &y, double &z) {
+    const double fx = (double)ix / (double)g.nx, fy = (double)iy / (double)g.ny, fz = (double)iz / (double)g.nz;
+    x = g.origin[0] + fx * g.a1[0] + fy * g.a2[0] + fz * g.a3[0];
+    y = g.origin[1] + fx * g.a1[1] + fy * g.a2[1] + fz * g.a3[1];
+    z = g.origin[2] + fx * g.a1[2] + fy * g.a2[2] + fz * g.a3[2];
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// tile_bin_kernel: one warp per tile.  Collects the ghost atoms that can reach any point of the tile
+// (|R - centre| < tile_radius + rcut_type) from the Cartesian cell list, in a deterministic order.
+// Tiles with no candidate are filled with the constant zero-neighbor descriptor right here; the others are
+// appended to the active list consumed by compute_ui / compute_zi_bi.
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) tile_bin_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers cb, double *out) {
+    const int lane = threadIdx.x & 31;
+    const int wt = (int)((blockIdx.x * (unsigned)blockDim.x + threadIdx.x) >> 5);
+    if (wt >= cb.ntiles) return;
+    const int tile = cb.tile_begin + wt;
+    int txi, tyi, tzi;
+    tile_coords(g, tile, txi, tyi, tzi);
+    // tile centre (fractional mid-point of the full tile, also for ragged tiles: conservative)
+    const double fx = (txi * g.tx + 0.5 * (g.tx - 1)) / (double)g.nx;
+    const double fy = (tyi * g.ty + 0.5 * (g.ty - 1)) / (double)g.ny;
+    const double fz = (g.z0 + tzi * g.tz + 0.5 * (g.tz - 1)) / (double)g.nz;
+    const double cx = g.origin[0] + fx * g.a1[0] + fy * g.a2[0] + fz * g.a3[0];
+    const double cy = g.origin[1] + fx * g.a1[1] + fy * g.a2[1] + fz * g.a3[1];
+    const double cz = g.origin[2] + fx * g.a1[2] + fy * g.a2[2] + fz * g.a3[2];
+    const double reach = g.tile_radius + g.rcutmax;
+    int lo[3], hi[3];
+    const double c3[3] = {cx, cy, cz};
+    const int nc3[3] = {g.ncx, g.ncy, g.ncz};
+    bool any = true;
+    for (int d = 0; d < 3; d++) {
+        const double l = floor((c3[d] - reach - g.cell_lo[d]) * g.cell_inv[d]);
+        const double h = floor((c3[d] + reach - g.cell_lo[d]) * g.cell_inv[d]);
+        if (h < 0.0 || l >= (double)nc3[d]) any = false;
+        lo[d] = (int)fmax(l, 0.0);
+        hi[d] = (int)fmin(h, (double)(nc3[d] - 1));
+    }
+    int n = 0;
+    int *mycand = cb.cand + (size_t)wt * cb.cand_cap;
+    if (any) {
+        for (int kz = lo[2]; kz <= hi[2]; kz++)
+            for (int ky = lo[1]; ky <= hi[1]; ky++) {
+                const int row = (kz * g.ncy + ky) * g.ncx;
+                const int g0 = cb.cell_start[row + lo[0]];
+                const int g1 = cb.cell_start[row + hi[0] + 1];
+                for (int base = g0; base < g1; base += 32) {
+                    const int gi = base + lane;
+                    bool ok = false;
+                    if (gi < g1) {
+                        const Ghost gh = cb.ghosts[gi];
+                        const double dx = gh.x - cx, dy = gh.y - cy, dz = gh.z - cz;
+                        const double rr = g.tile_radius + tb.type_rcut[gh.type];
+                        ok = (dx * dx + dy * dy + dz * dz) < rr * rr;
+                    }
+                    const unsigned bal = __ballot_sync(0xffffffffu, ok);
+                    const int p = n + __popc(bal & ((1u << lane) - 1u));
+                    if (ok && p < cb.cand_cap) mycand[p] = gi;
+                    n += __popc(bal);
+                }
+            }
+    }
+    if (n > cb.cand_cap) {  // cannot happen when the host bound is right; flagged, never silent
+        if (lane == 0) atomicExch(&cb.counters[3], 1);
+        n = cb.cand_cap;
+    }
+    if (lane == 0) cb.ncand[wt] = n;
+    if (n > 0) {
+        if (lane == 0) {
+            const int slot = atomicAdd(&cb.counters[0], 1);
+            cb.active[slot] = wt;
+        }
+        return;
+    }
+    if (out == nullptr) return;
+    // empty tile: constant descriptor, written as contiguous rows of tx points
+    const int nt = sc.ntriples;
+    const int ix0 = txi * g.tx;
+    const int npx = min(g.tx, g.nx - ix0);
+    for (int r = 0; r < g.ty * g.tz; r++) {
+        const int iy = tyi * g.ty + (r % g.ty);
+        const int iz = g.z0 + tzi * g.tz + (r / g.ty);
+        if (iy >= g.ny || iz >= g.z1) continue;
+        double *dst = out + ((size_t)((size_t)(iz - g.z0) * g.ny + iy) * g.nx + ix0) * nt;
+        for (int i = lane; i < npx * nt; i += 32) __stcs(dst + i, tb.bconst[i % nt]);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// one column (M) of all levels for two neighbors at once; accumulates levels J >= 2M into shared memory.
+// Ul points at element 0 of this lane (stride 32 double2 between elements).
+// ---------------------------------------------------------------------------------------------------------
+template <int M, int TJMAX, bool EXACT>
+__device__ __noinline__ void ui_column_pair(double2 *__restrict__ Ul, const int tj,
+                                               const double c0, const double a0r, const double a0i, const double b0r, const double b0i,
+                                               const double c1, const double a1r, const double a1i, const double b1r, const double b1i) {
+    double pr[2][TJMAX + 1], pi[2][TJMAX + 1];
+    const double ar[2] = {a0r, a1r}, ai[2] = {a0i, a1i}, br[2] = {b0r, b1r}, bi[2] = {b0i, b1i};
+    pr[0][0] = c0; pi[0][0] = 0.0;
+    pr[1][0] = c1; pi[1][0] = 0.0;
+    if (M == 0) {
+        double2 v = Ul[0];
+        v.x += c0 + c1;
+        Ul[0] = v;
+    }
+#pragma unroll
+    for (int r = 1; r <= TJMAX; r++) {
+        if (EXACT || r <= tj) {
+#pragma unroll
+            for (int n = 0; n < 2; n++) {
+                // linear factor f0 + f1 x :  (b + a x) for the first M rounds, (conj(a) - conj(b) x) afterwards
+                const double f0r = (r <= M) ? br[n] : ar[n];
+                const double f0i = (r <= M) ? bi[n] : -ai[n];
+                const double f1r = (r <= M) ? ar[n] : -br[n];
+                const double f1i = (r <= M) ? ai[n] : bi[n];
+                // in place, highest coefficient first; explicit fma chains: 4 FP64 instructions per component
+                pr[n][r] = fma(-f1i, pi[n][r - 1], f1r * pr[n][r - 1]);
+                pi[n][r] = fma(f1i, pr[n][r - 1], f1r * pi[n][r - 1]);
+#pragma unroll
+                for (int k = r - 1; k >= 1; k--) {
+                    double tr = f0r * pr[n][k];
+                    double ti = f0r * pi[n][k];
+                    tr = fma(-f0i, pi[n][k], tr);
+                    ti = fma(f0i, pr[n][k], ti);
+                    tr = fma(f1r, pr[n][k - 1], tr);
+                    ti = fma(f1r, pi[n][k - 1], ti);
+                    tr = fma(-f1i, pi[n][k - 1], tr);
+                    ti = fma(f1i, pr[n][k - 1], ti);
+                    pr[n][k] = tr;
+                    pi[n][k] = ti;
+                }
+                const double t0r = fma(-f0i, pi[n][0], f0r * pr[n][0]);
+                const double t0i = fma(f0i, pr[n][0], f0r * pi[n][0]);
+                pr[n][0] = t0r;
+                pi[n][0] = t0i;
+            }
+            if (r >= 2 * M) {
+                double2 *Ue = Ul + (size_t)(uhalf_off(r) + M * (r + 1)) * 32;
+#pragma unroll
+                for (int k = 0; k <= r; k++) {
+                    double2 v = Ue[k * 32];
+                    v.x += pr[0][k] + pr[1][k];
+                    v.y += pi[0][k] + pi[1][k];
+                    Ue[k * 32] = v;
+                }
+            }
+        }
+    }
+}
+
+// Cayley-Klein parameters and weight of one (grid point, neighbor) pair -- row a3.
+// d = R_neighbor - r_point, r2 = |d|^2 < rcut^2.
+__device__ __forceinline__ void pair_geometry(const double dx, const double dy, const double dz, const double r2, const double rcut,
+                                              const double w, const double rfac0, const double rmin0, double &c, double &ar, double &ai,
+                                              double &br, double &bi) {
+    const double r = sqrt(r2);
+    if (r < 1e-10 * rcut) {  // reading #11: continuous limit for an atom on the grid point
+        c = w; ar = 1.0; ai = 0.0; br = 0.0; bi = 0.0;
+        return;
+    }
+    double x = (r - rmin0) / (rcut - rmin0);
+    x = fmax(x, 0.0);
+    c = w * 0.5 * (cospi(x) + 1.0);
+    double s, co;
+    sincospi(rfac0 * x, &s, &co);
+    const double sr = s / r;
+    ar = co;
+    ai = -sr * dz;
+    br = sr * dy;
+    bi = -sr * dx;
+}
+
+template <int TJMAX, bool EXACT>
+__global__ void __launch_bounds__((TJMAX / 2 + 1) * 32, 1)
+compute_ui_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers cb) {
+    constexpr int NW = TJMAX / 2 + 1;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int nelem = sc.nelem;
+    double2 *uacc = reinterpret_cast<double2 *>(smem_raw);
+    double *geo = reinterpret_cast<double *>(uacc + (size_t)uhalf_size(TJMAX) * 32);
+    double *crec = geo + kGeoCap * 5 * 32;
+    __shared__ int s_slot;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int tj = sc.twojmax;
+
+    for (;;) {
+        __syncthreads();  // everybody is done with the previous tile (uacc reads, s_slot)
+        if (threadIdx.x == 0) s_slot = atomicAdd(&cb.counters[1], 1);
+        __syncthreads();
+        const int slot = s_slot;
+        if (slot >= cb.counters[0]) break;
+        const int wt = cb.active[slot];
+        const int tile = cb.tile_begin + wt;
+        int ix, iy, iz;
+        bool valid;
+        lane_point(g, tile, lane, ix, iy, iz, valid);
+        // ragged tiles: clamp onto a valid point (its result is never written)
+        ix = min(ix, g.nx - 1); iy = min(iy, g.ny - 1); iz = min(iz, g.z1 - 1);
+        double px, py, pz;
+        point_position(g, ix, iy, iz, px, py, pz);
+
+        for (int e = threadIdx.x; e < nelem * 32; e += NW * 32) uacc[e] = make_double2(0.0, 0.0);
+
+        auto accumulate = [&](const int cnt) {
+            if (warp > tj / 2) return;
+            const int nmax = __reduce_max_sync(0xffffffffu, cnt);
+            double2 *Ul = uacc + lane;
+            for (int i = 0; i < nmax; i += 2) {
+                double c0 = 0.0, a0r = 1.0, a0i = 0.0, b0r = 0.0, b0i = 0.0;
+                double c1 = 0.0, a1r = 1.0, a1i = 0.0, b1r = 0.0, b1i = 0.0;
+                if (i < cnt) {
+                    const double *q = geo + (size_t)i * 5 * 32 + lane;
+                    c0 = q[0]; a0r = q[32]; a0i = q[64]; b0r = q[96]; b0i = q[128];
+                }
+                if (i + 1 < cnt) {
+                    const double *q = geo + (size_t)(i + 1) * 5 * 32 + lane;
+                    c1 = q[0]; a1r = q[32]; a1i = q[64]; b1r = q[96]; b1i = q[128];
+                }
+                switch (warp) {
+                    case 0: ui_column_pair<0, TJMAX, EXACT>(Ul, tj, c0, a0r, a0i, b0r, b0i, c1, a1r, a1i, b1r, b1i); break;
+                    case 1: if (TJMAX >= 2) ui_column_pair<(TJMAX >= 2 ? 1 : 0), TJMAX, EXACT>(Ul, tj, c0, a0r, a0i, b0r, b0i, c1, a1r, a1i, b1r, b1i); break;
+                    case 2: if (TJMAX >= 4) ui_column_pair<(TJMAX >= 4 ? 2 : 0), TJMAX, EXACT>(Ul, tj, c0, a0r, a0i, b0r, b0i, c1, a1r, a1i, b1r, b1i); break;
+                    case 3: if (TJMAX >= 6) ui_column_pair<(TJMAX >= 6 ? 3 : 0), TJMAX, EXACT>(Ul, tj, c0, a0r, a0i, b0r, b0i, c1, a1r, a1i, b1r, b1i); break;
+                    case 4: if (TJMAX >= 8) ui_column_pair<(TJMAX >= 8 ? 4 : 0), TJMAX, EXACT>(Ul, tj, c0, a0r, a0i, b0r, b0i, c1, a1r, a1i, b1r, b1i); break;
+                    case 5: if (TJMAX >= 10) ui_column_pair<(TJMAX >= 10 ? 5 : 0), TJMAX, EXACT>(Ul, tj, c0, a0r, a0i, b0r, b0i, c1, a1r, a1i, b1r, b1i); break;
+                    default: break;
+                }
+            }
+        };
+
+        int cnt = 0;       // buffered neighbor entries of this lane (identical in every warp)
+        int appended = 0;  // candidates staged since the last accumulate pass (uniform over the CTA)
+        const int nc = cb.ncand[wt];
+        const int *mycand = cb.cand + (size_t)wt * cb.cand_cap;
+        for (int base = 0; base < nc; base += kCandBatch) {
+            const int nb = min(kCandBatch, nc - base);
+            if (appended + nb > kGeoCap) {
+                __syncthreads();
+                accumulate(cnt);
+                cnt = 0;
+                appended = 0;
+            }
+            __syncthreads();  // crec free again; first time: uacc zeroed
+            if (threadIdx.x < nb) {
+                const Ghost gh = cb.ghosts[mycand[base + threadIdx.x]];
+                const double rc = tb.type_rcut[gh.type];
+                double *q = crec + threadIdx.x * 6;
+                q[0] = gh.x; q[1] = gh.y; q[2] = gh.z; q[3] = rc; q[4] = tb.type_w[gh.type]; q[5] = rc * rc;
+            }
+            __syncthreads();
+            for (int k = 0; k < nb; k++) {
+                const double *q = crec + k * 6;
+                const double dx = q[0] - px, dy = q[1] - py, dz = q[2] - pz;
+                const double r2 = dx * dx + dy * dy + dz * dz;
+                if (r2 < q[5]) {
+                    if ((k % NW) == warp) {
+                        double c, ar, ai, br, bi;
+                        pair_geometry(dx, dy, dz, r2, q[3], q[4], sc.rfac0, sc.rmin0, c, ar, ai, br, bi);
+                        double *o = geo + (size_t)cnt * 5 * 32 + lane;
+                        o[0] = c; o[32] = ar; o[64] = ai; o[96] = br; o[128] = bi;
+                    }
+                    cnt++;
+                }
+            }
+            appended += nb;
+        }
+        __syncthreads();
+        accumulate(cnt);
+        __syncthreads();
+        // binomial normalisation, self term (delta(0) of Eq. (24)), coalesced store of the tile
+        double2 *dst = cb.utot + (size_t)slot * nelem * 32;
+        for (int e = warp; e < nelem; e += NW) {
+            double2 v = uacc[e * 32 + lane];
+            const double s = tb.unorm[e];
+            v.x = v.x * s + (tb.udiag[e] ? sc.wself : 0.0);
+            v.y = v.y * s;
+            dst[e * 32 + lane] = v;
+        }
+    }
+}
+
+inline size_t compute_ui_smem_bytes(int tjmax) {
+    return (size_t)uhalf_size(tjmax) * 32 * sizeof(double2) + (size_t)kGeoCap * 5 * 32 * sizeof(double) +
+           (size_t)kCandBatch * 6 * sizeof(double);
+}
+
+// debug: scatter U_tot tiles into [point][nelem] order; points of empty tiles get wself on the diagonal
+__global__ void utot_scatter_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers cb, double2 *u_out) {
+    const int lane = threadIdx.x & 31;
+    const int wt = (int)((blockIdx.x * (unsigned)blockDim.x + threadIdx.x) >> 5);
+    if (wt >= cb.ntiles) return;
+    const int tile = cb.tile_begin + wt;
+    int ix, iy, iz;
+    bool valid;
+    lane_point(g, tile, lane, ix, iy, iz, valid);
+    if (!valid) return;
+    // find the slot of this tile (linear search is fine for a test hook)
+    int slot = -1;
+    const int na = cb.counters[0];
+    for (int s = 0; s < na; s++)
+        if (cb.active[s] == wt) { slot = s; break; }
+    double2 *dst = u_out + ((size_t)((size_t)(iz - g.z0) * g.ny + iy) * g.nx + ix) * sc.nelem;
+    for (int e = 0; e < sc.nelem; e++) {
+        double2 v;
+        if (slot >= 0) v = cb.utot[((size_t)slot * sc.nelem + e) * 32 + lane];
+        else v = make_double2(tb.udiag[e] ? sc.wself : 0.0, 0.0);
+        dst[e] = v;
+    }
+}
+
+}  // namespace mala
