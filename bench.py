@@ -1,0 +1,358 @@
+#!/usr/bin/env python
+"""bench.py -- grid points/s of twojmax=10 fp64 bispectrum descriptors (BASELINE.json metric) on one B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl native|reference]
+
+A step = one pass of the whole hot path (tile binning -> compute_ui -> compute_zi/compute_bi -> writer)
+over the full grid of the workload (default: config 2, 256-atom solid Al on a 90^3 grid, the configuration the metric
+is quoted on).  `value` is measured through mala_bispectrum_grid with the output resident in HBM; `e2e` through
+mala_bispectrum_grid_host with a pinned HOST output (the device->host copy of all 91 x npoints doubles is inside the
+timed region).  N > 1: independent replicas, one per GPU, no collective on the data path.
+`--impl reference` times the CPU oracle (oracle/) as it stands on the host cores -- the only baseline that exists.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "grid points/s of twojmax=10 fp64 bispectrum descriptors; % of B200 FP64 peak"
+UNIT = "points/s"
+
+# Algorithmic flops: what the method must compute using the standard
+# half-column symmetries -- not instruction counts.
+F_PAIR = 20 * 235 + 4 * 271 + 60          # compute_ui per (grid point, neighbor) pair
+F_Z = 10 * 61332 + 4 * 13230              # compute_zi per non-empty grid point
+F_B = 4 * 3444 + 2 * 91                   # compute_bi per non-empty grid point
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed `ncu --set full`
+# capture (profiles/, file named in the value's comment); None until a capture of the current kernel exists.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {}
+FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 DFMA/clk/SM x 2 flop x 1.965 GHz = 37.2
+
+
+def parse_args():
+    p = argparse.ArgumentParser()
+    p.add_argument("--gpus", type=int, default=1)
+    p.add_argument("--steps", type=int, default=5)
+    p.add_argument("--warmup", type=int, default=3)
+    p.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5])
+    p.add_argument("--impl", default="native", choices=["native", "reference"])
+    p.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
+    p.add_argument("--no-e2e", action="store_true", help="skip the host-output leg (profiling runs)")
+    return p.parse_args()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# clocks during the timed region (B200_PROFILING.md "clocks line")
+# ---------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    FIELDS = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.gpu = gpu_index
+        self.rows = []
+        self.proc = None
+        self.thread = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits", "-lms", "100",
+                                          "-i", str(self.gpu)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._pump, daemon=True)
+        self.thread.start()
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, power, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); smax.append(float(f[2])); power.append(float(f[3]))
+            except ValueError:
+                continue
+            for name, v in zip(names, f[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)), "reasons": sorted(reasons),
+                "samples": len(sm), "power_w_max": float(max(power))}
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# workload facts used by the flop model
+# ---------------------------------------------------------------------------------------------------------------
+def workload_counts(w):
+    """(pairs, non-empty points) of the whole grid.  Periodic bulk systems: every point has neighbors and the mean
+    neighbor count of a uniform grid is exactly rho * 4/3 pi rcut^3.  The non-periodic cluster is counted directly."""
+    rcut = 2.0 * w.rcutfac * w.radelem[0]
+    if all(w.pbc):
+        vol = abs(np.linalg.det(w.box))
+        nbar = w.pos.shape[0] / vol * 4.0 / 3.0 * np.pi * rcut ** 3
+        return nbar * w.npoints, w.npoints
+    nx, ny, nz = w.ngrid
+    fx, fy, fz = np.arange(nx) / nx, np.arange(ny) / ny, np.arange(nz) / nz
+    cnt = np.zeros((nz, ny, nx), dtype=np.int32)
+    ax = fx[None, None, :, None] * w.box[0] + fy[None, :, None, None] * w.box[1]
+    for z0 in range(0, nz, 8):
+        pts = ax + fz[z0:z0 + 8, None, None, None] * w.box[2] + np.asarray(w.origin)
+        for a in w.pos:
+            cnt[z0:z0 + 8] += (((pts - a) ** 2).sum(-1) < rcut * rcut)
+    return float(cnt.sum()), int((cnt > 0).sum())
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return {"hbm_gbs": d.get("hbm_gbs"), "source": "measured (MEASURED_PEAKS.json)", "sm_max_mhz": d.get("sm_max_mhz")}
+    return {"hbm_gbs": 6650.0, "source": "fallback (B200_PROFILING.md)", "sm_max_mhz": 1965.0}
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# CPU oracle legs (the only places bench.py executes oracle/)
+# ---------------------------------------------------------------------------------------------------------------
+def oracle_rate(w, seconds, seed=7):
+    """points/s of the oracle, as it stands, on a seeded random sample of the grid sized to take about `seconds`."""
+    import oracle
+    rng = np.random.default_rng(seed)
+    kw = w.snap_params()
+    probe = rng.integers(0, w.npoints, 64 * max(oracle.num_threads(), 1))
+    t0 = time.perf_counter()
+    oracle.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, sample=probe, **kw)
+    dt = time.perf_counter() - t0
+    n = int(min(max(probe.size, seconds / max(dt, 1e-6) * probe.size), 400000))
+    sample = rng.integers(0, w.npoints, n)
+    t0 = time.perf_counter()
+    oracle.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, sample=sample, **kw)
+    dt = time.perf_counter() - t0
+    return n / dt, n, dt, oracle.num_threads()
+
+
+def run_reference(args, w, rank, world):
+    """--impl reference: the CPU oracle on the host cores, rank 0 only.  Each step = a bounded seeded sample."""
+    if rank != 0:
+        return
+    import oracle
+    rng = np.random.default_rng(11)
+    kw = w.snap_params()
+    threads = oracle.num_threads()
+    # calibrate the per-step sample so the whole run stays near two minutes
+    probe = rng.integers(0, w.npoints, 64 * max(threads, 1))
+    t0 = time.perf_counter()
+    oracle.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, sample=probe, **kw)
+    per_pt = (time.perf_counter() - t0) / probe.size
+    budget = 100.0 / max(args.steps + args.warmup, 1)
+    n = int(min(max(256, budget / per_pt), w.npoints))
+    times = []
+    for it in range(args.warmup + args.steps):
+        sample = rng.integers(0, w.npoints, n)
+        t0 = time.perf_counter()
+        oracle.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, sample=sample, **kw)
+        if it >= args.warmup:
+            times.append(time.perf_counter() - t0)
+    total = float(sum(times))
+    value = n * len(times) / total
+    sample_desc = f"{n} seeded random grid points of {w.name} per step (of {w.npoints}); rate is per point, not extrapolated"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(w, "cpu oracle"),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample_desc},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(w, path):
+    return {"workload": f"config{w.extra.get('cfg', '?')}:{w.name}", "natoms": int(w.pos.shape[0]), "ngrid": list(map(int, w.ngrid)),
+            "npoints": int(w.npoints), "twojmax": int(w.twojmax), "ncomp": 91, "rcut": float(2 * w.rcutfac * w.radelem[0]),
+            "path": path, "parallelism": "replicas",
+            "l2": "no flush: each step streams the U_tot workspace and the output (both far larger than the 126 MB L2)"}
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# multi-rank plumbing (torch.distributed; replicas only -- there is no exchange step on this path)
+# ---------------------------------------------------------------------------------------------------------------
+def dist_setup(args):
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+def reduce_max_sum(value_max, value_sum, world, backend_device=None):
+    """(max over ranks of value_max, sum over ranks of value_sum).  world == 1: identity."""
+    if world == 1:
+        return float(value_max), float(value_sum)
+    import torch
+    import torch.distributed as dist
+    dev = backend_device if backend_device is not None else "cpu"
+    a = torch.tensor([float(value_max)], dtype=torch.float64, device=dev)
+    b = torch.tensor([float(value_sum)], dtype=torch.float64, device=dev)
+    dist.all_reduce(a, op=dist.ReduceOp.MAX)
+    dist.all_reduce(b, op=dist.ReduceOp.SUM)
+    return float(a.item()), float(b.item())
+
+
+def run_native(args, w, rank, world, local):
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    from paper_2411_19617_b200 import MalaSnap, mala_snap_fp64_peak
+
+    def barrier():
+        if world > 1:
+            torch.distributed.barrier()
+        torch.cuda.synchronize()
+
+    npts, nt = w.npoints, 91
+    snap = MalaSnap(**w.snap_params())
+    stream = torch.cuda.current_stream()
+    out = torch.empty((npts, nt), dtype=torch.float64, device=dev)
+    call = lambda: snap.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, out=out, stream=stream)
+
+    # ---- device-resident leg ------------------------------------------------------------------------------
+    snap.set_option("timing", 1)
+    for _ in range(args.warmup):
+        call()
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.15)
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    ktimes = []
+    launches = 0
+    barrier()
+    for a, b in evs:
+        a.record(stream)
+        call()
+        b.record(stream)
+        launches += snap.last_stats()["kernels"]
+        ktimes.append(snap.kernel_times())  # waits for this step's kernels; steps are serial on the stream anyway
+    barrier()
+    clocks = sampler.stop()
+    step_ms = [a.elapsed_time(b) for a, b in evs]
+    total_ms = float(sum(step_ms))
+    total_ms, total_pts = reduce_max_sum(total_ms, npts * args.steps, world, dev)
+    value = total_pts / (total_ms * 1e-3)
+    stats = snap.last_stats()
+    snap.set_option("timing", 0)
+
+    # ---- roofline of the dominant kernel (compute_zi_bi: rows a5 + a6 + a7) --------------------------------
+    pairs, nonempty = workload_counts(w)
+    zi_ms = float(np.mean([k["compute_zi_bi"][0] for k in ktimes]))
+    zi_launches = ktimes[-1]["compute_zi_bi"][1]
+    ui_ms = float(np.mean([k["compute_ui"][0] for k in ktimes]))
+    bin_ms = float(np.mean([k["tile_bin"][0] for k in ktimes]))
+    zi_flop = nonempty * (F_Z + F_B)           # per step = summed over that step's launches
+    achieved = zi_flop / (zi_ms * 1e-3) / 1e12
+    peak_meas, mhz_eff = mala_snap_fp64_peak(stream)
+    roofline = {"bound": "alu", "kernel": "compute_zi_bi_spec_kernel", "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS,
+                "unit": "TFLOP/s", "frac": achieved / FP64_NOMINAL_TFLOPS,
+                "peak_source": "nominal FP64 FMA pipe: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md 'FP64 roofline')",
+                "peak_measured_dfma": peak_meas, "frac_of_measured_dfma": achieved / peak_meas if peak_meas > 0 else None,
+                "dfma_probe_sm_mhz": mhz_eff, "traffic": None,
+                "flop_per_launch": zi_flop / max(zi_launches, 1), "launches_per_step": zi_launches, "ms_per_launch": zi_ms / max(zi_launches, 1),
+                "kernel_ms_per_step": {"tile_bin": bin_ms, "compute_ui": ui_ms, "compute_zi_bi": zi_ms},
+                "compute_ui_tflops": pairs * F_PAIR / (ui_ms * 1e-3) / 1e12 if ui_ms > 0 else None,
+                "step_model_tflops": (pairs * F_PAIR + zi_flop) / (total_ms / args.steps * 1e-3) / 1e12 if world == 1 else None}
+    roofline["traffic"] = NCU_TRAFFIC_BYTES_PER_LAUNCH.get((args.config, roofline["kernel"]))
+    peaks = load_peaks()
+    roofline["hbm_gbs_step"] = (npts * nt * 8 + 2 * (nonempty / 32) * 271 * 32 * 16) / (total_ms / args.steps * 1e-3) / 1e9 if world == 1 else None
+    roofline["hbm_peak_gbs"] = peaks["hbm_gbs"]
+    roofline["hbm_peak_source"] = peaks["source"]
+
+    # ---- end-to-end leg: host output buffer, D2H inside the timed region ------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        host = torch.empty((npts, nt), dtype=torch.float64, pin_memory=True)
+        call_host = lambda: snap.bispectrum_grid_host(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, out=host, stream=stream)
+        for _ in range(max(1, min(args.warmup, 2))):
+            call_host()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            call_host()  # returns after the last device->host copy has completed
+        torch.cuda.synchronize()
+        e2e_s = time.perf_counter() - t0
+        e2e_s, e2e_pts = reduce_max_sum(e2e_s, npts * args.steps, world, dev)
+        h2d = int(w.pos.nbytes + w.types.nbytes + 9 * 8 + 3 * 8 + 3 * 4 + 3 * 4)
+        e2e = {"value": e2e_pts / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": int(npts * nt * 8),
+               "ms_per_step": 1e3 * e2e_s / args.steps,
+               "note": "mala_bispectrum_grid_host: HOST atoms in, pinned HOST descriptors out; D2H overlapped with the kernels of the next z-chunk"}
+        del host
+
+    # ---- CPU oracle beside it (rank 0, N = 1 only) ---------------------------------------------------------
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        rate, n, dt, threads = oracle_rate(w, seconds=12.0)
+        cpu = {"value": rate, "unit": UNIT, "cores": threads, "kind": "oracle",
+               "sample": f"{n} seeded random grid points of {w.name} (of {npts}) in {dt:.1f} s wall on {threads} threads"}
+
+    snap.close()
+    if world > 1:
+        torch.distributed.destroy_process_group()
+    if rank != 0:
+        return
+    cfg = workload_config(w, "mala_bispectrum_grid (device out)")
+    cfg.update({"chunks_per_step": stats["chunks"], "workspace_bytes": stats["workspace_bytes"], "ghost_atoms": stats["ghosts"]})
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": cfg, "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+            "roofline": roofline, "cpu_baseline": cpu, "pct_of_fp64_peak_step": None}
+    if roofline["step_model_tflops"] is not None:
+        line["pct_of_fp64_peak_step"] = 100.0 * roofline["step_model_tflops"] / FP64_NOMINAL_TFLOPS
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    args = parse_args()
+    rank, world, local = dist_setup(args)
+    if world != args.gpus and world > 1:
+        raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE={world}")
+    if args.gpus > 1 and world == 1:
+        raise SystemExit("launch N > 1 with: python -m torch.distributed.run --nnodes=1 --nproc-per-node N bench.py --gpus N ...")
+    from paper_2411_19617_b200 import workloads
+    w = workloads.make(args.config)
+    w.extra["cfg"] = args.config
+    if args.impl == "reference":
+        run_reference(args, w, rank, world)
+        return
+    run_native(args, w, rank, world, local)
+
+
+if __name__ == "__main__":
+    main()

@@ -101,6 +101,8 @@ int mala_bispectrum_grid_host(mala_snap_t *h, int natoms, const double *pos, con
  * Tuning / test knobs.  Unknown names give MALA_SNAP_EINVAL.
  *   "zi_impl"          0 = automatic (specialised kernel when twojmax == 10), 1 = generic table-driven
  *                      kernel, 2 = specialised kernel (EINVAL if twojmax != 10)
+ *   "timing"           1 = record a CUDA-event pair on the caller's stream around every kernel launch of the
+ *                      following calls (read back with mala_snap_kernel_times); 0 = off (default)
  *   "workspace_mb"     cap, in MiB, of the U_tot + candidate workspace (default 4096)
  *   "host_chunk_mb"    size, in MiB, of each of the two staging buffers of mala_bispectrum_grid_host
  */
@@ -112,6 +114,26 @@ int mala_snap_set_option(mala_snap_t *h, const char *name, long long value);
  *   [4] candidate capacity per tile   [5] workspace bytes in use   [6] points   [7] reserved
  */
 int mala_snap_last_stats(const mala_snap_t *h, long long stats[8]);
+
+/*
+ * Measurement: device time of the kernels of the last mala_bispectrum_grid* call on this handle, by class, from
+ * the event pairs recorded when the "timing" option is on (rows of SURVEY.md 8(a)):
+ *   ms[0] tile_bin (a2 + constant fill of empty tiles)   ms[1] compute_ui (a3 + a4)
+ *   ms[2] compute_zi_bi (a5 + a6 + a7)                    ms[3] other (test hooks)
+ *   launches[k] = number of launches summed into ms[k].   Both HOST arrays of 4.
+ * Waits for those events (so for the call's work).  All zeros if timing was off.
+ */
+int mala_snap_kernel_times(mala_snap_t *h, double ms[4], long long launches[4]);
+
+/*
+ * Measurement: achieved FP64 FMA rate of this device (TFLOP/s, 2 flop per DFMA) from a register-only
+ * microbenchmark -- 8 independent FMA chains per thread, 4 CTAs of 256 threads per SM, best of 5 timed launches
+ * after one warm-up -- the measured denominator of the FP64 roofline.
+ *   tflops            [out] HOST
+ *   sm_mhz_effective  [out] HOST, may be NULL: the SM clock that rate implies at 64 DFMA/clk/SM
+ * Synchronises the stream.
+ */
+int mala_snap_fp64_peak(double *tflops, double *sm_mhz_effective, void *cuda_stream);
 
 /*
  * Test hook: the Clebsch-Gordan coefficient the library's own table generator produces (doubled arguments).

@@ -110,6 +110,12 @@ struct mala_snap {
     GridGeom geom{};
     int cand_cap = 0;
     long long stats[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    // optional per-kernel timing ("timing" option): event pairs around every launch of the last call
+    bool timing = false;
+    struct Span { int kind; cudaEvent_t a, b; };
+    std::vector<Span> spans;           // recorded during the last call
+    std::vector<cudaEvent_t> ev_pool;  // reusable timing events
+    size_t ev_used = 0;
 
     DeviceTables tables() const {
         DeviceTables t;
@@ -142,10 +148,38 @@ int set_kernel_attributes(mala_snap *h) {
     return 0;
 }
 
+// kernel classes reported by mala_snap_kernel_times
+enum { kKindBin = 0, kKindUi = 1, kKindZi = 2, kKindOther = 3 };
+
+cudaEvent_t timing_event(mala_snap *h) {
+    if (h->ev_used == h->ev_pool.size()) {
+        cudaEvent_t e = nullptr;
+        if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        h->ev_pool.push_back(e);
+    }
+    return h->ev_pool[h->ev_used++];
+}
+
+// RAII bracket: records an event pair around the launches made while it is alive (no-op unless timing is on)
+struct TimedSpan {
+    mala_snap *h; cudaStream_t st; cudaEvent_t a = nullptr, b = nullptr; int kind;
+    TimedSpan(mala_snap *h_, cudaStream_t st_, int kind_) : h(h_), st(st_), kind(kind_) {
+        if (!h->timing) return;
+        a = timing_event(h); b = timing_event(h);
+        if (a && b) cudaEventRecord(a, st);
+    }
+    ~TimedSpan() {
+        if (!h->timing || !a || !b) return;
+        cudaEventRecord(b, st);
+        h->spans.push_back({kind, a, b});
+    }
+};
+
 // enqueue compute_zi_bi for one chunk
 int launch_zi(mala_snap *h, const ChunkBuffers &cb, double *out, cudaStream_t st) {
     const int grid = std::max(1, std::min(h->num_sms, cb.ntiles));
     const size_t smem = compute_zi_smem_bytes(h->sc.nelem, h->sc.ntriples);
+    TimedSpan span(h, st, kKindZi);
     if (h->use_spec())
         compute_zi_bi_spec_kernel<kSpecWarps><<<grid, kSpecWarps * 32, smem, st>>>(h->geom, h->sc, h->tables(), cb, out);
     else
@@ -234,6 +268,8 @@ int validate(const mala_snap *h, const CallArgs &a, bool need_out, const void *o
 // Ghost atoms + cell list for the slab [z_begin, z_end); fills h->geom (except the tile fields).
 int build_plan(mala_snap *h, const CallArgs &a, cudaStream_t st) {
     GridGeom &g = h->geom;
+    h->spans.clear();
+    h->ev_used = 0;
     h->cur = (int)(h->ncalls & 1ull);
     h->ncalls++;
     const int cur = h->cur;
@@ -464,19 +500,26 @@ int run_slab(mala_snap *h, int z0, int z1, double *out, double2 *u_out, cudaStre
         cb.ntiles = (int)std::min(chunk_tiles, total_tiles - t0);
         CUDA_TRY(cudaMemsetAsync(cb.counters, 0, 4 * sizeof(int), st));
         const int bin_blocks = (cb.ntiles + 7) / 8;
-        tile_bin_kernel<<<bin_blocks, 256, 0, st>>>(g, h->sc, tb, cb, out);
+        {
+            TimedSpan span(h, st, kKindBin);
+            tile_bin_kernel<<<bin_blocks, 256, 0, st>>>(g, h->sc, tb, cb, out);
+        }
         CUDA_TRY(cudaGetLastError());
         const int grid = std::max(1, std::min(h->num_sms, cb.ntiles));
-        if (h->twojmax == kMaxTwoJ)
-            compute_ui_kernel<kMaxTwoJ, true><<<grid, (kMaxTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kMaxTwoJ), st>>>(g, h->sc, tb, cb);
-        else  // smaller twojmax: same code with run-time guards on the levels
-            compute_ui_kernel<kMaxTwoJ, false><<<grid, (kMaxTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kMaxTwoJ), st>>>(g, h->sc, tb, cb);
+        {
+            TimedSpan span(h, st, kKindUi);
+            if (h->twojmax == kMaxTwoJ)
+                compute_ui_kernel<kMaxTwoJ, true><<<grid, (kMaxTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kMaxTwoJ), st>>>(g, h->sc, tb, cb);
+            else  // smaller twojmax: same code with run-time guards on the levels
+                compute_ui_kernel<kMaxTwoJ, false><<<grid, (kMaxTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kMaxTwoJ), st>>>(g, h->sc, tb, cb);
+        }
         CUDA_TRY(cudaGetLastError());
         h->stats[0] += 2;
         if (out) {
             int rc = launch_zi(h, cb, out, st);
             if (rc) return rc;
         } else if (u_out) {
+            TimedSpan span(h, st, kKindOther);
             utot_scatter_kernel<<<bin_blocks, 256, 0, st>>>(g, h->sc, tb, cb, u_out);
             CUDA_TRY(cudaGetLastError());
             h->stats[0]++;
@@ -495,6 +538,23 @@ int finish_call(mala_snap *h, cudaStream_t st) {
 }
 
 }  // namespace
+
+// FP64 FMA-pipe probe: kDfmaChains independent dependent-chains per thread, nothing else in the loop
+constexpr int kDfmaChains = 8;
+__global__ void __launch_bounds__(256) dfma_probe_kernel(double *sink, int iters, double m) {
+    double acc[kDfmaChains];
+#pragma unroll
+    for (int k = 0; k < kDfmaChains; k++) acc[k] = 1e-3 * (threadIdx.x + k);
+    const double c = 1e-7;
+    for (int i = 0; i < iters; i++) {
+#pragma unroll
+        for (int k = 0; k < kDfmaChains; k++) acc[k] = fma(acc[k], m, c);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < kDfmaChains; k++) s += acc[k];
+    if (s == 123.456) sink[threadIdx.x] = s;  // never true; keeps the chains alive
+}
 
 // =============================================================================================================
 // C ABI
@@ -606,6 +666,10 @@ int mala_snap_set_option(mala_snap_t *h, const char *name, long long value) {
         if (before != h->use_spec()) return compute_bconst(h);
         return MALA_SNAP_OK;
     }
+    if (n == "timing") {
+        h->timing = (value != 0);
+        return MALA_SNAP_OK;
+    }
     if (n == "workspace_mb") {
         if (value < 1) return fail(MALA_SNAP_EINVAL, "workspace_mb must be >= 1");
         h->workspace_mb = value;
@@ -622,6 +686,51 @@ int mala_snap_set_option(mala_snap_t *h, const char *name, long long value) {
 int mala_snap_last_stats(const mala_snap_t *h, long long stats[8]) {
     if (!h || !stats) return fail(MALA_SNAP_EINVAL, "handle or stats is NULL");
     for (int i = 0; i < 8; i++) stats[i] = h->stats[i];
+    return MALA_SNAP_OK;
+}
+
+int mala_snap_kernel_times(mala_snap_t *h, double ms[4], long long launches[4]) {
+    if (!h || !ms || !launches) return fail(MALA_SNAP_EINVAL, "handle or output is NULL");
+    for (int k = 0; k < 4; k++) { ms[k] = 0.0; launches[k] = 0; }
+    for (const mala_snap::Span &s : h->spans) {
+        CUDA_TRY(cudaEventSynchronize(s.b));
+        float t = 0.f;
+        CUDA_TRY(cudaEventElapsedTime(&t, s.a, s.b));
+        ms[s.kind] += (double)t;
+        launches[s.kind]++;
+    }
+    return MALA_SNAP_OK;
+}
+
+int mala_snap_fp64_peak(double *tflops, double *sm_mhz_effective, void *cuda_stream) {
+    if (!tflops) return fail(MALA_SNAP_EINVAL, "tflops is NULL");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    double *sink = nullptr;
+    CUDA_TRY(cudaMalloc((void **)&sink, sizeof(double) * 1024));
+    cudaEvent_t a = nullptr, b = nullptr;
+    cudaEventCreate(&a); cudaEventCreate(&b);
+    const int blocks = sms * 4, threads = 256, iters = 1 << 15;
+    double best = 0.0;
+    cudaError_t e = cudaSuccess;
+    for (int rep = 0; rep < 6 && e == cudaSuccess; rep++) {
+        cudaEventRecord(a, st);
+        dfma_probe_kernel<<<blocks, threads, 0, st>>>(sink, iters, 1.0 + 1e-9 * rep);
+        cudaEventRecord(b, st);
+        e = cudaEventSynchronize(b);
+        float t = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&t, a, b);
+        const double flop = 2.0 * kDfmaChains * (double)iters * blocks * threads;
+        if (rep > 0 && t > 0.f) best = std::max(best, flop / (t * 1e-3) / 1e12);
+    }
+    cudaEventDestroy(a); cudaEventDestroy(b);
+    cudaFree(sink);
+    if (e != cudaSuccess) return fail(MALA_SNAP_ECUDA, std::string("fp64 probe: ") + cudaGetErrorString(e));
+    *tflops = best;
+    // clock the rate implies if every SM retires 64 DFMA per cycle
+    if (sm_mhz_effective) *sm_mhz_effective = best * 1e12 / (2.0 * 64.0 * sms) / 1e6;
     return MALA_SNAP_OK;
 }
 
@@ -704,6 +813,7 @@ void mala_snap_destroy(mala_snap_t *h) {
         if (h->ev_copied[i]) cudaEventDestroy(h->ev_copied[i]);
     }
     h->d_cand.release(); h->d_ncand.release(); h->d_active.release(); h->d_counters.release(); h->d_utot.release();
+    for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
     if (h->ev_upload) cudaEventDestroy(h->ev_upload);
     if (h->upload_stream) cudaStreamDestroy(h->upload_stream);
     if (h->copy_stream) cudaStreamDestroy(h->copy_stream);

@@ -19,7 +19,7 @@ MALA_SNAP_ECUDA = -2
 MALA_SNAP_ENOMEM = -3
 
 EXPORTS = ("mala_snap_create", "mala_snap_ncomp", "mala_snap_triples", "mala_bispectrum_grid", "mala_bispectrum_grid_host",
-           "mala_snap_set_option", "mala_snap_last_stats", "mala_snap_clebsch_gordan", "mala_snap_debug_utot",
+           "mala_snap_set_option", "mala_snap_last_stats", "mala_snap_kernel_times", "mala_snap_fp64_peak", "mala_snap_clebsch_gordan", "mala_snap_debug_utot",
            "mala_snap_destroy", "mala_last_error")
 
 
@@ -65,6 +65,10 @@ def load_library():
     lib.mala_snap_set_option.argtypes = [vp, C.c_char_p, C.c_longlong]
     lib.mala_snap_last_stats.restype = C.c_int
     lib.mala_snap_last_stats.argtypes = [vp, C.POINTER(C.c_longlong)]
+    lib.mala_snap_kernel_times.restype = C.c_int
+    lib.mala_snap_kernel_times.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
+    lib.mala_snap_fp64_peak.restype = C.c_int
+    lib.mala_snap_fp64_peak.argtypes = [dp, dp, vp]
     lib.mala_snap_clebsch_gordan.restype = C.c_double
     lib.mala_snap_clebsch_gordan.argtypes = [C.c_int] * 6
     lib.mala_snap_destroy.restype = None
@@ -86,6 +90,15 @@ def _check(rc):
 
 def mala_snap_clebsch_gordan(J1, M1, J2, M2, J, M):
     return load_library().mala_snap_clebsch_gordan(int(J1), int(M1), int(J2), int(M2), int(J), int(M))
+
+
+def mala_snap_fp64_peak(stream=None):
+    """(TFLOP/s, implied SM MHz) of the device's FP64 FMA pipe, measured by the library's register-only probe."""
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    t, f = C.c_double(0.0), C.c_double(0.0)
+    _check(load_library().mala_snap_fp64_peak(C.byref(t), C.byref(f), C.c_void_p(s.cuda_stream)))
+    return t.value, f.value
 
 
 def _d(a):
@@ -152,6 +165,13 @@ class MalaSnap:
         _check(self._lib.mala_snap_last_stats(self._h, st))
         keys = ("kernels", "chunks", "tiles", "ghosts", "cand_cap", "workspace_bytes", "points", "reserved")
         return dict(zip(keys, [int(x) for x in st]))
+
+    def kernel_times(self):
+        """{class: (ms, launches)} of the last call; needs set_option("timing", 1) before it."""
+        ms = (C.c_double * 4)()
+        n = (C.c_longlong * 4)()
+        _check(self._lib.mala_snap_kernel_times(self._h, ms, n))
+        return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(("tile_bin", "compute_ui", "compute_zi_bi", "other"))}
 
     def _system(self, pos, types, box, origin, pbc, ngrid, z_begin, z_end):
         pos = _d(pos).reshape(-1, 3)

@@ -1,0 +1,296 @@
+"""GPU parity: the CUDA path behind the C ABI against the CPU oracle, element by element, on the same seeded inputs.
+
+Bar (BASELINE.json north_star): for each component k, max_p |B_gpu[p,k] - B_oracle[p,k]| <= 1e-9 * max_p |B_oracle[p,k]|.
+Small cases compare whole grids; the full-size configs compare seeded samples of points (the oracle computes any
+point on its own) plus properties that hold at any size (constant vector on empty points, slab-split identity).
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2411_19617_b200 import MalaSnap, MalaSnapError, workloads
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-9
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def assert_parity(got, ref, tol=TOL):
+    assert got.shape == ref.shape
+    assert np.isfinite(got).all()
+    scale = np.abs(ref).max(axis=0)
+    err = np.abs(got - ref).max(axis=0)
+    bad = err > tol * scale
+    assert not bad.any(), f"components {np.nonzero(bad)[0][:8]}: err/scale = {(err / scale)[bad][:8]}"
+    return float((err / scale).max())
+
+
+def gpu_grid(w, z0=0, z1=None, **opts):
+    torch = _torch()
+    with MalaSnap(**w.snap_params()) as snap:
+        for k, v in opts.items():
+            snap.set_option(k, v)
+        out = snap.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, z0, z1)
+        torch.cuda.synchronize()
+        return out.cpu().numpy()
+
+
+def oracle_grid(w, z0=0, z1=None, sample=None):
+    return oracle.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, z0, z1, sample=sample, **w.snap_params())
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# config 1 in full, both contraction kernels, whole grid = many tiles + ragged tails (18 is not a multiple of 4)
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.fixture(scope="module")
+def tiny_ref():
+    w = workloads.make(1)
+    return w, oracle_grid(w)
+
+
+@pytest.mark.parametrize("zi_impl", [1, 2])
+def test_config1_tiny_al_full_grid(tiny_ref, zi_impl):
+    w, ref = tiny_ref
+    got = gpu_grid(w, zi_impl=zi_impl)
+    assert_parity(got, ref)
+
+
+def test_triples_match_oracle_order():
+    with MalaSnap(twojmax=10) as s:
+        assert s.ncomp == 91
+        assert np.array_equal(s.triples(), oracle.triples(10))
+
+
+def test_slab_split_and_small_workspace_are_identical(tiny_ref):
+    """grid points are independent: any z split / internal chunking reproduces the full result"""
+    w, ref = tiny_ref
+    full = gpu_grid(w)
+    parts = [gpu_grid(w, a, b) for a, b in ((0, 5), (5, 6), (6, 18))]
+    assert np.array_equal(np.concatenate(parts), full)
+    chunked = gpu_grid(w, workspace_mb=1)
+    assert np.array_equal(chunked, full)
+    assert gpu_grid(w, 7, 7).shape[0] == 0
+
+
+def test_repeat_calls_are_bitwise_deterministic(tiny_ref):
+    w, _ = tiny_ref
+    torch = _torch()
+    with MalaSnap(**w.snap_params()) as snap:
+        a = snap.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid).clone()
+        b = snap.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid)
+        torch.cuda.synchronize()
+        assert torch.equal(a, b)
+
+
+def test_host_output_entry_point(tiny_ref):
+    w, ref = tiny_ref
+    torch = _torch()
+    with MalaSnap(**w.snap_params()) as snap:
+        snap.set_option("host_chunk_mb", 1)
+        out = snap.bispectrum_grid_host(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid)
+        dev = snap.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid)
+        torch.cuda.synchronize()
+    assert np.array_equal(out.numpy(), dev.cpu().numpy())
+    assert_parity(out.numpy(), ref)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# U_tot itself (rows a3 + a4) against the oracle's explicit Wigner-D sum
+# ---------------------------------------------------------------------------------------------------------------
+def test_utot_matches_explicit_wigner_D(tiny_ref):
+    w, _ = tiny_ref
+    torch = _torch()
+    with MalaSnap(**w.snap_params()) as snap:
+        u = snap.debug_utot(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, 2, 3).cpu().numpy()
+    nx, ny, nz = w.ngrid
+    ix, iy = np.meshgrid(np.arange(nx), np.arange(ny), indexing="xy")
+    frac = np.stack([ix.ravel() / nx, iy.ravel() / ny, np.full(nx * ny, 2 / nz)], axis=1)
+    pts = frac @ w.box + np.asarray(w.origin)
+    res = oracle.bispectrum_points(pts, w.pos, w.types, w.box, w.origin, w.pbc, want_U=True, **w.snap_params())
+    U = res["U"]
+    # B is the same for D, D^T, conj(D) and D^dagger (reading #16); the library may store any ONE of them, everywhere
+    worst = np.zeros(4)
+    e = 0
+    for J in range(w.twojmax + 1):
+        D = U[:, oracle.uoff(J):oracle.uoff(J) + (J + 1) ** 2].reshape(-1, J + 1, J + 1)
+        for mb in range(J // 2 + 1):
+            for ma in range(J + 1):
+                g = u[:, e, 0] + 1j * u[:, e, 1]
+                cands = (D[:, ma, mb], D[:, mb, ma], np.conj(D[:, ma, mb]), np.conj(D[:, mb, ma]))
+                for c, v in enumerate(cands):
+                    worst[c] = max(worst[c], np.abs(g - v).max())
+                e += 1
+    assert e == u.shape[1]
+    assert worst.min() < 1e-11 * np.abs(U).max(), worst
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# brute force on tiny inputs: every twojmax, triclinic box, mixed pbc, two types, box smaller than rcut
+# ---------------------------------------------------------------------------------------------------------------
+def _small_case(seed, twojmax, natoms, pbc, triclinic, two_types, ngrid=(7, 5, 6)):
+    rng = np.random.default_rng(seed)
+    box = np.diag([3.1, 3.7, 4.3])
+    if triclinic:
+        box = box + np.array([[0.0, 0.0, 0.0], [0.9, 0.0, 0.0], [-0.6, 0.8, 0.0]])
+        if seed % 2:
+            box = box[[1, 0, 2]]  # left-handed
+    pos = rng.random((natoms, 3)) @ box * 1.6 - 0.9  # unwrapped, partly outside the cell
+    ntypes = 2 if two_types else 1
+    types = rng.integers(0, ntypes, natoms).astype(np.int32)
+    params = dict(twojmax=twojmax, rcutfac=2.4, rfac0=0.99363, rmin0=0.0 if seed % 3 else 0.3, wself=1.0 if seed % 2 else 0.7,
+                  radelem=(0.5, 0.37)[:ntypes], wj=(1.0, 0.6)[:ntypes])
+    origin = (0.1, -0.2, 0.05)
+    return pos, types, box, origin, pbc, ngrid, params
+
+
+@pytest.mark.parametrize("twojmax", [0, 1, 2, 3, 4, 5, 7, 8, 9, 10])
+def test_small_cases_every_twojmax(twojmax):
+    torch = _torch()
+    for seed, (natoms, pbc, tri, two) in enumerate([(0, (1, 1, 1), False, False), (1, (0, 0, 0), False, False),
+                                                    (3, (1, 1, 1), True, True), (5, (1, 0, 1), True, True),
+                                                    (2, (0, 1, 0), False, True)]):
+        pos, types, box, origin, pbc, ngrid, params = _small_case(100 * twojmax + seed, twojmax, natoms, pbc, tri, two)
+        ref = oracle.bispectrum_grid(pos, types, box, origin, pbc, ngrid, **params)
+        with MalaSnap(**params) as snap:
+            got = snap.bispectrum_grid(pos, types, box, origin, pbc, ngrid)
+            torch.cuda.synchronize()
+            assert snap.ncomp == ref.shape[1]
+        assert_parity(got.cpu().numpy(), ref)
+
+
+def test_zero_atoms_gives_self_term_everywhere():
+    """closed form: B_{j1 j2 j} = wself^3 (j+1) for every triple (north_star: zero neighbors -> self term only)"""
+    torch = _torch()
+    with MalaSnap(twojmax=10, wself=1.3) as snap:
+        out = snap.bispectrum_grid(np.zeros((0, 3)), np.zeros(0, np.int32), np.eye(3) * 5.0, ngrid=(9, 6, 5))
+        torch.cuda.synchronize()
+        expect = 1.3 ** 3 * (snap.triples()[:, 2] + 1.0)
+    got = out.cpu().numpy()
+    assert got.shape == (270, 91)
+    assert np.abs(got - expect[None, :]).max() < 1e-12 * expect.max()
+
+
+def test_atom_exactly_on_a_grid_point_and_at_the_cutoff():
+    """reading #11 (continuous limit at r = 0) and #12 (strict < at rcut; f_c(rcut) = 0)"""
+    torch = _torch()
+    box = np.eye(3) * 8.0
+    ngrid = (8, 8, 8)
+    pos = np.array([[2.0, 3.0, 4.0],      # on grid point (2,3,4)
+                    [5.0, 3.0, 4.0 + 1e-13]])  # 3.0 = rcut away from (2,3,4) up to rounding
+    types = np.zeros(2, np.int32)
+    params = dict(twojmax=6, rcutfac=3.0)
+    ref = oracle.bispectrum_grid(pos, types, box, (0, 0, 0), (1, 1, 1), ngrid, **params)
+    with MalaSnap(**params) as snap:
+        got = snap.bispectrum_grid(pos, types, box, ngrid=ngrid)
+        torch.cuda.synchronize()
+    assert_parity(got.cpu().numpy(), ref)
+
+
+def test_invalid_arguments_are_rejected_without_enqueueing():
+    torch = _torch()
+    w = workloads.make(1)
+    with MalaSnap(**w.snap_params()) as snap:
+        out = torch.zeros((18 * 18, 91), dtype=torch.float64, device="cuda")
+        for kw in (dict(ngrid=(18, 18, 0)), dict(z_begin=3, z_end=2), dict(z_end=19), dict(types=np.array([0, 0, 1, 0])),
+                   dict(box=np.zeros((3, 3))), dict(pos=np.full((4, 3), np.nan))):
+            a = dict(pos=w.pos, types=w.types, box=w.box, origin=w.origin, pbc=w.pbc, ngrid=w.ngrid, z_begin=0, z_end=1)
+            a.update(kw)
+            with pytest.raises(MalaSnapError) as e:
+                snap.bispectrum_grid(out=out, **a)
+            assert e.value.code == -1
+        torch.cuda.synchronize()
+        assert float(out.abs().max()) == 0.0
+        with pytest.raises(MalaSnapError):
+            snap.set_option("no_such_option", 1)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# full-size configs in the launch configuration bench.py times: sampled points + any-size properties
+# ---------------------------------------------------------------------------------------------------------------
+def _sampled_parity(w, got, nsample, seed):
+    rng = np.random.default_rng(seed)
+    npts = w.npoints
+    sample = np.unique(np.concatenate([rng.integers(0, npts, nsample), [0, npts - 1, w.ngrid[0] - 1, npts - w.ngrid[0]]]))
+    ref = oracle_grid(w, sample=sample)
+    return assert_parity(got[sample], ref), sample, ref
+
+
+def test_config2_solid_al_full_size_sampled():
+    """headline workload: 256-atom Al, 90^3 grid; 3,000 seeded sample points + two complete z-planes"""
+    torch = _torch()
+    w = workloads.make(2)
+    with MalaSnap(**w.snap_params()) as snap:
+        out = snap.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid)
+        torch.cuda.synchronize()
+        got = out.cpu().numpy()
+        assert snap.last_stats()["points"] == 729000
+        # the same slab computed alone is bit-identical
+        part = snap.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, 44, 46).cpu().numpy()
+    _sampled_parity(w, got, 3000, 22)
+    plane = 90 * 90
+    assert np.array_equal(part, got[44 * plane:46 * plane])
+    assert_parity(part[:plane], oracle_grid(w, 44, 45))
+    # lattice translation of one atom / permutation of atoms: invariances (north_star) hold to rounding on the GPU too
+    pos2 = w.pos[::-1].copy()
+    pos2[3] += w.box[0] - 2 * w.box[2]
+    part2 = gpu_grid(workloads.Workload(**{**w.__dict__, "pos": pos2}), 44, 45)
+    assert np.abs(part2 - part[:plane]).max() <= 1e-11 * np.abs(part).max()
+
+
+def test_config3_liquid_al_full_size_sampled():
+    w = workloads.make(3)
+    got = gpu_grid(w)
+    _sampled_parity(w, got, 2000, 33)
+
+
+def test_config4_boron_cluster_full_size_sampled_and_empty_points():
+    """79 % of the points have no neighbor and must hold exactly the constant self-only vector"""
+    w = workloads.make(4)
+    got = gpu_grid(w)
+    nx, ny, nz = w.ngrid
+    rng = np.random.default_rng(44)
+    # sample biased towards the cluster (uniform sampling would mostly hit empty points)
+    near = []
+    while len(near) < 1500:
+        i = rng.integers(0, nx, 3)
+        p = i / np.array(w.ngrid) * 20.0
+        if np.linalg.norm(p - 10.0) < 8.5:
+            near.append((i[2] * ny + i[1]) * nx + i[0])
+    sample = np.unique(np.concatenate([near, rng.integers(0, w.npoints, 500)]))
+    ref = oracle_grid(w, sample=sample)
+    assert_parity(got[sample], ref)
+    # every point farther than rcut from all atoms: self term only, closed form wself^3 (j+1)
+    ix, iy, iz = np.meshgrid(np.arange(nx), np.arange(ny), np.arange(nz), indexing="ij")
+    idx = ((iz * ny + iy) * nx + ix).ravel()
+    pts = np.stack([ix.ravel(), iy.ravel(), iz.ravel()], axis=1) / np.array(w.ngrid) * 20.0
+    d2min = np.full(pts.shape[0], np.inf)
+    for a in w.pos:
+        d2min = np.minimum(d2min, ((pts - a) ** 2).sum(1))
+    empty = idx[d2min > (w.rcutfac * (1 + 1e-12)) ** 2]
+    assert 0.75 < empty.size / w.npoints < 0.83
+    expect = oracle.triples(10)[:, 2] + 1.0
+    assert np.abs(got[empty] - expect[None, :]).max() < 1e-12 * expect.max()
+
+
+def test_config5_be_slab_z_slabs_sampled():
+    """16,384-atom Be slab with the stacking fault; output streamed in z-slabs (here: the slab through the fault, one
+    at the periodic boundary and a ragged last slab), sampled against the oracle"""
+    torch = _torch()
+    w = workloads.make(5)
+    nx, ny, nz = w.ngrid
+    assert (nx, ny, nz) == (183, 317, 287)
+    rng = np.random.default_rng(55)
+    with MalaSnap(**w.snap_params()) as snap:
+        for z0, z1 in ((140, 148), (0, 3), (280, 287)):
+            out = snap.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, z0, z1)
+            torch.cuda.synchronize()
+            got = out.cpu().numpy()
+            n = (z1 - z0) * ny * nx
+            sample = np.unique(np.concatenate([rng.integers(0, n, 250), [0, n - 1]]))
+            ref = oracle.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, z0, z1, sample=sample, **w.snap_params())
+            assert_parity(got[sample], ref)
+            del out
