@@ -19,7 +19,7 @@
 #include "snap_tables.h"
 #include "snap_ui.cuh"
 #include "snap_zi.cuh"
-#include "snap_zi_spec.cuh"
+#include "snap_zi_coop.cuh"
 
 using namespace mala;
 
@@ -128,7 +128,6 @@ struct mala_snap {
 
 namespace {
 
-constexpr int kSpecWarps = 8;
 
 template <typename T>
 int upload(DevBuf<T> &b, const std::vector<T> &v) {
@@ -143,7 +142,7 @@ int set_kernel_attributes(mala_snap *h) {
     CUDA_TRY(cudaFuncSetAttribute(compute_ui_kernel<kMaxTwoJ, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ui_smem));
     const int zi_smem = (int)compute_zi_smem_bytes(uhalf_size(kMaxTwoJ), triple_count(kMaxTwoJ));
     CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, zi_smem));
-    CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_spec_kernel<kSpecWarps>, cudaFuncAttributeMaxDynamicSharedMemorySize, zi_smem));
+    CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_coop_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)compute_zi_coop_smem_bytes()));
     (void)h;
     return 0;
 }
@@ -181,7 +180,7 @@ int launch_zi(mala_snap *h, const ChunkBuffers &cb, double *out, cudaStream_t st
     const size_t smem = compute_zi_smem_bytes(h->sc.nelem, h->sc.ntriples);
     TimedSpan span(h, st, kKindZi);
     if (h->use_spec())
-        compute_zi_bi_spec_kernel<kSpecWarps><<<grid, kSpecWarps * 32, smem, st>>>(h->geom, h->sc, h->tables(), cb, out);
+        compute_zi_bi_coop_kernel<<<grid, kCoopWarps * 32, compute_zi_coop_smem_bytes(), st>>>(h->geom, h->sc, h->tables(), cb, out);
     else
         compute_zi_bi_generic_kernel<<<grid, kZiWarps * 32, smem, st>>>(h->geom, h->sc, h->tables(), cb, out);
     CUDA_TRY(cudaGetLastError());
@@ -355,9 +354,9 @@ int build_plan(mala_snap *h, const CallArgs &a, cudaStream_t st) {
         target *= 1.26;
     }
     for (int d = 0; d < 3; d++) {
-        const double ext = std::max(hi[d] - lo[d], 1e-9);
+        const double ext = hi[d] - lo[d];
         g.cell_lo[d] = lo[d];
-        g.cell_inv[d] = nc[d] / ext;
+        g.cell_inv[d] = (ext > 1e-9) ? nc[d] / ext : 0.0;  // degenerate extent: one cell, every index maps to 0
     }
     g.ncx = nc[0]; g.ncy = nc[1]; g.ncz = nc[2];
     const size_t ncell = (size_t)nc[0] * nc[1] * nc[2];
@@ -445,7 +444,7 @@ int candidate_bound(const mala_snap *h) {
     const int nc[3] = {g.ncx, g.ncy, g.ncz};
     const double reach = g.tile_radius + g.rcutmax;
     int w[3];
-    for (int d = 0; d < 3; d++) w[d] = std::min(nc[d], (int)std::floor(2.0 * reach * g.cell_inv[d]) + 2);
+    for (int d = 0; d < 3; d++) w[d] = (int)std::min((double)nc[d], std::floor(2.0 * reach * g.cell_inv[d]) + 2.0);
     const size_t sx = nc[0] + 1, sy = nc[1] + 1, sz = nc[2] + 1;
     std::vector<long long> S(sx * sy * sz, 0);
     auto at = [&](int x, int y, int z) -> long long & { return S[((size_t)z * sy + y) * sx + x]; };
@@ -620,6 +619,24 @@ int mala_snap_create(mala_snap_t **handle, int twojmax, double rcutfac, double r
             if ((int)h->tab.cg.size() != kSpecCG || h->tab.ntriples != kSpecNT) return fail(MALA_SNAP_ECUDA, "internal: table size mismatch");
             CUDA_TRY(cudaMemcpyToSymbol(c_cg_spec, h->tab.cg.data(), sizeof(double) * kSpecCG));
             CUDA_TRY(cudaMemcpyToSymbol(c_order_spec, h->tab.order.data(), sizeof(int) * kSpecNT));
+            // deal the (mb, mb1) items of every triple to the warps: run lengths of a round-robin deal over the whole
+            // tile, handed out as contiguous runs inside each triple (snap_zi_coop.cuh "Schedule")
+            unsigned short sched[kSpecNT][kCoopWarps][2];
+            long long start = 0;
+            for (int pos = 0; pos < kSpecNT; pos++) {
+                const int t = h->tab.order[pos];
+                const int n = triple_items(h->tab.triples[4 * t], h->tab.triples[4 * t + 1], h->tab.triples[4 * t + 2]);
+                const int q = n / kCoopWarps, r = n % kCoopWarps, s0 = (int)(start % kCoopWarps);
+                int begin = 0;
+                for (int w = 0; w < kCoopWarps; w++) {
+                    const int cnt = q + ((((w - s0) % kCoopWarps + kCoopWarps) % kCoopWarps) < r ? 1 : 0);
+                    sched[pos][w][0] = (unsigned short)begin;
+                    sched[pos][w][1] = (unsigned short)(begin + cnt);
+                    begin += cnt;
+                }
+                start += n;
+            }
+            CUDA_TRY(cudaMemcpyToSymbol(c_sched, sched, sizeof(sched)));
         }
         if ((rc = set_kernel_attributes(h))) return rc;
         CUDA_TRY(cudaStreamCreateWithFlags(&h->upload_stream, cudaStreamNonBlocking));

@@ -122,8 +122,10 @@ __global__ void __launch_bounds__(256) tile_bin_kernel(GridGeom g, SnapConst sc,
 // one column (M) of all levels for two neighbors at once; accumulates levels J >= 2M into shared memory.
 // Ul points at element 0 of this lane (stride 32 double2 between elements).
 // ---------------------------------------------------------------------------------------------------------
-template <int M, int TJMAX, bool EXACT>
-__device__ __noinline__ void ui_column_pair(double2 *__restrict__ Ul, const int tj,
+// M is a run-time argument on purpose: all column-warps then run the SAME instructions, so the SM fetches one
+// instruction stream instead of one per column (the per-column template instances stalled on instruction fetch).
+template <int TJMAX, bool EXACT>
+__device__ __noinline__ void ui_column_pair(double2 *__restrict__ Ul, const int tj, const int M,
                                                const double c0, const double a0r, const double a0i, const double b0r, const double b0i,
                                                const double c1, const double a1r, const double a1i, const double b1r, const double b1i) {
     double pr[2][TJMAX + 1], pi[2][TJMAX + 1];
@@ -248,15 +250,7 @@ compute_ui_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers cb) {
                     const double *q = geo + (size_t)(i + 1) * 5 * 32 + lane;
                     c1 = q[0]; a1r = q[32]; a1i = q[64]; b1r = q[96]; b1i = q[128];
                 }
-                switch (warp) {
-                    case 0: ui_column_pair<0, TJMAX, EXACT>(Ul, tj, c0, a0r, a0i, b0r, b0i, c1, a1r, a1i, b1r, b1i); break;
-                    case 1: if (TJMAX >= 2) ui_column_pair<(TJMAX >= 2 ? 1 : 0), TJMAX, EXACT>(Ul, tj, c0, a0r, a0i, b0r, b0i, c1, a1r, a1i, b1r, b1i); break;
-                    case 2: if (TJMAX >= 4) ui_column_pair<(TJMAX >= 4 ? 2 : 0), TJMAX, EXACT>(Ul, tj, c0, a0r, a0i, b0r, b0i, c1, a1r, a1i, b1r, b1i); break;
-                    case 3: if (TJMAX >= 6) ui_column_pair<(TJMAX >= 6 ? 3 : 0), TJMAX, EXACT>(Ul, tj, c0, a0r, a0i, b0r, b0i, c1, a1r, a1i, b1r, b1i); break;
-                    case 4: if (TJMAX >= 8) ui_column_pair<(TJMAX >= 8 ? 4 : 0), TJMAX, EXACT>(Ul, tj, c0, a0r, a0i, b0r, b0i, c1, a1r, a1i, b1r, b1i); break;
-                    case 5: if (TJMAX >= 10) ui_column_pair<(TJMAX >= 10 ? 5 : 0), TJMAX, EXACT>(Ul, tj, c0, a0r, a0i, b0r, b0i, c1, a1r, a1i, b1r, b1i); break;
-                    default: break;
-                }
+                ui_column_pair<TJMAX, EXACT>(Ul, tj, warp, c0, a0r, a0i, b0r, b0i, c1, a1r, a1i, b1r, b1i);
             }
         };
 

@@ -1,0 +1,231 @@
+// snap_zi_coop.cuh -- compute_zi / compute_bi specialised at compile time for twojmax = 10 (rows a5 + a6 + a7).
+//
+// Arithmetic.  For a triple (J1,J2,J), output column mb and one (mb1, mb2 = mb + sh - mb1) pair -- an "item" --
+//     z[ma] += cgb * sum_{ma1 + ma2 - sh = ma} CG(ma1, ma2) * x[ma1] * y[ma2],   x = U^{J1}[:, mb1], y = U^{J2}[:, mb2]
+// is a CG-weighted 1-D convolution of two columns.  x (<= 11 complex) and z (<= 11 complex) live in registers, y is
+// streamed one element at a time (pre-multiplied by cgb and by the sign/conjugation of the column-flip symmetry),
+// and the (ma1, ma2) loops are unrolled at compile time so every register index and every CG address is static; the
+// CG values are constant-memory operands of the DMUL instructions.  6 FP64-pipe instructions per product term,
+// ~0.25 B of shared-memory traffic per flop.  compute_bi is fused: a finished run of items of one column is folded
+// into B at once (B is linear in Z), so Z is never stored.
+//
+// Schedule.  A CTA owns one tile (32 grid points = the lanes of every warp; U_tot of the tile TMA-loaded into shared
+// memory).  ALL warps of the CTA work on the SAME triple at the same time: the items of a triple are dealt to the
+// warps as contiguous runs whose lengths follow a round-robin deal over the whole tile (so the load is balanced
+// across triples, not only within one).  The first version of this kernel gave every warp a triple of its own; with
+// ~13 KB of straight-line code per triple that made the SM fetch eight instruction streams at once and ncu showed
+// 25 "no instruction" stall cycles per issued instruction (profiles/r01_baseline.md).  Same-triple scheduling keeps the
+// instruction working set at one or two loop bodies.
+// Partial B values go through a small double-buffered shared-memory array and are summed in a fixed order every
+// eight triples, so results are bit-reproducible.
+#pragma once
+#include "snap_zi.cuh"
+
+namespace mala {
+
+constexpr int kSpecTJ = 10;
+constexpr int kSpecNT = triple_count(kSpecTJ);
+constexpr int kSpecCG = cg_block_off(kSpecTJ, kSpecNT);
+constexpr int kCoopWarps = 8;   // warps per CTA
+constexpr int kCoopGroup = 8;   // triples between two reductions of the partial sums
+
+__constant__ double c_cg_spec[kSpecCG];                        // dense CG blocks of every triple, [m2][m1]
+__constant__ int c_order_spec[kSpecNT];                        // triples by decreasing cost
+__constant__ unsigned short c_sched[kSpecNT][kCoopWarps][2];   // [position in c_order_spec][warp] = item range [begin, end)
+
+constexpr int kRowBytes = 32 * (int)sizeof(double2);  // bytes between consecutive elements of one lane
+
+// number of (mb, mb1) items of a triple: columns mb = 0..J/2, mb1 over the range with a valid mb2
+constexpr int triple_items(int J1, int J2, int J) {
+    const int sh = (J1 + J2 - J) / 2;
+    int n = 0;
+    for (int mb = 0; mb <= J / 2; mb++) {
+        const int lo = (mb + sh - J2) > 0 ? (mb + sh - J2) : 0;
+        const int hi = (mb + sh) < J1 ? (mb + sh) : J1;
+        n += hi - lo + 1;
+    }
+    return n;
+}
+
+__device__ __forceinline__ double flip_sign(double v, unsigned mask) {
+    return __hiloint2double(__double2hiint(v) ^ (int)mask, __double2loint(v));
+}
+
+// z[ma] += sum CG * x[ma1] * (scaled y[ma2]) for one item
+template <int J1, int J2, int J, int CGOFF>
+__device__ __forceinline__ void cg_convolve(double (&zr)[J + 1], double (&zi)[J + 1], const double (&xr)[J1 + 1],
+                                            const double (&xi)[J1 + 1], const unsigned char *ybase, const int ystep,
+                                            const double sre0, const double sre1, const double sim0, const double sim1) {
+    constexpr int SH = (J1 + J2 - J) / 2;
+#pragma unroll
+    for (int ma2 = 0; ma2 <= J2; ma2++) {
+        const int lo = (SH - ma2) > 0 ? (SH - ma2) : 0;
+        const int hi = (J + SH - ma2) < J1 ? (J + SH - ma2) : J1;
+        if (lo <= hi) {
+            const double2 yv = *reinterpret_cast<const double2 *>(ybase + ma2 * ystep);
+            const double yr = yv.x * ((ma2 & 1) ? sre1 : sre0);
+            const double yi = yv.y * ((ma2 & 1) ? sim1 : sim0);
+#pragma unroll
+            for (int ma1 = 0; ma1 <= J1; ma1++) {
+                if (ma1 >= lo && ma1 <= hi) {
+                    const int ma = ma1 + ma2 - SH;
+                    const double cg = c_cg_spec[CGOFF + ma2 * (J1 + 1) + ma1];
+                    const double tr = cg * xr[ma1];
+                    const double ti = cg * xi[ma1];
+                    zr[ma] = fma(tr, yr, zr[ma]);
+                    zr[ma] = fma(-ti, yi, zr[ma]);
+                    zi[ma] = fma(tr, yi, zi[ma]);
+                    zi[ma] = fma(ti, yr, zi[ma]);
+                }
+            }
+        }
+    }
+}
+
+// items mb1 in [mb1_begin, mb1_end) of output column mb: returns their contribution to B
+template <int J1, int J2, int J, int CGOFF>
+__device__ __forceinline__ double column_segment(const unsigned char *Ulane, const int mb, const int mb1_begin, const int mb1_end) {
+    constexpr int SH = (J1 + J2 - J) / 2;
+    double zr[J + 1], zi[J + 1];
+#pragma unroll
+    for (int k = 0; k <= J; k++) { zr[k] = 0.0; zi[k] = 0.0; }
+#pragma unroll 1
+    for (int mb1 = mb1_begin; mb1 < mb1_end; mb1++) {
+        const int mb2 = mb + SH - mb1;
+        const double cgb = c_cg_spec[CGOFF + mb2 * (J1 + 1) + mb1];
+        // x = U^{J1}[:, mb1]; columns beyond the middle come from the stored half by
+        // u[ma][mb] = (-1)^(ma-mb) conj(u[J-ma][J-mb])
+        const bool fx = mb1 > J1 / 2;
+        const int cx = fx ? J1 - mb1 : mb1;
+        const unsigned char *xb = Ulane + (uhalf_off(J1) + cx * (J1 + 1) + (fx ? J1 : 0)) * kRowBytes;
+        const int xstep = fx ? -kRowBytes : kRowBytes;
+        // sign masks by parity of ma1: real part (-1)^(ma1-mb1), imaginary part the opposite (conjugation)
+        const unsigned mxr0 = (fx && (mb1 & 1)) ? 0x80000000u : 0u;
+        const unsigned mxr1 = (fx && !(mb1 & 1)) ? 0x80000000u : 0u;
+        const unsigned mxi0 = fx ? (mxr0 ^ 0x80000000u) : 0u;
+        const unsigned mxi1 = fx ? (mxr1 ^ 0x80000000u) : 0u;
+        double xr[J1 + 1], xi[J1 + 1];
+#pragma unroll
+        for (int k = 0; k <= J1; k++) {
+            const double2 v = *reinterpret_cast<const double2 *>(xb + k * xstep);
+            xr[k] = flip_sign(v.x, (k & 1) ? mxr1 : mxr0);
+            xi[k] = flip_sign(v.y, (k & 1) ? mxi1 : mxi0);
+        }
+        // y = U^{J2}[:, mb2], same symmetry, folded with cgb into four scale factors
+        const bool fy = mb2 > J2 / 2;
+        const int cy = fy ? J2 - mb2 : mb2;
+        const unsigned char *yb = Ulane + (uhalf_off(J2) + cy * (J2 + 1) + (fy ? J2 : 0)) * kRowBytes;
+        const int ystep = fy ? -kRowBytes : kRowBytes;
+        const double p0 = (fy && (mb2 & 1)) ? -cgb : cgb;  // parity-0 rows, real part
+        const double p1 = fy ? -p0 : cgb;                  // parity-1 rows, real part
+        const double q0 = fy ? -p0 : cgb;                  // imaginary parts: conjugation flips the sign again
+        const double q1 = fy ? -p1 : cgb;
+        cg_convolve<J1, J2, J, CGOFF>(zr, zi, xr, xi, yb, ystep, p0, p1, q0, q1);
+    }
+    // compute_bi: B += w * Re(conj(U^J[ma][mb]) * z[ma]).  Columns below the middle stand for their mirror images
+    // too (w = 2); the middle column of an even J is computed in full and counted once.
+    const unsigned char *ub = Ulane + (uhalf_off(J) + mb * (J + 1)) * kRowBytes;
+    const double w = (((J & 1) == 0) && mb == J / 2) ? 1.0 : 2.0;
+    double b = 0.0;
+#pragma unroll
+    for (int ma = 0; ma <= J; ma++) {
+        const double2 u = *reinterpret_cast<const double2 *>(ub + ma * kRowBytes);
+        b = fma(u.x, zr[ma], b);
+        b = fma(u.y, zi[ma], b);
+    }
+    return w * b;
+}
+
+// this warp's items [begin, end) of triple T (items numbered column by column)
+template <int T>
+__device__ __noinline__ double triple_items_b(const unsigned char *Ulane, const int begin, const int end) {
+    constexpr Triple tr = triple_at(kSpecTJ, T);
+    constexpr int J1 = tr.j1, J2 = tr.j2, J = tr.j;
+    constexpr int SH = (J1 + J2 - J) / 2;
+    constexpr int CGOFF = cg_block_off(kSpecTJ, T);
+    double b = 0.0;
+    int base = 0;
+#pragma unroll 1
+    for (int mb = 0; mb <= J / 2; mb++) {
+        const int lo = max(0, mb + SH - J2), hi = min(J1, mb + SH);
+        const int nb = hi - lo + 1;
+        const int s = max(begin, base), e = min(end, base + nb);
+        if (s < e) b += column_segment<J1, J2, J, CGOFF>(Ulane, mb, lo + s - base, lo + e - base);
+        base += nb;
+    }
+    return b;
+}
+
+__device__ __forceinline__ double dispatch_triple(const int t, const unsigned char *Ulane, const int begin, const int end) {
+    double b = 0.0;
+    switch (t) {
+#define MALA_CASE(N) \
+    case N:          \
+        if (N < kSpecNT) b = triple_items_b<(N < kSpecNT ? N : 0)>(Ulane, begin, end); \
+        break;
+#define MALA_CASE10(D) \
+    MALA_CASE(D * 10 + 0) MALA_CASE(D * 10 + 1) MALA_CASE(D * 10 + 2) MALA_CASE(D * 10 + 3) MALA_CASE(D * 10 + 4) \
+    MALA_CASE(D * 10 + 5) MALA_CASE(D * 10 + 6) MALA_CASE(D * 10 + 7) MALA_CASE(D * 10 + 8) MALA_CASE(D * 10 + 9)
+        MALA_CASE10(0) MALA_CASE10(1) MALA_CASE10(2) MALA_CASE10(3) MALA_CASE10(4)
+        MALA_CASE10(5) MALA_CASE10(6) MALA_CASE10(7) MALA_CASE10(8) MALA_CASE10(9)
+#undef MALA_CASE10
+#undef MALA_CASE
+        default: break;
+    }
+    return b;
+}
+
+__global__ void __launch_bounds__(kCoopWarps * 32, 1)
+compute_zi_bi_coop_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers cb, double *out) {
+    static_assert(kSpecNT <= 100, "dispatch_triple covers 100 cases");
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int nelem = uhalf_size(kSpecTJ), nt = kSpecNT, NW = kCoopWarps;
+    double2 *U = reinterpret_cast<double2 *>(smem_raw);
+    double *Bs = reinterpret_cast<double *>(U + (size_t)nelem * 32);
+    double *red = Bs + 32 * nt;  // [2][kCoopGroup][NW][32]
+    __shared__ uint64_t bar;
+    __shared__ int s_slot;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) mbar_init(&bar, 1);
+    uint32_t parity = 0;
+    for (;;) {
+        __syncthreads();  // previous tile written out: Bs, U and s_slot are free
+        if (threadIdx.x == 0) s_slot = atomicAdd(&cb.counters[2], 1);
+        __syncthreads();
+        const int slot = s_slot;
+        if (slot >= cb.counters[0]) break;
+        const int wt = cb.active[slot];
+        if (threadIdx.x == 0) tma_load_tile(U, cb.utot + (size_t)slot * nelem * 32, nelem, &bar);
+        mbar_wait(&bar, parity);
+        parity ^= 1u;
+        const unsigned char *Ulane = reinterpret_cast<const unsigned char *>(U + lane);
+        for (int pos = 0; pos < nt; pos++) {
+            const int t = c_order_spec[pos];
+            const int begin = c_sched[pos][warp][0], end = c_sched[pos][warp][1];
+            double b = 0.0;
+            if (begin < end) b = dispatch_triple(t, Ulane, begin, end);
+            const int buf = (pos / kCoopGroup) & 1, k = pos % kCoopGroup;
+            red[((buf * kCoopGroup + k) * NW + warp) * 32 + lane] = b;
+            if (k == kCoopGroup - 1 || pos == nt - 1) {
+                __syncthreads();
+                // fixed-order sum of the partials of the triples of this group
+                for (int kk = warp; kk <= k; kk += NW) {
+                    const double *r = red + ((buf * kCoopGroup + kk) * NW) * 32 + lane;
+                    double s = 0.0;
+#pragma unroll
+                    for (int w2 = 0; w2 < NW; w2++) s += r[w2 * 32];
+                    Bs[lane * nt + c_order_spec[pos - k + kk]] = s;
+                }
+            }
+        }
+        __syncthreads();
+        write_tile(g, cb.tile_begin + wt, Bs, nt, out, NW);
+    }
+}
+
+inline size_t compute_zi_coop_smem_bytes() {
+    return (size_t)uhalf_size(kSpecTJ) * 32 * sizeof(double2) + (size_t)32 * kSpecNT * sizeof(double) +
+           (size_t)2 * kCoopGroup * kCoopWarps * 32 * sizeof(double) + 16;
+}
+
+}  // namespace mala

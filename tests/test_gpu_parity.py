@@ -69,8 +69,11 @@ def test_slab_split_and_small_workspace_are_identical(tiny_ref):
     """grid points are independent: any z split / internal chunking reproduces the full result"""
     w, ref = tiny_ref
     full = gpu_grid(w)
-    parts = [gpu_grid(w, a, b) for a, b in ((0, 5), (5, 6), (6, 18))]
-    assert np.array_equal(np.concatenate(parts), full)
+    # a slab may get another tile shape, hence another neighbor summation order: equal to rounding (SURVEY.md section 4)
+    parts = np.concatenate([gpu_grid(w, a, b) for a, b in ((0, 5), (5, 6), (6, 18))])
+    assert np.abs(parts - full).max() <= 1e-13 * np.abs(full).max()
+    assert_parity(parts, ref)
+    # internal chunking keeps the tiles, so it is bit-identical
     chunked = gpu_grid(w, workspace_mb=1)
     assert np.array_equal(chunked, full)
     assert gpu_grid(w, 7, 7).shape[0] == 0
@@ -194,7 +197,7 @@ def test_invalid_arguments_are_rejected_without_enqueueing():
     torch = _torch()
     w = workloads.make(1)
     with MalaSnap(**w.snap_params()) as snap:
-        out = torch.zeros((18 * 18, 91), dtype=torch.float64, device="cuda")
+        out = torch.zeros((20 * 18 * 18, 91), dtype=torch.float64, device="cuda")
         for kw in (dict(ngrid=(18, 18, 0)), dict(z_begin=3, z_end=2), dict(z_end=19), dict(types=np.array([0, 0, 1, 0])),
                    dict(box=np.zeros((3, 3))), dict(pos=np.full((4, 3), np.nan))):
             a = dict(pos=w.pos, types=w.types, box=w.box, origin=w.origin, pbc=w.pbc, ngrid=w.ngrid, z_begin=0, z_end=1)
@@ -228,11 +231,11 @@ def test_config2_solid_al_full_size_sampled():
         torch.cuda.synchronize()
         got = out.cpu().numpy()
         assert snap.last_stats()["points"] == 729000
-        # the same slab computed alone is bit-identical
+        # the same slab computed alone agrees to rounding
         part = snap.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, 44, 46).cpu().numpy()
     _sampled_parity(w, got, 3000, 22)
     plane = 90 * 90
-    assert np.array_equal(part, got[44 * plane:46 * plane])
+    assert np.abs(part - got[44 * plane:46 * plane]).max() <= 1e-13 * np.abs(part).max()
     assert_parity(part[:plane], oracle_grid(w, 44, 45))
     # lattice translation of one atom / permutation of atoms: invariances (north_star) hold to rounding on the GPU too
     pos2 = w.pos[::-1].copy()
