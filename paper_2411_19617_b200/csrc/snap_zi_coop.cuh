@@ -26,8 +26,14 @@ namespace mala {
 constexpr int kSpecTJ = 10;
 constexpr int kSpecNT = triple_count(kSpecTJ);
 constexpr int kSpecCG = cg_block_off(kSpecTJ, kSpecNT);
-constexpr int kCoopWarps = 8;   // warps per CTA
-constexpr int kCoopGroup = 8;   // triples between two reductions of the partial sums
+#ifndef MALA_COOP_WARPS
+#define MALA_COOP_WARPS 8
+#endif
+#ifndef MALA_COOP_GROUP
+#define MALA_COOP_GROUP 8
+#endif
+constexpr int kCoopWarps = MALA_COOP_WARPS;   // warps per CTA
+constexpr int kCoopGroup = MALA_COOP_GROUP;   // triples between two reductions of the partial sums
 
 __constant__ double c_cg_spec[kSpecCG];                        // dense CG blocks of every triple, [m2][m1]
 __constant__ int c_order_spec[kSpecNT];                        // triples by decreasing cost
