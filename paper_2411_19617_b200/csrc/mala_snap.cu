@@ -619,22 +619,38 @@ int mala_snap_create(mala_snap_t **handle, int twojmax, double rcutfac, double r
             if ((int)h->tab.cg.size() != kSpecCG || h->tab.ntriples != kSpecNT) return fail(MALA_SNAP_ECUDA, "internal: table size mismatch");
             CUDA_TRY(cudaMemcpyToSymbol(c_cg_spec, h->tab.cg.data(), sizeof(double) * kSpecCG));
             CUDA_TRY(cudaMemcpyToSymbol(c_order_spec, h->tab.order.data(), sizeof(int) * kSpecNT));
-            // deal the (mb, mb1) items of every triple to the warps: run lengths of a round-robin deal over the whole
-            // tile, handed out as contiguous runs inside each triple (snap_zi_coop.cuh "Schedule")
-            unsigned short sched[kSpecNT][kCoopWarps][2];
-            long long start = 0;
+            // deal the (mb, mb1) items of every triple to the warps as contiguous runs (snap_zi_coop.cuh "Schedule"):
+            // run boundaries are placed so that every warp's cumulative cost (product terms plus a fixed per-item
+            // overhead) tracks the mean over the whole tile, not only within one triple
+            static unsigned short sched[kSpecNT][kCoopWarps][2];
+            const double kItemOverhead = 8.0;
+            std::vector<double> load(kCoopWarps, 0.0);
+            double total = 0.0;
             for (int pos = 0; pos < kSpecNT; pos++) {
                 const int t = h->tab.order[pos];
-                const int n = triple_items(h->tab.triples[4 * t], h->tab.triples[4 * t + 1], h->tab.triples[4 * t + 2]);
-                const int q = n / kCoopWarps, r = n % kCoopWarps, s0 = (int)(start % kCoopWarps);
-                int begin = 0;
-                for (int w = 0; w < kCoopWarps; w++) {
-                    const int cnt = q + ((((w - s0) % kCoopWarps + kCoopWarps) % kCoopWarps) < r ? 1 : 0);
-                    sched[pos][w][0] = (unsigned short)begin;
-                    sched[pos][w][1] = (unsigned short)(begin + cnt);
-                    begin += cnt;
+                const int J1 = h->tab.triples[4 * t], J2 = h->tab.triples[4 * t + 1], J = h->tab.triples[4 * t + 2];
+                std::vector<double> cost;
+                for (int mb = 0; mb <= J / 2; mb++) {
+                    const int nb = item_hi(J1, J2, J, mb) - item_lo(J1, J2, J, mb) + 1;
+                    for (int i = 0; i < nb; i++) cost.push_back(item_terms(J1, J2, J, mb) + kItemOverhead);
                 }
-                start += n;
+                const int n = (int)cost.size();
+                for (double c : cost) total += c;
+                const double target = total / kCoopWarps;
+                int i = 0;
+                for (int w = 0; w < kCoopWarps; w++) {
+                    const int begin = i;
+                    double acc = 0.0;
+                    if (w == kCoopWarps - 1) {
+                        for (; i < n; i++) acc += cost[i];
+                    } else {
+                        const double want = target - load[w];
+                        while (i < n && acc + 0.5 * cost[i] <= want) acc += cost[i++];
+                    }
+                    load[w] += acc;
+                    sched[pos][w][0] = (unsigned short)begin;
+                    sched[pos][w][1] = (unsigned short)i;
+                }
             }
             CUDA_TRY(cudaMemcpyToSymbol(c_sched, sched, sizeof(sched)));
         }

@@ -27,7 +27,7 @@ constexpr int kSpecTJ = 10;
 constexpr int kSpecNT = triple_count(kSpecTJ);
 constexpr int kSpecCG = cg_block_off(kSpecTJ, kSpecNT);
 #ifndef MALA_COOP_WARPS
-#define MALA_COOP_WARPS 8
+#define MALA_COOP_WARPS 12
 #endif
 #ifndef MALA_COOP_GROUP
 #define MALA_COOP_GROUP 8
@@ -41,15 +41,36 @@ __constant__ unsigned short c_sched[kSpecNT][kCoopWarps][2];   // [position in c
 
 constexpr int kRowBytes = 32 * (int)sizeof(double2);  // bytes between consecutive elements of one lane
 
-// number of (mb, mb1) items of a triple: columns mb = 0..J/2, mb1 over the range with a valid mb2
+// Items of output column mb: mb1 in [item_lo, item_hi], mb2 = mb + sh - mb1.
+// J1 == J2: the items (mb1, mb2) and (mb2, mb1) contribute the same Z column (swap the two factors and use
+// CG(j1 m1 j1 m2 | j m) = +-CG(j1 m2 j1 m1 | j m) for both coefficients), so only mb1 <= mb2 is computed, with weight 2
+// when mb1 < mb2.
+constexpr int item_lo(int J1, int J2, int J, int mb) {
+    const int s = mb + (J1 + J2 - J) / 2;
+    return (s - J2) > 0 ? (s - J2) : 0;
+}
+constexpr int item_hi(int J1, int J2, int J, int mb) {
+    const int s = mb + (J1 + J2 - J) / 2;
+    int hi = s < J1 ? s : J1;
+    if (J1 == J2 && s / 2 < hi) hi = s / 2;
+    return hi;
+}
+// the middle column of an even J needs rows ma <= J/2 only (the others are its mirror images)
+constexpr bool is_mid(int J, int mb) { return (J % 2 == 0) && (mb == J / 2); }
+
+// number of (mb, mb1) items of a triple: columns mb = 0..J/2
 constexpr int triple_items(int J1, int J2, int J) {
-    const int sh = (J1 + J2 - J) / 2;
     int n = 0;
-    for (int mb = 0; mb <= J / 2; mb++) {
-        const int lo = (mb + sh - J2) > 0 ? (mb + sh - J2) : 0;
-        const int hi = (mb + sh) < J1 ? (mb + sh) : J1;
-        n += hi - lo + 1;
-    }
+    for (int mb = 0; mb <= J / 2; mb++) n += item_hi(J1, J2, J, mb) - item_lo(J1, J2, J, mb) + 1;
+    return n;
+}
+// product terms of one item of column mb (the cost unit of the schedule)
+constexpr int item_terms(int J1, int J2, int J, int mb) {
+    const int sh = (J1 + J2 - J) / 2, mahi = is_mid(J, mb) ? J / 2 : J;
+    int n = 0;
+    for (int m2 = 0; m2 <= J2; m2++)
+        for (int m1 = 0; m1 <= J1; m1++)
+            if (m1 + m2 - sh >= 0 && m1 + m2 - sh <= mahi) n++;
     return n;
 }
 
@@ -58,7 +79,7 @@ __device__ __forceinline__ double flip_sign(double v, unsigned mask) {
 }
 
 // z[ma] += sum CG * x[ma1] * (scaled y[ma2]) for one item
-template <int J1, int J2, int J, int CGOFF>
+template <int J1, int J2, int J, int CGOFF, int MAHI>
 __device__ __forceinline__ void cg_convolve(double (&zr)[J + 1], double (&zi)[J + 1], const double (&xr)[J1 + 1],
                                             const double (&xi)[J1 + 1], const unsigned char *ybase, const int ystep,
                                             const double sre0, const double sre1, const double sim0, const double sim1) {
@@ -66,7 +87,7 @@ __device__ __forceinline__ void cg_convolve(double (&zr)[J + 1], double (&zi)[J 
 #pragma unroll
     for (int ma2 = 0; ma2 <= J2; ma2++) {
         const int lo = (SH - ma2) > 0 ? (SH - ma2) : 0;
-        const int hi = (J + SH - ma2) < J1 ? (J + SH - ma2) : J1;
+        const int hi = (MAHI + SH - ma2) < J1 ? (MAHI + SH - ma2) : J1;
         if (lo <= hi) {
             const double2 yv = *reinterpret_cast<const double2 *>(ybase + ma2 * ystep);
             const double yr = yv.x * ((ma2 & 1) ? sre1 : sre0);
@@ -88,17 +109,20 @@ __device__ __forceinline__ void cg_convolve(double (&zr)[J + 1], double (&zi)[J 
     }
 }
 
-// items mb1 in [mb1_begin, mb1_end) of output column mb: returns their contribution to B
-template <int J1, int J2, int J, int CGOFF>
+// items mb1 in [mb1_begin, mb1_end) of output column mb: returns their contribution to B.
+// MID: mb is the middle column of an even J; only rows ma <= J/2 are formed.
+template <int J1, int J2, int J, int CGOFF, bool MID>
 __device__ __forceinline__ double column_segment(const unsigned char *Ulane, const int mb, const int mb1_begin, const int mb1_end) {
     constexpr int SH = (J1 + J2 - J) / 2;
+    constexpr int MAHI = MID ? J / 2 : J;
     double zr[J + 1], zi[J + 1];
 #pragma unroll
     for (int k = 0; k <= J; k++) { zr[k] = 0.0; zi[k] = 0.0; }
 #pragma unroll 1
     for (int mb1 = mb1_begin; mb1 < mb1_end; mb1++) {
         const int mb2 = mb + SH - mb1;
-        const double cgb = c_cg_spec[CGOFF + mb2 * (J1 + 1) + mb1];
+        double cgb = c_cg_spec[CGOFF + mb2 * (J1 + 1) + mb1];
+        if (J1 == J2 && mb1 != mb2) cgb += cgb;  // stands for its mirror item (mb2, mb1) too
         // x = U^{J1}[:, mb1]; columns beyond the middle come from the stored half by
         // u[ma][mb] = (-1)^(ma-mb) conj(u[J-ma][J-mb])
         const bool fx = mb1 > J1 / 2;
@@ -126,20 +150,25 @@ __device__ __forceinline__ double column_segment(const unsigned char *Ulane, con
         const double p1 = fy ? -p0 : cgb;                  // parity-1 rows, real part
         const double q0 = fy ? -p0 : cgb;                  // imaginary parts: conjugation flips the sign again
         const double q1 = fy ? -p1 : cgb;
-        cg_convolve<J1, J2, J, CGOFF>(zr, zi, xr, xi, yb, ystep, p0, p1, q0, q1);
+        cg_convolve<J1, J2, J, CGOFF, MAHI>(zr, zi, xr, xi, yb, ystep, p0, p1, q0, q1);
     }
     // compute_bi: B += w * Re(conj(U^J[ma][mb]) * z[ma]).  Columns below the middle stand for their mirror images
-    // too (w = 2); the middle column of an even J is computed in full and counted once.
+    // too (w = 2); in the middle column of an even J rows ma < J/2 stand for rows J - ma (w = 2), the centre counts once.
     const unsigned char *ub = Ulane + (uhalf_off(J) + mb * (J + 1)) * kRowBytes;
-    const double w = (((J & 1) == 0) && mb == J / 2) ? 1.0 : 2.0;
     double b = 0.0;
 #pragma unroll
-    for (int ma = 0; ma <= J; ma++) {
+    for (int ma = 0; ma < (MID ? J / 2 : J + 1); ma++) {
         const double2 u = *reinterpret_cast<const double2 *>(ub + ma * kRowBytes);
         b = fma(u.x, zr[ma], b);
         b = fma(u.y, zi[ma], b);
     }
-    return w * b;
+    b += b;
+    if (MID) {
+        const double2 u = *reinterpret_cast<const double2 *>(ub + (J / 2) * kRowBytes);
+        b = fma(u.x, zr[J / 2], b);
+        b = fma(u.y, zi[J / 2], b);
+    }
+    return b;
 }
 
 // this warp's items [begin, end) of triple T (items numbered column by column)
@@ -147,17 +176,21 @@ template <int T>
 __device__ __noinline__ double triple_items_b(const unsigned char *Ulane, const int begin, const int end) {
     constexpr Triple tr = triple_at(kSpecTJ, T);
     constexpr int J1 = tr.j1, J2 = tr.j2, J = tr.j;
-    constexpr int SH = (J1 + J2 - J) / 2;
     constexpr int CGOFF = cg_block_off(kSpecTJ, T);
+    constexpr int NFULL = (J % 2 == 0) ? J / 2 : J / 2 + 1;  // columns computed in full
     double b = 0.0;
     int base = 0;
 #pragma unroll 1
-    for (int mb = 0; mb <= J / 2; mb++) {
-        const int lo = max(0, mb + SH - J2), hi = min(J1, mb + SH);
-        const int nb = hi - lo + 1;
+    for (int mb = 0; mb < NFULL; mb++) {
+        const int lo = item_lo(J1, J2, J, mb), nb = item_hi(J1, J2, J, mb) - lo + 1;
         const int s = max(begin, base), e = min(end, base + nb);
-        if (s < e) b += column_segment<J1, J2, J, CGOFF>(Ulane, mb, lo + s - base, lo + e - base);
+        if (s < e) b += column_segment<J1, J2, J, CGOFF, false>(Ulane, mb, lo + s - base, lo + e - base);
         base += nb;
+    }
+    if (J % 2 == 0) {
+        constexpr int lo = item_lo(J1, J2, J, J / 2), nb = item_hi(J1, J2, J, J / 2) - lo + 1;
+        const int s = max(begin, base), e = min(end, base + nb);
+        if (s < e) b += column_segment<J1, J2, J, CGOFF, true>(Ulane, J / 2, lo + s - base, lo + e - base);
     }
     return b;
 }
