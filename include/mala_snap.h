@@ -99,8 +99,11 @@ int mala_bispectrum_grid_host(mala_snap_t *h, int natoms, const double *pos, con
 
 /*
  * Tuning / test knobs.  Unknown names give MALA_SNAP_EINVAL.
- *   "zi_impl"          0 = automatic (specialised kernel when twojmax == 10), 1 = generic table-driven
- *                      kernel, 2 = specialised kernel (EINVAL if twojmax != 10)
+ *   "zi_impl"          0 = automatic (per-triple specialised kernel when twojmax == 10, anti-diagonal kernel
+ *                      otherwise), 1 = generic table-driven kernel, 2 = per-triple specialised kernel (EINVAL if
+ *                      twojmax != 10), 3 = anti-diagonal kernel (code specialised on j1 only, any twojmax).
+ *                      The anti-diagonal kernel keeps its tables in __constant__ memory, one image per process:
+ *                      handles with different twojmax must not run it concurrently on different streams.
  *   "timing"           1 = record a CUDA-event pair on the caller's stream around every kernel launch of the
  *                      following calls (read back with mala_snap_kernel_times); 0 = off (default)
  *   "workspace_mb"     cap, in MiB, of the U_tot + candidate workspace (default 4096)

@@ -9,6 +9,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -20,6 +21,7 @@
 #include "snap_ui.cuh"
 #include "snap_zi.cuh"
 #include "snap_zi_coop.cuh"
+#include "snap_zi_diag.cuh"
 
 using namespace mala;
 
@@ -85,6 +87,11 @@ struct mala_snap {
     int device = 0, num_sms = 0;
     // options
     int zi_impl = 0;
+    // constant-memory images of the diag kernel (uploaded again when another handle used the constants last)
+    std::vector<double> k_dcg;
+    std::vector<DiagTriple> k_dtriple;
+    std::vector<unsigned short> k_dsched;
+    int k_duoff[kMaxTwoJ + 2] = {0};
     long long workspace_mb = 4096;
     long long host_chunk_mb = 512;
     // device tables
@@ -123,7 +130,9 @@ struct mala_snap {
         t.type_rcut = d_rcut.p; t.type_w = d_w.p; t.bconst = d_bconst.p;
         return t;
     }
-    bool use_spec() const { return (zi_impl == 2) || (zi_impl == 0 && twojmax == kSpecTJ); }
+    // 0 = automatic: the per-triple specialised kernel at twojmax = 10, the anti-diagonal kernel otherwise
+    bool use_spec() const { return zi_impl == 2 || (zi_impl == 0 && twojmax == kSpecTJ); }
+    bool use_diag() const { return zi_impl == 3 || (zi_impl == 0 && twojmax != kSpecTJ); }
 };
 
 namespace {
@@ -143,6 +152,8 @@ int set_kernel_attributes(mala_snap *h) {
     const int zi_smem = (int)compute_zi_smem_bytes(uhalf_size(kMaxTwoJ), triple_count(kMaxTwoJ));
     CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, zi_smem));
     CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_coop_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)compute_zi_coop_smem_bytes()));
+    CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_diag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)compute_zi_diag_smem_bytes(uhalf_size(kMaxTwoJ), triple_count(kMaxTwoJ))));
     (void)h;
     return 0;
 }
@@ -174,12 +185,87 @@ struct TimedSpan {
     }
 };
 
+// The diag kernel reads its tables from __constant__ memory, which is one image per process: the handle that used it
+// last is remembered and another handle uploads its own image (stream-ordered) before launching.
+const mala_snap *g_diag_owner = nullptr;
+
+int bind_diag_constants(mala_snap *h, cudaStream_t st) {
+    if (g_diag_owner == h) return 0;
+    CUDA_TRY(cudaMemcpyToSymbolAsync(c_dcg, h->k_dcg.data(), h->k_dcg.size() * sizeof(double), 0, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyToSymbolAsync(c_dtriple, h->k_dtriple.data(), h->k_dtriple.size() * sizeof(DiagTriple), 0, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyToSymbolAsync(c_dsched, h->k_dsched.data(), h->k_dsched.size() * sizeof(unsigned short), 0, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyToSymbolAsync(c_duoff, h->k_duoff, sizeof(h->k_duoff), 0, cudaMemcpyHostToDevice, st));
+    g_diag_owner = h;
+    return 0;
+}
+
+// processing order (J1 descending, then cost) and the per-warp item schedule of the diag kernel
+void build_diag_schedule(mala_snap *h) {
+    const SnapTables &T = h->tab;
+    const int nt = T.ntriples;
+    h->k_dcg = T.cg;
+    h->k_dcg.resize(T.cg.size() + 16, 0.0);
+    for (int J = 0; J <= kMaxTwoJ + 1; J++) h->k_duoff[J] = uhalf_off(J);
+    const double kItemOverhead = 10.0;
+    std::vector<double> tcost(nt, 0.0);
+    std::vector<std::vector<double>> icost(nt);
+    for (int t = 0; t < nt; t++) {
+        const int J1 = T.triples[4 * t], J2 = T.triples[4 * t + 1], J = T.triples[4 * t + 2];
+        for (int mb = 0; mb <= J / 2; mb++) {
+            int lo, hi;
+            diag_item_range(J1, J2, J, mb, lo, hi);
+            for (int i = lo; i <= hi; i++) icost[t].push_back((double)(J1 + 1) * (J2 + 1) + kItemOverhead);
+        }
+        for (double c : icost[t]) tcost[t] += c;
+    }
+    std::vector<int> order(nt);
+    for (int i = 0; i < nt; i++) order[i] = i;
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) {
+        if (T.triples[4 * a] != T.triples[4 * b]) return T.triples[4 * a] > T.triples[4 * b];
+        return tcost[a] > tcost[b];
+    });
+    h->k_dtriple.assign(nt, DiagTriple{});
+    h->k_dsched.assign((size_t)kDiagMaxNT * kDiagWarps * 2, 0);
+    std::vector<double> load(kDiagWarps, 0.0);
+    double total = 0.0;
+    for (int pos = 0; pos < nt; pos++) {
+        const int t = order[pos];
+        DiagTriple &d = h->k_dtriple[pos];
+        d.J1 = (short)T.triples[4 * t]; d.J2 = (short)T.triples[4 * t + 1]; d.J = (short)T.triples[4 * t + 2];
+        d.index = (short)t; d.cgoff = T.triples[4 * t + 3]; d.pad = 0;
+        const std::vector<double> &cost = icost[t];
+        const int n = (int)cost.size();
+        total += tcost[t];
+        const double target = total / kDiagWarps;
+        int i = 0;
+        for (int w = 0; w < kDiagWarps; w++) {
+            const int begin = i;
+            double acc = 0.0;
+            if (w == kDiagWarps - 1) {
+                for (; i < n; i++) acc += cost[i];
+            } else {
+                const double want = target - load[w];
+                while (i < n && acc + 0.5 * cost[i] <= want) acc += cost[i++];
+            }
+            load[w] += acc;
+            h->k_dsched[((size_t)pos * kDiagWarps + w) * 2] = (unsigned short)begin;
+            h->k_dsched[((size_t)pos * kDiagWarps + w) * 2 + 1] = (unsigned short)i;
+        }
+    }
+}
+
 // enqueue compute_zi_bi for one chunk
 int launch_zi(mala_snap *h, const ChunkBuffers &cb, double *out, cudaStream_t st) {
     const int grid = std::max(1, std::min(h->num_sms, cb.ntiles));
     const size_t smem = compute_zi_smem_bytes(h->sc.nelem, h->sc.ntriples);
+    if (h->use_diag()) {
+        int rc = bind_diag_constants(h, st);
+        if (rc) return rc;
+    }
     TimedSpan span(h, st, kKindZi);
-    if (h->use_spec())
+    if (h->use_diag())
+        compute_zi_bi_diag_kernel<<<grid, kDiagWarps * 32, compute_zi_diag_smem_bytes(h->sc.nelem, h->sc.ntriples), st>>>(h->geom, h->sc, h->tables(), cb, out);
+    else if (h->use_spec())
         compute_zi_bi_coop_kernel<<<grid, kCoopWarps * 32, compute_zi_coop_smem_bytes(), st>>>(h->geom, h->sc, h->tables(), cb, out);
     else
         compute_zi_bi_generic_kernel<<<grid, kZiWarps * 32, smem, st>>>(h->geom, h->sc, h->tables(), cb, out);
@@ -623,9 +709,17 @@ int mala_snap_create(mala_snap_t **handle, int twojmax, double rcutfac, double r
             // run boundaries are placed so that every warp's cumulative cost (product terms plus a fixed per-item
             // overhead) tracks the mean over the whole tile, not only within one triple
             static unsigned short sched[kSpecNT][kCoopWarps][2];
+            // The warps form `teams` teams; a triple goes to the team with the smallest load (triples come in order of
+            // decreasing cost) and its items are dealt to that team's warps as contiguous runs whose boundaries keep
+            // every warp's cumulative cost on the team mean.  More teams = longer runs per call but more instruction
+            // streams in flight: measured on B200 (config 2) 1 team 30.8 ms, 2 teams 28.9 ms, 3 teams 35.7 ms,
+            // 4 teams 52.9 ms -- the 32 KB instruction cache holds two loop bodies, not three.
             const double kItemOverhead = 8.0;
-            std::vector<double> load(kCoopWarps, 0.0);
-            double total = 0.0;
+            int teams = kCoopTeams;
+            if (const char *e = std::getenv("MALA_SNAP_COOP_TEAMS")) teams = std::atoi(e);
+            if (teams < 1 || kCoopWarps % teams != 0) teams = 1;
+            const int tw = kCoopWarps / teams;  // warps per team
+            std::vector<double> load(kCoopWarps, 0.0), team_load(teams, 0.0);
             for (int pos = 0; pos < kSpecNT; pos++) {
                 const int t = h->tab.order[pos];
                 const int J1 = h->tab.triples[4 * t], J2 = h->tab.triples[4 * t + 1], J = h->tab.triples[4 * t + 2];
@@ -635,13 +729,20 @@ int mala_snap_create(mala_snap_t **handle, int twojmax, double rcutfac, double r
                     for (int i = 0; i < nb; i++) cost.push_back(item_terms(J1, J2, J, mb) + kItemOverhead);
                 }
                 const int n = (int)cost.size();
-                for (double c : cost) total += c;
-                const double target = total / kCoopWarps;
+                double sum = 0.0;
+                for (double c : cost) sum += c;
+                int team = 0;
+                for (int k = 1; k < teams; k++)
+                    if (team_load[k] < team_load[team]) team = k;
+                team_load[team] += sum;
+                const double target = team_load[team] / tw;
+                for (int w = 0; w < kCoopWarps; w++) sched[pos][w][0] = sched[pos][w][1] = 0;
                 int i = 0;
-                for (int w = 0; w < kCoopWarps; w++) {
+                for (int k = 0; k < tw; k++) {
+                    const int w = team * tw + k;
                     const int begin = i;
                     double acc = 0.0;
-                    if (w == kCoopWarps - 1) {
+                    if (k == tw - 1) {
                         for (; i < n; i++) acc += cost[i];
                     } else {
                         const double want = target - load[w];
@@ -654,6 +755,7 @@ int mala_snap_create(mala_snap_t **handle, int twojmax, double rcutfac, double r
             }
             CUDA_TRY(cudaMemcpyToSymbol(c_sched, sched, sizeof(sched)));
         }
+        build_diag_schedule(h);
         if ((rc = set_kernel_attributes(h))) return rc;
         CUDA_TRY(cudaStreamCreateWithFlags(&h->upload_stream, cudaStreamNonBlocking));
         CUDA_TRY(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
@@ -692,12 +794,10 @@ int mala_snap_set_option(mala_snap_t *h, const char *name, long long value) {
     if (!h || !name) return fail(MALA_SNAP_EINVAL, "handle or name is NULL");
     const std::string n(name);
     if (n == "zi_impl") {
-        if (value < 0 || value > 2) return fail(MALA_SNAP_EINVAL, "zi_impl must be 0, 1 or 2");
+        if (value < 0 || value > 3) return fail(MALA_SNAP_EINVAL, "zi_impl must be 0, 1, 2 or 3");
         if (value == 2 && h->twojmax != kSpecTJ) return fail(MALA_SNAP_EINVAL, "the specialised kernel exists for twojmax = 10 only");
-        const bool before = h->use_spec();
         h->zi_impl = (int)value;
-        if (before != h->use_spec()) return compute_bconst(h);
-        return MALA_SNAP_OK;
+        return compute_bconst(h);
     }
     if (n == "timing") {
         h->timing = (value != 0);
@@ -836,6 +936,7 @@ int mala_snap_debug_utot(mala_snap_t *h, int natoms, const double *pos, const in
 
 void mala_snap_destroy(mala_snap_t *h) {
     if (!h) return;
+    if (g_diag_owner == h) g_diag_owner = nullptr;
     cudaDeviceSynchronize();
     h->d_triples.release(); h->d_udiag.release(); h->d_order.release();
     h->d_cg.release(); h->d_unorm.release(); h->d_rcut.release(); h->d_w.release(); h->d_bconst.release();

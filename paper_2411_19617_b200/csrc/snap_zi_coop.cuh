@@ -33,6 +33,10 @@ constexpr int kSpecCG = cg_block_off(kSpecTJ, kSpecNT);
 #define MALA_COOP_GROUP 8
 #endif
 constexpr int kCoopWarps = MALA_COOP_WARPS;   // warps per CTA
+#ifndef MALA_COOP_TEAMS
+#define MALA_COOP_TEAMS 2
+#endif
+constexpr int kCoopTeams = MALA_COOP_TEAMS;   // warp teams working on different triples at the same time
 constexpr int kCoopGroup = MALA_COOP_GROUP;   // triples between two reductions of the partial sums
 
 __constant__ double c_cg_spec[kSpecCG];                        // dense CG blocks of every triple, [m2][m1]
@@ -155,13 +159,14 @@ __device__ __forceinline__ double column_segment(const unsigned char *Ulane, con
     // compute_bi: B += w * Re(conj(U^J[ma][mb]) * z[ma]).  Columns below the middle stand for their mirror images
     // too (w = 2); in the middle column of an even J rows ma < J/2 stand for rows J - ma (w = 2), the centre counts once.
     const unsigned char *ub = Ulane + (uhalf_off(J) + mb * (J + 1)) * kRowBytes;
-    double b = 0.0;
+    double bp[4] = {0.0, 0.0, 0.0, 0.0};  // independent partial sums: no 2(J+1)-deep dependent DFMA chain
 #pragma unroll
     for (int ma = 0; ma < (MID ? J / 2 : J + 1); ma++) {
         const double2 u = *reinterpret_cast<const double2 *>(ub + ma * kRowBytes);
-        b = fma(u.x, zr[ma], b);
-        b = fma(u.y, zi[ma], b);
+        bp[(2 * ma) & 3] = fma(u.x, zr[ma], bp[(2 * ma) & 3]);
+        bp[(2 * ma + 1) & 3] = fma(u.y, zi[ma], bp[(2 * ma + 1) & 3]);
     }
+    double b = (bp[0] + bp[1]) + (bp[2] + bp[3]);
     b += b;
     if (MID) {
         const double2 u = *reinterpret_cast<const double2 *>(ub + (J / 2) * kRowBytes);

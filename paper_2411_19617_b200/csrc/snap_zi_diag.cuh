@@ -1,0 +1,252 @@
+// snap_zi_diag.cuh -- compute_zi / compute_bi with anti-diagonal accumulators (rows a5 + a6 + a7), any twojmax <= 10.
+//
+// Same arithmetic as snap_zi_coop.cuh (an *item* = triple (J1,J2,J), output column mb, one (mb1, mb2) pair; its Z column
+// is a CG-weighted 1-D convolution of x = U^{J1}[:, mb1] and y = U^{J2}[:, mb2]), organised so that the code depends on
+// J1 only:
+//   * the accumulators are indexed by the anti-diagonal d = ma1 + k of the (ma1, row) rectangle, r[0 .. 2 J1], with
+//     the rows k = ma2 + (J1 - J2) right-aligned.  Row k touches r[k .. k + J1]: all register indices are static for a
+//     body unrolled over the J1 + 1 possible rows, and a triple with fewer rows enters the body at row J1 - J2
+//     (a switch with fall-through), so the rows run without any branch between them;
+//   * J2, J, the shift sh = (J1 + J2 - J)/2 and the CG block are run-time values: z[ma] = r[ma + sh + J1 - J2] is
+//     resolved when the column is folded into B (compute_bi), where only the *address* of conj(U^J[ma][mb]) depends on
+//     it.  Products outside the band 0 <= ma <= J are computed with the zero entries of the dense CG table (+24 % FP64
+//     work at twojmax = 10) -- the price for an instruction footprint of 11 bodies (~50 KB, mostly resident in the
+//     instruction caches) instead of one body per triple (~750 KB streamed from L2 for every tile; profiles/r01_*.md).
+// Scheduling, the fixed-order reduction of the partial sums and the writer are those of the coop kernel.
+#pragma once
+#include "snap_zi.cuh"
+
+namespace mala {
+
+#ifndef MALA_DIAG_WARPS
+#define MALA_DIAG_WARPS 12
+#endif
+#ifndef MALA_DIAG_GROUP
+#define MALA_DIAG_GROUP 8
+#endif
+constexpr int kDiagWarps = MALA_DIAG_WARPS;  // warps per CTA
+constexpr int kDiagGroup = MALA_DIAG_GROUP;  // triples between two reductions of the partial sums
+constexpr int kDiagMaxNT = triple_count(kMaxTwoJ);
+constexpr int kDiagMaxCG = cg_block_off(kMaxTwoJ, kDiagMaxNT);
+
+struct DiagTriple {  // one entry per position of the processing order
+    short J1, J2, J, index;  // index = component number in output order
+    int cgoff;               // offset of the dense CG block [m2][m1] in c_dcg
+    int pad;
+};
+
+__constant__ double c_dcg[kDiagMaxCG + 16];                         // dense CG blocks (zero where m is out of range)
+__constant__ DiagTriple c_dtriple[kDiagMaxNT];                       // processing order: J1 descending, then cost
+__constant__ unsigned short c_dsched[kDiagMaxNT][kDiagWarps][2];     // [position][warp] = item range [begin, end)
+__constant__ int c_duoff[kMaxTwoJ + 2];                              // half-column offset of every level
+
+constexpr int kDiagRowBytes = 32 * (int)sizeof(double2);
+
+// item range of output column mb (run-time version of item_lo / item_hi of snap_zi_coop.cuh)
+__host__ __device__ inline void diag_item_range(int J1, int J2, int J, int mb, int &lo, int &hi) {
+    const int s = mb + (J1 + J2 - J) / 2;
+    lo = (s - J2) > 0 ? (s - J2) : 0;
+    hi = s < J1 ? s : J1;
+    if (J1 == J2 && s / 2 < hi) hi = s / 2;  // mirror items (mb2, mb1) are folded into weight 2
+}
+
+__device__ __forceinline__ double diag_flip(double v, unsigned mask) {
+    return __hiloint2double(__double2hiint(v) ^ (int)mask, __double2loint(v));
+}
+
+// one row of the rectangle: r[ma1 + K] += CG[row][ma1] * x[ma1] * y,  y pre-scaled
+template <int J1, int K>
+__device__ __forceinline__ void diag_row(double (&rr)[2 * J1 + 1], double (&ri)[2 * J1 + 1], const double (&xr)[J1 + 1],
+                                         const double (&xi)[J1 + 1], const unsigned char *yrow0, const int ystep, const int cbase,
+                                         const double se, const double so, const double te, const double to) {
+    const double2 yv = *reinterpret_cast<const double2 *>(yrow0 + K * ystep);
+    const double yr = yv.x * ((K & 1) ? so : se);
+    const double yi = yv.y * ((K & 1) ? to : te);
+#pragma unroll
+    for (int ma1 = 0; ma1 <= J1; ma1++) {
+        const double cg = c_dcg[cbase + K * (J1 + 1) + ma1];
+        const double tr = cg * xr[ma1];
+        const double ti = cg * xi[ma1];
+        rr[ma1 + K] = fma(tr, yr, rr[ma1 + K]);
+        rr[ma1 + K] = fma(-ti, yi, rr[ma1 + K]);
+        ri[ma1 + K] = fma(tr, yi, ri[ma1 + K]);
+        ri[ma1 + K] = fma(ti, yr, ri[ma1 + K]);
+    }
+}
+
+// items mb1 in [mb1_begin, mb1_end) of output column mb of one triple: their contribution to B
+template <int J1>
+__device__ __forceinline__ double diag_segment(const unsigned char *Ulane, const int J2, const int J, const int sh, const int cgoff,
+                                               const int mb, const int mb1_begin, const int mb1_end) {
+    constexpr int ND = 2 * J1 + 1;
+    double rr[ND], ri[ND];
+#pragma unroll
+    for (int d = 0; d < ND; d++) { rr[d] = 0.0; ri[d] = 0.0; }
+    const int off = J1 - J2;  // first row of the unrolled body
+    const int uoff2 = c_duoff[J2];
+#pragma unroll 1
+    for (int mb1 = mb1_begin; mb1 < mb1_end; mb1++) {
+        const int mb2 = mb + sh - mb1;
+        double cgb = c_dcg[cgoff + mb2 * (J1 + 1) + mb1];
+        if (J1 == J2 && mb1 != mb2) cgb += cgb;
+        // x = U^{J1}[:, mb1]; columns beyond the middle come from the stored half by
+        // u[ma][mb] = (-1)^(ma-mb) conj(u[J-ma][J-mb])
+        const bool fx = mb1 > J1 / 2;
+        const int cx = fx ? J1 - mb1 : mb1;
+        const unsigned char *xb = Ulane + (uhalf_off(J1) + cx * (J1 + 1) + (fx ? J1 : 0)) * kDiagRowBytes;
+        const int xstep = fx ? -kDiagRowBytes : kDiagRowBytes;
+        const unsigned mxr0 = (fx && (mb1 & 1)) ? 0x80000000u : 0u;
+        const unsigned mxr1 = (fx && !(mb1 & 1)) ? 0x80000000u : 0u;
+        const unsigned mxi0 = fx ? (mxr0 ^ 0x80000000u) : 0u;
+        const unsigned mxi1 = fx ? (mxr1 ^ 0x80000000u) : 0u;
+        double xr[J1 + 1], xi[J1 + 1];
+#pragma unroll
+        for (int k = 0; k <= J1; k++) {
+            const double2 v = *reinterpret_cast<const double2 *>(xb + k * xstep);
+            xr[k] = diag_flip(v.x, (k & 1) ? mxr1 : mxr0);
+            xi[k] = diag_flip(v.y, (k & 1) ? mxi1 : mxi0);
+        }
+        // y = U^{J2}[:, mb2], same symmetry, folded with cgb into scale factors by the parity of ma2
+        const bool fy = mb2 > J2 / 2;
+        const int cy = fy ? J2 - mb2 : mb2;
+        const int ystep = fy ? -kDiagRowBytes : kDiagRowBytes;
+        const unsigned char *yb = Ulane + (uoff2 + cy * (J2 + 1) + (fy ? J2 : 0)) * kDiagRowBytes;
+        const double p0 = (fy && (mb2 & 1)) ? -cgb : cgb;  // even ma2, real part
+        const double p1 = fy ? -p0 : cgb;                  // odd ma2, real part
+        const double q0 = fy ? -p0 : cgb;                  // imaginary parts: conjugation flips the sign again
+        const double q1 = fy ? -p1 : cgb;
+        // rows are numbered k = ma2 + off: re-base the row pointer, the CG offset and the parities to k
+        const unsigned char *yrow0 = yb - off * ystep;
+        const int cbase = cgoff - off * (J1 + 1);
+        const bool odd = off & 1;
+        const double se = odd ? p1 : p0, so = odd ? p0 : p1, te = odd ? q1 : q0, to = odd ? q0 : q1;
+        switch (off) {
+#define MALA_DIAG_ROW(K)                                                                                      \
+    case K:                                                                                                   \
+        if constexpr (K <= J1) diag_row<J1, (K <= J1 ? K : 0)>(rr, ri, xr, xi, yrow0, ystep, cbase, se, so, te, to); \
+        [[fallthrough]];
+            MALA_DIAG_ROW(0) MALA_DIAG_ROW(1) MALA_DIAG_ROW(2) MALA_DIAG_ROW(3) MALA_DIAG_ROW(4) MALA_DIAG_ROW(5)
+            MALA_DIAG_ROW(6) MALA_DIAG_ROW(7) MALA_DIAG_ROW(8) MALA_DIAG_ROW(9) MALA_DIAG_ROW(10)
+#undef MALA_DIAG_ROW
+            default: break;
+        }
+    }
+    // compute_bi: B += w * Re(conj(U^J[ma][mb]) * z[ma]), z[ma] = r[ma + sh + off].  Columns below the middle stand for
+    // their mirror images too (w = 2); in the middle column of an even J rows ma < J/2 stand for rows J - ma (w = 2),
+    // the centre counts once and rows above it are not used (w = 0).
+    const bool mid = ((J & 1) == 0) && (mb == J / 2);
+    const int d0 = sh + off;
+    const int mahi = mid ? J / 2 : J;
+    const unsigned char *ub = Ulane + (c_duoff[J] + mb * (J + 1)) * kDiagRowBytes;
+    double bp[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+    for (int d = 0; d < ND; d++) {
+        const int ma = d - d0;
+        if (ma >= 0 && ma <= mahi) {
+            const double2 u = *reinterpret_cast<const double2 *>(ub + ma * kDiagRowBytes);
+            const double w = (mid && ma == mahi) ? 1.0 : 2.0;
+            bp[(2 * d) & 3] = fma(u.x * w, rr[d], bp[(2 * d) & 3]);
+            bp[(2 * d + 1) & 3] = fma(u.y * w, ri[d], bp[(2 * d + 1) & 3]);
+        }
+    }
+    return (bp[0] + bp[1]) + (bp[2] + bp[3]);
+}
+
+// this warp's items [begin, end) of one triple (items numbered column by column)
+template <int J1>
+__device__ __noinline__ double diag_items(const unsigned char *Ulane, const int J2_, const int J_, const int cgoff_, const int begin_,
+                                          const int end_) {
+    // every argument but Ulane is warp-uniform; a broadcast from lane 0 tells the compiler so (uniform registers,
+    // uniform branches, CG values as uniform-register operands instead of per-thread constant loads)
+    const int J2 = __shfl_sync(0xffffffffu, J2_, 0), J = __shfl_sync(0xffffffffu, J_, 0);
+    const int cgoff = __shfl_sync(0xffffffffu, cgoff_, 0);
+    const int begin = __shfl_sync(0xffffffffu, begin_, 0), end = __shfl_sync(0xffffffffu, end_, 0);
+    const int sh = (J1 + J2 - J) / 2;
+    double b = 0.0;
+    int base = 0;
+#pragma unroll 1
+    for (int mb = 0; mb <= J / 2 && base < end; mb++) {
+        int lo, hi;
+        diag_item_range(J1, J2, J, mb, lo, hi);
+        const int nb = hi - lo + 1;
+        const int s = max(begin, base), e = min(end, base + nb);
+        if (s < e) b += diag_segment<J1>(Ulane, J2, J, sh, cgoff, mb, lo + s - base, lo + e - base);
+        base += nb;
+    }
+    return b;
+}
+
+__device__ __forceinline__ double diag_dispatch(const int J1, const unsigned char *Ulane, const int J2, const int J, const int cgoff,
+                                                const int begin, const int end) {
+    switch (J1) {
+        case 0: return diag_items<0>(Ulane, J2, J, cgoff, begin, end);
+        case 1: return diag_items<1>(Ulane, J2, J, cgoff, begin, end);
+        case 2: return diag_items<2>(Ulane, J2, J, cgoff, begin, end);
+        case 3: return diag_items<3>(Ulane, J2, J, cgoff, begin, end);
+        case 4: return diag_items<4>(Ulane, J2, J, cgoff, begin, end);
+        case 5: return diag_items<5>(Ulane, J2, J, cgoff, begin, end);
+        case 6: return diag_items<6>(Ulane, J2, J, cgoff, begin, end);
+        case 7: return diag_items<7>(Ulane, J2, J, cgoff, begin, end);
+        case 8: return diag_items<8>(Ulane, J2, J, cgoff, begin, end);
+        case 9: return diag_items<9>(Ulane, J2, J, cgoff, begin, end);
+        case 10: return diag_items<10>(Ulane, J2, J, cgoff, begin, end);
+        default: return 0.0;
+    }
+}
+
+__global__ void __launch_bounds__(kDiagWarps * 32, 1)
+compute_zi_bi_diag_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers cb, double *out) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int NW = kDiagWarps;
+    const int nelem = sc.nelem, nt = sc.ntriples;
+    double2 *U = reinterpret_cast<double2 *>(smem_raw);
+    double *Bs = reinterpret_cast<double *>(U + (size_t)nelem * 32);
+    double *red = Bs + 32 * nt;  // [2][kDiagGroup][NW][32]
+    __shared__ uint64_t bar;
+    __shared__ int s_slot;
+    const int lane = threadIdx.x & 31, warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
+    if (threadIdx.x == 0) mbar_init(&bar, 1);
+    uint32_t parity = 0;
+    for (;;) {
+        __syncthreads();  // previous tile written out: Bs, U and s_slot are free
+        if (threadIdx.x == 0) s_slot = atomicAdd(&cb.counters[2], 1);
+        __syncthreads();
+        const int slot = s_slot;
+        if (slot >= cb.counters[0]) break;
+        const int wt = cb.active[slot];
+        if (threadIdx.x == 0) tma_load_tile(U, cb.utot + (size_t)slot * nelem * 32, nelem, &bar);
+        mbar_wait(&bar, parity);
+        parity ^= 1u;
+        const unsigned char *Ulane = reinterpret_cast<const unsigned char *>(U + lane);
+        for (int pos = 0; pos < nt; pos++) {
+            const int begin = c_dsched[pos][warp][0], end = c_dsched[pos][warp][1];
+            double b = 0.0;
+            if (begin < end) {
+                const DiagTriple t = c_dtriple[pos];
+                b = diag_dispatch(t.J1, Ulane, t.J2, t.J, t.cgoff, begin, end);
+            }
+            const int buf = (pos / kDiagGroup) & 1, k = pos % kDiagGroup;
+            red[((buf * kDiagGroup + k) * NW + warp) * 32 + lane] = b;
+            if (k == kDiagGroup - 1 || pos == nt - 1) {
+                __syncthreads();
+                // fixed-order sum of the partials of the triples of this group
+                for (int kk = warp; kk <= k; kk += NW) {
+                    const double *r = red + ((buf * kDiagGroup + kk) * NW) * 32 + lane;
+                    double s = 0.0;
+#pragma unroll
+                    for (int w2 = 0; w2 < NW; w2++) s += r[w2 * 32];
+                    Bs[lane * nt + c_dtriple[pos - k + kk].index] = s;
+                }
+            }
+        }
+        __syncthreads();
+        write_tile(g, cb.tile_begin + wt, Bs, nt, out, NW);
+    }
+}
+
+inline size_t compute_zi_diag_smem_bytes(int nelem, int nt) {
+    return (size_t)nelem * 32 * sizeof(double2) + (size_t)32 * nt * sizeof(double) +
+           (size_t)2 * kDiagGroup * kDiagWarps * 32 * sizeof(double) + 16;
+}
+
+}  // namespace mala

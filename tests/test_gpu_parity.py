@@ -52,7 +52,7 @@ def tiny_ref():
     return w, oracle_grid(w)
 
 
-@pytest.mark.parametrize("zi_impl", [1, 2])
+@pytest.mark.parametrize("zi_impl", [1, 2, 3])
 def test_config1_tiny_al_full_grid(tiny_ref, zi_impl):
     w, ref = tiny_ref
     got = gpu_grid(w, zi_impl=zi_impl)
