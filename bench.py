@@ -280,7 +280,7 @@ def run_native(args, w, rank, world, local):
     zi_flop = nonempty * (F_Z + F_B)           # per step = summed over that step's launches
     achieved = zi_flop / (zi_ms * 1e-3) / 1e12
     peak_meas, mhz_eff = mala_snap_fp64_peak(stream)
-    roofline = {"bound": "alu", "kernel": "compute_zi_bi_spec_kernel", "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS,
+    roofline = {"bound": "alu", "kernel": "compute_zi_bi_coop_kernel", "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS,
                 "unit": "TFLOP/s", "frac": achieved / FP64_NOMINAL_TFLOPS,
                 "peak_source": "nominal FP64 FMA pipe: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md 'FP64 roofline')",
                 "peak_measured_dfma": peak_meas, "frac_of_measured_dfma": achieved / peak_meas if peak_meas > 0 else None,

@@ -191,7 +191,7 @@ const mala_snap *g_diag_owner = nullptr;
 
 int bind_diag_constants(mala_snap *h, cudaStream_t st) {
     if (g_diag_owner == h) return 0;
-    CUDA_TRY(cudaMemcpyToSymbolAsync(c_dcg, h->k_dcg.data(), h->k_dcg.size() * sizeof(double), 0, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyToSymbolAsync(c_dcg2, h->k_dcg.data(), h->k_dcg.size() * sizeof(double), 0, cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaMemcpyToSymbolAsync(c_dtriple, h->k_dtriple.data(), h->k_dtriple.size() * sizeof(DiagTriple), 0, cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaMemcpyToSymbolAsync(c_dsched, h->k_dsched.data(), h->k_dsched.size() * sizeof(unsigned short), 0, cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaMemcpyToSymbolAsync(c_duoff, h->k_duoff, sizeof(h->k_duoff), 0, cudaMemcpyHostToDevice, st));
@@ -199,22 +199,39 @@ int bind_diag_constants(mala_snap *h, cudaStream_t st) {
     return 0;
 }
 
-// processing order (J1 descending, then cost) and the per-warp item schedule of the diag kernel
+// processing order (J1 descending, then cost), padded CG blocks and the per-warp item schedule of the diag kernel
 void build_diag_schedule(mala_snap *h) {
     const SnapTables &T = h->tab;
     const int nt = T.ntriples;
-    h->k_dcg = T.cg;
-    h->k_dcg.resize(T.cg.size() + 16, 0.0);
     for (int J = 0; J <= kMaxTwoJ + 1; J++) h->k_duoff[J] = uhalf_off(J);
-    const double kItemOverhead = 10.0;
-    std::vector<double> tcost(nt, 0.0);
+    // CG blocks with an even row stride (16-byte rows: two coefficients per uniform load)
+    std::vector<int> cgoff(nt, 0);
+    h->k_dcg.clear();
+    for (int t = 0; t < nt; t++) {
+        const int J1 = T.triples[4 * t], J2 = T.triples[4 * t + 1], src = T.triples[4 * t + 3], S = diag_stride(J1);
+        cgoff[t] = (int)h->k_dcg.size();
+        for (int m2 = 0; m2 <= J2; m2++)
+            for (int m1 = 0; m1 < S; m1++) h->k_dcg.push_back(m1 <= J1 ? T.cg[src + m2 * (J1 + 1) + m1] : 0.0);
+    }
+    h->k_dcg.resize(h->k_dcg.size() + 16, 0.0);
+    // cost model in issue cycles (an FP64 instruction holds the issue port for two cycles, anything else for one):
+    // one row of an item = 6 (J1+1) FP64 + (J1+1) constant loads + ~4; an item adds its x loads and set-up; every
+    // column segment a warp starts pays for zeroing and folding the 2 J1 + 1 accumulators; every call ~120.
+    std::vector<double> tcost(nt, 0.0), segcost(nt, 0.0);
     std::vector<std::vector<double>> icost(nt);
+    std::vector<std::vector<int>> icol(nt);
+    const double kCallCost = 120.0;
     for (int t = 0; t < nt; t++) {
         const int J1 = T.triples[4 * t], J2 = T.triples[4 * t + 1], J = T.triples[4 * t + 2];
+        segcost[t] = 7.0 * (2 * J1 + 1) + 40.0;
         for (int mb = 0; mb <= J / 2; mb++) {
             int lo, hi;
             diag_item_range(J1, J2, J, mb, lo, hi);
-            for (int i = lo; i <= hi; i++) icost[t].push_back((double)(J1 + 1) * (J2 + 1) + kItemOverhead);
+            for (int i = lo; i <= hi; i++) {
+                icost[t].push_back((J2 + 1) * (13.0 * (J1 + 1) + 4.0) + 4.0 * (J1 + 1) + 60.0);
+                icol[t].push_back(mb);
+            }
+            if (hi >= lo) tcost[t] += segcost[t];
         }
         for (double c : icost[t]) tcost[t] += c;
     }
@@ -226,26 +243,38 @@ void build_diag_schedule(mala_snap *h) {
     });
     h->k_dtriple.assign(nt, DiagTriple{});
     h->k_dsched.assign((size_t)kDiagMaxNT * kDiagWarps * 2, 0);
-    std::vector<double> load(kDiagWarps, 0.0);
-    double total = 0.0;
+    int teams = kDiagTeams;
+    if (const char *e = std::getenv("MALA_SNAP_DIAG_TEAMS")) teams = std::atoi(e);
+    if (teams < 1 || kDiagWarps % teams != 0) teams = 1;
+    const int tw = kDiagWarps / teams;
+    std::vector<double> load(kDiagWarps, 0.0), team_load(teams, 0.0);
     for (int pos = 0; pos < nt; pos++) {
         const int t = order[pos];
         DiagTriple &d = h->k_dtriple[pos];
         d.J1 = (short)T.triples[4 * t]; d.J2 = (short)T.triples[4 * t + 1]; d.J = (short)T.triples[4 * t + 2];
-        d.index = (short)t; d.cgoff = T.triples[4 * t + 3]; d.pad = 0;
+        d.index = (short)t; d.cgoff = cgoff[t]; d.pad = 0;
         const std::vector<double> &cost = icost[t];
         const int n = (int)cost.size();
-        total += tcost[t];
-        const double target = total / kDiagWarps;
+        int team = 0;
+        for (int k = 1; k < teams; k++)
+            if (team_load[k] < team_load[team]) team = k;
+        team_load[team] += tcost[t];
+        double sum_load = tcost[t] + 0.5 * tw * kCallCost;
+        for (int k = 0; k < tw; k++) sum_load += load[team * tw + k];
+        const double target = sum_load / tw;
         int i = 0;
-        for (int w = 0; w < kDiagWarps; w++) {
+        for (int k = 0; k < tw; k++) {
+            const int w = team * tw + k;
             const int begin = i;
             double acc = 0.0;
-            if (w == kDiagWarps - 1) {
-                for (; i < n; i++) acc += cost[i];
-            } else {
-                const double want = target - load[w];
-                while (i < n && acc + 0.5 * cost[i] <= want) acc += cost[i++];
+            const bool last = (k == tw - 1);
+            const double want = target - load[w];
+            while (i < n) {
+                const bool newseg = (i == begin) || (icol[t][i] != icol[t][i - 1]);
+                const double c = cost[i] + (newseg ? segcost[t] : 0.0) + (i == begin ? kCallCost : 0.0);
+                if (!last && acc + 0.5 * c > want) break;
+                acc += c;
+                i++;
             }
             load[w] += acc;
             h->k_dsched[((size_t)pos * kDiagWarps + w) * 2] = (unsigned short)begin;

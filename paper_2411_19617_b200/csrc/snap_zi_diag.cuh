@@ -27,15 +27,26 @@ namespace mala {
 constexpr int kDiagWarps = MALA_DIAG_WARPS;  // warps per CTA
 constexpr int kDiagGroup = MALA_DIAG_GROUP;  // triples between two reductions of the partial sums
 constexpr int kDiagMaxNT = triple_count(kMaxTwoJ);
-constexpr int kDiagMaxCG = cg_block_off(kMaxTwoJ, kDiagMaxNT);
+constexpr int diag_stride(int J1) { return (J1 + 2) & ~1; }  // CG row stride: J1 + 1 rounded up to even (16-byte rows)
+constexpr int diag_cg_size(int twojmax) {
+    int n = 0;
+    for (int i = 0; i < triple_count(twojmax); i++) {
+        Triple t = triple_at(twojmax, i);
+        n += (t.j2 + 1) * diag_stride(t.j1);
+    }
+    return n;
+}
+constexpr int kDiagMaxCG = diag_cg_size(kMaxTwoJ);
+constexpr int kDiagTeams = 2;        // warp teams working on different triples at the same time
+constexpr int kDiagPadBytes = 5120;  // zeros in front of U in shared memory (see the fold in diag_segment)
 
 struct DiagTriple {  // one entry per position of the processing order
     short J1, J2, J, index;  // index = component number in output order
-    int cgoff;               // offset of the dense CG block [m2][m1] in c_dcg
+    int cgoff;               // offset (in doubles, even) of the dense CG block [m2][diag_stride(J1)] in c_dcg2
     int pad;
 };
 
-__constant__ double c_dcg[kDiagMaxCG + 16];                         // dense CG blocks (zero where m is out of range)
+__constant__ double2 c_dcg2[kDiagMaxCG / 2 + 8];                     // dense CG blocks, zero where m is out of range
 __constant__ DiagTriple c_dtriple[kDiagMaxNT];                       // processing order: J1 descending, then cost
 __constant__ unsigned short c_dsched[kDiagMaxNT][kDiagWarps][2];     // [position][warp] = item range [begin, end)
 __constant__ int c_duoff[kMaxTwoJ + 2];                              // half-column offset of every level
@@ -54,23 +65,32 @@ __device__ __forceinline__ double diag_flip(double v, unsigned mask) {
     return __hiloint2double(__double2hiint(v) ^ (int)mask, __double2loint(v));
 }
 
-// one row of the rectangle: r[ma1 + K] += CG[row][ma1] * x[ma1] * y,  y pre-scaled
+// one row of the rectangle: r[ma1 + K] += CG[row][ma1] * x[ma1] * y,  y pre-scaled.  yp walks down the y column.
 template <int J1, int K>
 __device__ __forceinline__ void diag_row(double (&rr)[2 * J1 + 1], double (&ri)[2 * J1 + 1], const double (&xr)[J1 + 1],
-                                         const double (&xi)[J1 + 1], const unsigned char *yrow0, const int ystep, const int cbase,
+                                         const double (&xi)[J1 + 1], const unsigned char *&yp, const int ystep, const int cbase2,
                                          const double se, const double so, const double te, const double to) {
-    const double2 yv = *reinterpret_cast<const double2 *>(yrow0 + K * ystep);
+    constexpr int S = diag_stride(J1);
+    const double2 yv = *reinterpret_cast<const double2 *>(yp);
+    yp += ystep;
     const double yr = yv.x * ((K & 1) ? so : se);
     const double yi = yv.y * ((K & 1) ? to : te);
 #pragma unroll
-    for (int ma1 = 0; ma1 <= J1; ma1++) {
-        const double cg = c_dcg[cbase + K * (J1 + 1) + ma1];
-        const double tr = cg * xr[ma1];
-        const double ti = cg * xi[ma1];
-        rr[ma1 + K] = fma(tr, yr, rr[ma1 + K]);
-        rr[ma1 + K] = fma(-ti, yi, rr[ma1 + K]);
-        ri[ma1 + K] = fma(tr, yi, ri[ma1 + K]);
-        ri[ma1 + K] = fma(ti, yr, ri[ma1 + K]);
+    for (int p = 0; p <= J1 / 2; p++) {
+        const double2 c2 = c_dcg2[cbase2 + (K * S) / 2 + p];  // 16-byte uniform load: CG of ma1 = 2p and 2p + 1
+#pragma unroll
+        for (int q = 0; q < 2; q++) {
+            const int ma1 = 2 * p + q;
+            if (ma1 <= J1) {
+                const double cg = q ? c2.y : c2.x;
+                const double tr = cg * xr[ma1];
+                const double ti = cg * xi[ma1];
+                rr[ma1 + K] = fma(tr, yr, rr[ma1 + K]);
+                rr[ma1 + K] = fma(-ti, yi, rr[ma1 + K]);
+                ri[ma1 + K] = fma(tr, yi, ri[ma1 + K]);
+                ri[ma1 + K] = fma(ti, yr, ri[ma1 + K]);
+            }
+        }
     }
 }
 
@@ -79,51 +99,56 @@ template <int J1>
 __device__ __forceinline__ double diag_segment(const unsigned char *Ulane, const int J2, const int J, const int sh, const int cgoff,
                                                const int mb, const int mb1_begin, const int mb1_end) {
     constexpr int ND = 2 * J1 + 1;
+    constexpr int S = diag_stride(J1);
     double rr[ND], ri[ND];
 #pragma unroll
     for (int d = 0; d < ND; d++) { rr[d] = 0.0; ri[d] = 0.0; }
     const int off = J1 - J2;  // first row of the unrolled body
     const int uoff2 = c_duoff[J2];
+    const int cbase2 = (cgoff - off * S) / 2;  // rows are numbered k = ma2 + off
+    const double *cgs = reinterpret_cast<const double *>(c_dcg2);
 #pragma unroll 1
     for (int mb1 = mb1_begin; mb1 < mb1_end; mb1++) {
         const int mb2 = mb + sh - mb1;
-        double cgb = c_dcg[cgoff + mb2 * (J1 + 1) + mb1];
+        double cgb = cgs[cgoff + mb2 * S + mb1];
         if (J1 == J2 && mb1 != mb2) cgb += cgb;
         // x = U^{J1}[:, mb1]; columns beyond the middle come from the stored half by
         // u[ma][mb] = (-1)^(ma-mb) conj(u[J-ma][J-mb])
-        const bool fx = mb1 > J1 / 2;
-        const int cx = fx ? J1 - mb1 : mb1;
-        const unsigned char *xb = Ulane + (uhalf_off(J1) + cx * (J1 + 1) + (fx ? J1 : 0)) * kDiagRowBytes;
-        const int xstep = fx ? -kDiagRowBytes : kDiagRowBytes;
-        const unsigned mxr0 = (fx && (mb1 & 1)) ? 0x80000000u : 0u;
-        const unsigned mxr1 = (fx && !(mb1 & 1)) ? 0x80000000u : 0u;
-        const unsigned mxi0 = fx ? (mxr0 ^ 0x80000000u) : 0u;
-        const unsigned mxi1 = fx ? (mxr1 ^ 0x80000000u) : 0u;
         double xr[J1 + 1], xi[J1 + 1];
+        if (mb1 <= J1 / 2) {
+            const unsigned char *xb = Ulane + (uhalf_off(J1) + mb1 * (J1 + 1)) * kDiagRowBytes;
 #pragma unroll
-        for (int k = 0; k <= J1; k++) {
-            const double2 v = *reinterpret_cast<const double2 *>(xb + k * xstep);
-            xr[k] = diag_flip(v.x, (k & 1) ? mxr1 : mxr0);
-            xi[k] = diag_flip(v.y, (k & 1) ? mxi1 : mxi0);
+            for (int k = 0; k <= J1; k++) {
+                const double2 v = *reinterpret_cast<const double2 *>(xb + k * kDiagRowBytes);
+                xr[k] = v.x;
+                xi[k] = v.y;
+            }
+        } else {
+            const unsigned char *xb = Ulane + (uhalf_off(J1) + (J1 - mb1) * (J1 + 1) + J1) * kDiagRowBytes;
+            const unsigned m0 = (mb1 & 1) ? 0x80000000u : 0u;  // sign of the real part on even rows
+#pragma unroll
+            for (int k = 0; k <= J1; k++) {
+                const double2 v = *reinterpret_cast<const double2 *>(xb - k * kDiagRowBytes);
+                xr[k] = diag_flip(v.x, (k & 1) ? (m0 ^ 0x80000000u) : m0);
+                xi[k] = diag_flip(v.y, (k & 1) ? m0 : (m0 ^ 0x80000000u));
+            }
         }
         // y = U^{J2}[:, mb2], same symmetry, folded with cgb into scale factors by the parity of ma2
         const bool fy = mb2 > J2 / 2;
         const int cy = fy ? J2 - mb2 : mb2;
-        const int ystep = fy ? -kDiagRowBytes : kDiagRowBytes;
-        const unsigned char *yb = Ulane + (uoff2 + cy * (J2 + 1) + (fy ? J2 : 0)) * kDiagRowBytes;
+        int ystep = fy ? -kDiagRowBytes : kDiagRowBytes;
+        const unsigned char *yp = Ulane + (uoff2 + cy * (J2 + 1) + (fy ? J2 : 0)) * kDiagRowBytes;
+        asm volatile("" : "+r"(ystep));  // keep the step in a register: one add per row, nothing recomputed
         const double p0 = (fy && (mb2 & 1)) ? -cgb : cgb;  // even ma2, real part
         const double p1 = fy ? -p0 : cgb;                  // odd ma2, real part
         const double q0 = fy ? -p0 : cgb;                  // imaginary parts: conjugation flips the sign again
         const double q1 = fy ? -p1 : cgb;
-        // rows are numbered k = ma2 + off: re-base the row pointer, the CG offset and the parities to k
-        const unsigned char *yrow0 = yb - off * ystep;
-        const int cbase = cgoff - off * (J1 + 1);
-        const bool odd = off & 1;
+        const bool odd = off & 1;  // parities re-based from ma2 to the row number k
         const double se = odd ? p1 : p0, so = odd ? p0 : p1, te = odd ? q1 : q0, to = odd ? q0 : q1;
         switch (off) {
-#define MALA_DIAG_ROW(K)                                                                                      \
-    case K:                                                                                                   \
-        if constexpr (K <= J1) diag_row<J1, (K <= J1 ? K : 0)>(rr, ri, xr, xi, yrow0, ystep, cbase, se, so, te, to); \
+#define MALA_DIAG_ROW(K)                                                                                       \
+    case K:                                                                                                    \
+        if constexpr (K <= J1) diag_row<J1, (K <= J1 ? K : 0)>(rr, ri, xr, xi, yp, ystep, cbase2, se, so, te, to); \
         [[fallthrough]];
             MALA_DIAG_ROW(0) MALA_DIAG_ROW(1) MALA_DIAG_ROW(2) MALA_DIAG_ROW(3) MALA_DIAG_ROW(4) MALA_DIAG_ROW(5)
             MALA_DIAG_ROW(6) MALA_DIAG_ROW(7) MALA_DIAG_ROW(8) MALA_DIAG_ROW(9) MALA_DIAG_ROW(10)
@@ -131,25 +156,33 @@ __device__ __forceinline__ double diag_segment(const unsigned char *Ulane, const
             default: break;
         }
     }
-    // compute_bi: B += w * Re(conj(U^J[ma][mb]) * z[ma]), z[ma] = r[ma + sh + off].  Columns below the middle stand for
-    // their mirror images too (w = 2); in the middle column of an even J rows ma < J/2 stand for rows J - ma (w = 2),
-    // the centre counts once and rows above it are not used (w = 0).
+    // compute_bi: B += w * Re(conj(U^J[ma][mb]) * z[ma]), z[ma] = r[ma + d0], d0 = sh + off.  Columns below the middle
+    // stand for their mirror images too (w = 2).  r[d] is exactly zero wherever ma = d - d0 falls outside [0, J] (those
+    // products used the zero entries of the CG table), so the fold runs over all d with plain loads: addresses outside
+    // the column read other finite shared-memory words (the zero pad in front of U, other elements of U, or Bs) and
+    // multiply them by zero.  In the middle column of an even J rows ma < J/2 stand for rows J - ma, the centre counts
+    // once and rows above it are dropped: r is masked first.
     const bool mid = ((J & 1) == 0) && (mb == J / 2);
     const int d0 = sh + off;
-    const int mahi = mid ? J / 2 : J;
-    const unsigned char *ub = Ulane + (c_duoff[J] + mb * (J + 1)) * kDiagRowBytes;
+    if (mid) {
+#pragma unroll
+        for (int d = 0; d < ND; d++) {
+            const int ma = d - d0;
+            const double w = (ma < J / 2) ? 1.0 : ((ma == J / 2) ? 0.5 : 0.0);
+            rr[d] *= w;
+            ri[d] *= w;
+        }
+    }
+    const unsigned char *ub = Ulane + (c_duoff[J] + mb * (J + 1) - d0) * kDiagRowBytes;
     double bp[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
     for (int d = 0; d < ND; d++) {
-        const int ma = d - d0;
-        if (ma >= 0 && ma <= mahi) {
-            const double2 u = *reinterpret_cast<const double2 *>(ub + ma * kDiagRowBytes);
-            const double w = (mid && ma == mahi) ? 1.0 : 2.0;
-            bp[(2 * d) & 3] = fma(u.x * w, rr[d], bp[(2 * d) & 3]);
-            bp[(2 * d + 1) & 3] = fma(u.y * w, ri[d], bp[(2 * d + 1) & 3]);
-        }
+        const double2 u = *reinterpret_cast<const double2 *>(ub + d * kDiagRowBytes);
+        bp[(2 * d) & 3] = fma(u.x, rr[d], bp[(2 * d) & 3]);
+        bp[(2 * d + 1) & 3] = fma(u.y, ri[d], bp[(2 * d + 1) & 3]);
     }
-    return (bp[0] + bp[1]) + (bp[2] + bp[3]);
+    const double b = (bp[0] + bp[1]) + (bp[2] + bp[3]);
+    return b + b;
 }
 
 // this warp's items [begin, end) of one triple (items numbered column by column)
@@ -199,13 +232,16 @@ compute_zi_bi_diag_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffer
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int NW = kDiagWarps;
     const int nelem = sc.nelem, nt = sc.ntriples;
-    double2 *U = reinterpret_cast<double2 *>(smem_raw);
+    double2 *U = reinterpret_cast<double2 *>(smem_raw + kDiagPadBytes);
     double *Bs = reinterpret_cast<double *>(U + (size_t)nelem * 32);
     double *red = Bs + 32 * nt;  // [2][kDiagGroup][NW][32]
     __shared__ uint64_t bar;
     __shared__ int s_slot;
     const int lane = threadIdx.x & 31, warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
     if (threadIdx.x == 0) mbar_init(&bar, 1);
+    // the fold of diag_segment may read (and multiply by zero) words of the pad and of Bs: make them finite
+    for (int i = threadIdx.x; i < kDiagPadBytes / 8; i += NW * 32) reinterpret_cast<double *>(smem_raw)[i] = 0.0;
+    for (int i = threadIdx.x; i < 32 * nt + 2 * kDiagGroup * NW * 32; i += NW * 32) Bs[i] = 0.0;  // Bs and red
     uint32_t parity = 0;
     for (;;) {
         __syncthreads();  // previous tile written out: Bs, U and s_slot are free
@@ -245,7 +281,7 @@ compute_zi_bi_diag_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffer
 }
 
 inline size_t compute_zi_diag_smem_bytes(int nelem, int nt) {
-    return (size_t)nelem * 32 * sizeof(double2) + (size_t)32 * nt * sizeof(double) +
+    return (size_t)kDiagPadBytes + (size_t)nelem * 32 * sizeof(double2) + (size_t)32 * nt * sizeof(double) +
            (size_t)2 * kDiagGroup * kDiagWarps * 32 * sizeof(double) + 16;
 }
 
