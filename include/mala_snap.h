@@ -107,7 +107,8 @@ int mala_bispectrum_grid_host(mala_snap_t *h, int natoms, const double *pos, con
  *   "timing"           1 = record a CUDA-event pair on the caller's stream around every kernel launch of the
  *                      following calls (read back with mala_snap_kernel_times); 0 = off (default)
  *   "workspace_mb"     cap, in MiB, of the U_tot + candidate workspace (default 4096)
- *   "host_chunk_mb"    size, in MiB, of each of the two staging buffers of mala_bispectrum_grid_host
+ *   "host_chunk_mb"    cap, in MiB, of each of the two staging buffers of mala_bispectrum_grid_host (default 256;
+ *                      outputs above 96 MiB are split into at least three chunks so the copies overlap the kernels)
  */
 int mala_snap_set_option(mala_snap_t *h, const char *name, long long value);
 

@@ -93,7 +93,7 @@ struct mala_snap {
     std::vector<unsigned short> k_dsched;
     int k_duoff[kMaxTwoJ + 2] = {0};
     long long workspace_mb = 4096;
-    long long host_chunk_mb = 512;
+    long long host_chunk_mb = 256;
     // device tables
     DevBuf<int> d_triples, d_udiag, d_order;
     DevBuf<double> d_cg, d_unorm, d_rcut, d_w, d_bconst;
@@ -744,11 +744,10 @@ int mala_snap_create(mala_snap_t **handle, int twojmax, double rcutfac, double r
             // streams in flight: measured on B200 (config 2) 1 team 30.8 ms, 2 teams 28.9 ms, 3 teams 35.7 ms,
             // 4 teams 52.9 ms -- the 32 KB instruction cache holds two loop bodies, not three.
             const double kItemOverhead = 8.0;
-            int teams = kCoopTeams;
-            if (const char *e = std::getenv("MALA_SNAP_COOP_TEAMS")) teams = std::atoi(e);
-            if (teams < 1 || kCoopWarps % teams != 0) teams = 1;
+            const int teams = kCoopTeams;  // compile-time: the kernel's reduction sums kTeamWarps partials
             const int tw = kCoopWarps / teams;  // warps per team
             std::vector<double> load(kCoopWarps, 0.0), team_load(teams, 0.0);
+            std::vector<int> pos_team(kSpecNT, 0);
             for (int pos = 0; pos < kSpecNT; pos++) {
                 const int t = h->tab.order[pos];
                 const int J1 = h->tab.triples[4 * t], J2 = h->tab.triples[4 * t + 1], J = h->tab.triples[4 * t + 2];
@@ -764,6 +763,7 @@ int mala_snap_create(mala_snap_t **handle, int twojmax, double rcutfac, double r
                 for (int k = 1; k < teams; k++)
                     if (team_load[k] < team_load[team]) team = k;
                 team_load[team] += sum;
+                pos_team[pos] = team;
                 const double target = team_load[team] / tw;
                 for (int w = 0; w < kCoopWarps; w++) sched[pos][w][0] = sched[pos][w][1] = 0;
                 int i = 0;
@@ -782,7 +782,28 @@ int mala_snap_create(mala_snap_t **handle, int twojmax, double rcutfac, double r
                     sched[pos][w][1] = (unsigned short)i;
                 }
             }
-            CUDA_TRY(cudaMemcpyToSymbol(c_sched, sched, sizeof(sched)));
+            // flatten into one work list per warp (snap_zi_coop.cuh, c_wlist)
+            static unsigned int wlist[kCoopWarps][kListMax];
+            int wn[kCoopWarps];
+            for (int w = 0; w < kCoopWarps; w++) wn[w] = 0;
+            for (int pos = 0; pos < kSpecNT; pos++) {
+                const int t = h->tab.order[pos];
+                const int k = pos % kCoopGroup, buf = (pos / kCoopGroup) & 1;
+                const int team = pos_team[pos];
+                for (int q = 0; q < tw; q++) {
+                    const int w = team * tw + q;
+                    wlist[w][wn[w]++] = ((unsigned)(buf * kCoopGroup + k) << 23) | ((unsigned)sched[pos][w][1] << 15) |
+                                        ((unsigned)sched[pos][w][0] << 7) | (unsigned)t;
+                }
+                if (k == kCoopGroup - 1 || pos == kSpecNT - 1)
+                    for (int w = 0; w < kCoopWarps; w++)
+                        wlist[w][wn[w]++] = 0x80000000u | ((unsigned)(pos - k) << 8) | ((unsigned)buf << 4) | (unsigned)k;
+            }
+            for (int w = 0; w < kCoopWarps; w++) {
+                if (wn[w] >= kListMax) return fail(MALA_SNAP_ECUDA, "internal: work list overflow");
+                for (int i = wn[w]; i < kListMax; i++) wlist[w][i] = 0xffffffffu;
+            }
+            CUDA_TRY(cudaMemcpyToSymbol(c_wlist, wlist, sizeof(wlist)));
         }
         build_diag_schedule(h);
         if ((rc = set_kernel_attributes(h))) return rc;
@@ -923,6 +944,10 @@ int mala_bispectrum_grid_host(mala_snap_t *h, int natoms, const double *pos, con
     const size_t plane = (size_t)ngrid[0] * ngrid[1] * h->sc.ntriples;  // doubles per z-plane
     const size_t budget = ((size_t)h->host_chunk_mb << 20) / sizeof(double);
     int planes = (int)std::max<size_t>(1, std::min<size_t>(budget / std::max<size_t>(plane, 1), (size_t)(z_end - z_begin)));
+    // at least three chunks once the output is large enough for the copy to matter: the device->host copy of a chunk
+    // overlaps the kernels of the next one, so only the last chunk's copy is exposed
+    const size_t total = plane * (size_t)(z_end - z_begin);
+    if (total * sizeof(double) > ((size_t)96 << 20)) planes = std::min(planes, (z_end - z_begin + 2) / 3);
     if (planes >= 8) planes = planes / 8 * 8;  // whole tiles for every tile shape
     for (int b = 0; b < 2; b++)
         if (h->d_stage[b].reserve(plane * planes)) return fail(MALA_SNAP_ENOMEM, "cudaMalloc (staging) failed");

@@ -41,7 +41,14 @@ constexpr int kCoopGroup = MALA_COOP_GROUP;   // triples between two reductions 
 
 __constant__ double c_cg_spec[kSpecCG];                        // dense CG blocks of every triple, [m2][m1]
 __constant__ int c_order_spec[kSpecNT];                        // triples by decreasing cost
-__constant__ unsigned short c_sched[kSpecNT][kCoopWarps][2];   // [position in c_order_spec][warp] = item range [begin, end)
+constexpr int kTeamWarps = kCoopWarps / kCoopTeams;           // warps per team
+constexpr int kListMax = kSpecNT + kSpecNT / kCoopGroup + 4;  // entries of one warp's work list
+// One work list per warp, built on the host (mala_snap.cu): the triples of the warp's team in processing order with the
+// warp's item range, interleaved with one entry per reduction group.
+//   work entry:  bit 31 = 0 | buf << 27 | k << 23 | end << 15 | begin << 7 | triple      (k = slot of the triple in its group)
+//   sync entry:  bit 31 = 1 | first position of the group << 8 | buf << 4 | last k
+//   0xffffffff terminates the list
+__constant__ unsigned int c_wlist[kCoopWarps][kListMax];
 
 constexpr int kRowBytes = 32 * (int)sizeof(double2);  // bytes between consecutive elements of one lane
 
@@ -223,13 +230,15 @@ __global__ void __launch_bounds__(kCoopWarps * 32, 1)
 compute_zi_bi_coop_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers cb, double *out) {
     static_assert(kSpecNT <= 100, "dispatch_triple covers 100 cases");
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    constexpr int nelem = uhalf_size(kSpecTJ), nt = kSpecNT, NW = kCoopWarps;
+    constexpr int nelem = uhalf_size(kSpecTJ), nt = kSpecNT, NW = kCoopWarps, TW = kTeamWarps;
     double2 *U = reinterpret_cast<double2 *>(smem_raw);
     double *Bs = reinterpret_cast<double *>(U + (size_t)nelem * 32);
-    double *red = Bs + 32 * nt;  // [2][kCoopGroup][NW][32]
+    double *red = Bs + 32 * nt;  // [2][kCoopGroup][TW][32]: partial sums of the warps of the triple's team
     __shared__ uint64_t bar;
     __shared__ int s_slot;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    const int wk = warp % TW;
     if (threadIdx.x == 0) mbar_init(&bar, 1);
     uint32_t parity = 0;
     for (;;) {
@@ -243,22 +252,24 @@ compute_zi_bi_coop_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffer
         mbar_wait(&bar, parity);
         parity ^= 1u;
         const unsigned char *Ulane = reinterpret_cast<const unsigned char *>(U + lane);
-        for (int pos = 0; pos < nt; pos++) {
-            const int t = c_order_spec[pos];
-            const int begin = c_sched[pos][warp][0], end = c_sched[pos][warp][1];
-            double b = 0.0;
-            if (begin < end) b = dispatch_triple(t, Ulane, begin, end);
-            const int buf = (pos / kCoopGroup) & 1, k = pos % kCoopGroup;
-            red[((buf * kCoopGroup + k) * NW + warp) * 32 + lane] = b;
-            if (k == kCoopGroup - 1 || pos == nt - 1) {
+        for (int i = 0;; i++) {
+            const unsigned e = c_wlist[warp][i];
+            if (e == 0xffffffffu) break;
+            if ((e >> 31) == 0u) {
+                const int t = (int)(e & 127u), begin = (int)((e >> 7) & 255u), end = (int)((e >> 15) & 255u);
+                double b = 0.0;
+                if (begin < end) b = dispatch_triple(t, Ulane, begin, end);
+                red[(((e >> 23) & 31u) * TW + wk) * 32 + lane] = b;  // (buf * kCoopGroup + k) in one field
+            } else {
                 __syncthreads();
                 // fixed-order sum of the partials of the triples of this group
-                for (int kk = warp; kk <= k; kk += NW) {
-                    const double *r = red + ((buf * kCoopGroup + kk) * NW) * 32 + lane;
+                const int klast = (int)(e & 15u), base = (int)((e >> 4) & 1u) * kCoopGroup, pos0 = (int)((e >> 8) & 255u);
+                for (int kk = warp; kk <= klast; kk += NW) {
+                    const double *r = red + ((base + kk) * TW) * 32 + lane;
                     double s = 0.0;
 #pragma unroll
-                    for (int w2 = 0; w2 < NW; w2++) s += r[w2 * 32];
-                    Bs[lane * nt + c_order_spec[pos - k + kk]] = s;
+                    for (int w2 = 0; w2 < TW; w2++) s += r[w2 * 32];
+                    Bs[lane * nt + c_order_spec[pos0 + kk]] = s;
                 }
             }
         }
@@ -269,7 +280,7 @@ compute_zi_bi_coop_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffer
 
 inline size_t compute_zi_coop_smem_bytes() {
     return (size_t)uhalf_size(kSpecTJ) * 32 * sizeof(double2) + (size_t)32 * kSpecNT * sizeof(double) +
-           (size_t)2 * kCoopGroup * kCoopWarps * 32 * sizeof(double) + 16;
+           (size_t)2 * kCoopGroup * kTeamWarps * 32 * sizeof(double) + 16;
 }
 
 }  // namespace mala
