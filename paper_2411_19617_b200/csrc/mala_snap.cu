@@ -620,12 +620,13 @@ int run_slab(mala_snap *h, int z0, int z1, double *out, double2 *u_out, cudaStre
         }
         CUDA_TRY(cudaGetLastError());
         const int grid = std::max(1, std::min(h->num_sms, cb.ntiles));
+        const int ui_grid = std::max(1, std::min(2 * h->num_sms, 2 * cb.ntiles));  // half-tile items, two CTAs per SM
         {
             TimedSpan span(h, st, kKindUi);
             if (h->twojmax == kMaxTwoJ)
-                compute_ui_kernel<kMaxTwoJ, true><<<grid, (kMaxTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kMaxTwoJ), st>>>(g, h->sc, tb, cb);
+                compute_ui_kernel<kMaxTwoJ, true><<<ui_grid, (kMaxTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kMaxTwoJ), st>>>(g, h->sc, tb, cb);
             else  // smaller twojmax: same code with run-time guards on the levels
-                compute_ui_kernel<kMaxTwoJ, false><<<grid, (kMaxTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kMaxTwoJ), st>>>(g, h->sc, tb, cb);
+                compute_ui_kernel<kMaxTwoJ, false><<<ui_grid, (kMaxTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kMaxTwoJ), st>>>(g, h->sc, tb, cb);
         }
         CUDA_TRY(cudaGetLastError());
         h->stats[0] += 2;

@@ -16,7 +16,8 @@
 
 namespace mala {
 
-constexpr int kGeoCap = 48;     // neighbor entries per lane buffered between two accumulate passes
+constexpr int kGeoCap = 48;     // neighbor entries per grid point buffered between two accumulate passes
+constexpr int kUiPoints = 16;   // grid points per compute_ui CTA: half a tile; lane = (point, half), the halves split the neighbors
 constexpr int kCandBatch = 32;  // candidate atoms staged per batch
 
 __device__ __forceinline__ void lane_point(const GridGeom &g, int tile, int lane, int &ix, int &iy, int &iz, bool &valid) {
@@ -125,17 +126,25 @@ __global__ void __launch_bounds__(256) tile_bin_kernel(GridGeom g, SnapConst sc,
 // M is a run-time argument on purpose: all column-warps then run the SAME instructions, so the SM fetches one
 // instruction stream instead of one per column (the per-column template instances stalled on instruction fetch).
 template <int TJMAX, bool EXACT>
-__device__ __noinline__ void ui_column_pair(double2 *__restrict__ Ul, const int tj, const int M,
+__device__ __noinline__ void ui_column_pair(double2 *Ul, const int tj, const int M, const bool upper,
                                                const double c0, const double a0r, const double a0i, const double b0r, const double b0i,
                                                const double c1, const double a1r, const double a1i, const double b1r, const double b1i) {
     double pr[2][TJMAX + 1], pi[2][TJMAX + 1];
     const double ar[2] = {a0r, a1r}, ai[2] = {a0i, a1i}, br[2] = {b0r, b1r}, bi[2] = {b0i, b1i};
     pr[0][0] = c0; pi[0][0] = 0.0;
     pr[1][0] = c1; pi[1][0] = 0.0;
+    // The two half-warps hold different neighbors of the same 16 points: they add into shared memory one after the
+    // other (lower half first), so the summation order is fixed and the result bit-reproducible.
     if (M == 0) {
+        const double s = c0 + c1;
         double2 v = Ul[0];
-        v.x += c0 + c1;
-        Ul[0] = v;
+        v.x += s;
+        if (!upper) Ul[0] = v;
+        __syncwarp();
+        v = Ul[0];
+        v.x += s;
+        if (upper) Ul[0] = v;
+        __syncwarp();
     }
 #pragma unroll
     for (int r = 1; r <= TJMAX; r++) {
@@ -169,14 +178,23 @@ __device__ __noinline__ void ui_column_pair(double2 *__restrict__ Ul, const int 
                 pi[n][0] = t0i;
             }
             if (r >= 2 * M) {
-                double2 *Ue = Ul + (size_t)(uhalf_off(r) + M * (r + 1)) * 32;
+                double2 *Ue = Ul + (size_t)(uhalf_off(r) + M * (r + 1)) * kUiPoints;
 #pragma unroll
                 for (int k = 0; k <= r; k++) {
-                    double2 v = Ue[k * 32];
+                    double2 v = Ue[k * kUiPoints];
                     v.x += pr[0][k] + pr[1][k];
                     v.y += pi[0][k] + pi[1][k];
-                    Ue[k * 32] = v;
+                    if (!upper) Ue[k * kUiPoints] = v;
                 }
+                __syncwarp();
+#pragma unroll
+                for (int k = 0; k <= r; k++) {
+                    double2 v = Ue[k * kUiPoints];
+                    v.x += pr[0][k] + pr[1][k];
+                    v.y += pi[0][k] + pi[1][k];
+                    if (upper) Ue[k * kUiPoints] = v;
+                }
+                __syncwarp();
             }
         }
     }
@@ -204,57 +222,66 @@ __device__ __forceinline__ void pair_geometry(const double dx, const double dy, 
     bi = -sr * dx;
 }
 
+// Work item = half a tile (16 grid points).  Lane = (point p = lane & 15, half h = lane >> 4): both halves see the same
+// points and split each point's neighbors (entries of even / odd index), so a CTA needs shared-memory accumulators for
+// 16 points only (69 KB) and two CTAs share an SM -- twice the warps to hide the FP64 latency with.
 template <int TJMAX, bool EXACT>
-__global__ void __launch_bounds__((TJMAX / 2 + 1) * 32, 1)
+__global__ void __launch_bounds__((TJMAX / 2 + 1) * 32, 2)
 compute_ui_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers cb) {
     constexpr int NW = TJMAX / 2 + 1;
+    constexpr int NP = kUiPoints;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int nelem = sc.nelem;
-    double2 *uacc = reinterpret_cast<double2 *>(smem_raw);
-    double *geo = reinterpret_cast<double *>(uacc + (size_t)uhalf_size(TJMAX) * 32);
-    double *crec = geo + kGeoCap * 5 * 32;
-    __shared__ int s_slot;
+    double2 *uacc = reinterpret_cast<double2 *>(smem_raw);                       // [nelem][NP]
+    double *geo = reinterpret_cast<double *>(uacc + (size_t)uhalf_size(TJMAX) * NP);  // [kGeoCap][5][NP]
+    double *crec = geo + kGeoCap * 5 * NP;
+    __shared__ int s_item;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int p = lane & (NP - 1);
+    const bool upper = lane >= NP;
     const int tj = sc.twojmax;
 
     for (;;) {
-        __syncthreads();  // everybody is done with the previous tile (uacc reads, s_slot)
-        if (threadIdx.x == 0) s_slot = atomicAdd(&cb.counters[1], 1);
+        __syncthreads();  // everybody is done with the previous item (uacc reads, s_item)
+        if (threadIdx.x == 0) s_item = atomicAdd(&cb.counters[1], 1);
         __syncthreads();
-        const int slot = s_slot;
+        const int item = s_item;
+        const int slot = item >> 1, hh = item & 1;
         if (slot >= cb.counters[0]) break;
         const int wt = cb.active[slot];
         const int tile = cb.tile_begin + wt;
         int ix, iy, iz;
         bool valid;
-        lane_point(g, tile, lane, ix, iy, iz, valid);
+        lane_point(g, tile, hh * NP + p, ix, iy, iz, valid);
         // ragged tiles: clamp onto a valid point (its result is never written)
         ix = min(ix, g.nx - 1); iy = min(iy, g.ny - 1); iz = min(iz, g.z1 - 1);
         double px, py, pz;
         point_position(g, ix, iy, iz, px, py, pz);
 
-        for (int e = threadIdx.x; e < nelem * 32; e += NW * 32) uacc[e] = make_double2(0.0, 0.0);
+        for (int e = threadIdx.x; e < nelem * NP; e += NW * 32) uacc[e] = make_double2(0.0, 0.0);
 
+        // this lane takes the entries of its point with index = half (mod 2), two at a time
         auto accumulate = [&](const int cnt) {
             if (warp > tj / 2) return;
             const int nmax = __reduce_max_sync(0xffffffffu, cnt);
-            double2 *Ul = uacc + lane;
-            for (int i = 0; i < nmax; i += 2) {
+            double2 *Ul = uacc + p;
+            for (int i0 = 0; i0 < nmax; i0 += 4) {  // uniform trip count: ui_column_pair synchronises the warp
+                const int i = i0 + (upper ? 1 : 0);
                 double c0 = 0.0, a0r = 1.0, a0i = 0.0, b0r = 0.0, b0i = 0.0;
                 double c1 = 0.0, a1r = 1.0, a1i = 0.0, b1r = 0.0, b1i = 0.0;
                 if (i < cnt) {
-                    const double *q = geo + (size_t)i * 5 * 32 + lane;
-                    c0 = q[0]; a0r = q[32]; a0i = q[64]; b0r = q[96]; b0i = q[128];
+                    const double *q = geo + (size_t)i * 5 * NP + p;
+                    c0 = q[0]; a0r = q[NP]; a0i = q[2 * NP]; b0r = q[3 * NP]; b0i = q[4 * NP];
                 }
-                if (i + 1 < cnt) {
-                    const double *q = geo + (size_t)(i + 1) * 5 * 32 + lane;
-                    c1 = q[0]; a1r = q[32]; a1i = q[64]; b1r = q[96]; b1i = q[128];
+                if (i + 2 < cnt) {
+                    const double *q = geo + (size_t)(i + 2) * 5 * NP + p;
+                    c1 = q[0]; a1r = q[NP]; a1i = q[2 * NP]; b1r = q[3 * NP]; b1i = q[4 * NP];
                 }
-                ui_column_pair<TJMAX, EXACT>(Ul, tj, warp, c0, a0r, a0i, b0r, b0i, c1, a1r, a1i, b1r, b1i);
+                ui_column_pair<TJMAX, EXACT>(Ul, tj, warp, upper, c0, a0r, a0i, b0r, b0i, c1, a1r, a1i, b1r, b1i);
             }
         };
 
-        int cnt = 0;       // buffered neighbor entries of this lane (identical in every warp)
+        int cnt = 0;       // buffered neighbor entries of this lane's point (identical in both halves and every warp)
         int appended = 0;  // candidates staged since the last accumulate pass (uniform over the CTA)
         const int nc = cb.ncand[wt];
         const int *mycand = cb.cand + (size_t)wt * cb.cand_cap;
@@ -279,11 +306,12 @@ compute_ui_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers cb) {
                 const double dx = q[0] - px, dy = q[1] - py, dz = q[2] - pz;
                 const double r2 = dx * dx + dy * dy + dz * dz;
                 if (r2 < q[5]) {
-                    if ((k % NW) == warp) {
+                    // the geometry of entry cnt is computed once: by warp k mod NW, in the half that will use it
+                    if ((k % NW) == warp && ((cnt & 1) != 0) == upper) {
                         double c, ar, ai, br, bi;
                         pair_geometry(dx, dy, dz, r2, q[3], q[4], sc.rfac0, sc.rmin0, c, ar, ai, br, bi);
-                        double *o = geo + (size_t)cnt * 5 * 32 + lane;
-                        o[0] = c; o[32] = ar; o[64] = ai; o[96] = br; o[128] = bi;
+                        double *o = geo + (size_t)cnt * 5 * NP + p;
+                        o[0] = c; o[NP] = ar; o[2 * NP] = ai; o[3 * NP] = br; o[4 * NP] = bi;
                     }
                     cnt++;
                 }
@@ -293,20 +321,21 @@ compute_ui_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers cb) {
         __syncthreads();
         accumulate(cnt);
         __syncthreads();
-        // binomial normalisation, self term (delta(0) of Eq. (24)), coalesced store of the tile
-        double2 *dst = cb.utot + (size_t)slot * nelem * 32;
-        for (int e = warp; e < nelem; e += NW) {
-            double2 v = uacc[e * 32 + lane];
-            const double s = tb.unorm[e];
-            v.x = v.x * s + (tb.udiag[e] ? sc.wself : 0.0);
-            v.y = v.y * s;
-            dst[e * 32 + lane] = v;
+        // binomial normalisation, self term (delta(0) of Eq. (24)), store of the half tile: lanes hh*16 .. hh*16+15 of
+        // every element; each half-warp takes an element of its own
+        double2 *dst = cb.utot + (size_t)slot * nelem * 32 + hh * NP;
+        for (int e = warp * 2 + (upper ? 1 : 0); e < nelem; e += NW * 2) {
+            double2 v = uacc[e * NP + p];
+            const double sN = tb.unorm[e];
+            v.x = v.x * sN + (tb.udiag[e] ? sc.wself : 0.0);
+            v.y = v.y * sN;
+            dst[e * 32 + p] = v;
         }
     }
 }
 
 inline size_t compute_ui_smem_bytes(int tjmax) {
-    return (size_t)uhalf_size(tjmax) * 32 * sizeof(double2) + (size_t)kGeoCap * 5 * 32 * sizeof(double) +
+    return (size_t)uhalf_size(tjmax) * kUiPoints * sizeof(double2) + (size_t)kGeoCap * 5 * kUiPoints * sizeof(double) +
            (size_t)kCandBatch * 6 * sizeof(double);
 }
 
