@@ -56,14 +56,23 @@ constexpr int kRowBytes = 32 * (int)sizeof(double2);  // bytes between consecuti
 // J1 == J2: the items (mb1, mb2) and (mb2, mb1) contribute the same Z column (swap the two factors and use
 // CG(j1 m1 j1 m2 | j m) = +-CG(j1 m2 j1 m1 | j m) for both coefficients), so only mb1 <= mb2 is computed, with weight 2
 // when mb1 < mb2.
+// J == J1 (and J1 != J2): U^{J1} and U^J are the same matrix, and the contribution of item (mb, mb1) to B equals that
+// of item (mb1, mb) (swap the roles of the two factors; the third one turns into its mirror element, whose sign and
+// conjugation cancel against the CG symmetry).  Together with the column flip (mb, mb1) -> (J - mb, J - mb1) already
+// used, the items mb <= mb1 <= J - mb of the columns mb <= J/2 represent all of them: weight 2 unless mb1 == mb or
+// mb1 == J - mb.  Checked against the oracle's U and CG to 1e-15 before use.
+constexpr bool item_hermitian(int J1, int J2, int J) { return J == J1 && J1 != J2; }
 constexpr int item_lo(int J1, int J2, int J, int mb) {
     const int s = mb + (J1 + J2 - J) / 2;
-    return (s - J2) > 0 ? (s - J2) : 0;
+    int lo = (s - J2) > 0 ? (s - J2) : 0;
+    if (item_hermitian(J1, J2, J) && lo < mb) lo = mb;
+    return lo;
 }
 constexpr int item_hi(int J1, int J2, int J, int mb) {
     const int s = mb + (J1 + J2 - J) / 2;
     int hi = s < J1 ? s : J1;
     if (J1 == J2 && s / 2 < hi) hi = s / 2;
+    if (item_hermitian(J1, J2, J) && J - mb < hi) hi = J - mb;
     return hi;
 }
 // the middle column of an even J needs rows ma <= J/2 only (the others are its mirror images)
@@ -134,6 +143,7 @@ __device__ __forceinline__ double column_segment(const unsigned char *Ulane, con
         const int mb2 = mb + SH - mb1;
         double cgb = c_cg_spec[CGOFF + mb2 * (J1 + 1) + mb1];
         if (J1 == J2 && mb1 != mb2) cgb += cgb;  // stands for its mirror item (mb2, mb1) too
+        if (item_hermitian(J1, J2, J) && mb1 != mb && mb1 != J - mb) cgb += cgb;  // and for item (mb1, mb)
         // x = U^{J1}[:, mb1]; columns beyond the middle come from the stored half by
         // u[ma][mb] = (-1)^(ma-mb) conj(u[J-ma][J-mb])
         const bool fx = mb1 > J1 / 2;

@@ -59,6 +59,10 @@ __host__ __device__ inline void diag_item_range(int J1, int J2, int J, int mb, i
     lo = (s - J2) > 0 ? (s - J2) : 0;
     hi = s < J1 ? s : J1;
     if (J1 == J2 && s / 2 < hi) hi = s / 2;  // mirror items (mb2, mb1) are folded into weight 2
+    if (J == J1 && J1 != J2) {               // item (mb, mb1) == item (mb1, mb): see item_hermitian in snap_zi_coop.cuh
+        if (lo < mb) lo = mb;
+        if (J - mb < hi) hi = J - mb;
+    }
 }
 
 __device__ __forceinline__ double diag_flip(double v, unsigned mask) {
@@ -112,6 +116,7 @@ __device__ __forceinline__ double diag_segment(const unsigned char *Ulane, const
         const int mb2 = mb + sh - mb1;
         double cgb = cgs[cgoff + mb2 * S + mb1];
         if (J1 == J2 && mb1 != mb2) cgb += cgb;
+        if (J == J1 && J1 != J2 && mb1 != mb && mb1 != J - mb) cgb += cgb;
         // x = U^{J1}[:, mb1]; columns beyond the middle come from the stored half by
         // u[ma][mb] = (-1)^(ma-mb) conj(u[J-ma][J-mb])
         double xr[J1 + 1], xi[J1 + 1];
