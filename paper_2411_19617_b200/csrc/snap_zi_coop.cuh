@@ -86,7 +86,7 @@ constexpr int triple_items(int J1, int J2, int J) {
 }
 // product terms of one item of column mb (the cost unit of the schedule)
 constexpr int item_terms(int J1, int J2, int J, int mb) {
-    const int sh = (J1 + J2 - J) / 2, mahi = is_mid(J, mb) ? J / 2 : J;
+    const int sh = (J1 + J2 - J) / 2, mahi = (is_mid(J, mb) && !item_hermitian(J1, J2, J)) ? J / 2 : J;
     int n = 0;
     for (int m2 = 0; m2 <= J2; m2++)
         for (int m1 = 0; m1 <= J1; m1++)
@@ -212,7 +212,13 @@ __device__ __noinline__ double triple_items_b(const unsigned char *Ulane, const 
     if (J % 2 == 0) {
         constexpr int lo = item_lo(J1, J2, J, J / 2), nb = item_hi(J1, J2, J, J / 2) - lo + 1;
         const int s = max(begin, base), e = min(end, base + nb);
-        if (s < e) b += column_segment<J1, J2, J, CGOFF, true>(Ulane, J / 2, lo + s - base, lo + e - base);
+        // the half-row body pays for its code only when the middle column has several items; with the j == j1 symmetry
+        // it has a single one, which then runs through the full-column body (weight 2 there, hence the 0.5)
+        if constexpr (item_hermitian(J1, J2, J)) {
+            if (s < e) b += 0.5 * column_segment<J1, J2, J, CGOFF, false>(Ulane, J / 2, lo + s - base, lo + e - base);
+        } else {
+            if (s < e) b += column_segment<J1, J2, J, CGOFF, true>(Ulane, J / 2, lo + s - base, lo + e - base);
+        }
     }
     return b;
 }
