@@ -77,6 +77,14 @@ constexpr int item_hi(int J1, int J2, int J, int mb) {
 }
 // the middle column of an even J needs rows ma <= J/2 only (the others are its mirror images)
 constexpr bool is_mid(int J, int mb) { return (J % 2 == 0) && (mb == J / 2); }
+// The half-row body of the middle column is extra code to fetch for every tile: it pays only when the middle column has
+// enough items (MALA_COOP_MID_MIN, tuned on B200); otherwise the column runs through the full-column body at half weight.
+#ifndef MALA_COOP_MID_MIN
+#define MALA_COOP_MID_MIN 2
+#endif
+constexpr bool use_mid_body(int J1, int J2, int J) {
+    return (J % 2 == 0) && (item_hi(J1, J2, J, J / 2) - item_lo(J1, J2, J, J / 2) + 1 >= MALA_COOP_MID_MIN);
+}
 
 // number of (mb, mb1) items of a triple: columns mb = 0..J/2
 constexpr int triple_items(int J1, int J2, int J) {
@@ -86,7 +94,7 @@ constexpr int triple_items(int J1, int J2, int J) {
 }
 // product terms of one item of column mb (the cost unit of the schedule)
 constexpr int item_terms(int J1, int J2, int J, int mb) {
-    const int sh = (J1 + J2 - J) / 2, mahi = (is_mid(J, mb) && !item_hermitian(J1, J2, J)) ? J / 2 : J;
+    const int sh = (J1 + J2 - J) / 2, mahi = (is_mid(J, mb) && use_mid_body(J1, J2, J)) ? J / 2 : J;
     int n = 0;
     for (int m2 = 0; m2 <= J2; m2++)
         for (int m1 = 0; m1 <= J1; m1++)
@@ -214,7 +222,7 @@ __device__ __noinline__ double triple_items_b(const unsigned char *Ulane, const 
         const int s = max(begin, base), e = min(end, base + nb);
         // the half-row body pays for its code only when the middle column has several items; with the j == j1 symmetry
         // it has a single one, which then runs through the full-column body (weight 2 there, hence the 0.5)
-        if constexpr (item_hermitian(J1, J2, J)) {
+        if constexpr (!use_mid_body(J1, J2, J)) {
             if (s < e) b += 0.5 * column_segment<J1, J2, J, CGOFF, false>(Ulane, J / 2, lo + s - base, lo + e - base);
         } else {
             if (s < e) b += column_segment<J1, J2, J, CGOFF, true>(Ulane, J / 2, lo + s - base, lo + e - base);
