@@ -98,6 +98,20 @@ int mala_bispectrum_grid_host(mala_snap_t *h, int natoms, const double *pos, con
                               int z_begin, int z_end, double *out_host, void *cuda_stream);
 
 /*
+ * Gaussian descriptors on the same grid ("a sum of Gaussians centered at R", the Gaussian representation of
+ * the ionic configuration behind Eqs. (40)-(43)).  One channel per atom type t:
+ *     G_t(r) = wj[t] * (2 pi sigma^2)^(-3/2) * sum exp(-|R - r|^2 / (2 sigma^2))
+ * over the atoms of type t and their periodic images with |R - r| < rcut_t (the handle's cutoffs; strict).  The paper
+ * fixes neither the normalisation nor the truncation: this is DESIGN.md reading G1.  twojmax of the handle is not used.
+ *   sigma    > 0, the Gaussian width w_G of PAPER.md:416, in the length unit of pos
+ *   out      DEVICE [(z_end-z_begin)*ny*nx][ntypes] fp64, ix fastest; all other arguments as mala_bispectrum_grid
+ * At most 4 atom types (MALA_SNAP_EINVAL otherwise).  Work is enqueued on cuda_stream; the call does not synchronise.
+ */
+int mala_gaussian_grid(mala_snap_t *h, double sigma, int natoms, const double *pos, const int *types, const double box[9],
+                       const double origin[3], const int pbc[3], const int ngrid[3], int z_begin, int z_end, double *out,
+                       void *cuda_stream);
+
+/*
  * Tuning / test knobs.  Unknown names give MALA_SNAP_EINVAL.
  *   "zi_impl"          0 = automatic (per-triple specialised kernel when twojmax == 10, anti-diagonal kernel
  *                      otherwise), 1 = generic table-driven kernel, 2 = per-triple specialised kernel (EINVAL if

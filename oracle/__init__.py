@@ -158,6 +158,40 @@ def bispectrum_grid(pos, types, box, origin, pbc, ngrid, z_begin=0, z_end=None, 
     return out
 
 
+def gaussian_points(points, pos, types, box, origin=(0, 0, 0), pbc=(1, 1, 1), *, sigma, rcutfac=4.67637, radelem=(0.5,),
+                    wj=(1.0,)):
+    """Gaussian descriptors [np, ntypes] at explicit Cartesian points (snap_oracle.c for the reading)."""
+    points = _d(points).reshape(-1, 3)
+    radelem = _d(radelem).ravel()
+    wj = _d(wj).ravel()
+    pos = _d(pos).reshape(-1, 3)
+    types = _i(types).ravel()
+    box = _d(box).reshape(3, 3)
+    origin = _d(origin).ravel()
+    pbc = _i(pbc).ravel()
+    out = np.zeros((points.shape[0], radelem.shape[0]))
+    rc = lib().oracle_gaussian_points(C.c_double(rcutfac), C.c_double(sigma), C.c_int(radelem.shape[0]), _p(radelem, C.c_double),
+                                      _p(wj, C.c_double), C.c_int(pos.shape[0]), _p(pos, C.c_double), _p(types, C.c_int),
+                                      _p(box, C.c_double), _p(origin, C.c_double), _p(pbc, C.c_int),
+                                      C.c_int(points.shape[0]), _p(points, C.c_double), _p(out, C.c_double))
+    if rc != 0:
+        raise ValueError("oracle_gaussian_points: invalid argument")
+    return out
+
+
+def grid_points(box, origin, ngrid, z_begin=0, z_end=None, sample=None):
+    """Cartesian positions of the grid points of a slab in output order (ix fastest), or of flat indices `sample`."""
+    box = _d(box).reshape(3, 3)
+    nx, ny, nz = (int(v) for v in ngrid)
+    if sample is None:
+        z_end = nz if z_end is None else z_end
+        idx = np.arange(z_begin * ny * nx, z_end * ny * nx)
+    else:
+        idx = np.asarray(sample, dtype=np.int64)
+    ix, iy, iz = idx % nx, (idx // nx) % ny, idx // (nx * ny)
+    return (_d(origin)[None, :] + (ix / nx)[:, None] * box[0] + (iy / ny)[:, None] * box[1] + (iz / nz)[:, None] * box[2])
+
+
 def num_threads():
     return lib().oracle_num_threads()
 

@@ -491,6 +491,53 @@ int oracle_bispectrum_grid(int twojmax, double rcutfac, double rfac0, double rmi
     return rc;
 }
 
+/* ------------------------------------------------------------------ */
+/* Gaussian descriptors ("a sum of  */
+/* Gaussians centered at R", Eqs. (40)-(43) PAPER.md:396-412).          */
+/* Reading: per atom type t one channel,         */
+/*   G_t(r) = w_t (2 pi sigma^2)^(-3/2) sum exp(-|R - r|^2 / (2 sigma^2)) */
+/* over the atoms of type t and their periodic images with              */
+/* |R - r| < rcut_t (strict), i.e. unit-integral Gaussians of width     */
+/* sigma = w_G truncated at the descriptor cutoff.  Plain definition:   */
+/* all atoms x all images.                                              */
+/* ------------------------------------------------------------------ */
+int oracle_gaussian_points(double rcutfac, double sigma, int ntypes, const double *radelem, const double *wj, int natoms,
+                           const double *pos, const int *types, const double *box, const double *origin, const int *pbc,
+                           int npoints, const double *points, double *out /* [npoints*ntypes] */)
+{
+    if (!(sigma > 0.0) || ntypes < 1 || natoms < 0 || npoints < 0) return -1;
+    sys_t s;
+    memset(&s, 0, sizeof(s));
+    s.rcutfac = rcutfac; s.ntypes = ntypes; s.radelem = radelem; s.wj = wj;
+    s.natoms = natoms; s.pos = pos; s.types = types; s.box = box; s.origin = origin; s.pbc = pbc;
+    if (sys_prepare(&s)) return -1;
+    const double pi = 3.14159265358979323846;
+    const double pref = 1.0 / (pow(2.0 * pi, 1.5) * sigma * sigma * sigma);
+    const double *a1 = box, *a2 = box + 3, *a3 = box + 6;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int p = 0; p < npoints; p++) {
+        const double *rp = points + 3 * p;
+        double *g = out + (size_t)p * ntypes;
+        for (int t = 0; t < ntypes; t++) g[t] = 0.0;
+        for (int n = 0; n < natoms; n++) {
+            int t = types[n];
+            double rcut = 2.0 * rcutfac * radelem[t];
+            for (int n1 = -s.nimg[0]; n1 <= s.nimg[0]; n1++)
+                for (int n2 = -s.nimg[1]; n2 <= s.nimg[1]; n2++)
+                    for (int n3 = -s.nimg[2]; n3 <= s.nimg[2]; n3++) {
+                        double d[3];
+                        for (int k = 0; k < 3; k++)
+                            d[k] = s.wpos[3 * n + k] + n1 * a1[k] + n2 * a2[k] + n3 * a3[k] - rp[k];
+                        double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+                        if (!(sqrt(r2) < rcut)) continue;
+                        g[t] += wj[t] * pref * exp(-r2 / (2.0 * sigma * sigma));
+                    }
+        }
+    }
+    free(s.wpos);
+    return 0;
+}
+
 int oracle_num_threads(void)
 {
 #ifdef _OPENMP

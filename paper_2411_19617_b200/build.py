@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmala_snap.so")
 SOURCES = ["mala_snap.cu"]
-DEPS = ["mala_snap.cu", "snap_common.cuh", "snap_tables.h", "snap_ui.cuh", "snap_zi.cuh", "snap_zi_coop.cuh", "snap_zi_diag.cuh",
+DEPS = ["mala_snap.cu", "snap_common.cuh", "snap_tables.h", "snap_ui.cuh", "snap_zi.cuh", "snap_zi_coop.cuh", "snap_zi_diag.cuh", "snap_gauss.cuh",
         os.path.join("..", "..", "include", "mala_snap.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "--expt-relaxed-constexpr", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-diag-suppress", "177"]

@@ -22,6 +22,7 @@
 #include "snap_zi.cuh"
 #include "snap_zi_coop.cuh"
 #include "snap_zi_diag.cuh"
+#include "snap_gauss.cuh"
 
 using namespace mala;
 
@@ -646,6 +647,52 @@ int run_slab(mala_snap *h, int z0, int z1, double *out, double2 *u_out, cudaStre
     return 0;
 }
 
+// Gaussian descriptors of the slab [z0, z1) into out (DEVICE, [points][ntypes]): tile binning + one pass over the candidates
+int run_slab_gauss(mala_snap *h, int z0, int z1, double sigma, double *out, cudaStream_t st) {
+    if (z1 <= z0) return 0;
+    choose_tiles(h, z0, z1);
+    GridGeom &g = h->geom;
+    h->cand_cap = candidate_bound(h);
+    const long long total_tiles = (long long)g.ntx * g.nty * g.ntz;
+    if (total_tiles > 2000000000LL) return fail(MALA_SNAP_EINVAL, "slab has too many tiles; use smaller z-slabs");
+    const size_t per_tile = (size_t)h->cand_cap * sizeof(int) + 2 * sizeof(int);
+    const size_t budget = (size_t)std::max<long long>(h->workspace_mb, 1) << 20;
+    long long chunk_tiles = (long long)std::max<size_t>(budget / per_tile, (size_t)h->num_sms);
+    chunk_tiles = std::min(chunk_tiles, total_tiles);
+    if (h->d_cand.reserve((size_t)chunk_tiles * h->cand_cap) || h->d_ncand.reserve(chunk_tiles) || h->d_active.reserve(chunk_tiles) ||
+        h->d_counters.reserve(4))
+        return fail(MALA_SNAP_ENOMEM, "cudaMalloc (workspace) failed");
+    const double pi = 3.14159265358979323846;
+    const double pref = 1.0 / (std::pow(2.0 * pi, 1.5) * sigma * sigma * sigma), inv2s2 = 1.0 / (2.0 * sigma * sigma);
+    const DeviceTables tb = h->tables();
+    for (long long t0 = 0; t0 < total_tiles; t0 += chunk_tiles) {
+        ChunkBuffers cb{};
+        cb.ghosts = h->d_ghosts[h->cur].p; cb.cell_start = h->d_cell_start[h->cur].p;
+        cb.cand = h->d_cand.p; cb.ncand = h->d_ncand.p; cb.active = h->d_active.p; cb.counters = h->d_counters.p;
+        cb.cand_cap = h->cand_cap;
+        cb.tile_begin = (int)t0;
+        cb.ntiles = (int)std::min(chunk_tiles, total_tiles - t0);
+        CUDA_TRY(cudaMemsetAsync(cb.counters, 0, 4 * sizeof(int), st));
+        const int blocks = (cb.ntiles + 7) / 8;
+        {
+            TimedSpan span(h, st, kKindBin);
+            tile_bin_kernel<<<blocks, 256, 0, st>>>(g, h->sc, tb, cb, nullptr);
+        }
+        CUDA_TRY(cudaGetLastError());
+        {
+            TimedSpan span(h, st, kKindOther);
+            gaussian_grid_kernel<<<blocks, 256, 0, st>>>(g, h->sc, tb, cb, inv2s2, pref, out);
+        }
+        CUDA_TRY(cudaGetLastError());
+        h->stats[0] += 2;
+        h->stats[1]++;
+    }
+    h->stats[2] += total_tiles;
+    h->stats[4] = h->cand_cap;
+    h->stats[6] += (long long)g.nx * g.ny * (z1 - z0);
+    return 0;
+}
+
 int finish_call(mala_snap *h, cudaStream_t st) {
     CUDA_TRY(cudaEventRecord(h->ev_call_done[h->cur], st));
     h->call_done_valid[h->cur] = true;
@@ -970,6 +1017,22 @@ int mala_bispectrum_grid_host(mala_snap_t *h, int natoms, const double *pos, con
     CUDA_TRY(cudaStreamSynchronize(h->copy_stream));
     CUDA_TRY(cudaStreamSynchronize(st));
     return MALA_SNAP_OK;
+}
+
+int mala_gaussian_grid(mala_snap_t *h, double sigma, int natoms, const double *pos, const int *types, const double box[9],
+                       const double origin[3], const int pbc[3], const int ngrid[3], int z_begin, int z_end, double *out,
+                       void *cuda_stream) {
+    const CallArgs a{natoms, pos, types, box, origin, pbc, ngrid, z_begin, z_end};
+    int rc = validate(h, a, true, out);
+    if (rc) return rc;
+    if (!(sigma > 0.0) || !std::isfinite(sigma)) return fail(MALA_SNAP_EINVAL, "sigma must be positive");
+    if (h->ntypes > kGaussMaxTypes) return fail(MALA_SNAP_EINVAL, "mala_gaussian_grid supports at most 4 atom types");
+    std::fill(h->stats, h->stats + 8, 0LL);
+    if (z_end == z_begin) return MALA_SNAP_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if ((rc = build_plan(h, a, st))) return rc;
+    if ((rc = run_slab_gauss(h, z_begin, z_end, sigma, out, st))) return rc;
+    return finish_call(h, st);
 }
 
 int mala_snap_debug_utot(mala_snap_t *h, int natoms, const double *pos, const int *types, const double box[9],

@@ -19,6 +19,7 @@ MALA_SNAP_ECUDA = -2
 MALA_SNAP_ENOMEM = -3
 
 EXPORTS = ("mala_snap_create", "mala_snap_ncomp", "mala_snap_triples", "mala_bispectrum_grid", "mala_bispectrum_grid_host",
+           "mala_gaussian_grid",
            "mala_snap_set_option", "mala_snap_last_stats", "mala_snap_kernel_times", "mala_snap_fp64_peak", "mala_snap_clebsch_gordan", "mala_snap_debug_utot",
            "mala_snap_destroy", "mala_last_error")
 
@@ -59,6 +60,8 @@ def load_library():
     lib.mala_bispectrum_grid.argtypes = grid_args
     lib.mala_bispectrum_grid_host.restype = C.c_int
     lib.mala_bispectrum_grid_host.argtypes = grid_args
+    lib.mala_gaussian_grid.restype = C.c_int
+    lib.mala_gaussian_grid.argtypes = [vp, C.c_double] + grid_args[1:]
     lib.mala_snap_debug_utot.restype = C.c_int
     lib.mala_snap_debug_utot.argtypes = grid_args
     lib.mala_snap_set_option.restype = C.c_int
@@ -132,6 +135,7 @@ class MalaSnap:
                                     int(radelem.shape[0]), _dp(radelem), _dp(wj)))
         self.twojmax = int(twojmax)
         self.ncomp = lib.mala_snap_ncomp(self._h)
+        self.ntypes = int(radelem.shape[0])
 
     # -- mala_snap_destroy
     def close(self):
@@ -214,6 +218,20 @@ class MalaSnap:
             raise ValueError("out must be a contiguous CPU float64 tensor with at least npoints*ncomp elements")
         s = torch.cuda.current_stream() if stream is None else stream
         _check(self._lib.mala_bispectrum_grid_host(self._h, *args, C.c_void_p(out.data_ptr()), C.c_void_p(s.cuda_stream)))
+        return out
+
+    # -- mala_gaussian_grid: Gaussian descriptors [npoints, ntypes]
+    def gaussian_grid(self, sigma, pos, types, box, origin=(0, 0, 0), pbc=(1, 1, 1), ngrid=(1, 1, 1), z_begin=0, z_end=None,
+                      out=None, stream=None):
+        import torch
+        args, keep, npts = self._system(pos, types, box, origin, pbc, ngrid, z_begin, z_end)
+        if out is None:
+            out = torch.empty((npts, self.ntypes), dtype=torch.float64, device="cuda")
+        if (not out.is_cuda) or out.dtype != torch.float64 or (not out.is_contiguous()) or out.numel() < npts * self.ntypes:
+            raise ValueError("out must be a contiguous CUDA float64 tensor with at least npoints*ntypes elements")
+        s = torch.cuda.current_stream() if stream is None else stream
+        _check(self._lib.mala_gaussian_grid(self._h, C.c_double(float(sigma)), *args, C.c_void_p(out.data_ptr()),
+                                            C.c_void_p(s.cuda_stream)))
         return out
 
     # -- mala_snap_debug_utot (test hook)
