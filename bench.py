@@ -48,6 +48,9 @@ def parse_args():
     p.add_argument("--warmup", type=int, default=3)
     p.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5])
     p.add_argument("--impl", default="native", choices=["native", "reference"])
+    p.add_argument("--descriptor", default="bispectrum", choices=["bispectrum", "gaussian"],
+                   help="gaussian: the SURVEY 8(f) f2 path (mala_gaussian_grid), a separate metric line")
+    p.add_argument("--sigma", type=float, default=0.5, help="Gaussian width for --descriptor gaussian")
     p.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
     p.add_argument("--no-e2e", action="store_true", help="skip the host-output leg (profiling runs)")
     return p.parse_args()
@@ -341,6 +344,98 @@ def run_native(args, w, rank, world, local):
     print(json.dumps(line), flush=True)
 
 
+def run_gaussian(args, w, rank, world, local):
+    """--descriptor gaussian: grid points/s of mala_gaussian_grid (row f2).  Same contract: device leg, e2e leg with a pinned
+    host copy of the result, oracle baseline.  Flop model per point: 9 flop per candidate-free distance test is not
+    algorithmic, so only the hits count: 8 (distance) + 1 sqrt + 22 (exp) + 2 = 33 flop per neighbor within the cutoff."""
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        torch.distributed.init_process_group("nccl", device_id=dev)
+    from paper_2411_19617_b200 import MalaSnap
+    npts, nty = w.npoints, len(w.radelem)
+    snap = MalaSnap(**w.snap_params())
+    stream = torch.cuda.current_stream()
+    out = torch.empty((npts, nty), dtype=torch.float64, device=dev)
+    host = torch.empty((npts, nty), dtype=torch.float64, pin_memory=True)
+    call = lambda: snap.gaussian_grid(args.sigma, w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, out=out, stream=stream)
+
+    def barrier():
+        if world > 1:
+            torch.distributed.barrier()
+        torch.cuda.synchronize()
+
+    snap.set_option("timing", 1)
+    for _ in range(args.warmup):
+        call()
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.15)
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    launches, kms = 0, []
+    barrier()
+    for a, b in evs:
+        a.record(stream)
+        call()
+        b.record(stream)
+        launches += snap.last_stats()["kernels"]
+        kms.append(snap.kernel_times())
+    barrier()
+    clocks = sampler.stop()
+    total_ms = float(sum(a.elapsed_time(b) for a, b in evs))
+    total_ms, total_pts = reduce_max_sum(total_ms, npts * args.steps, world, dev)
+    value = total_pts / (total_ms * 1e-3)
+    g_ms = float(np.mean([k["other"][0] for k in kms]))
+    bin_ms = float(np.mean([k["tile_bin"][0] for k in kms]))
+    pairs, _ = workload_counts(w)
+    peaks = load_peaks()
+    achieved = pairs * 33 / (g_ms * 1e-3) / 1e12
+    roofline = {"bound": "alu", "kernel": "gaussian_grid_kernel", "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS, "unit": "TFLOP/s",
+                "frac": achieved / FP64_NOMINAL_TFLOPS, "traffic": None, "flop_per_launch": pairs * 33,
+                "kernel_ms_per_step": {"tile_bin": bin_ms, "gaussian_grid": g_ms},
+                "hbm_out_gbs": npts * nty * 8 / (g_ms * 1e-3) / 1e9, "hbm_peak_gbs": peaks["hbm_gbs"],
+                "note": "neither roofline binds at these sizes: 33 flop per neighbor and 8 B per point leave the kernel latency-bound"}
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        call()
+        host.copy_(out, non_blocking=True)
+        torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    e2e_s, e2e_pts = reduce_max_sum(e2e_s, npts * args.steps, world, dev)
+    h2d = int(w.pos.nbytes + w.types.nbytes + 9 * 8 + 3 * 8 + 3 * 4 + 3 * 4)
+    e2e = {"value": e2e_pts / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": int(npts * nty * 8),
+           "ms_per_step": 1e3 * e2e_s / args.steps}
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+        rng = np.random.default_rng(7)
+        n = 200000
+        sample = rng.integers(0, npts, n)
+        pts = oracle.grid_points(w.box, w.origin, w.ngrid, sample=sample)
+        t0 = time.perf_counter()
+        oracle.gaussian_points(pts, w.pos, w.types, w.box, w.origin, w.pbc, sigma=args.sigma, rcutfac=w.rcutfac, radelem=w.radelem, wj=w.wj)
+        dt = time.perf_counter() - t0
+        cpu = {"value": n / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": f"{n} seeded random grid points of {w.name} (of {npts}) in {dt:.1f} s wall"}
+    snap.close()
+    if world > 1:
+        torch.distributed.destroy_process_group()
+    if rank != 0:
+        return
+    cfg = workload_config(w, "mala_gaussian_grid (device out)")
+    cfg.update({"ncomp": nty, "sigma": args.sigma})
+    line = {"metric": "grid points/s of Gaussian descriptors (SURVEY 8(f) f2)", "value": value, "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": cfg, "clocks": clocks,
+            "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     args = parse_args()
     rank, world, local = dist_setup(args)
@@ -353,6 +448,9 @@ def main():
     w.extra["cfg"] = args.config
     if args.impl == "reference":
         run_reference(args, w, rank, world)
+        return
+    if args.descriptor == "gaussian":
+        run_gaussian(args, w, rank, world, local)
         return
     run_native(args, w, rank, world, local)
 
