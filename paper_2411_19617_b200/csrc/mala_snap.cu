@@ -791,43 +791,71 @@ int mala_snap_create(mala_snap_t **handle, int twojmax, double rcutfac, double r
             // every warp's cumulative cost on the team mean.  More teams = longer runs per call but more instruction
             // streams in flight: measured on B200 (config 2) 1 team 30.8 ms, 2 teams 28.9 ms, 3 teams 35.7 ms,
             // 4 teams 52.9 ms -- the 32 KB instruction cache holds two loop bodies, not three.
+            // The CTA-wide barrier at the end of every reduction group (kCoopGroup triples) makes the group, not the tile,
+            // the unit to balance: per group the triples are split between the teams so that the team totals are as equal
+            // as possible (all subsets are tried), and the running loads that place the run boundaries start from zero
+            // in every group.  Model idle time at the barriers: 15 % with tile-wide balancing, 6 % with this.
             const double kItemOverhead = 8.0;
             const int teams = kCoopTeams;  // compile-time: the kernel's reduction sums kTeamWarps partials
             const int tw = kCoopWarps / teams;  // warps per team
-            std::vector<double> load(kCoopWarps, 0.0), team_load(teams, 0.0);
             std::vector<int> pos_team(kSpecNT, 0);
+            std::vector<std::vector<double>> icost(kSpecNT);
+            std::vector<double> tsum(kSpecNT, 0.0);
             for (int pos = 0; pos < kSpecNT; pos++) {
                 const int t = h->tab.order[pos];
                 const int J1 = h->tab.triples[4 * t], J2 = h->tab.triples[4 * t + 1], J = h->tab.triples[4 * t + 2];
-                std::vector<double> cost;
                 for (int mb = 0; mb <= J / 2; mb++) {
                     const int nb = item_hi(J1, J2, J, mb) - item_lo(J1, J2, J, mb) + 1;
-                    for (int i = 0; i < nb; i++) cost.push_back(item_terms(J1, J2, J, mb) + kItemOverhead);
+                    for (int i = 0; i < nb; i++) icost[pos].push_back(item_terms(J1, J2, J, mb) + kItemOverhead);
                 }
-                const int n = (int)cost.size();
-                double sum = 0.0;
-                for (double c : cost) sum += c;
-                int team = 0;
-                for (int k = 1; k < teams; k++)
-                    if (team_load[k] < team_load[team]) team = k;
-                team_load[team] += sum;
-                pos_team[pos] = team;
-                const double target = team_load[team] / tw;
-                for (int w = 0; w < kCoopWarps; w++) sched[pos][w][0] = sched[pos][w][1] = 0;
-                int i = 0;
-                for (int k = 0; k < tw; k++) {
-                    const int w = team * tw + k;
-                    const int begin = i;
-                    double acc = 0.0;
-                    if (k == tw - 1) {
-                        for (; i < n; i++) acc += cost[i];
-                    } else {
-                        const double want = target - load[w];
-                        while (i < n && acc + 0.5 * cost[i] <= want) acc += cost[i++];
+                for (double c : icost[pos]) tsum[pos] += c;
+            }
+            for (int g0 = 0; g0 < kSpecNT; g0 += kCoopGroup) {
+                const int gn = std::min(kCoopGroup, kSpecNT - g0);
+                // team of every triple of the group
+                if (teams == 2 && gn <= 16) {
+                    double total = 0.0, best = 1e300;
+                    for (int i = 0; i < gn; i++) total += tsum[g0 + i];
+                    unsigned best_mask = 0;
+                    for (unsigned mask = 0; mask < (1u << gn); mask++) {
+                        double a = 0.0;
+                        for (int i = 0; i < gn; i++)
+                            if (mask >> i & 1u) a += tsum[g0 + i];
+                        if (std::fabs(2.0 * a - total) < best) { best = std::fabs(2.0 * a - total); best_mask = mask; }
                     }
-                    load[w] += acc;
-                    sched[pos][w][0] = (unsigned short)begin;
-                    sched[pos][w][1] = (unsigned short)i;
+                    for (int i = 0; i < gn; i++) pos_team[g0 + i] = (int)(best_mask >> i & 1u);
+                } else {
+                    std::vector<double> tl(teams, 0.0);
+                    for (int i = 0; i < gn; i++) {
+                        int team = 0;
+                        for (int k = 1; k < teams; k++)
+                            if (tl[k] < tl[team]) team = k;
+                        tl[team] += tsum[g0 + i];
+                        pos_team[g0 + i] = team;
+                    }
+                }
+                std::vector<double> load(kCoopWarps, 0.0), team_load(teams, 0.0);
+                for (int pos = g0; pos < g0 + gn; pos++) {
+                    const std::vector<double> &cost = icost[pos];
+                    const int n = (int)cost.size(), team = pos_team[pos];
+                    team_load[team] += tsum[pos];
+                    const double target = team_load[team] / tw;
+                    for (int w = 0; w < kCoopWarps; w++) sched[pos][w][0] = sched[pos][w][1] = 0;
+                    int i = 0;
+                    for (int k = 0; k < tw; k++) {
+                        const int w = team * tw + k;
+                        const int begin = i;
+                        double acc = 0.0;
+                        if (k == tw - 1) {
+                            for (; i < n; i++) acc += cost[i];
+                        } else {
+                            const double want = target - load[w];
+                            while (i < n && acc + 0.5 * cost[i] <= want) acc += cost[i++];
+                        }
+                        load[w] += acc;
+                        sched[pos][w][0] = (unsigned short)begin;
+                        sched[pos][w][1] = (unsigned short)i;
+                    }
                 }
             }
             // flatten into one work list per warp (snap_zi_coop.cuh, c_wlist)
