@@ -116,6 +116,7 @@ struct mala_snap {
     cudaEvent_t ev_done[2] = {nullptr, nullptr}, ev_copied[2] = {nullptr, nullptr};
     // plan of the current call
     GridGeom geom{};
+    long long total_tiles = 0;
     int cand_cap = 0;
     long long stats[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     // optional per-kernel timing ("timing" option): event pairs around every launch of the last call
@@ -321,7 +322,10 @@ int compute_bconst(mala_snap *h) {
     CUDA_TRY(cudaMemcpy(h->d_counters.p, counters, sizeof(counters), cudaMemcpyHostToDevice));
     GridGeom g{};
     g.a1[0] = g.a2[1] = g.a3[2] = 1.0;
-    g.nx = 4; g.ny = 4; g.nz = 2; g.z0 = 0; g.z1 = 2; g.tx = 4; g.ty = 4; g.tz = 2; g.ntx = g.nty = g.ntz = 1;
+    g.nx = 4; g.ny = 4; g.nz = 2; g.z0 = 0; g.z1 = 2;
+    g.nreg = 1; g.total_tiles = 1;
+    g.reg[0].x0 = 0; g.reg[0].y0 = 0; g.reg[0].nxr = 4; g.reg[0].nyr = 4; g.reg[0].tx = 4; g.reg[0].ty = 4; g.reg[0].tz = 2;
+    g.reg[0].ntx = g.reg[0].nty = g.reg[0].ntz = 1; g.reg[0].tile_begin = 0;
     const GridGeom saved = h->geom;
     h->geom = g;
     ChunkBuffers cb{};
@@ -510,20 +514,19 @@ int build_plan(mala_snap *h, const CallArgs &a, cudaStream_t st) {
 
 namespace {
 
-// tile shape: 32 points as a small brick; prefer the most compact brick among those that waste the fewest lanes
+// Tile shapes: 32 points as a small brick.  The (x, y) extent is split into the part the main brick covers exactly, the
+// strips left over along x and along y, and their corner; every part gets the brick that minimises
+// (number of tiles) x (1 + radius / rcut)^3 -- wasted lanes cost whole tiles, a larger radius costs candidate tests.
 void choose_tiles(mala_snap *h, int z0, int z1) {
     GridGeom &g = h->geom;
     static const int shapes[][3] = {{4, 4, 2}, {4, 2, 4}, {2, 4, 4}, {8, 2, 2}, {2, 8, 2}, {2, 2, 8}, {8, 4, 1}, {4, 8, 1},
                                     {16, 2, 1}, {2, 16, 1}, {32, 1, 1}, {1, 32, 1}, {1, 1, 32}, {16, 1, 2}, {1, 16, 2},
                                     {8, 1, 4}, {1, 8, 4}, {4, 1, 8}, {1, 4, 8}, {2, 1, 16}, {1, 2, 16}};
+    constexpr int nshapes = (int)(sizeof(shapes) / sizeof(shapes[0]));
     const int nzs = std::max(z1 - z0, 1);
-    double best_score = -1.0;
-    int best = 0;
-    for (int s = 0; s < (int)(sizeof(shapes) / sizeof(shapes[0])); s++) {
-        const int *t = shapes[s];
-        const double tiles = (double)((g.nx + t[0] - 1) / t[0]) * ((g.ny + t[1] - 1) / t[1]) * ((nzs + t[2] - 1) / t[2]);
-        const double util = (double)g.nx * g.ny * nzs / (tiles * 32.0);
-        // radius of the brick in units of the grid spacings (a proxy that does not need the metric)
+    const double rcut = std::max(h->rcutmax, 1e-9);
+    // radius of a brick: half its longest body diagonal
+    auto radius_of = [&](const int *t) {
         double e[3][3];
         for (int k = 0; k < 3; k++) {
             e[0][k] = g.a1[k] * (t[0] - 1) / g.nx;
@@ -537,20 +540,57 @@ void choose_tiles(mala_snap *h, int z0, int z1) {
             for (int k = 0; k < 3; k++) d[k] = e[0][k] + s1 * e[1][k] + s2 * e[2][k];
             r = std::max(r, 0.5 * std::sqrt(dot3(d, d)));
         }
-        // fewer wasted lanes first; a larger radius costs candidate tests, roughly (1 + r/rcut)^3
-        const double reach = 1.0 + r / std::max(h->rcutmax, 1e-9);
-        const double score = util / (reach * reach * reach);
-        if (score > best_score * (1.0 + 1e-12)) {
-            best_score = score;
-            best = s;
-            g.tile_radius = r * (1.0 + 1e-9) + 1e-12;
+        return r * (1.0 + 1e-9) + 1e-12;
+    };
+    auto cost_of = [&](int nxr, int nyr, const int *t) {
+        if (nxr <= 0 || nyr <= 0) return 0.0;
+        const double tiles = (double)((nxr + t[0] - 1) / t[0]) * ((nyr + t[1] - 1) / t[1]) * ((nzs + t[2] - 1) / t[2]);
+        const double reach = 1.0 + radius_of(t) / rcut;
+        return tiles * reach * reach * reach;
+    };
+    auto best_shape = [&](int nxr, int nyr, double &cost) {
+        int best = 0;
+        cost = 1e300;
+        for (int s = 0; s < nshapes; s++) {
+            const double c = cost_of(nxr, nyr, shapes[s]);
+            if (c < cost * (1.0 - 1e-12)) { cost = c; best = s; }
+        }
+        return best;
+    };
+    double best_cost = 1e300;
+    int pick[4] = {0, 0, 0, 0}, X0 = 0, Y0 = 0;
+    for (int s = 0; s < nshapes; s++) {
+        const int *t = shapes[s];
+        const int x0 = g.nx / t[0] * t[0], y0 = g.ny / t[1] * t[1];
+        double c1, c2, c3;
+        const int s1 = best_shape(g.nx - x0, y0, c1), s2 = best_shape(x0, g.ny - y0, c2), s3 = best_shape(g.nx - x0, g.ny - y0, c3);
+        const double c = cost_of(x0, y0, t) + c1 + c2 + c3;
+        if (c < best_cost * (1.0 - 1e-12)) {
+            best_cost = c;
+            pick[0] = s; pick[1] = s1; pick[2] = s2; pick[3] = s3;
+            X0 = x0; Y0 = y0;
         }
     }
-    g.tx = shapes[best][0]; g.ty = shapes[best][1]; g.tz = shapes[best][2];
+    const int ext[4][4] = {{0, 0, X0, Y0}, {X0, 0, g.nx - X0, Y0}, {0, Y0, X0, g.ny - Y0}, {X0, Y0, g.nx - X0, g.ny - Y0}};
     g.z0 = z0; g.z1 = z1;
-    g.ntx = (g.nx + g.tx - 1) / g.tx;
-    g.nty = (g.ny + g.ty - 1) / g.ty;
-    g.ntz = (nzs + g.tz - 1) / g.tz;
+    g.nreg = 0;
+    g.tile_radius = 0.0;
+    long long total = 0;
+    for (int r = 0; r < 4; r++) {
+        if (ext[r][2] <= 0 || ext[r][3] <= 0) continue;
+        GridGeom::Region &R = g.reg[g.nreg++];
+        const int *t = shapes[pick[r]];
+        R.x0 = ext[r][0]; R.y0 = ext[r][1]; R.nxr = ext[r][2]; R.nyr = ext[r][3];
+        R.tx = t[0]; R.ty = t[1]; R.tz = t[2];
+        R.ntx = (R.nxr + R.tx - 1) / R.tx; R.nty = (R.nyr + R.ty - 1) / R.ty; R.ntz = (nzs + R.tz - 1) / R.tz;
+        R.tile_begin = (int)std::min<long long>(total, 2000000000LL);
+        R.pad = 0;
+        R.tile_radius = radius_of(t);
+        g.tile_radius = std::max(g.tile_radius, R.tile_radius);
+        total += (long long)R.ntx * R.nty * R.ntz;
+    }
+    h->total_tiles = total;
+    g.total_tiles = (int)std::min<long long>(total, 2000000000LL);
 }
 
 // upper bound of the candidates tile_bin_kernel can collect for any tile: maximum ghost count over all windows
@@ -594,7 +634,7 @@ int run_slab(mala_snap *h, int z0, int z1, double *out, double2 *u_out, cudaStre
     choose_tiles(h, z0, z1);
     GridGeom &g = h->geom;
     h->cand_cap = candidate_bound(h);
-    const long long total_tiles = (long long)g.ntx * g.nty * g.ntz;
+    const long long total_tiles = h->total_tiles;
     if (total_tiles > 2000000000LL) return fail(MALA_SNAP_EINVAL, "slab has too many tiles; use smaller z-slabs");
     const size_t per_tile = (size_t)h->sc.nelem * 32 * sizeof(double2) + (size_t)h->cand_cap * sizeof(int) + 2 * sizeof(int);
     const size_t budget = (size_t)std::max<long long>(h->workspace_mb, 1) << 20;
@@ -653,7 +693,7 @@ int run_slab_gauss(mala_snap *h, int z0, int z1, double sigma, double *out, cuda
     choose_tiles(h, z0, z1);
     GridGeom &g = h->geom;
     h->cand_cap = candidate_bound(h);
-    const long long total_tiles = (long long)g.ntx * g.nty * g.ntz;
+    const long long total_tiles = h->total_tiles;
     if (total_tiles > 2000000000LL) return fail(MALA_SNAP_EINVAL, "slab has too many tiles; use smaller z-slabs");
     const size_t per_tile = (size_t)h->cand_cap * sizeof(int) + 2 * sizeof(int);
     const size_t budget = (size_t)std::max<long long>(h->workspace_mb, 1) << 20;

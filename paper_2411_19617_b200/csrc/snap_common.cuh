@@ -15,9 +15,20 @@ struct GridGeom {
     double a1[3], a2[3], a3[3], origin[3];  // cell rows and the position of grid point (0,0,0)
     int nx, ny, nz;                          // grid
     int z0, z1;                              // slab [z0, z1) handled by this launch sequence
-    int tx, ty, tz;                          // tile shape in points, tx*ty*tz == 32
-    int ntx, nty, ntz;                       // tiles per axis (ntz counts from z0)
-    double tile_radius;                      // bounding-sphere radius of one tile around its centre
+    // The slab is covered by up to four regions in (x, y), each tiled by its own 32-point brick: the part the main brick
+    // covers exactly, the strips left over along x and along y, and their corner.  A grid whose extents are not
+    // multiples of the brick (90 = 22 * 4 + 2) then wastes lanes only where the strips are ragged themselves.
+    int nreg;
+    struct Region {
+        int x0, y0, nxr, nyr;                // first point and extent of the region
+        int tx, ty, tz;                      // tile shape in points, tx*ty*tz == 32
+        int ntx, nty, ntz;                   // tiles per axis (ntz counts from z0)
+        int tile_begin;                      // id of the region's first tile
+        int pad;
+        double tile_radius;                  // bounding-sphere radius of one tile around its centre
+    } reg[4];
+    double tile_radius;                      // largest of the regions' radii (host-side candidate bound)
+    int total_tiles;
     // Cartesian cell list over the ghost atoms
     double cell_lo[3], cell_inv[3];
     int ncx, ncy, ncz;
@@ -62,11 +73,26 @@ struct ChunkBuffers {
     int ntiles;              // tiles in the chunk
 };
 
-__host__ __device__ inline void tile_coords(const GridGeom &g, int tile, int &txi, int &tyi, int &tzi) {
-    txi = tile % g.ntx;
-    int r = tile / g.ntx;
-    tyi = r % g.nty;
-    tzi = r / g.nty;
+// one tile: its first grid point, its shape, and the end of its region (points beyond it do not belong to the tile)
+struct TileInfo {
+    int ix0, iy0, iz0, tx, ty, tz, xend, yend;
+    double radius;
+};
+
+__host__ __device__ inline TileInfo tile_info(const GridGeom &g, int tile) {
+    int r = 0;
+    while (r + 1 < g.nreg && tile >= g.reg[r + 1].tile_begin) r++;
+    const GridGeom::Region &R = g.reg[r];
+    int t = tile - R.tile_begin;
+    const int txi = t % R.ntx;
+    t /= R.ntx;
+    const int tyi = t % R.nty, tzi = t / R.nty;
+    TileInfo ti;
+    ti.ix0 = R.x0 + txi * R.tx; ti.iy0 = R.y0 + tyi * R.ty; ti.iz0 = g.z0 + tzi * R.tz;
+    ti.tx = R.tx; ti.ty = R.ty; ti.tz = R.tz;
+    ti.xend = R.x0 + R.nxr; ti.yend = R.y0 + R.nyr;
+    ti.radius = R.tile_radius;
+    return ti;
 }
 
 }  // namespace mala

@@ -21,13 +21,12 @@ constexpr int kUiPoints = 16;   // grid points per compute_ui CTA: half a tile; 
 constexpr int kCandBatch = 32;  // candidate atoms staged per batch
 
 __device__ __forceinline__ void lane_point(const GridGeom &g, int tile, int lane, int &ix, int &iy, int &iz, bool &valid) {
-    int txi, tyi, tzi;
-    tile_coords(g, tile, txi, tyi, tzi);
-    const int lx = lane % g.tx, ly = (lane / g.tx) % g.ty, lz = lane / (g.tx * g.ty);
-    ix = txi * g.tx + lx;
-    iy = tyi * g.ty + ly;
-    iz = g.z0 + tzi * g.tz + lz;
-    valid = (ix < g.nx) && (iy < g.ny) && (iz < g.z1);
+    const TileInfo ti = tile_info(g, tile);
+    const int lx = lane % ti.tx, ly = (lane / ti.tx) % ti.ty, lz = lane / (ti.tx * ti.ty);
+    ix = ti.ix0 + lx;
+    iy = ti.iy0 + ly;
+    iz = ti.iz0 + lz;
+    valid = (ix < ti.xend) && (iy < ti.yend) && (iz < g.z1);
 }
 
 __device__ __forceinline__ void point_position(const GridGeom &g, int ix, int iy, int iz, double &x, double &y, double &z) {
@@ -48,16 +47,15 @@ __global__ void __launch_bounds__(256) tile_bin_kernel(GridGeom g, SnapConst sc,
     const int wt = (int)((blockIdx.x * (unsigned)blockDim.x + threadIdx.x) >> 5);
     if (wt >= cb.ntiles) return;
     const int tile = cb.tile_begin + wt;
-    int txi, tyi, tzi;
-    tile_coords(g, tile, txi, tyi, tzi);
+    const TileInfo ti = tile_info(g, tile);
     // tile centre (fractional mid-point of the full tile, also for ragged tiles: conservative)
-    const double fx = (txi * g.tx + 0.5 * (g.tx - 1)) / (double)g.nx;
-    const double fy = (tyi * g.ty + 0.5 * (g.ty - 1)) / (double)g.ny;
-    const double fz = (g.z0 + tzi * g.tz + 0.5 * (g.tz - 1)) / (double)g.nz;
+    const double fx = (ti.ix0 + 0.5 * (ti.tx - 1)) / (double)g.nx;
+    const double fy = (ti.iy0 + 0.5 * (ti.ty - 1)) / (double)g.ny;
+    const double fz = (ti.iz0 + 0.5 * (ti.tz - 1)) / (double)g.nz;
     const double cx = g.origin[0] + fx * g.a1[0] + fy * g.a2[0] + fz * g.a3[0];
     const double cy = g.origin[1] + fx * g.a1[1] + fy * g.a2[1] + fz * g.a3[1];
     const double cz = g.origin[2] + fx * g.a1[2] + fy * g.a2[2] + fz * g.a3[2];
-    const double reach = g.tile_radius + g.rcutmax;
+    const double reach = ti.radius + g.rcutmax;
     int lo[3], hi[3];
     const double c3[3] = {cx, cy, cz};
     const int nc3[3] = {g.ncx, g.ncy, g.ncz};
@@ -83,7 +81,7 @@ __global__ void __launch_bounds__(256) tile_bin_kernel(GridGeom g, SnapConst sc,
                     if (gi < g1) {
                         const Ghost gh = cb.ghosts[gi];
                         const double dx = gh.x - cx, dy = gh.y - cy, dz = gh.z - cz;
-                        const double rr = g.tile_radius + tb.type_rcut[gh.type];
+                        const double rr = ti.radius + tb.type_rcut[gh.type];
                         ok = (dx * dx + dy * dy + dz * dz) < rr * rr;
                     }
                     const unsigned bal = __ballot_sync(0xffffffffu, ok);
@@ -108,12 +106,12 @@ __global__ void __launch_bounds__(256) tile_bin_kernel(GridGeom g, SnapConst sc,
     if (out == nullptr) return;
     // empty tile: constant descriptor, written as contiguous rows of tx points
     const int nt = sc.ntriples;
-    const int ix0 = txi * g.tx;
-    const int npx = min(g.tx, g.nx - ix0);
-    for (int r = 0; r < g.ty * g.tz; r++) {
-        const int iy = tyi * g.ty + (r % g.ty);
-        const int iz = g.z0 + tzi * g.tz + (r / g.ty);
-        if (iy >= g.ny || iz >= g.z1) continue;
+    const int ix0 = ti.ix0;
+    const int npx = min(ti.tx, ti.xend - ix0);
+    for (int r = 0; r < ti.ty * ti.tz; r++) {
+        const int iy = ti.iy0 + (r % ti.ty);
+        const int iz = ti.iz0 + (r / ti.ty);
+        if (iy >= ti.yend || iz >= g.z1) continue;
         double *dst = out + ((size_t)((size_t)(iz - g.z0) * g.ny + iy) * g.nx + ix0) * nt;
         for (int i = lane; i < npx * nt; i += 32) __stcs(dst + i, tb.bconst[i % nt]);
     }

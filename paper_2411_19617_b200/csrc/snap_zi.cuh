@@ -64,16 +64,15 @@ __device__ __forceinline__ void tma_load_tile(double2 *dst, const double2 *src, 
 // Points of one tile row (fixed iy, iz) are consecutive in x, so a row is one contiguous run of npx*nt doubles.
 __device__ __forceinline__ void write_tile(const GridGeom &g, int tile, const double *Bs, int nt, double *out, int nwarps) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    int txi, tyi, tzi;
-    tile_coords(g, tile, txi, tyi, tzi);
-    const int ix0 = txi * g.tx;
-    const int npx = min(g.tx, g.nx - ix0);
-    for (int r = warp; r < g.ty * g.tz; r += nwarps) {
-        const int iy = tyi * g.ty + (r % g.ty);
-        const int iz = g.z0 + tzi * g.tz + (r / g.ty);
-        if (iy >= g.ny || iz >= g.z1) continue;
+    const TileInfo ti = tile_info(g, tile);
+    const int ix0 = ti.ix0;
+    const int npx = min(ti.tx, ti.xend - ix0);
+    for (int r = warp; r < ti.ty * ti.tz; r += nwarps) {
+        const int iy = ti.iy0 + (r % ti.ty);
+        const int iz = ti.iz0 + (r / ti.ty);
+        if (iy >= ti.yend || iz >= g.z1) continue;
         double *dst = out + ((size_t)((size_t)(iz - g.z0) * g.ny + iy) * g.nx + ix0) * nt;
-        const double *src = Bs + (size_t)(r * g.tx) * nt;  // lanes r*tx .. r*tx+npx-1 are contiguous in Bs
+        const double *src = Bs + (size_t)(r * ti.tx) * nt;  // lanes r*tx .. r*tx+npx-1 are contiguous in Bs
         const int n = npx * nt;
         if (((((uintptr_t)dst) | ((uintptr_t)src)) & 15) == 0) {
             // 16-byte vector stores over the even part, scalar tail
