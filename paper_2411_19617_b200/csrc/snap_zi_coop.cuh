@@ -154,21 +154,24 @@ __device__ __forceinline__ double column_segment(const unsigned char *Ulane, con
         if (item_hermitian(J1, J2, J) && mb1 != mb && mb1 != J - mb) cgb += cgb;  // and for item (mb1, mb)
         // x = U^{J1}[:, mb1]; columns beyond the middle come from the stored half by
         // u[ma][mb] = (-1)^(ma-mb) conj(u[J-ma][J-mb])
-        const bool fx = mb1 > J1 / 2;
-        const int cx = fx ? J1 - mb1 : mb1;
-        const unsigned char *xb = Ulane + (uhalf_off(J1) + cx * (J1 + 1) + (fx ? J1 : 0)) * kRowBytes;
-        const int xstep = fx ? -kRowBytes : kRowBytes;
-        // sign masks by parity of ma1: real part (-1)^(ma1-mb1), imaginary part the opposite (conjugation)
-        const unsigned mxr0 = (fx && (mb1 & 1)) ? 0x80000000u : 0u;
-        const unsigned mxr1 = (fx && !(mb1 & 1)) ? 0x80000000u : 0u;
-        const unsigned mxi0 = fx ? (mxr0 ^ 0x80000000u) : 0u;
-        const unsigned mxi1 = fx ? (mxr1 ^ 0x80000000u) : 0u;
         double xr[J1 + 1], xi[J1 + 1];
+        if (mb1 <= J1 / 2) {  // stored column: plain loads (the branch is warp-uniform)
+            const unsigned char *xb = Ulane + (uhalf_off(J1) + mb1 * (J1 + 1)) * kRowBytes;
 #pragma unroll
-        for (int k = 0; k <= J1; k++) {
-            const double2 v = *reinterpret_cast<const double2 *>(xb + k * xstep);
-            xr[k] = flip_sign(v.x, (k & 1) ? mxr1 : mxr0);
-            xi[k] = flip_sign(v.y, (k & 1) ? mxi1 : mxi0);
+            for (int k = 0; k <= J1; k++) {
+                const double2 v = *reinterpret_cast<const double2 *>(xb + k * kRowBytes);
+                xr[k] = v.x;
+                xi[k] = v.y;
+            }
+        } else {  // mirror column, read backwards; real part (-1)^(ma1-mb1), imaginary part the opposite (conjugation)
+            const unsigned char *xb = Ulane + (uhalf_off(J1) + (J1 - mb1) * (J1 + 1) + J1) * kRowBytes;
+            const unsigned m0 = (mb1 & 1) ? 0x80000000u : 0u;
+#pragma unroll
+            for (int k = 0; k <= J1; k++) {
+                const double2 v = *reinterpret_cast<const double2 *>(xb - k * kRowBytes);
+                xr[k] = flip_sign(v.x, (k & 1) ? (m0 ^ 0x80000000u) : m0);
+                xi[k] = flip_sign(v.y, (k & 1) ? m0 : (m0 ^ 0x80000000u));
+            }
         }
         // y = U^{J2}[:, mb2], same symmetry, folded with cgb into four scale factors
         const bool fy = mb2 > J2 / 2;
