@@ -60,6 +60,15 @@ __device__ __forceinline__ void tma_load_tile(double2 *dst, const double2 *src, 
     }
 }
 
+// L2 prefetch of one U_tot tile (no completion tracking: a hint)
+__device__ __forceinline__ void prefetch_l2_tile(const double2 *src, int nelem) {
+    const uint32_t total = (uint32_t)nelem * 32u * (uint32_t)sizeof(double2);
+    for (uint32_t done = 0; done < total; done += 32768u) {
+        const uint32_t n = min(total - done, 32768u);
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(reinterpret_cast<const unsigned char *>(src) + done), "r"(n) : "memory");
+    }
+}
+
 // ---- writer (row a7): B of one tile, staged as Bs[lane][nt] in shared memory, to out[point][nt] --------------
 // Points of one tile row (fixed iy, iz) are consecutive in x, so a row is one contiguous run of npx*nt doubles.
 __device__ __forceinline__ void write_tile(const GridGeom &g, int tile, const double *Bs, int nt, double *out, int nwarps) {

@@ -268,14 +268,21 @@ compute_zi_bi_coop_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffer
     const int wk = warp % TW;
     if (threadIdx.x == 0) mbar_init(&bar, 1);
     uint32_t parity = 0;
+    const int nactive = cb.counters[0];
+    if (threadIdx.x == 0) s_slot = atomicAdd(&cb.counters[2], 1);
     for (;;) {
-        __syncthreads();  // previous tile written out: Bs, U and s_slot are free
-        if (threadIdx.x == 0) s_slot = atomicAdd(&cb.counters[2], 1);
-        __syncthreads();
+        __syncthreads();  // previous tile written out: Bs and U are free; s_slot is visible
         const int slot = s_slot;
-        if (slot >= cb.counters[0]) break;
+        if (slot >= nactive) break;
         const int wt = cb.active[slot];
-        if (threadIdx.x == 0) tma_load_tile(U, cb.utot + (size_t)slot * nelem * 32, nelem, &bar);
+        __syncthreads();  // everybody has read s_slot
+        if (threadIdx.x == 0) {
+            tma_load_tile(U, cb.utot + (size_t)slot * nelem * 32, nelem, &bar);
+            // claim the next tile now and pull its U_tot into L2 while this one is being worked on
+            const int next = atomicAdd(&cb.counters[2], 1);
+            s_slot = next;
+            if (next < nactive) prefetch_l2_tile(cb.utot + (size_t)next * nelem * 32, nelem);
+        }
         mbar_wait(&bar, parity);
         parity ^= 1u;
         const unsigned char *Ulane = reinterpret_cast<const unsigned char *>(U + lane);
