@@ -165,6 +165,22 @@ def test_small_cases_every_twojmax(twojmax):
         assert_parity(got.cpu().numpy(), ref)
 
 
+@pytest.mark.parametrize("ngrid,zr", [((1, 1, 1), (0, 1)), ((2, 3, 1), (0, 1)), ((9, 1, 5), (1, 4)), ((5, 13, 7), (0, 7)),
+                                      ((33, 2, 3), (0, 3)), ((6, 10, 9), (2, 9)), ((17, 17, 2), (0, 2))])
+def test_ragged_grid_shapes_cover_every_point_once(ngrid, zr):
+    """the region tiling (main bricks, x strip, y strip, corner) on extents that are not multiples of any brick, with z-slabs"""
+    torch = _torch()
+    pos, types, box, origin, pbc, _, params = _small_case(77, 3, 4, (1, 1, 0), True, True)
+    ref = oracle.bispectrum_grid(pos, types, box, origin, pbc, ngrid, zr[0], zr[1], **params)
+    with MalaSnap(**params) as snap:
+        out = torch.full((ref.shape[0] + 3, ref.shape[1]), float("nan"), dtype=torch.float64, device="cuda")
+        snap.bispectrum_grid(pos, types, box, origin, pbc, ngrid, zr[0], zr[1], out=out)
+        torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    assert np.isnan(got[ref.shape[0]:]).all()          # nothing written past the slab
+    assert_parity(got[:ref.shape[0]], ref)
+
+
 def test_zero_atoms_gives_self_term_everywhere():
     """closed form: B_{j1 j2 j} = wself^3 (j+1) for every triple (north_star: zero neighbors -> self term only)"""
     torch = _torch()
