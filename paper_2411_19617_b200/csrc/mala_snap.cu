@@ -822,6 +822,16 @@ int mala_snap_create(mala_snap_t **handle, int twojmax, double rcutfac, double r
             if ((int)h->tab.cg.size() != kSpecCG || h->tab.ntriples != kSpecNT) return fail(MALA_SNAP_ECUDA, "internal: table size mismatch");
             CUDA_TRY(cudaMemcpyToSymbol(c_cg_spec, h->tab.cg.data(), sizeof(double) * kSpecCG));
             CUDA_TRY(cudaMemcpyToSymbol(c_order_spec, h->tab.order.data(), sizeof(int) * kSpecNT));
+            {
+                static double sq[kSpecTJ + 1][kSpecTJ + 1], isq[kSpecTJ + 1][kSpecTJ + 1];
+                for (int J = 0; J <= kSpecTJ; J++)
+                    for (int m = 0; m <= kSpecTJ; m++) {
+                        sq[J][m] = (m <= J) ? std::sqrt(binom_d(J, m)) : 0.0;
+                        isq[J][m] = (m <= J) ? 1.0 / std::sqrt(binom_d(J, m)) : 0.0;
+                    }
+                CUDA_TRY(cudaMemcpyToSymbol(c_sqbin, sq, sizeof(sq)));
+                CUDA_TRY(cudaMemcpyToSymbol(c_isqbin, isq, sizeof(isq)));
+            }
             // deal the (mb, mb1) items of every triple to the warps as contiguous runs (snap_zi_coop.cuh "Schedule"):
             // run boundaries are placed so that every warp's cumulative cost (product terms plus a fixed per-item
             // overhead) tracks the mean over the whole tile, not only within one triple
