@@ -69,10 +69,25 @@ constexpr bool item_stretched(int J1, int J2, int J) { return J == J1 + J2 && J2
 // used, the items mb <= mb1 <= J - mb of the columns mb <= J/2 represent all of them: weight 2 unless mb1 == mb or
 // mb1 == J - mb.  Checked against the oracle's U and CG to 1e-15 before use.
 constexpr bool item_hermitian(int J1, int J2, int J) { return J == J1 && J1 != J2; }
+// J1 == J2 == J: both of the above hold, i.e. the contribution of an item is symmetric under every permutation of its
+// three column indices mu1 = mb1 - J/2, mu2 = mb2 - J/2, mu3 = J/2 - mb (sum zero) and under their common sign change.
+// One item per class is computed: mu1 <= mu2 <= mu3 with mu2 <= 0, i.e. mb <= mb1 <= (mb + J/2)/2 in the columns
+// mb <= J/2, weighted with the class size (permutations 6, 3 or 1, times 2 unless mu2 == 0).
+// Used by the anti-diagonal kernel (snap_zi_diag.cuh).  In this kernel it is switched off: it halves the items of the five
+// (J, J, J) triples (-4 % product terms), but those are the triples with the largest loop bodies, whose time is set by
+// fetching the body, not by the number of passes through it -- measured 23.91 ms with it against 23.52 ms without.
+constexpr bool kCoopSymmetric3 = false;
+constexpr bool item_symmetric3(int J1, int J2, int J) { return kCoopSymmetric3 && J == J1 && J1 == J2; }
+__host__ __device__ constexpr double item_weight3(int J, int mb, int mb1) {
+    const int mu1 = mb1 - J / 2, mu3 = J / 2 - mb, mu2 = -mu1 - mu3;
+    const int perms = (mu1 == mu2 && mu2 == mu3) ? 1 : ((mu1 == mu2 || mu2 == mu3) ? 3 : 6);
+    const int both = (mu2 == 0) ? 1 : 2;
+    return (double)(perms * both) / ((mb == J / 2) ? 1.0 : 2.0);  // columns below the middle are doubled at the fold
+}
 constexpr int item_lo(int J1, int J2, int J, int mb) {
     const int s = mb + (J1 + J2 - J) / 2;
     int lo = (s - J2) > 0 ? (s - J2) : 0;
-    if (item_hermitian(J1, J2, J) && lo < mb) lo = mb;
+    if ((item_hermitian(J1, J2, J) || item_symmetric3(J1, J2, J)) && lo < mb) lo = mb;
     return lo;
 }
 constexpr int item_hi(int J1, int J2, int J, int mb) {
@@ -161,7 +176,8 @@ __device__ __forceinline__ double column_segment(const unsigned char *Ulane, con
     for (int mb1 = mb1_begin; mb1 < mb1_end; mb1++) {
         const int mb2 = mb + SH - mb1;
         double cgb = c_cg_spec[CGOFF + mb2 * (J1 + 1) + mb1];
-        if (J1 == J2 && mb1 != mb2) cgb += cgb;  // stands for its mirror item (mb2, mb1) too
+        if (item_symmetric3(J1, J2, J)) cgb *= item_weight3(J, mb, mb1);  // stands for its whole symmetry class
+        else if (J1 == J2 && mb1 != mb2) cgb += cgb;                        // stands for its mirror item (mb2, mb1) too
         if (item_hermitian(J1, J2, J) && mb1 != mb && mb1 != J - mb) cgb += cgb;  // and for item (mb1, mb)
         // x = U^{J1}[:, mb1]; columns beyond the middle come from the stored half by
         // u[ma][mb] = (-1)^(ma-mb) conj(u[J-ma][J-mb])

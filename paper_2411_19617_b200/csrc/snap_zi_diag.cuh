@@ -63,6 +63,15 @@ __host__ __device__ inline void diag_item_range(int J1, int J2, int J, int mb, i
         if (lo < mb) lo = mb;
         if (J - mb < hi) hi = J - mb;
     }
+    if (J == J1 && J1 == J2 && lo < mb) lo = mb;  // one item per S3 x Z2 class: item_symmetric3 in snap_zi_coop.cuh
+}
+
+// class size of an item of a (J, J, J) triple over the column doubling of the fold (item_weight3 of snap_zi_coop.cuh)
+__device__ __forceinline__ double diag_weight3(int J, int mb, int mb1) {
+    const int mu1 = mb1 - J / 2, mu3 = J / 2 - mb, mu2 = -mu1 - mu3;
+    const int perms = (mu1 == mu2 && mu2 == mu3) ? 1 : ((mu1 == mu2 || mu2 == mu3) ? 3 : 6);
+    const int both = (mu2 == 0) ? 1 : 2;
+    return (double)(perms * both) / ((mb == J / 2) ? 1.0 : 2.0);
 }
 
 __device__ __forceinline__ double diag_flip(double v, unsigned mask) {
@@ -115,7 +124,8 @@ __device__ __forceinline__ double diag_segment(const unsigned char *Ulane, const
     for (int mb1 = mb1_begin; mb1 < mb1_end; mb1++) {
         const int mb2 = mb + sh - mb1;
         double cgb = cgs[cgoff + mb2 * S + mb1];
-        if (J1 == J2 && mb1 != mb2) cgb += cgb;
+        if (J == J1 && J1 == J2) cgb *= diag_weight3(J, mb, mb1);
+        else if (J1 == J2 && mb1 != mb2) cgb += cgb;
         if (J == J1 && J1 != J2 && mb1 != mb && mb1 != J - mb) cgb += cgb;
         // x = U^{J1}[:, mb1]; columns beyond the middle come from the stored half by
         // u[ma][mb] = (-1)^(ma-mb) conj(u[J-ma][J-mb])

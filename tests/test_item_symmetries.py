@@ -6,7 +6,9 @@ columns mb1 and mb2 = mb + sh - mb1) to B_{j1 j2 j},
 
 satisfies  (F) b(mb, mb1) = b(J - mb, J1 - mb1)   column flip (half-column storage),
            (S) j1 == j2:  b(mb, mb1) = b(mb, mb2)  the two factors swapped,
-           (H) j == j1:   b(mb, mb1) = b(mb1, mb)  output and first factor swapped.
+           (H) j == j1:   b(mb, mb1) = b(mb1, mb)  output and first factor swapped,
+           (S3) j1 == j2 == j: b depends only on the class of (mu1, mu2, mu3) = (mb1 - J/2, mb2 - J/2, J/2 - mb) under
+                permutations and a common sign change; the class sizes are the weights of the anti-diagonal kernel.
 """
 import os
 import sys
@@ -71,3 +73,32 @@ def test_item_symmetries(utot, triple):
                 assert abs(x - item_b(utot, J1, J2, J, mb1, mb)) < 1e-12 * scale                # (H)
             checked += 1
     assert checked > 10
+
+
+@pytest.mark.parametrize("J", [2, 4, 6])
+def test_fully_symmetric_triples_have_s3_classes(utot, J):
+    sh = J // 2
+    classes = {}
+    for mb in range(J + 1):
+        for mb1 in range(J + 1):
+            x = item_b(utot, J, J, J, mb, mb1)
+            if x is None:
+                continue
+            mu = (mb1 - J // 2, mb + sh - mb1 - J // 2, J // 2 - mb)
+            key = min(tuple(sorted(mu)), tuple(sorted(-m for m in mu)))
+            classes.setdefault(key, []).append(x)
+    scale = max(abs(v) for vals in classes.values() for v in vals)
+    for key, vals in classes.items():
+        assert max(vals) - min(vals) < 1e-12 * scale
+        m1, m2, m3 = key
+        perms = 1 if m1 == m2 == m3 else (3 if (m1 == m2 or m2 == m3) else 6)
+        both = 1 if sorted(key)[1] == 0 else 2
+        assert perms * both == len(vals)          # the weight the kernel gives the class representative
+    # the representative the kernel computes: mu1 <= mu2 <= mu3, mu2 <= 0  <=>  mb <= mb1 <= (mb + J/2) / 2, mb <= J/2
+    kept = set()
+    for mb in range(J // 2 + 1):
+        for mb1 in range(mb, (mb + sh) // 2 + 1):
+            mu = (mb1 - J // 2, mb + sh - mb1 - J // 2, J // 2 - mb)
+            assert mu[0] <= mu[1] <= mu[2] and mu[1] <= 0
+            kept.add(min(tuple(sorted(mu)), tuple(sorted(-m for m in mu))))
+    assert kept == set(classes)
