@@ -181,6 +181,43 @@ def test_ragged_grid_shapes_cover_every_point_once(ngrid, zr):
     assert_parity(got[:ref.shape[0]], ref)
 
 
+def test_random_small_systems_all_kernels():
+    """60 seeded random systems (twojmax 0..10, 0..6 atoms, one or two types, triclinic / left-handed boxes, any periodicity,
+    grids 1..13 per axis, random z-slabs, sometimes a 1 MB workspace) through every zi kernel"""
+    torch = _torch()
+    rng = np.random.default_rng(2024)
+    n = 0
+    for it in range(60):
+        tj = int(rng.integers(0, 11))
+        box = np.diag(rng.uniform(2.5, 6.0, 3))
+        if rng.random() < 0.5:
+            box = box + np.tril(rng.uniform(-1, 1, (3, 3)), -1)
+        if rng.random() < 0.3:
+            box = box[[1, 0, 2]]
+        natoms = int(rng.integers(0, 7))
+        pos = rng.random((natoms, 3)) @ box * 1.5 - 0.5
+        ntypes = int(rng.integers(1, 3))
+        types = rng.integers(0, ntypes, natoms).astype(np.int32)
+        pbc = tuple(int(x) for x in rng.integers(0, 2, 3))
+        ngrid = tuple(int(x) for x in rng.integers(1, 14, 3))
+        z0 = int(rng.integers(0, ngrid[2]))
+        z1 = int(rng.integers(z0 + 1, ngrid[2] + 1))
+        params = dict(twojmax=tj, rcutfac=float(rng.uniform(1.5, 3.2)), rfac0=0.99363, rmin0=float(rng.choice([0.0, 0.2])),
+                      wself=float(rng.choice([1.0, 0.5])), radelem=(0.5, 0.4)[:ntypes], wj=(1.0, 0.7)[:ntypes])
+        origin = tuple(rng.uniform(-0.3, 0.3, 3))
+        ref = oracle.bispectrum_grid(pos, types, box, origin, pbc, ngrid, z0, z1, **params)
+        with MalaSnap(**params) as snap:
+            for zi in ([1, 3] if tj != 10 else [1, 2, 3]):
+                snap.set_option("zi_impl", zi)
+                if rng.random() < 0.3:
+                    snap.set_option("workspace_mb", 1)
+                got = snap.bispectrum_grid(pos, types, box, origin, pbc, ngrid, z0, z1)
+                torch.cuda.synchronize()
+                assert_parity(got.cpu().numpy(), ref)
+                n += 1
+    assert n >= 120
+
+
 def test_zero_atoms_gives_self_term_everywhere():
     """closed form: B_{j1 j2 j} = wself^3 (j+1) for every triple (north_star: zero neighbors -> self term only)"""
     torch = _torch()
