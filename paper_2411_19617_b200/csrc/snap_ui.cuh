@@ -18,7 +18,6 @@ namespace mala {
 
 constexpr int kGeoCap = 48;     // neighbor entries per grid point buffered between two accumulate passes
 constexpr int kUiPoints = 16;   // grid points per compute_ui CTA: half a tile; lane = (point, half), the halves split the neighbors
-constexpr int kCandBatch = 32;  // candidate atoms staged per batch
 
 __device__ __forceinline__ void lane_point(const GridGeom &g, int tile, int lane, int &ix, int &iy, int &iz, bool &valid) {
     const TileInfo ti = tile_info(g, tile);
@@ -232,7 +231,8 @@ compute_ui_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers cb) {
     const int nelem = sc.nelem;
     double2 *uacc = reinterpret_cast<double2 *>(smem_raw);                       // [nelem][NP]
     double *geo = reinterpret_cast<double *>(uacc + (size_t)uhalf_size(TJMAX) * NP);  // [kGeoCap][5][NP]
-    double *crec = geo + kGeoCap * 5 * NP;
+    double *crec = geo + kGeoCap * 5 * NP;                                          // [kGeoCap][6]
+    unsigned char *hitk = reinterpret_cast<unsigned char *>(crec + kGeoCap * 6);    // [NP][kGeoCap]
     __shared__ int s_item;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int p = lane & (NP - 1);
@@ -279,45 +279,45 @@ compute_ui_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers cb) {
             }
         };
 
-        int cnt = 0;       // buffered neighbor entries of this lane's point (identical in both halves and every warp)
-        int appended = 0;  // candidates staged since the last accumulate pass (uniform over the CTA)
+        // Candidates are taken in windows of kGeoCap.  Per window: (A) every lane runs the distance tests of its point
+        // (the count must be known everywhere) and one half-warp records which candidates hit; (B) the hits of a point are
+        // dealt to the twelve (warp, half) lanes of that point, which compute the pair geometry with all lanes busy
+        // instead of whichever lanes happen to hit a given candidate; (C) the column warps accumulate.
         const int nc = cb.ncand[wt];
         const int *mycand = cb.cand + (size_t)wt * cb.cand_cap;
-        for (int base = 0; base < nc; base += kCandBatch) {
-            const int nb = min(kCandBatch, nc - base);
-            if (appended + nb > kGeoCap) {
-                __syncthreads();
-                accumulate(cnt);
-                cnt = 0;
-                appended = 0;
-            }
-            __syncthreads();  // crec free again; first time: uacc zeroed
-            if (threadIdx.x < nb) {
-                const Ghost gh = cb.ghosts[mycand[base + threadIdx.x]];
+        for (int wbase = 0; wbase < nc || wbase == 0; wbase += kGeoCap) {
+            const int nw = min(kGeoCap, nc - wbase);
+            __syncthreads();  // crec, hitk and geo free again; first time: uacc zeroed
+            if ((int)threadIdx.x < nw) {
+                const Ghost gh = cb.ghosts[mycand[wbase + threadIdx.x]];
                 const double rc = tb.type_rcut[gh.type];
                 double *q = crec + threadIdx.x * 6;
                 q[0] = gh.x; q[1] = gh.y; q[2] = gh.z; q[3] = rc; q[4] = tb.type_w[gh.type]; q[5] = rc * rc;
             }
             __syncthreads();
-            for (int k = 0; k < nb; k++) {
+            int cnt = 0;  // neighbors of this lane's point in the window (identical in both halves and every warp)
+            for (int k = 0; k < nw; k++) {
                 const double *q = crec + k * 6;
                 const double dx = q[0] - px, dy = q[1] - py, dz = q[2] - pz;
-                const double r2 = dx * dx + dy * dy + dz * dz;
-                if (r2 < q[5]) {
-                    // the geometry of entry cnt is computed once: by warp k mod NW, in the half that will use it
-                    if ((k % NW) == warp && ((cnt & 1) != 0) == upper) {
-                        double c, ar, ai, br, bi;
-                        pair_geometry(dx, dy, dz, r2, q[3], q[4], sc.rfac0, sc.rmin0, c, ar, ai, br, bi);
-                        double *o = geo + (size_t)cnt * 5 * NP + p;
-                        o[0] = c; o[NP] = ar; o[2 * NP] = ai; o[3 * NP] = br; o[4 * NP] = bi;
-                    }
+                if (dx * dx + dy * dy + dz * dz < q[5]) {
+                    if (warp == 0 && !upper) hitk[p * kGeoCap + cnt] = (unsigned char)k;
                     cnt++;
                 }
             }
-            appended += nb;
+            __syncthreads();
+            for (int e = warp * 2 + (upper ? 1 : 0); e < cnt; e += NW * 2) {
+                const double *q = crec + (int)hitk[p * kGeoCap + e] * 6;
+                const double dx = q[0] - px, dy = q[1] - py, dz = q[2] - pz;
+                const double r2 = dx * dx + dy * dy + dz * dz;
+                double c, ar, ai, br, bi;
+                pair_geometry(dx, dy, dz, r2, q[3], q[4], sc.rfac0, sc.rmin0, c, ar, ai, br, bi);
+                double *o = geo + (size_t)e * 5 * NP + p;
+                o[0] = c; o[NP] = ar; o[2 * NP] = ai; o[3 * NP] = br; o[4 * NP] = bi;
+            }
+            __syncthreads();
+            accumulate(cnt);
+            if (nc == 0) break;
         }
-        __syncthreads();
-        accumulate(cnt);
         __syncthreads();
         // binomial normalisation, self term (delta(0) of Eq. (24)), store of the half tile: lanes hh*16 .. hh*16+15 of
         // every element; each half-warp takes an element of its own
@@ -334,7 +334,7 @@ compute_ui_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers cb) {
 
 inline size_t compute_ui_smem_bytes(int tjmax) {
     return (size_t)uhalf_size(tjmax) * kUiPoints * sizeof(double2) + (size_t)kGeoCap * 5 * kUiPoints * sizeof(double) +
-           (size_t)kCandBatch * 6 * sizeof(double);
+           (size_t)kGeoCap * 6 * sizeof(double) + (size_t)kUiPoints * kGeoCap;
 }
 
 // debug: scatter U_tot tiles into [point][nelem] order; points of empty tiles get wself on the diagonal
