@@ -35,8 +35,8 @@ F_B = 4 * 3444 + 2 * 91                   # compute_bi per non-empty grid point
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed `ncu --set full`
 # capture (profiles/, file named in the value's comment); None until a capture of the current kernel exists.
 NCU_TRAFFIC_BYTES_PER_LAUNCH = {
-    # profiles/r01_final_ncu_full.csv: 3.168514 GB read + 0.520276 GB written (U_tot tiles 3.16 GB + output 0.53 GB)
-    (2, "compute_zi_bi_coop_kernel"): 3.688790e9,
+    # profiles/r01_final_ncu_full.csv: 3.169535 GB read + 0.520816 GB written (U_tot tiles 3.16 GB + output 0.53 GB)
+    (2, "compute_zi_bi_coop_kernel"): 3.690351e9,
 }
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 DFMA/clk/SM x 2 flop x 1.965 GHz = 37.2
 
