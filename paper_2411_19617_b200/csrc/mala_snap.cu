@@ -249,38 +249,60 @@ void build_diag_schedule(mala_snap *h) {
     if (const char *e = std::getenv("MALA_SNAP_DIAG_TEAMS")) teams = std::atoi(e);
     if (teams < 1 || kDiagWarps % teams != 0) teams = 1;
     const int tw = kDiagWarps / teams;
-    std::vector<double> load(kDiagWarps, 0.0), team_load(teams, 0.0);
-    for (int pos = 0; pos < nt; pos++) {
-        const int t = order[pos];
-        DiagTriple &d = h->k_dtriple[pos];
-        d.J1 = (short)T.triples[4 * t]; d.J2 = (short)T.triples[4 * t + 1]; d.J = (short)T.triples[4 * t + 2];
-        d.index = (short)t; d.cgoff = cgoff[t]; d.pad = 0;
-        const std::vector<double> &cost = icost[t];
-        const int n = (int)cost.size();
-        int team = 0;
-        for (int k = 1; k < teams; k++)
-            if (team_load[k] < team_load[team]) team = k;
-        team_load[team] += tcost[t];
-        double sum_load = tcost[t] + 0.5 * tw * kCallCost;
-        for (int k = 0; k < tw; k++) sum_load += load[team * tw + k];
-        const double target = sum_load / tw;
-        int i = 0;
-        for (int k = 0; k < tw; k++) {
-            const int w = team * tw + k;
-            const int begin = i;
-            double acc = 0.0;
-            const bool last = (k == tw - 1);
-            const double want = target - load[w];
-            while (i < n) {
-                const bool newseg = (i == begin) || (icol[t][i] != icol[t][i - 1]);
-                const double c = cost[i] + (newseg ? segcost[t] : 0.0) + (i == begin ? kCallCost : 0.0);
-                if (!last && acc + 0.5 * c > want) break;
-                acc += c;
-                i++;
+    // balanced per reduction group, like the per-triple kernel: team split by exhaustive search, per-group running loads
+    std::vector<int> pos_team(nt, 0);
+    for (int g0 = 0; g0 < nt; g0 += kDiagGroup) {
+        const int gn = std::min(kDiagGroup, nt - g0);
+        if (teams == 2 && gn <= 16) {
+            double total = 0.0, best = 1e300;
+            for (int i = 0; i < gn; i++) total += tcost[order[g0 + i]];
+            unsigned best_mask = 0;
+            for (unsigned mask = 0; mask < (1u << gn); mask++) {
+                double a = 0.0;
+                for (int i = 0; i < gn; i++)
+                    if (mask >> i & 1u) a += tcost[order[g0 + i]];
+                if (std::fabs(2.0 * a - total) < best) { best = std::fabs(2.0 * a - total); best_mask = mask; }
             }
-            load[w] += acc;
-            h->k_dsched[((size_t)pos * kDiagWarps + w) * 2] = (unsigned short)begin;
-            h->k_dsched[((size_t)pos * kDiagWarps + w) * 2 + 1] = (unsigned short)i;
+            for (int i = 0; i < gn; i++) pos_team[g0 + i] = (int)(best_mask >> i & 1u);
+        } else {
+            std::vector<double> tl(teams, 0.0);
+            for (int i = 0; i < gn; i++) {
+                int team = 0;
+                for (int k = 1; k < teams; k++)
+                    if (tl[k] < tl[team]) team = k;
+                tl[team] += tcost[order[g0 + i]];
+                pos_team[g0 + i] = team;
+            }
+        }
+        std::vector<double> load(kDiagWarps, 0.0);
+        for (int pos = g0; pos < g0 + gn; pos++) {
+            const int t = order[pos], team = pos_team[pos];
+            DiagTriple &d = h->k_dtriple[pos];
+            d.J1 = (short)T.triples[4 * t]; d.J2 = (short)T.triples[4 * t + 1]; d.J = (short)T.triples[4 * t + 2];
+            d.index = (short)t; d.cgoff = cgoff[t]; d.pad = 0;
+            const std::vector<double> &cost = icost[t];
+            const int n = (int)cost.size();
+            double sum_load = tcost[t] + 0.5 * tw * kCallCost;
+            for (int k = 0; k < tw; k++) sum_load += load[team * tw + k];
+            const double target = sum_load / tw;
+            int i = 0;
+            for (int k = 0; k < tw; k++) {
+                const int w = team * tw + k;
+                const int begin = i;
+                double acc = 0.0;
+                const bool last = (k == tw - 1);
+                const double want = target - load[w];
+                while (i < n) {
+                    const bool newseg = (i == begin) || (icol[t][i] != icol[t][i - 1]);
+                    const double c = cost[i] + (newseg ? segcost[t] : 0.0) + (i == begin ? kCallCost : 0.0);
+                    if (!last && acc + 0.5 * c > want) break;
+                    acc += c;
+                    i++;
+                }
+                load[w] += acc;
+                h->k_dsched[((size_t)pos * kDiagWarps + w) * 2] = (unsigned short)begin;
+                h->k_dsched[((size_t)pos * kDiagWarps + w) * 2 + 1] = (unsigned short)i;
+            }
         }
     }
 }
