@@ -245,9 +245,7 @@ void build_diag_schedule(mala_snap *h) {
     });
     h->k_dtriple.assign(nt, DiagTriple{});
     h->k_dsched.assign((size_t)kDiagMaxNT * kDiagWarps * 2, 0);
-    int teams = kDiagTeams;
-    if (const char *e = std::getenv("MALA_SNAP_DIAG_TEAMS")) teams = std::atoi(e);
-    if (teams < 1 || kDiagWarps % teams != 0) teams = 1;
+    const int teams = (kDiagWarps % kDiagTeams == 0) ? kDiagTeams : 1;
     const int tw = kDiagWarps / teams;
     // balanced per reduction group, like the per-triple kernel: team split by exhaustive search, per-group running loads
     std::vector<int> pos_team(nt, 0);
