@@ -37,6 +37,9 @@
  * cross-check, B_000 closed form, zero- and one-neighbor closed forms,
  * Chebyshev closed form of B_{j,0,j}, index symmetries of B, rotation /
  * reflection / permutation / translation invariances.
+ * oracle_bj0j_grid (Chebyshev closed form of B_{j,0,j}, whole grids) and
+ * oracle_gaussian_points (Gaussian descriptors, row f2) have their own
+ * pins in tests/test_oracle_pins.py and tests/test_gaussian_descriptors.py.
  * Parity unpinned: component ORDER versus LAMMPS/MALA files (no such file in
  * the container); the order is the loop order of oracle_triples().
  */
@@ -536,6 +539,89 @@ int oracle_gaussian_points(double rcutfac, double sigma, int ntypes, const doubl
     }
     free(s.wpos);
     return 0;
+}
+
+/* ------------------------------------------------------------------ */
+/* Second, independent oracle for the 11 components B_{j,0,j}           */
+/* (SURVEY.md 8(c) pins): with the self term (c = wself, q = (1,0,0,0)) */
+/* and the neighbors (c = w f_c, unit quaternion q = (cos t0, sin t0    */
+/* d/r)) indexed together,                                              */
+/*   B_{j,0,j} = (sum_k c_k) * sum_{k,l} c_k c_l U_j(<q_k, q_l>),        */
+/* U_j the Chebyshev polynomial of the second kind of degree j          */
+/* (doubled j).  Needs neither Wigner-D nor Clebsch-Gordan, only the     */
+/* neighbor gather, f_c and the theta0 map -- cheap enough for whole     */
+/* grids.  Pinned against oracle_bispectrum_points (the Wigner-D / CG    */
+/* path) in tests/test_oracle_pins.py.  out[(z1-z0)*ny*nx][twojmax+1].   */
+/* ------------------------------------------------------------------ */
+int oracle_bj0j_grid(int twojmax, double rcutfac, double rfac0, double rmin0, double wself, int ntypes, const double *radelem,
+                     const double *wj, int natoms, const double *pos, const int *types, const double *box,
+                     const double *origin, const int *pbc, const int *ngrid, int z0, int z1, double *out)
+{
+    if (twojmax < 0 || twojmax > ORACLE_MAX_TWOJ || ntypes < 1 || z0 < 0 || z1 > ngrid[2] || z0 > z1) return -1;
+    sys_t s;
+    memset(&s, 0, sizeof(s));
+    s.twojmax = twojmax; s.rcutfac = rcutfac; s.rfac0 = rfac0; s.rmin0 = rmin0; s.wself = wself;
+    s.ntypes = ntypes; s.radelem = radelem; s.wj = wj;
+    s.natoms = natoms; s.pos = pos; s.types = types; s.box = box; s.origin = origin; s.pbc = pbc;
+    if (sys_prepare(&s)) return -1;
+    const double *a1 = box, *a2 = box + 3, *a3 = box + 6;
+    const int nx = ngrid[0], ny = ngrid[1], nz = ngrid[2];
+    const long npts = (long)(z1 - z0) * ny * nx;
+    int bad = 0;
+#pragma omp parallel for schedule(dynamic, 64)
+    for (long ip = 0; ip < npts; ip++) {
+        const int ix = (int)(ip % nx), iy = (int)((ip / nx) % ny), iz = z0 + (int)(ip / ((long)nx * ny));
+        double rp[3];
+        for (int k = 0; k < 3; k++)
+            rp[k] = origin[k] + ((double)ix / nx) * a1[k] + ((double)iy / ny) * a2[k] + ((double)iz / nz) * a3[k];
+        int cap = 128, n = 1;
+        double *c = (double *)malloc(sizeof(double) * cap), *q = (double *)malloc(sizeof(double) * 4 * cap);
+        c[0] = wself; q[0] = 1.0; q[1] = q[2] = q[3] = 0.0;
+        for (int a = 0; a < natoms; a++) {
+            const int t = types[a];
+            const double rcut = 2.0 * rcutfac * radelem[t];
+            for (int n1 = -s.nimg[0]; n1 <= s.nimg[0]; n1++)
+                for (int n2 = -s.nimg[1]; n2 <= s.nimg[1]; n2++)
+                    for (int n3 = -s.nimg[2]; n3 <= s.nimg[2]; n3++) {
+                        double d[3];
+                        for (int k = 0; k < 3; k++)
+                            d[k] = s.wpos[3 * a + k] + n1 * a1[k] + n2 * a2[k] + n3 * a3[k] - rp[k];
+                        if (fabs(d[0]) >= rcut || fabs(d[1]) >= rcut || fabs(d[2]) >= rcut) continue;
+                        double ab[4], fc;
+                        if (!oracle_pair(d, rcut, rfac0, rmin0, ab, &fc)) continue;
+                        if (n == cap) {
+                            cap *= 2;
+                            c = (double *)realloc(c, sizeof(double) * cap);
+                            q = (double *)realloc(q, sizeof(double) * 4 * cap);
+                        }
+                        /* a = q0 - i q3, b = q2 - i q1 (oracle_pair) */
+                        c[n] = wj[t] * fc;
+                        q[4 * n + 0] = ab[0]; q[4 * n + 1] = -ab[3]; q[4 * n + 2] = ab[2]; q[4 * n + 3] = -ab[1];
+                        n++;
+                    }
+        }
+        double csum = 0.0, acc[ORACLE_MAX_TWOJ + 1];
+        for (int j = 0; j <= twojmax; j++) acc[j] = 0.0;
+        for (int k = 0; k < n; k++) csum += c[k];
+        for (int k = 0; k < n; k++)
+            for (int l = 0; l < n; l++) {
+                const double x = q[4 * k] * q[4 * l] + q[4 * k + 1] * q[4 * l + 1] + q[4 * k + 2] * q[4 * l + 2] + q[4 * k + 3] * q[4 * l + 3];
+                double um = 0.0, u = 1.0; /* U_{-1}, U_0 */
+                const double w = c[k] * c[l];
+                for (int j = 0; j <= twojmax; j++) {
+                    acc[j] += w * u;
+                    const double un = 2.0 * x * u - um;
+                    um = u;
+                    u = un;
+                }
+            }
+        for (int j = 0; j <= twojmax; j++) out[(size_t)ip * (twojmax + 1) + j] = csum * acc[j];
+        free(c);
+        free(q);
+        if (n < 1) bad = 1;
+    }
+    free(s.wpos);
+    return bad ? -1 : 0;
 }
 
 int oracle_num_threads(void)

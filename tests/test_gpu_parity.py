@@ -275,6 +275,18 @@ def _sampled_parity(w, got, nsample, seed):
     return assert_parity(got[sample], ref), sample, ref
 
 
+def _bj0j_full_grid(w, got, z_begin=0, z_end=None):
+    """every grid point of the slab: the 11 components B_{j,0,j} against the Chebyshev closed form (second oracle: no
+    Wigner-D, no CG; SURVEY 8(c) pins) -- a wrong tile, lane or region anywhere on the grid shows up here"""
+    tr = oracle.triples(10)
+    idx = [int(np.where((tr[:, 0] == j) & (tr[:, 1] == 0) & (tr[:, 2] == j))[0][0]) for j in range(11)]
+    ref = oracle.bj0j_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, z_begin, z_end, **w.snap_params())
+    sub = got[:, idx]
+    assert sub.shape == ref.shape
+    scale = np.abs(ref).max(axis=0)
+    assert (np.abs(sub - ref).max(axis=0) <= TOL * scale).all()
+
+
 def test_config2_solid_al_full_size_sampled():
     """headline workload: 256-atom Al, 90^3 grid; 3,000 seeded sample points + two complete z-planes"""
     torch = _torch()
@@ -287,6 +299,7 @@ def test_config2_solid_al_full_size_sampled():
         # the same slab computed alone agrees to rounding
         part = snap.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, 44, 46).cpu().numpy()
     _sampled_parity(w, got, 3000, 22)
+    _bj0j_full_grid(w, got)
     plane = 90 * 90
     assert np.abs(part - got[44 * plane:46 * plane]).max() <= 1e-13 * np.abs(part).max()
     assert_parity(part[:plane], oracle_grid(w, 44, 45))
@@ -301,6 +314,7 @@ def test_config3_liquid_al_full_size_sampled():
     w = workloads.make(3)
     got = gpu_grid(w)
     _sampled_parity(w, got, 2000, 33)
+    _bj0j_full_grid(w, got)
 
 
 def test_config4_boron_cluster_full_size_sampled_and_empty_points():
@@ -330,6 +344,7 @@ def test_config4_boron_cluster_full_size_sampled_and_empty_points():
     assert 0.75 < empty.size / w.npoints < 0.83
     expect = oracle.triples(10)[:, 2] + 1.0
     assert np.abs(got[empty] - expect[None, :]).max() < 1e-12 * expect.max()
+    _bj0j_full_grid(w, got)
 
 
 def test_config5_be_slab_z_slabs_sampled():
@@ -349,4 +364,6 @@ def test_config5_be_slab_z_slabs_sampled():
             sample = np.unique(np.concatenate([rng.integers(0, n, 250), [0, n - 1]]))
             ref = oracle.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, z0, z1, sample=sample, **w.snap_params())
             assert_parity(got[sample], ref)
+            if z0 == 140:  # one complete plane through the stacking fault against the Chebyshev closed form
+                _bj0j_full_grid(w, got[3 * ny * nx:4 * ny * nx], 143, 144)
             del out

@@ -250,6 +250,27 @@ def test_chebyshev_closed_form_for_Bj0j(case):
         np.testing.assert_allclose(B[idx], ref, rtol=1e-11)
 
 
+def test_chebyshev_grid_oracle_agrees_with_the_wigner_cg_path():
+    """oracle.bj0j_grid (closed form, C) is the second oracle of the full-size GPU tests: here it is tied to the main path
+    (explicit Wigner-D + Racah CG) on a whole tiny-Al grid and on a two-type triclinic mixed-pbc slab"""
+    from paper_2411_19617_b200 import workloads
+    w = workloads.make(1)
+    tr = oracle.triples(10)
+    idx = [int(np.where((tr[:, 0] == j) & (tr[:, 1] == 0) & (tr[:, 2] == j))[0][0]) for j in range(11)]
+    ref = oracle.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, 0, 6, **w.snap_params())
+    ch = oracle.bj0j_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, 0, 6, **w.snap_params())
+    np.testing.assert_allclose(ch, ref[:, idx], rtol=1e-11)
+    rng = np.random.default_rng(12)
+    box = np.array([[5.0, 0.3, 0.0], [1.0, 4.5, 0.2], [0.0, -0.6, 6.0]])
+    pos = rng.uniform(-0.3, 1.3, size=(6, 3)) @ box
+    kw = dict(twojmax=6, rcutfac=4.2, radelem=(0.5, 0.45), wj=(1.0, 0.8), wself=0.7, rmin0=0.2)
+    tr6 = oracle.triples(6)
+    idx6 = [int(np.where((tr6[:, 0] == j) & (tr6[:, 1] == 0) & (tr6[:, 2] == j))[0][0]) for j in range(7)]
+    ref = oracle.bispectrum_grid(pos, [0, 1, 1, 0, 1, 0], box, (0.1, -0.2, 0.05), (1, 0, 1), (5, 4, 6), 1, 5, **kw)
+    ch = oracle.bj0j_grid(pos, [0, 1, 1, 0, 1, 0], box, (0.1, -0.2, 0.05), (1, 0, 1), (5, 4, 6), 1, 5, **kw)
+    np.testing.assert_allclose(ch, ref[:, idx6], rtol=1e-11)
+
+
 def test_atom_exactly_on_grid_point_uses_continuous_limit():
     # reading #11: r -> 0 contributes w * I
     r = oracle.bispectrum_points([[2.0, 2.0, 2.0]], [[2.0, 2.0, 2.0]], [0], BIG, pbc=(0, 0, 0), wj=(0.5,))
