@@ -1,14 +1,17 @@
 #!/usr/bin/env python
 """bench.py -- grid points/s of twojmax=10 fp64 bispectrum descriptors (BASELINE.json metric) on one B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl native|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--twojmax 10] [--shard none|z] [--impl native|reference]
 
 A step = one pass of the whole hot path (tile binning -> compute_ui -> compute_zi/compute_bi -> writer)
 over the full grid of the workload (default: config 2, 256-atom solid Al on a 90^3 grid, the configuration the metric
 is quoted on).  `value` is measured through mala_bispectrum_grid with the output resident in HBM; `e2e` through
-mala_bispectrum_grid_host with a pinned HOST output (the device->host copy of all 91 x npoints doubles is inside the
-timed region).  N > 1: independent replicas, one per GPU, no collective on the data path.
+mala_bispectrum_grid_host with a pinned HOST output (the device->host copy of all ncomp x npoints doubles is inside the
+timed region).  N > 1: one process per GPU (spawned here through torch.distributed.run when the launcher has not done
+it), no collective on the data path: `--shard none` = independent replicas of the whole grid
+(weak scaling), `--shard z` = ONE grid split into z-slabs balanced by non-empty points (strong scaling).
 `--impl reference` times the CPU oracle (oracle/) as it stands on the host cores -- the only baseline that exists.
+Other workloads: --config 200cube | binary, --twojmax 2..14.
 """
 import argparse
 import json
@@ -26,19 +29,48 @@ if ROOT not in sys.path:
 
 METRIC = "grid points/s of twojmax=10 fp64 bispectrum descriptors; % of B200 FP64 peak"
 UNIT = "points/s"
-
-# Algorithmic flops: what the method must compute using the standard
-# half-column symmetries -- not instruction counts.
-F_PAIR = 20 * 235 + 4 * 271 + 60          # compute_ui per (grid point, neighbor) pair
-F_Z = 10 * 61332 + 4 * 13230              # compute_zi per non-empty grid point
-F_B = 4 * 3444 + 2 * 91                   # compute_bi per non-empty grid point
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed `ncu --set full`
-# capture (profiles/, file named in the value's comment); None until a capture of the current kernel exists.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {
-    # profiles/r01_final_ncu_full.csv: 3.169535 GB read + 0.520816 GB written (U_tot tiles 3.16 GB + output 0.53 GB)
-    (2, "compute_zi_bi_coop_kernel"): 3.690351e9,
-}
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 DFMA/clk/SM x 2 flop x 1.965 GHz = 37.2
+
+
+def flop_model(twojmax):
+    """Algorithmic flops: what the method must compute using the standard
+    half-column symmetry -- not instruction counts.  Counted here from the index ranges themselves; at twojmax = 10:
+    235 recursion steps, 271 U elements, 3,444 Z elements, 61,332 product terms, 13,230 outer steps, i.e.
+    F_pair = 5,844, F_Z = 666,240, F_B = 13,958."""
+    tj = int(twojmax)
+    triples = [(j1, j2, j) for j1 in range(tj + 1) for j2 in range(j1 + 1) for j in range(j1 - j2, min(tj, j1 + j2) + 1, 2) if j >= j1]
+    nelem = sum((J + 1) * (J // 2 + 1) for J in range(tj + 1))
+    steps = sum((J + 1) * (J // 2 + 1) for J in range(1, tj + 1)) - sum(J + 1 for J in range(2, tj + 1, 2))
+    nz = terms = outer = 0
+    for J1, J2, J in triples:
+        sh = (J1 + J2 - J) // 2
+        for mb in range(J // 2 + 1):
+            mid = (J % 2 == 0) and (mb == J // 2)
+            nb = min(J1, mb + sh) - max(0, mb + sh - J2) + 1
+            for ma in range((J // 2 if mid else J) + 1):
+                na = min(J1, ma + sh) - max(0, ma + sh - J2) + 1
+                nz += 1
+                terms += na * nb
+                outer += nb
+    return {"ncomp": len(triples), "nelem": nelem, "F_PAIR": 20 * steps + 4 * nelem + 60, "F_Z": 10 * terms + 4 * outer,
+            "F_B": 4 * nz + 2 * len(triples), "terms": terms}
+
+
+def ncu_traffic(workload_key, kernel, live_ms):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed `ncu --set full` capture
+    (profiles/traffic.json, written from the capture named there).  Returned only when that capture's kernel duration
+    agrees with the duration measured live in this run within 3 % -- otherwise the capture is stale and the answer is None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            table = json.load(f)
+    except (OSError, ValueError):
+        return None, "no profiles/traffic.json"
+    ent = table.get(f"{workload_key}:{kernel}")
+    if not ent:
+        return None, "no capture for this workload/kernel"
+    if live_ms <= 0 or abs(ent["ncu_ms"] - live_ms) > 0.03 * live_ms:
+        return None, f"capture {ent['source']} is stale: {ent['ncu_ms']:.2f} ms under ncu vs {live_ms:.2f} ms live"
+    return float(ent["dram_bytes"]), ent["source"]
 
 
 def parse_args():
@@ -46,14 +78,20 @@ def parse_args():
     p.add_argument("--gpus", type=int, default=1)
     p.add_argument("--steps", type=int, default=5)
     p.add_argument("--warmup", type=int, default=3)
-    p.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5])
+    p.add_argument("--config", default="2", choices=["1", "2", "3", "4", "5", "200cube", "binary"],
+                   help="1-5: BASELINE.json configs; 200cube: config 2's atoms on the paper's 200^3 grid; binary: two species")
+    p.add_argument("--twojmax", type=int, default=None, help="override the workload's twojmax (default 10)")
+    p.add_argument("--shard", default="none", choices=["none", "z"],
+                   help="N > 1: none = every rank computes the whole grid (replicas), z = one grid split into z-slabs")
     p.add_argument("--impl", default="native", choices=["native", "reference"])
     p.add_argument("--descriptor", default="bispectrum", choices=["bispectrum", "gaussian"],
                    help="gaussian: the SURVEY 8(f) f2 path (mala_gaussian_grid), a separate metric line")
     p.add_argument("--sigma", type=float, default=0.5, help="Gaussian width for --descriptor gaussian")
     p.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
     p.add_argument("--no-e2e", action="store_true", help="skip the host-output leg (profiling runs)")
-    return p.parse_args()
+    args = p.parse_args()
+    args.config = int(args.config) if args.config.isdigit() else args.config
+    return args
 
 
 # ---------------------------------------------------------------------------------------------------------------
@@ -117,11 +155,11 @@ class ClockSampler:
 def workload_counts(w):
     """(pairs, non-empty points) of the whole grid.  Periodic bulk systems: every point has neighbors and the mean
     neighbor count of a uniform grid is exactly rho * 4/3 pi rcut^3.  The non-periodic cluster is counted directly."""
-    rcut = 2.0 * w.rcutfac * w.radelem[0]
     if all(w.pbc):
         vol = abs(np.linalg.det(w.box))
-        nbar = w.pos.shape[0] / vol * 4.0 / 3.0 * np.pi * rcut ** 3
+        nbar = sum(int((w.types == t).sum()) / vol * 4.0 / 3.0 * np.pi * (2.0 * w.rcutfac * r) ** 3 for t, r in enumerate(w.radelem))
         return nbar * w.npoints, w.npoints
+    rcut = 2.0 * w.rcutfac * w.radelem[0]
     nx, ny, nz = w.ngrid
     fx, fy, fz = np.arange(nx) / nx, np.arange(ny) / ny, np.arange(nz) / nz
     cnt = np.zeros((nz, ny, nx), dtype=np.int32)
@@ -131,6 +169,36 @@ def workload_counts(w):
         for a in w.pos:
             cnt[z0:z0 + 8] += (((pts - a) ** 2).sum(-1) < rcut * rcut)
     return float(cnt.sum()), int((cnt > 0).sum())
+
+
+def plane_costs(w):
+    """relative cost of every z-plane for the slab partition of --shard z: non-empty points (exact for the cluster in
+    vacuum, uniform for periodic bulk)"""
+    nx, ny, nz = w.ngrid
+    if all(w.pbc):
+        return [1.0] * nz
+    rcut = 2.0 * w.rcutfac * max(w.radelem)
+    fx, fy, fz = np.arange(nx) / nx, np.arange(ny) / ny, np.arange(nz) / nz
+    ax = fx[None, :, None] * w.box[0] + fy[:, None, None] * w.box[1]
+    cost = []
+    for z in range(nz):
+        pts = ax + fz[z] * w.box[2] + np.asarray(w.origin)
+        hit = np.zeros((ny, nx), dtype=bool)
+        for a in w.pos:
+            hit |= ((pts - a) ** 2).sum(-1) < rcut * rcut
+        cost.append(float(hit.sum()) + 0.02 * nx * ny)   # empty points still cost their 8 * ncomp bytes of fill
+    return cost
+
+
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.lower().startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
 
 
 def load_peaks():
@@ -159,7 +227,16 @@ def oracle_rate(w, seconds, seed=7):
     t0 = time.perf_counter()
     oracle.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, sample=sample, **kw)
     dt = time.perf_counter() - t0
-    return n / dt, n, dt, oracle.num_threads()
+    # per-core rate: one thread on >= 2,000 points (SURVEY.md 8(d) "Oracle timing beside it" (ii)), bounded to ~6 s
+    threads = oracle.num_threads()
+    n1 = int(min(max(2000, 0.25 * n / max(threads, 1)), 6.0 * (n / dt) / max(threads, 1) + 2000))
+    s1 = rng.integers(0, w.npoints, n1)
+    oracle.set_num_threads(1)
+    t0 = time.perf_counter()
+    oracle.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, sample=s1, **kw)
+    dt1 = time.perf_counter() - t0
+    oracle.set_num_threads(threads)
+    return n / dt, n, dt, threads, n1 / dt1, n1
 
 
 def run_reference(args, w, rank, world):
@@ -197,10 +274,11 @@ def run_reference(args, w, rank, world):
     print(json.dumps(line), flush=True)
 
 
-def workload_config(w, path):
+def workload_config(w, path, parallelism="replicas"):
     return {"workload": f"config{w.extra.get('cfg', '?')}:{w.name}", "natoms": int(w.pos.shape[0]), "ngrid": list(map(int, w.ngrid)),
-            "npoints": int(w.npoints), "twojmax": int(w.twojmax), "ncomp": 91, "rcut": float(2 * w.rcutfac * w.radelem[0]),
-            "path": path, "parallelism": "replicas",
+            "npoints": int(w.npoints), "twojmax": int(w.twojmax), "ncomp": flop_model(w.twojmax)["ncomp"],
+            "rcut": [float(2 * w.rcutfac * r) for r in w.radelem] if len(w.radelem) > 1 else float(2 * w.rcutfac * w.radelem[0]),
+            "path": path, "parallelism": parallelism,
             "l2": "no flush: each step streams the U_tot workspace and the output (both far larger than the 126 MB L2)"}
 
 
@@ -237,18 +315,26 @@ def run_native(args, w, rank, world, local):
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
-    from paper_2411_19617_b200 import MalaSnap, mala_snap_fp64_peak
+    from paper_2411_19617_b200 import MalaSnap, mala_snap_fp64_peak, slabs
 
     def barrier():
         if world > 1:
             torch.distributed.barrier()
         torch.cuda.synchronize()
 
-    npts, nt = w.npoints, 91
+    fm = flop_model(w.twojmax)
+    nt = fm["ncomp"]
+    nx, ny, nz = (int(v) for v in w.ngrid)
+    sharded = (args.shard == "z" and world > 1)
+    z0, z1 = (0, nz)
+    if sharded:   # one grid, rank r takes slab r of a partition balanced by non-empty points; atoms replicated, nothing exchanged
+        z0, z1 = slabs.weighted_z_slabs(plane_costs(w), world)[rank]
+    npts = (z1 - z0) * ny * nx
     snap = MalaSnap(**w.snap_params())
+    assert snap.ncomp == nt
     stream = torch.cuda.current_stream()
-    out = torch.empty((npts, nt), dtype=torch.float64, device=dev)
-    call = lambda: snap.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, out=out, stream=stream)
+    out = torch.empty((max(npts, 1), nt), dtype=torch.float64, device=dev)
+    call = lambda: snap.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, z0, z1, out=out, stream=stream)
 
     # ---- device-resident leg ------------------------------------------------------------------------------
     snap.set_option("timing", 1)
@@ -266,8 +352,8 @@ def run_native(args, w, rank, world, local):
         a.record(stream)
         call()
         b.record(stream)
-        launches += snap.last_stats()["kernels"]
         ktimes.append(snap.kernel_times())  # waits for this step's kernels; steps are serial on the stream anyway
+        launches += snap.last_stats()["kernels"]
     barrier()
     clocks = sampler.stop()
     step_ms = [a.elapsed_time(b) for a, b in evs]
@@ -279,33 +365,43 @@ def run_native(args, w, rank, world, local):
 
     # ---- roofline of the dominant kernel (compute_zi_bi: rows a5 + a6 + a7) --------------------------------
     pairs, nonempty = workload_counts(w)
+    if sharded:   # this rank's share (uniform bulk: by points; the cluster: by its plane costs)
+        pc = plane_costs(w)
+        frac = sum(pc[z0:z1]) / sum(pc)
+        pairs, nonempty = pairs * frac, nonempty * frac
     zi_ms = float(np.mean([k["compute_zi_bi"][0] for k in ktimes]))
     zi_launches = ktimes[-1]["compute_zi_bi"][1]
     ui_ms = float(np.mean([k["compute_ui"][0] for k in ktimes]))
     bin_ms = float(np.mean([k["tile_bin"][0] for k in ktimes]))
-    zi_flop = nonempty * (F_Z + F_B)           # per step = summed over that step's launches
-    achieved = zi_flop / (zi_ms * 1e-3) / 1e12
+    zi_flop = nonempty * (fm["F_Z"] + fm["F_B"])           # per step = summed over that step's launches
+    achieved = zi_flop / (zi_ms * 1e-3) / 1e12 if zi_ms > 0 else 0.0
     peak_meas, mhz_eff = mala_snap_fp64_peak(stream)
-    roofline = {"bound": "alu", "kernel": "compute_zi_bi_coop_kernel", "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS,
+    kernel = snap.zi_kernel_name()
+    roofline = {"bound": "alu", "kernel": kernel, "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS,
                 "unit": "TFLOP/s", "frac": achieved / FP64_NOMINAL_TFLOPS,
                 "peak_source": "nominal FP64 FMA pipe: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md 'FP64 roofline')",
                 "peak_measured_dfma": peak_meas, "frac_of_measured_dfma": achieved / peak_meas if peak_meas > 0 else None,
                 "dfma_probe_sm_mhz": mhz_eff, "traffic": None,
+                "flop_per_point": {"pair": fm["F_PAIR"], "zi": fm["F_Z"], "bi": fm["F_B"]},
                 "flop_per_launch": zi_flop / max(zi_launches, 1), "launches_per_step": zi_launches, "ms_per_launch": zi_ms / max(zi_launches, 1),
                 "kernel_ms_per_step": {"tile_bin": bin_ms, "compute_ui": ui_ms, "compute_zi_bi": zi_ms},
-                "compute_ui_tflops": pairs * F_PAIR / (ui_ms * 1e-3) / 1e12 if ui_ms > 0 else None,
-                "step_model_tflops": (pairs * F_PAIR + zi_flop) / (total_ms / args.steps * 1e-3) / 1e12 if world == 1 else None}
-    roofline["traffic"] = NCU_TRAFFIC_BYTES_PER_LAUNCH.get((args.config, roofline["kernel"]))
+                "compute_ui_tflops": pairs * fm["F_PAIR"] / (ui_ms * 1e-3) / 1e12 if ui_ms > 0 else None,
+                "step_model_tflops": (pairs * fm["F_PAIR"] + zi_flop) / (total_ms / args.steps * 1e-3) / 1e12 if world == 1 else None}
+    wl_key = f"config{w.extra.get('cfg')}/tj{w.twojmax}"
+    roofline["traffic"], roofline["traffic_source"] = ncu_traffic(wl_key, kernel, zi_ms / max(zi_launches, 1))
     peaks = load_peaks()
-    roofline["hbm_gbs_step"] = (npts * nt * 8 + 2 * (nonempty / 32) * 271 * 32 * 16) / (total_ms / args.steps * 1e-3) / 1e9 if world == 1 else None
+    roofline["hbm_gbs_step"] = (npts * nt * 8 + 2 * (nonempty / 32) * fm["nelem"] * 32 * 16) / (total_ms / args.steps * 1e-3) / 1e9 if world == 1 else None
     roofline["hbm_peak_gbs"] = peaks["hbm_gbs"]
     roofline["hbm_peak_source"] = peaks["source"]
+    # the fill of empty tiles is the HBM-bound part of tile_bin (config 4): 8 * ncomp bytes per empty point
+    if nonempty < npts and bin_ms > 0 and not sharded:
+        roofline["tile_bin_fill_gbs"] = (npts - nonempty) * nt * 8 / (bin_ms * 1e-3) / 1e9
 
     # ---- end-to-end leg: host output buffer, D2H inside the timed region ------------------------------------
     e2e = None
     if not args.no_e2e:
-        host = torch.empty((npts, nt), dtype=torch.float64, pin_memory=True)
-        call_host = lambda: snap.bispectrum_grid_host(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, out=host, stream=stream)
+        host = torch.empty((max(npts, 1), nt), dtype=torch.float64, pin_memory=True)
+        call_host = lambda: snap.bispectrum_grid_host(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, z0, z1, out=host, stream=stream)
         for _ in range(max(1, min(args.warmup, 2))):
             call_host()
         barrier()
@@ -324,19 +420,24 @@ def run_native(args, w, rank, world, local):
     # ---- CPU oracle beside it (rank 0, N = 1 only) ---------------------------------------------------------
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        rate, n, dt, threads = oracle_rate(w, seconds=12.0)
+        rate, n, dt, threads, rate1, n1 = oracle_rate(w, seconds=12.0)
         cpu = {"value": rate, "unit": UNIT, "cores": threads, "kind": "oracle",
-               "sample": f"{n} seeded random grid points of {w.name} (of {npts}) in {dt:.1f} s wall on {threads} threads"}
+               "sample": f"{n} seeded random grid points of {w.name} (of {w.npoints}) in {dt:.1f} s wall on {threads} threads",
+               "one_thread": {"value": rate1, "unit": UNIT, "sample": f"{n1} seeded random grid points on 1 thread"},
+               "cpu_model": cpu_model(), "host_cores_online": os.cpu_count()}
 
     snap.close()
     if world > 1:
         torch.distributed.destroy_process_group()
     if rank != 0:
         return
-    cfg = workload_config(w, "mala_bispectrum_grid (device out)")
+    cfg = workload_config(w, "mala_bispectrum_grid (device out)", "z-slab shards of one grid" if sharded else "replicas")
     cfg.update({"chunks_per_step": stats["chunks"], "workspace_bytes": stats["workspace_bytes"], "ghost_atoms": stats["ghosts"]})
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+    if sharded:
+        cfg["rank0_slab"] = [z0, z1]
+    line = {"metric": METRIC if w.twojmax == 10 else METRIC.replace("twojmax=10", f"twojmax={w.twojmax}"),
+            "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic", "config": cfg, "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
             "roofline": roofline, "cpu_baseline": cpu, "pct_of_fp64_peak_step": None}
     if roofline["step_model_tflops"] is not None:
@@ -436,15 +537,30 @@ def run_gaussian(args, w, rank, world, local):
     print(json.dumps(line), flush=True)
 
 
+def spawn_ranks(args):
+    """`python bench.py --gpus N` without a launcher: start the N ranks ourselves, exactly as the driver would
+    (torch.distributed.run, one process per GPU, rendezvous on 127.0.0.1), and pass their output through."""
+    import socket
+    with socket.socket() as so:
+        so.bind(("127.0.0.1", 0))
+        port = so.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
 def main():
     args = parse_args()
     rank, world, local = dist_setup(args)
     if world != args.gpus and world > 1:
         raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE={world}")
     if args.gpus > 1 and world == 1:
-        raise SystemExit("launch N > 1 with: python -m torch.distributed.run --nnodes=1 --nproc-per-node N bench.py --gpus N ...")
+        if args.impl == "reference":
+            args.gpus = 1    # the oracle arm runs on rank 0 alone
+        else:
+            raise SystemExit(spawn_ranks(args))
     from paper_2411_19617_b200 import workloads
-    w = workloads.make(args.config)
+    w = workloads.make(args.config, twojmax=args.twojmax)
     w.extra["cfg"] = args.config
     if args.impl == "reference":
         run_reference(args, w, rank, world)

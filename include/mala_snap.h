@@ -20,8 +20,10 @@
  *       MALA_SNAP_ECUDA   (-2)  CUDA runtime error      (message names the call)
  *       MALA_SNAP_ENOMEM  (-3)  host or device allocation failed
  *     and mala_last_error() returns a thread-local description of the last failure.
- *   - one handle must not be used by two host threads at once.  There is no CPU fallback: without a CUDA
- *     device mala_snap_create fails with MALA_SNAP_ECUDA.
+ *   - one handle must not be used by two host threads at once.  Calls on one handle are serialised on the device
+ *     whatever streams they are given (the handle owns one workspace): a call waits, on the device, for the previous
+ *     call on the same handle.  mala_snap_create / mala_snap_set_option("zi_impl") synchronise the device.
+ *     There is no CPU fallback: without a CUDA device mala_snap_create fails with MALA_SNAP_ECUDA.
  */
 #ifndef MALA_SNAP_H
 #define MALA_SNAP_H
@@ -121,6 +123,9 @@ int mala_gaussian_grid(mala_snap_t *h, double sigma, int natoms, const double *p
  *   "timing"           1 = record a CUDA-event pair on the caller's stream around every kernel launch of the
  *                      following calls (read back with mala_snap_kernel_times); 0 = off (default)
  *   "workspace_mb"     cap, in MiB, of the U_tot + candidate workspace (default 4096)
+ *   "cand_cap_limit"   test hook: clamp the per-tile candidate capacity to this value (0 = off, default).  A value below
+ *                      the true bound makes tile_bin_kernel overflow, which must surface as MALA_SNAP_ECUDA (see
+ *                      mala_snap_last_stats); never set it in production
  *   "host_chunk_mb"    cap, in MiB, of each of the two staging buffers of mala_bispectrum_grid_host (default 256;
  *                      outputs above 96 MiB are split into at least three chunks so the copies overlap the kernels)
  */
@@ -129,9 +134,14 @@ int mala_snap_set_option(mala_snap_t *h, const char *name, long long value);
 /*
  * Counters of the last mala_bispectrum_grid* call on this handle (HOST array of 8):
  *   [0] kernels launched   [1] chunks   [2] tiles   [3] ghost atoms (atoms + periodic images kept)
- *   [4] candidate capacity per tile   [5] workspace bytes in use   [6] points   [7] reserved
+ *   [4] candidate capacity per tile   [5] workspace bytes in use   [6] points
+ *   [7] status bits of the handle (0 = healthy; bit 0: a neighbor-candidate list overflowed its host-computed bound and was
+ *       truncated, i.e. results of that call are invalid)
+ * Waits for the last call on the handle (its status word is part of the answer) and returns MALA_SNAP_ECUDA when a status
+ * bit is set.  A raised bit is sticky: every later mala_*_grid call on the handle fails with MALA_SNAP_ECUDA at entry as soon
+ * as the offending call has drained; mala_bispectrum_grid_host, which synchronises anyway, reports it on return.
  */
-int mala_snap_last_stats(const mala_snap_t *h, long long stats[8]);
+int mala_snap_last_stats(mala_snap_t *h, long long stats[8]);
 
 /*
  * Measurement: device time of the kernels of the last mala_bispectrum_grid* call on this handle, by class, from
@@ -142,6 +152,10 @@ int mala_snap_last_stats(const mala_snap_t *h, long long stats[8]);
  * Waits for those events (so for the call's work).  All zeros if timing was off.
  */
 int mala_snap_kernel_times(mala_snap_t *h, double ms[4], long long launches[4]);
+
+/* Measurement: name of the compute_zi / compute_bi kernel the handle launches with its current options (the kernel the
+ * roofline of bench.py is reported for); a static string, "" on a NULL handle */
+const char *mala_snap_zi_kernel(const mala_snap_t *h);
 
 /*
  * Measurement: achieved FP64 FMA rate of this device (TFLOP/s, 2 flop per DFMA) from a register-only

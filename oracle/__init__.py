@@ -192,15 +192,19 @@ def grid_points(box, origin, ngrid, z_begin=0, z_end=None, sample=None):
     return (_d(origin)[None, :] + (ix / nx)[:, None] * box[0] + (iy / ny)[:, None] * box[1] + (iz / nz)[:, None] * box[2])
 
 
-def bj0j_grid(pos, types, box, origin, pbc, ngrid, z_begin=0, z_end=None, *, twojmax=10, rcutfac=4.67637, rfac0=0.99363,
-              rmin0=0.0, wself=1.0, radelem=(0.5,), wj=(1.0,)):
-    """The 11 components B_{j,0,j} on a grid slab by the Chebyshev closed form (no Wigner-D, no CG): [npoints, twojmax+1]."""
+def bj0j_grid(pos, types, box, origin, pbc, ngrid, z_begin=0, z_end=None, *, sample=None, twojmax=10, rcutfac=4.67637,
+              rfac0=0.99363, rmin0=0.0, wself=1.0, radelem=(0.5,), wj=(1.0,)):
+    """The 11 components B_{j,0,j} on a grid slab by the Chebyshev closed form (no Wigner-D, no CG): [npoints, twojmax+1];
+    with `sample` (flat point indices relative to the slab) only those points: [len(sample), twojmax+1]."""
     nx, ny, nz = (int(v) for v in ngrid)
     z_end = nz if z_end is None else int(z_end)
     args, keep = _sys_args(twojmax, rcutfac, rfac0, rmin0, wself, radelem, wj, pos, types, box, origin, pbc)
     ng = _i([nx, ny, nz])
-    out = np.zeros(((z_end - z_begin) * ny * nx, twojmax + 1))
-    rc = lib().oracle_bj0j_grid(*args, _p(ng, C.c_int), C.c_int(int(z_begin)), C.c_int(z_end), _p(out, C.c_double))
+    smp = None if sample is None else np.ascontiguousarray(sample, dtype=np.int64)
+    npts = (z_end - z_begin) * ny * nx if smp is None else smp.size
+    out = np.zeros((npts, twojmax + 1))
+    rc = lib().oracle_bj0j_grid(*args, _p(ng, C.c_int), C.c_int(int(z_begin)), C.c_int(z_end),
+                                C.c_long(0 if smp is None else smp.size), _p(smp, C.c_long), _p(out, C.c_double))
     if rc != 0:
         raise ValueError("oracle_bj0j_grid: invalid argument")
     return out

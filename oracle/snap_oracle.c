@@ -149,7 +149,8 @@ double oracle_cg(int J1, int M1, int J2, int M2, int J, int M)
 /* Pair geometry, SURVEY.md 8(c) step 5 / north_star.                   */
 /* d = R_neighbor - r_point.  Returns 0 if not a neighbor (r >= rcut).  */
 /* a = q0 - i q3, b = q2 - i q1, q = (cos th0, sin th0 * d/r).          */
-/* r -> 0 limit (reading #11): a = 1, b = 0, fc = 1.                    */
+/* r -> 0 limit (reading #11): a = 1, b = 0, fc = 1 (for rmin0 > 0 the  */
+/* direction is undefined at r = 0 and the same U = I is used).         */
 /* ------------------------------------------------------------------ */
 int oracle_pair(const double d[3], double rcut, double rfac0, double rmin0,
                 double ab[4] /* a.re a.im b.re b.im */, double *fc)
@@ -161,9 +162,11 @@ int oracle_pair(const double d[3], double rcut, double rfac0, double rmin0,
         *fc = 1.0;
         return 1;
     }
+    /* reading #22: for r <= rmin0 the switching function
+     * saturates at 1, while the theta0 map stays the same linear function of r
+     * (theta0 < 0 there); only rmin0 = 0 occurs in the five configs. */
     double x = (r - rmin0) / (rcut - rmin0);
-    if (x < 0.0) x = 0.0; /* r <= rmin0: switching function saturates at 1 */
-    *fc = 0.5 * (cos(M_PI * x) + 1.0);
+    *fc = (x <= 0.0) ? 1.0 : 0.5 * (cos(M_PI * x) + 1.0);
     double th0 = rfac0 * M_PI * x;
     double q0 = cos(th0), s = sin(th0);
     double q1 = s * d[0] / r, q2 = s * d[1] / r, q3 = s * d[2] / r;
@@ -551,11 +554,13 @@ int oracle_gaussian_points(double rcutfac, double sigma, int ntypes, const doubl
 /* (doubled j).  Needs neither Wigner-D nor Clebsch-Gordan, only the     */
 /* neighbor gather, f_c and the theta0 map -- cheap enough for whole     */
 /* grids.  Pinned against oracle_bispectrum_points (the Wigner-D / CG    */
-/* path) in tests/test_oracle_pins.py.  out[(z1-z0)*ny*nx][twojmax+1].   */
+/* path) in tests/test_oracle_pins.py.  out[(z1-z0)*ny*nx][twojmax+1],   */
+/* or out[nsample][twojmax+1] when a list of point indices is given.     */
 /* ------------------------------------------------------------------ */
 int oracle_bj0j_grid(int twojmax, double rcutfac, double rfac0, double rmin0, double wself, int ntypes, const double *radelem,
                      const double *wj, int natoms, const double *pos, const int *types, const double *box,
-                     const double *origin, const int *pbc, const int *ngrid, int z0, int z1, double *out)
+                     const double *origin, const int *pbc, const int *ngrid, int z0, int z1,
+                     long nsample, const long *sample /* optional flat point indices relative to the slab */, double *out)
 {
     if (twojmax < 0 || twojmax > ORACLE_MAX_TWOJ || ntypes < 1 || z0 < 0 || z1 > ngrid[2] || z0 > z1) return -1;
     sys_t s;
@@ -566,11 +571,12 @@ int oracle_bj0j_grid(int twojmax, double rcutfac, double rfac0, double rmin0, do
     if (sys_prepare(&s)) return -1;
     const double *a1 = box, *a2 = box + 3, *a3 = box + 6;
     const int nx = ngrid[0], ny = ngrid[1], nz = ngrid[2];
-    const long npts = (long)(z1 - z0) * ny * nx;
+    const long npts = nsample > 0 ? nsample : (long)(z1 - z0) * ny * nx;
     int bad = 0;
 #pragma omp parallel for schedule(dynamic, 64)
     for (long ip = 0; ip < npts; ip++) {
-        const int ix = (int)(ip % nx), iy = (int)((ip / nx) % ny), iz = z0 + (int)(ip / ((long)nx * ny));
+        const long fp = nsample > 0 ? sample[ip] : ip;
+        const int ix = (int)(fp % nx), iy = (int)((fp / nx) % ny), iz = z0 + (int)(fp / ((long)nx * ny));
         double rp[3];
         for (int k = 0; k < 3; k++)
             rp[k] = origin[k] + ((double)ix / nx) * a1[k] + ((double)iy / ny) * a2[k] + ((double)iz / nz) * a3[k];

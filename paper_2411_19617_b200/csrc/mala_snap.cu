@@ -44,21 +44,24 @@ static int fail(int code, const std::string &msg) {
 
 namespace {
 
+// Device buffer that only grows.  Tables are allocated once at create time (plain cudaMalloc); the per-call workspace
+// grows through the stream-ordered allocator on the caller's stream, so enlarging it inside an enqueue-only call neither
+// synchronises the device nor pulls memory from under kernels that are still queued on that stream.
 template <typename T>
 struct DevBuf {
     T *p = nullptr;
     size_t cap = 0;  // elements
-    int reserve(size_t n) {
+    bool pooled = false;
+    int reserve(size_t n, cudaStream_t st = nullptr, bool stream_ordered = false) {
         if (n <= cap) return 0;
-        if (p) cudaFree(p);
-        p = nullptr;
-        cap = 0;
+        release(st);
         size_t want = n + n / 4 + 16;
-        cudaError_t e = cudaMalloc((void **)&p, want * sizeof(T));
+        pooled = stream_ordered;
+        cudaError_t e = stream_ordered ? cudaMallocAsync((void **)&p, want * sizeof(T), st) : cudaMalloc((void **)&p, want * sizeof(T));
         if (e != cudaSuccess) {
             cudaGetLastError();
-            e = cudaMalloc((void **)&p, n * sizeof(T));
             want = n;
+            e = stream_ordered ? cudaMallocAsync((void **)&p, want * sizeof(T), st) : cudaMalloc((void **)&p, want * sizeof(T));
         }
         if (e != cudaSuccess) {
             cudaGetLastError();
@@ -68,8 +71,11 @@ struct DevBuf {
         cap = want;
         return 0;
     }
-    void release() {
-        if (p) cudaFree(p);
+    void release(cudaStream_t st = nullptr) {
+        if (p) {
+            if (pooled) cudaFreeAsync(p, st);
+            else cudaFree(p);
+        }
         p = nullptr;
         cap = 0;
     }
@@ -110,6 +116,10 @@ struct mala_snap {
     int cur = 0;  // buffer set of the current call
     std::vector<int> h_cell_start;
     DevBuf<int> d_cand, d_ncand, d_active, d_counters;
+    DevBuf<int> d_status;          // kStatus* bits raised by the kernels; never cleared by a chunk
+    int *h_status = nullptr;       // pinned mirror, refreshed at the end of every call
+    int sticky_status = 0;         // bits seen so far (a raised bit makes every later call fail)
+    int cand_cap_limit = 0;        // test hook: clamp the candidate capacity (0 = off) to provoke the overflow path
     DevBuf<double2> d_utot;
     DevBuf<double> d_stage[2];
     cudaStream_t copy_stream = nullptr;
@@ -325,37 +335,44 @@ int launch_zi(mala_snap *h, const ChunkBuffers &cb, double *out, cudaStream_t st
     return 0;
 }
 
-// B of a point without neighbors, computed by the same kernel that handles every other point
+// B of a point without neighbors, computed by the same kernel that handles every other point.  Set-up time only
+// (create, set_option): drains the device first, works on private temporaries and synchronises before returning.
 int compute_bconst(mala_snap *h) {
-    const int nelem = h->sc.nelem, nt = h->sc.ntriples;
-    std::vector<double2> u((size_t)nelem * 32);
+    const int nelem = h->sc.nelem, nt = h->sc.ntriples, P = kTilePoints;
+    CUDA_TRY(cudaDeviceSynchronize());
+    std::vector<double2> u((size_t)nelem * P);
     for (int e = 0; e < nelem; e++)
-        for (int l = 0; l < 32; l++) u[(size_t)e * 32 + l] = make_double2(h->tab.udiag[e] ? h->wself : 0.0, 0.0);
-    if (h->d_utot.reserve(u.size())) return fail(MALA_SNAP_ENOMEM, "cudaMalloc (utot) failed");
-    if (h->d_active.reserve(1) || h->d_counters.reserve(4) || h->d_bconst.reserve(nt)) return fail(MALA_SNAP_ENOMEM, "cudaMalloc failed");
+        for (int l = 0; l < P; l++) u[(size_t)e * P + l] = make_double2(h->tab.udiag[e] ? h->wself : 0.0, 0.0);
+    DevBuf<double2> t_utot;
+    DevBuf<int> t_active, t_counters;
     DevBuf<double> tmp;
-    if (tmp.reserve((size_t)32 * nt)) return fail(MALA_SNAP_ENOMEM, "cudaMalloc failed");
-    CUDA_TRY(cudaMemcpy(h->d_utot.p, u.data(), u.size() * sizeof(double2), cudaMemcpyHostToDevice));
+    auto cleanup = [&]() { t_utot.release(); t_active.release(); t_counters.release(); tmp.release(); };
+    if (t_utot.reserve(u.size()) || t_active.reserve(1) || t_counters.reserve(4) || tmp.reserve((size_t)32 * nt) || h->d_bconst.reserve(nt)) {
+        cleanup();
+        return fail(MALA_SNAP_ENOMEM, "cudaMalloc failed");
+    }
     const int zero = 0;
     const int counters[4] = {1, 0, 0, 0};
-    CUDA_TRY(cudaMemcpy(h->d_active.p, &zero, sizeof(int), cudaMemcpyHostToDevice));
-    CUDA_TRY(cudaMemcpy(h->d_counters.p, counters, sizeof(counters), cudaMemcpyHostToDevice));
+    cudaError_t e = cudaMemcpy(t_utot.p, u.data(), u.size() * sizeof(double2), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(t_active.p, &zero, sizeof(int), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(t_counters.p, counters, sizeof(counters), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { cleanup(); return fail(MALA_SNAP_ECUDA, std::string("compute_bconst: ") + cudaGetErrorString(e)); }
     GridGeom g{};
     g.a1[0] = g.a2[1] = g.a3[2] = 1.0;
-    g.nx = 4; g.ny = 4; g.nz = 2; g.z0 = 0; g.z1 = 2;
+    g.nx = 4; g.ny = 4; g.nz = P / 16; g.z0 = 0; g.z1 = P / 16;
     g.nreg = 1; g.total_tiles = 1;
-    g.reg[0].x0 = 0; g.reg[0].y0 = 0; g.reg[0].nxr = 4; g.reg[0].nyr = 4; g.reg[0].tx = 4; g.reg[0].ty = 4; g.reg[0].tz = 2;
+    g.reg[0].x0 = 0; g.reg[0].y0 = 0; g.reg[0].nxr = 4; g.reg[0].nyr = 4; g.reg[0].tx = 4; g.reg[0].ty = 4; g.reg[0].tz = P / 16;
     g.reg[0].ntx = g.reg[0].nty = g.reg[0].ntz = 1; g.reg[0].tile_begin = 0;
     const GridGeom saved = h->geom;
     h->geom = g;
     ChunkBuffers cb{};
-    cb.active = h->d_active.p; cb.counters = h->d_counters.p; cb.utot = h->d_utot.p; cb.tile_begin = 0; cb.ntiles = 1;
+    cb.active = t_active.p; cb.counters = t_counters.p; cb.status = h->d_status.p; cb.utot = t_utot.p; cb.tile_begin = 0; cb.ntiles = 1;
     int rc = launch_zi(h, cb, tmp.p, nullptr);
     h->geom = saved;
-    if (rc) { tmp.release(); return rc; }
-    cudaError_t e = cudaMemcpy(h->d_bconst.p, tmp.p, nt * sizeof(double), cudaMemcpyDeviceToDevice);
+    if (rc) { cleanup(); return rc; }
+    e = cudaMemcpy(h->d_bconst.p, tmp.p, nt * sizeof(double), cudaMemcpyDeviceToDevice);
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
-    tmp.release();
+    cleanup();
     if (e != cudaSuccess) return fail(MALA_SNAP_ECUDA, std::string("compute_bconst: ") + cudaGetErrorString(e));
     return 0;
 }
@@ -516,10 +533,14 @@ int build_plan(mala_snap *h, const CallArgs &a, cudaStream_t st) {
         std::vector<int> fill(start.begin(), start.end() - 1);
         for (size_t i = 0; i < ng; i++) sorted[fill[cell_of[i]]++] = ghosts[i];
     }
+    // The workspace (U_tot, candidate lists, counters) is one set per handle: a call on another stream must not start
+    // before the previous call on this handle has drained (calls on one handle are serialised, whatever their streams).
+    if (h->call_done_valid[cur ^ 1]) CUDA_TRY(cudaStreamWaitEvent(st, h->ev_call_done[cur ^ 1], 0));
     // upload on the private stream once the call that last used this buffer set has drained
     if (h->call_done_valid[cur]) CUDA_TRY(cudaStreamWaitEvent(h->upload_stream, h->ev_call_done[cur], 0));
-    if (h->d_ghosts[cur].reserve(std::max<size_t>(ng, 1)) || h->d_cell_start[cur].reserve(ncell + 1))
-        return fail(MALA_SNAP_ENOMEM, "cudaMalloc (ghosts) failed");
+    if (h->d_ghosts[cur].reserve(std::max<size_t>(ng, 1), h->upload_stream, true) ||
+        h->d_cell_start[cur].reserve(ncell + 1, h->upload_stream, true))
+        return fail(MALA_SNAP_ENOMEM, "cudaMallocAsync (ghosts) failed");
     if (ng) CUDA_TRY(cudaMemcpyAsync(h->d_ghosts[cur].p, sorted.data(), ng * sizeof(Ghost), cudaMemcpyHostToDevice, h->upload_stream));
     CUDA_TRY(cudaMemcpyAsync(h->d_cell_start[cur].p, start.data(), (ncell + 1) * sizeof(int), cudaMemcpyHostToDevice, h->upload_stream));
     // (pageable sources: cudaMemcpyAsync returns only after they have been staged, so they may die with this scope)
@@ -644,7 +665,9 @@ int candidate_bound(const mala_snap *h) {
             }
     best = std::max<long long>(best, 1);
     best = (best + 31) / 32 * 32;
-    return (int)std::min<long long>(best, 1 << 24);
+    if (best > (1 << 24)) return -1;  // caller reports it: no silent clamp
+    if (h->cand_cap_limit > 0) best = std::min<long long>(best, h->cand_cap_limit);  // test hook (provokes kStatusCandOverflow)
+    return (int)best;
 }
 
 // enqueue the whole path for the slab [z0, z1) into out (DEVICE, relative to z0); out == nullptr: stop after compute_ui
@@ -654,15 +677,16 @@ int run_slab(mala_snap *h, int z0, int z1, double *out, double2 *u_out, cudaStre
     choose_tiles(h, z0, z1);
     GridGeom &g = h->geom;
     h->cand_cap = candidate_bound(h);
+    if (h->cand_cap < 0) return fail(MALA_SNAP_EINVAL, "more than 2^24 candidate atoms per tile; use a finer cell or smaller z-slabs");
     const long long total_tiles = h->total_tiles;
     if (total_tiles > 2000000000LL) return fail(MALA_SNAP_EINVAL, "slab has too many tiles; use smaller z-slabs");
     const size_t per_tile = (size_t)h->sc.nelem * 32 * sizeof(double2) + (size_t)h->cand_cap * sizeof(int) + 2 * sizeof(int);
     const size_t budget = (size_t)std::max<long long>(h->workspace_mb, 1) << 20;
     long long chunk_tiles = (long long)std::max<size_t>(budget / per_tile, (size_t)h->num_sms);
     chunk_tiles = std::min(chunk_tiles, total_tiles);
-    if (h->d_utot.reserve((size_t)chunk_tiles * h->sc.nelem * 32) || h->d_cand.reserve((size_t)chunk_tiles * h->cand_cap) ||
-        h->d_ncand.reserve(chunk_tiles) || h->d_active.reserve(chunk_tiles) || h->d_counters.reserve(4))
-        return fail(MALA_SNAP_ENOMEM, "cudaMalloc (workspace) failed");
+    if (h->d_utot.reserve((size_t)chunk_tiles * h->sc.nelem * 32, st, true) || h->d_cand.reserve((size_t)chunk_tiles * h->cand_cap, st, true) ||
+        h->d_ncand.reserve(chunk_tiles, st, true) || h->d_active.reserve(chunk_tiles, st, true) || h->d_counters.reserve(4, st, true))
+        return fail(MALA_SNAP_ENOMEM, "cudaMallocAsync (workspace) failed");
     h->stats[4] = h->cand_cap;
     h->stats[5] = (long long)(per_tile * (size_t)chunk_tiles);
     const DeviceTables tb = h->tables();
@@ -670,6 +694,7 @@ int run_slab(mala_snap *h, int z0, int z1, double *out, double2 *u_out, cudaStre
         ChunkBuffers cb{};
         cb.ghosts = h->d_ghosts[h->cur].p; cb.cell_start = h->d_cell_start[h->cur].p;
         cb.cand = h->d_cand.p; cb.ncand = h->d_ncand.p; cb.active = h->d_active.p; cb.counters = h->d_counters.p;
+        cb.status = h->d_status.p;
         cb.utot = h->d_utot.p; cb.cand_cap = h->cand_cap;
         cb.tile_begin = (int)t0;
         cb.ntiles = (int)std::min(chunk_tiles, total_tiles - t0);
@@ -713,15 +738,16 @@ int run_slab_gauss(mala_snap *h, int z0, int z1, double sigma, double *out, cuda
     choose_tiles(h, z0, z1);
     GridGeom &g = h->geom;
     h->cand_cap = candidate_bound(h);
+    if (h->cand_cap < 0) return fail(MALA_SNAP_EINVAL, "more than 2^24 candidate atoms per tile; use a finer cell or smaller z-slabs");
     const long long total_tiles = h->total_tiles;
     if (total_tiles > 2000000000LL) return fail(MALA_SNAP_EINVAL, "slab has too many tiles; use smaller z-slabs");
     const size_t per_tile = (size_t)h->cand_cap * sizeof(int) + 2 * sizeof(int);
     const size_t budget = (size_t)std::max<long long>(h->workspace_mb, 1) << 20;
     long long chunk_tiles = (long long)std::max<size_t>(budget / per_tile, (size_t)h->num_sms);
     chunk_tiles = std::min(chunk_tiles, total_tiles);
-    if (h->d_cand.reserve((size_t)chunk_tiles * h->cand_cap) || h->d_ncand.reserve(chunk_tiles) || h->d_active.reserve(chunk_tiles) ||
-        h->d_counters.reserve(4))
-        return fail(MALA_SNAP_ENOMEM, "cudaMalloc (workspace) failed");
+    if (h->d_cand.reserve((size_t)chunk_tiles * h->cand_cap, st, true) || h->d_ncand.reserve(chunk_tiles, st, true) ||
+        h->d_active.reserve(chunk_tiles, st, true) || h->d_counters.reserve(4, st, true))
+        return fail(MALA_SNAP_ENOMEM, "cudaMallocAsync (workspace) failed");
     const double pi = 3.14159265358979323846;
     const double pref = 1.0 / (std::pow(2.0 * pi, 1.5) * sigma * sigma * sigma), inv2s2 = 1.0 / (2.0 * sigma * sigma);
     const DeviceTables tb = h->tables();
@@ -729,6 +755,7 @@ int run_slab_gauss(mala_snap *h, int z0, int z1, double sigma, double *out, cuda
         ChunkBuffers cb{};
         cb.ghosts = h->d_ghosts[h->cur].p; cb.cell_start = h->d_cell_start[h->cur].p;
         cb.cand = h->d_cand.p; cb.ncand = h->d_ncand.p; cb.active = h->d_active.p; cb.counters = h->d_counters.p;
+        cb.status = h->d_status.p;
         cb.cand_cap = h->cand_cap;
         cb.tile_begin = (int)t0;
         cb.ntiles = (int)std::min(chunk_tiles, total_tiles - t0);
@@ -754,8 +781,26 @@ int run_slab_gauss(mala_snap *h, int z0, int z1, double sigma, double *out, cuda
 }
 
 int finish_call(mala_snap *h, cudaStream_t st) {
+    // the status word travels back with every call: one 4-byte copy into pinned memory, ordered before ev_call_done
+    CUDA_TRY(cudaMemcpyAsync(h->h_status, h->d_status.p, sizeof(int), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaEventRecord(h->ev_call_done[h->cur], st));
     h->call_done_valid[h->cur] = true;
+    return 0;
+}
+
+// Status of the calls issued so far.  wait = false: looks only at calls that have already drained (used at the start of an
+// enqueue-only call, which must not block); wait = true: waits for the last call first.  A raised bit is sticky.
+int check_status(mala_snap *h, bool wait) {
+    const int last = (int)((h->ncalls + 1ull) & 1ull);  // buffer set of the most recent call
+    if (h->ncalls > 0 && h->call_done_valid[last]) {
+        cudaError_t e = wait ? cudaEventSynchronize(h->ev_call_done[last]) : cudaEventQuery(h->ev_call_done[last]);
+        if (e == cudaSuccess) h->sticky_status |= *(volatile int *)h->h_status;
+        else if (e != cudaErrorNotReady) return fail(MALA_SNAP_ECUDA, std::string("status check: ") + cudaGetErrorString(e));
+        else cudaGetLastError();
+    }
+    if (h->sticky_status & kStatusCandOverflow)
+        return fail(MALA_SNAP_ECUDA, "candidate overflow: tile_bin_kernel truncated a neighbor-candidate list in an earlier call on this "
+                                     "handle (its results are invalid); the host bound was violated");
     return 0;
 }
 
@@ -953,6 +998,18 @@ int mala_snap_create(mala_snap_t **handle, int twojmax, double rcutfac, double r
         }
         build_diag_schedule(h);
         if ((rc = set_kernel_attributes(h))) return rc;
+        if (h->d_status.reserve(1)) return fail(MALA_SNAP_ENOMEM, "cudaMalloc (status) failed");
+        CUDA_TRY(cudaMemset(h->d_status.p, 0, sizeof(int)));
+        CUDA_TRY(cudaMallocHost((void **)&h->h_status, sizeof(int)));
+        *h->h_status = 0;
+        {   // keep freed workspace blocks in the stream-ordered pool instead of returning them to the driver at every sync
+            cudaMemPool_t pool = nullptr;
+            if (cudaDeviceGetDefaultMemPool(&pool, h->device) == cudaSuccess) {
+                unsigned long long keep = ~0ull;
+                cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+            }
+            cudaGetLastError();
+        }
         CUDA_TRY(cudaStreamCreateWithFlags(&h->upload_stream, cudaStreamNonBlocking));
         CUDA_TRY(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
         CUDA_TRY(cudaEventCreateWithFlags(&h->ev_upload, cudaEventDisableTiming));
@@ -1004,6 +1061,11 @@ int mala_snap_set_option(mala_snap_t *h, const char *name, long long value) {
         h->workspace_mb = value;
         return MALA_SNAP_OK;
     }
+    if (n == "cand_cap_limit") {  // test hook: see mala_snap.h
+        if (value < 0 || value > (1 << 24)) return fail(MALA_SNAP_EINVAL, "cand_cap_limit must lie in [0, 2^24]");
+        h->cand_cap_limit = (int)value;
+        return MALA_SNAP_OK;
+    }
     if (n == "host_chunk_mb") {
         if (value < 1) return fail(MALA_SNAP_EINVAL, "host_chunk_mb must be >= 1");
         h->host_chunk_mb = value;
@@ -1012,10 +1074,12 @@ int mala_snap_set_option(mala_snap_t *h, const char *name, long long value) {
     return fail(MALA_SNAP_EINVAL, "unknown option: " + n);
 }
 
-int mala_snap_last_stats(const mala_snap_t *h, long long stats[8]) {
+int mala_snap_last_stats(mala_snap_t *h, long long stats[8]) {
     if (!h || !stats) return fail(MALA_SNAP_EINVAL, "handle or stats is NULL");
+    const int rc = check_status(h, true);  // waits for the last call: its status word is part of the answer
+    h->stats[7] = h->sticky_status;
     for (int i = 0; i < 8; i++) stats[i] = h->stats[i];
-    return MALA_SNAP_OK;
+    return rc;
 }
 
 int mala_snap_kernel_times(mala_snap_t *h, double ms[4], long long launches[4]) {
@@ -1029,6 +1093,11 @@ int mala_snap_kernel_times(mala_snap_t *h, double ms[4], long long launches[4]) 
         launches[s.kind]++;
     }
     return MALA_SNAP_OK;
+}
+
+const char *mala_snap_zi_kernel(const mala_snap_t *h) {
+    if (!h) return "";
+    return h->use_diag() ? "compute_zi_bi_diag_kernel" : (h->use_spec() ? "compute_zi_bi_coop_kernel" : "compute_zi_bi_generic_kernel");
 }
 
 int mala_snap_fp64_peak(double *tflops, double *sm_mhz_effective, void *cuda_stream) {
@@ -1069,6 +1138,7 @@ int mala_bispectrum_grid(mala_snap_t *h, int natoms, const double *pos, const in
     const CallArgs a{natoms, pos, types, box, origin, pbc, ngrid, z_begin, z_end};
     int rc = validate(h, a, true, out);
     if (rc) return rc;
+    if ((rc = check_status(h, false))) return rc;
     std::fill(h->stats, h->stats + 8, 0LL);
     if (z_end == z_begin) return MALA_SNAP_OK;
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -1083,6 +1153,7 @@ int mala_bispectrum_grid_host(mala_snap_t *h, int natoms, const double *pos, con
     const CallArgs a{natoms, pos, types, box, origin, pbc, ngrid, z_begin, z_end};
     int rc = validate(h, a, true, out_host);
     if (rc) return rc;
+    if ((rc = check_status(h, false))) return rc;
     std::fill(h->stats, h->stats + 8, 0LL);
     if (z_end == z_begin) return MALA_SNAP_OK;
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -1096,7 +1167,7 @@ int mala_bispectrum_grid_host(mala_snap_t *h, int natoms, const double *pos, con
     if (total * sizeof(double) > ((size_t)96 << 20)) planes = std::min(planes, (z_end - z_begin + 2) / 3);
     if (planes >= 8) planes = planes / 8 * 8;  // whole tiles for every tile shape
     for (int b = 0; b < 2; b++)
-        if (h->d_stage[b].reserve(plane * planes)) return fail(MALA_SNAP_ENOMEM, "cudaMalloc (staging) failed");
+        if (h->d_stage[b].reserve(plane * planes, st, true)) return fail(MALA_SNAP_ENOMEM, "cudaMallocAsync (staging) failed");
     bool used[2] = {false, false};
     int i = 0;
     for (int z = z_begin; z < z_end; z += planes, i++) {
@@ -1114,7 +1185,7 @@ int mala_bispectrum_grid_host(mala_snap_t *h, int natoms, const double *pos, con
     if ((rc = finish_call(h, st))) return rc;
     CUDA_TRY(cudaStreamSynchronize(h->copy_stream));
     CUDA_TRY(cudaStreamSynchronize(st));
-    return MALA_SNAP_OK;
+    return check_status(h, true);
 }
 
 int mala_gaussian_grid(mala_snap_t *h, double sigma, int natoms, const double *pos, const int *types, const double box[9],
@@ -1123,6 +1194,7 @@ int mala_gaussian_grid(mala_snap_t *h, double sigma, int natoms, const double *p
     const CallArgs a{natoms, pos, types, box, origin, pbc, ngrid, z_begin, z_end};
     int rc = validate(h, a, true, out);
     if (rc) return rc;
+    if ((rc = check_status(h, false))) return rc;
     if (!(sigma > 0.0) || !std::isfinite(sigma)) return fail(MALA_SNAP_EINVAL, "sigma must be positive");
     if (h->ntypes > kGaussMaxTypes) return fail(MALA_SNAP_EINVAL, "mala_gaussian_grid supports at most 4 atom types");
     std::fill(h->stats, h->stats + 8, 0LL);
@@ -1139,6 +1211,7 @@ int mala_snap_debug_utot(mala_snap_t *h, int natoms, const double *pos, const in
     const CallArgs a{natoms, pos, types, box, origin, pbc, ngrid, z_begin, z_end};
     int rc = validate(h, a, true, u_out);
     if (rc) return rc;
+    if ((rc = check_status(h, false))) return rc;
     std::fill(h->stats, h->stats + 8, 0LL);
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (z_end > z_begin) {
@@ -1147,6 +1220,7 @@ int mala_snap_debug_utot(mala_snap_t *h, int natoms, const double *pos, const in
         if ((rc = finish_call(h, st))) return rc;
     }
     CUDA_TRY(cudaStreamSynchronize(st));
+    if ((rc = check_status(h, true))) return rc;
     return h->sc.nelem;
 }
 
@@ -1163,6 +1237,8 @@ void mala_snap_destroy(mala_snap_t *h) {
         if (h->ev_copied[i]) cudaEventDestroy(h->ev_copied[i]);
     }
     h->d_cand.release(); h->d_ncand.release(); h->d_active.release(); h->d_counters.release(); h->d_utot.release();
+    h->d_status.release();
+    if (h->h_status) cudaFreeHost(h->h_status);
     for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
     if (h->ev_upload) cudaEventDestroy(h->ev_upload);
     if (h->upload_stream) cudaStreamDestroy(h->upload_stream);

@@ -66,12 +66,15 @@ struct ChunkBuffers {
     int *cand;               // [chunk_tiles * cand_cap] ghost indices per tile
     int *ncand;              // [chunk_tiles]
     int *active;             // [chunk_tiles] compacted list of non-empty tiles (local tile ids)
-    int *counters;           // [0] number of active tiles, [1] ui work counter, [2] zi work counter
+    int *counters;           // [0] number of active tiles, [1] ui work counter, [2] zi work counter (zeroed per chunk)
+    int *status;             // handle-wide status word, never cleared by a chunk: kStatus* bits
     double2 *utot;           // [chunk_tiles][nelem][32]
     int cand_cap;
     int tile_begin;          // first global tile id of the chunk
     int ntiles;              // tiles in the chunk
 };
+
+constexpr int kStatusCandOverflow = 1;  // tile_bin_kernel had to truncate a candidate list (host bound violated)
 
 // one tile: its first grid point, its shape, and the end of its region (points beyond it do not belong to the tile)
 struct TileInfo {

@@ -90,8 +90,8 @@ __global__ void __launch_bounds__(256) tile_bin_kernel(GridGeom g, SnapConst sc,
                 }
             }
     }
-    if (n > cb.cand_cap) {  // cannot happen when the host bound is right; flagged, never silent
-        if (lane == 0) atomicExch(&cb.counters[3], 1);
+    if (n > cb.cand_cap) {  // cannot happen when the host bound is right: raise the handle's status word (read back by the host)
+        if (lane == 0) atomicOr(cb.status, kStatusCandOverflow);
         n = cb.cand_cap;
     }
     if (lane == 0) cb.ncand[wt] = n;
@@ -207,9 +207,9 @@ __device__ __forceinline__ void pair_geometry(const double dx, const double dy, 
         c = w; ar = 1.0; ai = 0.0; br = 0.0; bi = 0.0;
         return;
     }
-    double x = (r - rmin0) / (rcut - rmin0);
-    x = fmax(x, 0.0);
-    c = w * 0.5 * (cospi(x) + 1.0);
+    // reading #22: inside rmin0 the switching function saturates at 1; the theta0 map stays linear in r (theta0 < 0 there)
+    const double x = (r - rmin0) / (rcut - rmin0);
+    c = (x <= 0.0) ? w : w * 0.5 * (cospi(x) + 1.0);
     double s, co;
     sincospi(rfac0 * x, &s, &co);
     const double sr = s / r;

@@ -20,7 +20,7 @@ MALA_SNAP_ENOMEM = -3
 
 EXPORTS = ("mala_snap_create", "mala_snap_ncomp", "mala_snap_triples", "mala_bispectrum_grid", "mala_bispectrum_grid_host",
            "mala_gaussian_grid",
-           "mala_snap_set_option", "mala_snap_last_stats", "mala_snap_kernel_times", "mala_snap_fp64_peak", "mala_snap_clebsch_gordan", "mala_snap_debug_utot",
+           "mala_snap_set_option", "mala_snap_last_stats", "mala_snap_kernel_times", "mala_snap_zi_kernel", "mala_snap_fp64_peak", "mala_snap_clebsch_gordan", "mala_snap_debug_utot",
            "mala_snap_destroy", "mala_last_error")
 
 
@@ -70,6 +70,8 @@ def load_library():
     lib.mala_snap_last_stats.argtypes = [vp, C.POINTER(C.c_longlong)]
     lib.mala_snap_kernel_times.restype = C.c_int
     lib.mala_snap_kernel_times.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
+    lib.mala_snap_zi_kernel.restype = C.c_char_p
+    lib.mala_snap_zi_kernel.argtypes = [vp]
     lib.mala_snap_fp64_peak.restype = C.c_int
     lib.mala_snap_fp64_peak.argtypes = [dp, dp, vp]
     lib.mala_snap_clebsch_gordan.restype = C.c_double
@@ -167,8 +169,11 @@ class MalaSnap:
     def last_stats(self):
         st = (C.c_longlong * 8)()
         _check(self._lib.mala_snap_last_stats(self._h, st))
-        keys = ("kernels", "chunks", "tiles", "ghosts", "cand_cap", "workspace_bytes", "points", "reserved")
+        keys = ("kernels", "chunks", "tiles", "ghosts", "cand_cap", "workspace_bytes", "points", "status")
         return dict(zip(keys, [int(x) for x in st]))
+
+    def zi_kernel_name(self):
+        return self._lib.mala_snap_zi_kernel(self._h).decode()
 
     def kernel_times(self):
         """{class: (ms, launches)} of the last call; needs set_option("timing", 1) before it."""

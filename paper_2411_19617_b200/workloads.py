@@ -144,11 +144,35 @@ def be_slab(seed=1005, ncell=(16, 16, 16), spacing=0.2):
                           "plane (reading #19), sigma=0.05, grid spacing ~0.2 A")
 
 
+def solid_al_200(seed=1002):
+    """paper-scale grid for the same 256-atom cell: 200^3 = 8.0e6 points (Tab. 5)"""
+    w = solid_al(seed, ngrid=(200, 200, 200))
+    w.name = "solid_al_200cube"
+    w.notes = "256-atom 4x4x4 fcc Al, sigma=0.1, 200^3 grid (8.0e6 points: the grid of the paper's 256-atom Al runs, Tab. 5)"
+    return w
+
+
+def binary_alloy(seed=1006, ngrid=(90, 90, 90)):
+    """two species with distinct radii and weights (PAPER.md:252 per-species cutoff R^eta, weights w_eta of Eq. (24)):
+    the 256-site fcc cell of config 2 with every site assigned type 0 or 1 by a seeded coin; rcut = 4.676 / 3.74 A."""
+    a = 4.05
+    rng = _Rng(seed)
+    pos = _fcc(4, a) + 0.1 * rng.normal((256, 3))
+    types = (rng.uniform(256) < 0.5).astype(np.int32)
+    return Workload("binary_alloy", pos, types, np.eye(3) * 4 * a, (1, 1, 1), tuple(ngrid), 4.676, radelem=(0.5, 0.4), wj=(1.0, 0.6),
+                    seed=seed, notes="256-site fcc cell, two species by a seeded coin: radelem (0.5, 0.4), wj (1.0, 0.6), 90^3 grid")
+
+
 CONFIGS = {
     1: tiny_al, 2: solid_al, 3: liquid_al, 4: boron_cluster, 5: be_slab,
     "tiny_al": tiny_al, "solid_al": solid_al, "liquid_al": liquid_al, "boron_cluster": boron_cluster, "be_slab": be_slab,
+    "200cube": solid_al_200, "binary": binary_alloy,
 }
 
 
-def make(config, **kw):
-    return CONFIGS[config](**kw)
+def make(config, twojmax=None, **kw):
+    """config: 1..5 (BASELINE.json `configs`), "200cube" or "binary"; twojmax overrides the default 10."""
+    w = CONFIGS[config](**kw)
+    if twojmax is not None:
+        w.twojmax = int(twojmax)
+    return w

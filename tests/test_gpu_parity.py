@@ -246,6 +246,81 @@ def test_atom_exactly_on_a_grid_point_and_at_the_cutoff():
     assert_parity(got.cpu().numpy(), ref)
 
 
+def test_neighbor_inside_rmin0_reading22():
+    """reading #22: f_c saturates at 1 and theta0 turns negative for r < rmin0 (pinned on the oracle side by closed forms)"""
+    torch = _torch()
+    box = np.eye(3) * 6.0
+    ngrid = (6, 6, 6)
+    pos = np.array([[1.0 + 0.12, 2.0 - 0.1, 3.0 + 0.12],   # 0.197 from grid point (1,2,3): inside rmin0 = 0.3
+                    [4.0, 4.0 + 0.31, 1.0],                # just outside rmin0 of grid point (4,4,1)
+                    [2.5, 2.6, 0.4], [5.1, 0.3, 3.3]])
+    types = np.array([0, 1, 0, 1], np.int32)
+    params = dict(twojmax=8, rcutfac=2.6, rmin0=0.3, wself=0.9, radelem=(0.5, 0.45), wj=(1.0, 0.7))
+    ref = oracle.bispectrum_grid(pos, types, box, (0, 0, 0), (1, 1, 1), ngrid, **params)
+    with MalaSnap(**params) as snap:
+        got = snap.bispectrum_grid(pos, types, box, ngrid=ngrid)
+        torch.cuda.synchronize()
+    assert_parity(got.cpu().numpy(), ref)
+
+
+def test_candidate_overflow_is_reported_not_silent():
+    """the per-tile candidate capacity is an exact host bound; if it is ever violated (forced here through the test hook) the
+    truncation must surface as an error code, both from the status query and from the next call on the handle"""
+    torch = _torch()
+    w = workloads.make(1)
+    with MalaSnap(**w.snap_params()) as snap:
+        ok = snap.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid)
+        assert snap.last_stats()["status"] == 0 and snap.last_stats()["cand_cap"] > 32
+        snap.set_option("cand_cap_limit", 32)
+        snap.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, out=ok)   # enqueued; overflows on the device
+        with pytest.raises(MalaSnapError) as e:
+            snap.last_stats()
+        assert e.value.code == -2 and "overflow" in str(e.value)
+        snap.set_option("cand_cap_limit", 0)
+        with pytest.raises(MalaSnapError) as e:      # sticky: the handle refuses further work
+            snap.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, out=ok)
+        assert e.value.code == -2
+        with pytest.raises(MalaSnapError):
+            snap.bispectrum_grid_host(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid)
+    torch.cuda.synchronize()
+    with MalaSnap(**w.snap_params()) as snap:       # a fresh handle is healthy; the host entry point reports it on return
+        snap.set_option("cand_cap_limit", 32)
+        with pytest.raises(MalaSnapError) as e:
+            snap.bispectrum_grid_host(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid)
+        assert e.value.code == -2
+
+
+def test_calls_on_two_streams_and_two_handles_do_not_interfere(tiny_ref):
+    """one handle used from two streams back to back (serialised on the device by the library), interleaved with a second
+    handle of another twojmax on a third stream: every result equals its stand-alone value bit for bit"""
+    torch = _torch()
+    w, ref = tiny_ref
+    pos, types, box, origin, pbc, ngrid, params = _small_case(5, 6, 5, (1, 1, 1), True, True, ngrid=(11, 9, 10))
+    s1, s2, s3 = torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()
+    with MalaSnap(**w.snap_params()) as a, MalaSnap(**params) as b, MalaSnap(**{**params, "twojmax": 8}) as c:
+        alone_a = a.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid).clone()
+        alone_b = b.bispectrum_grid(pos, types, box, origin, pbc, ngrid).clone()
+        alone_c = c.bispectrum_grid(pos, types, box, origin, pbc, ngrid).clone()
+        torch.cuda.synchronize()
+        outs = []
+        for it in range(3):
+            oa1 = torch.empty_like(alone_a); oa2 = torch.empty_like(alone_a)
+            ob = torch.empty_like(alone_b); oc = torch.empty_like(alone_c)
+            a.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, out=oa1, stream=s1)
+            b.bispectrum_grid(pos, types, box, origin, pbc, ngrid, out=ob, stream=s3)
+            a.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, 0, 9, out=oa2, stream=s2)
+            c.bispectrum_grid(pos, types, box, origin, pbc, ngrid, out=oc, stream=s1)
+            outs.append((oa1, oa2, ob, oc))
+        torch.cuda.synchronize()
+        n9 = 9 * w.ngrid[0] * w.ngrid[1]
+        part = a.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, 0, 9)
+        torch.cuda.synchronize()
+        for oa1, oa2, ob, oc in outs:
+            assert torch.equal(oa1, alone_a) and torch.equal(ob, alone_b) and torch.equal(oc, alone_c)
+            assert torch.equal(oa2[:n9], part)
+    assert_parity(alone_a.cpu().numpy(), ref)
+
+
 def test_invalid_arguments_are_rejected_without_enqueueing():
     torch = _torch()
     w = workloads.make(1)
@@ -310,6 +385,24 @@ def test_config2_solid_al_full_size_sampled():
     assert np.abs(part2 - part[:plane]).max() <= 1e-11 * np.abs(part).max()
 
 
+def test_config2_multi_chunk_workspace_is_bit_identical():
+    """the workspace-capped chunk loop at real size: 1 GiB cap -> >= 3 chunks of the 90^3 grid, same tiles, same bits"""
+    torch = _torch()
+    w = workloads.make(2)
+    with MalaSnap(**w.snap_params()) as snap:
+        one = snap.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid)
+        assert snap.last_stats()["chunks"] == 1
+        snap.set_option("workspace_mb", 1024)
+        many = snap.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid)
+        st = snap.last_stats()
+        assert st["chunks"] >= 3 and st["workspace_bytes"] <= 1024 << 20
+        assert torch.equal(one, many)
+        snap.set_option("workspace_mb", 300)
+        many = snap.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid)
+        assert snap.last_stats()["chunks"] >= 10
+        assert torch.equal(one, many)
+
+
 def test_config3_liquid_al_full_size_sampled():
     w = workloads.make(3)
     got = gpu_grid(w)
@@ -367,3 +460,42 @@ def test_config5_be_slab_z_slabs_sampled():
             if z0 == 140:  # one complete plane through the stacking fault against the Chebyshev closed form
                 _bj0j_full_grid(w, got[3 * ny * nx:4 * ny * nx], 143, 144)
             del out
+
+
+def test_config5_whole_grid_streamed_to_host():
+    """north_star: "fp64 output streamed in z-slabs" -- the WHOLE 183 x 317 x 287 grid (16.6 M points, 12.1 GB) through
+    mala_bispectrum_grid_host into one host buffer.  Checked with the stratified sample of SURVEY.md 8(d): the closed-form
+    second oracle (11 components B_{j,0,j}) on every 8th z-plane plus the planes at both fault interfaces, and 2,000 seeded
+    random points on all 91 components against the full oracle."""
+    torch = _torch()
+    w = workloads.make(5)
+    nx, ny, nz = w.ngrid
+    plane = nx * ny
+    try:
+        host = torch.empty((w.npoints, 91), dtype=torch.float64, pin_memory=True)
+    except RuntimeError:
+        host = torch.empty((w.npoints, 91), dtype=torch.float64)
+    host[::plane].fill_(float("nan"))
+    with MalaSnap(**w.snap_params()) as snap:
+        snap.bispectrum_grid_host(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, out=host)
+        st = snap.last_stats()
+    assert st["status"] == 0
+    got = host.numpy()
+    assert np.isfinite(got[::plane]).all() and np.isfinite(got[-1]).all()
+    # the two fault interfaces: basal layers 15|16 (middle of the cell) and 31|0 (periodic boundary), c/2 = 1.792 A per layer.
+    # The oracle visits all 16,384 atoms x 125 images per point (~20 ms of one core), so complete planes are checked at the two
+    # interfaces and 500 seeded points in every 8th plane and in the planes next to the interfaces.
+    zf = int(round(16 * 1.792 / 57.344 * nz))
+    for z in (zf, 0):
+        _bj0j_full_grid(w, got[z * plane:(z + 1) * plane], z, z + 1)
+    rng = np.random.default_rng(555)
+    tr = oracle.triples(10)
+    idx = [int(np.where((tr[:, 0] == j) & (tr[:, 1] == 0) & (tr[:, 2] == j))[0][0]) for j in range(11)]
+    for z in sorted(set(range(0, nz, 8)) | {zf - 1, zf + 1, nz - 1}):
+        smp = np.unique(np.concatenate([rng.integers(0, plane, 500), [0, nx - 1, plane - nx, plane - 1]]))
+        ref = oracle.bj0j_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, z, z + 1, sample=smp, **w.snap_params())
+        sub = got[z * plane + smp][:, idx]
+        assert (np.abs(sub - ref).max(axis=0) <= TOL * np.abs(ref).max(axis=0)).all(), z
+    sample = np.unique(np.concatenate([rng.integers(0, w.npoints, 2000), [0, w.npoints - 1]]))
+    ref = oracle_grid(w, sample=sample)
+    assert_parity(got[sample], ref)

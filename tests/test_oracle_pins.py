@@ -39,8 +39,11 @@ def brute_neighbors(point, pos, types, box, origin, pbc, rcut_t, nimg=4):
 
 
 def fc_theta(r, rcut, rmin0=0.0):
+    """(f_c, theta0), written from DESIGN.md readings #3, #4 and #22: the switching function saturates at 1 for
+    r <= rmin0, the theta0 map is linear in r throughout (negative below rmin0)."""
     x = (r - rmin0) / (rcut - rmin0)
-    return 0.5 * (np.cos(np.pi * x) + 1.0), RFAC0 * np.pi * x
+    fc = 1.0 if x <= 0.0 else 0.5 * (np.cos(np.pi * x) + 1.0)
+    return fc, RFAC0 * np.pi * x
 
 
 def rand_unit_quat(rng):
@@ -208,14 +211,14 @@ def test_B000_closed_form_twojmax0_periodic_two_types():
         np.testing.assert_allclose(B[0], s ** 3, rtol=1e-13)
 
 
-def chebyshev_bj0j(point, pos, types, box, origin, pbc, rcut_t, wj, wself, twojmax):
+def chebyshev_bj0j(point, pos, types, box, origin, pbc, rcut_t, wj, wself, twojmax, rmin0=0.0):
     """B_{j,0,j} = (sum_k c_k) * sum_{k,l} c_k c_l U_j(<q_k,q_l>), k,l over the self term and all neighbors
     (SURVEY.md 8(c)); needs neither Wigner-D nor CG."""
     nb = brute_neighbors(point, pos, types, box, origin, pbc, rcut_t)
     cs, qs = [wself], [np.array([1.0, 0, 0, 0])]
     for d, t in nb:
         r = np.linalg.norm(d)
-        fc, th0 = fc_theta(r, rcut_t[t])
+        fc, th0 = fc_theta(r, rcut_t[t], rmin0)
         cs.append(wj[t] * fc)
         qs.append(np.concatenate([[np.cos(th0)], np.sin(th0) * d / r]))
     cs, qs = np.array(cs), np.array(qs)
@@ -248,6 +251,48 @@ def test_chebyshev_closed_form_for_Bj0j(case):
         ref, n_ref = chebyshev_bj0j(p, pos, types, box, origin, pbc, rcut_t, wj, 1.0, 10)
         assert nn == n_ref and nn > 0
         np.testing.assert_allclose(B[idx], ref, rtol=1e-11)
+
+
+def test_rmin0_branch_B000_and_Bj0j_closed_forms():
+    """reading #22 (rmin0 != 0): f_c = 1 and theta0 < 0 for a neighbor inside rmin0.  Pinned by the two closed forms with an
+    independent numpy neighbor list: B_000 = (wself + sum w f_c)^3 sees the saturation of f_c, the Chebyshev form of
+    B_{j,0,j} sees the sign of theta0 through the quaternion dot products with the other neighbors."""
+    rng = np.random.default_rng(21)
+    rmin0, rcutfac, wself = 0.3, 3.9, 1.3
+    radelem, wj = (0.5, 0.4), (1.0, 0.6)
+    rcut_t = [2 * rcutfac * x for x in radelem]
+    pts = np.array([[25.0, 25.0, 25.0], [25.4, 24.8, 25.1]])
+    # neighbors of the first point: one inside rmin0 (r = 0.2), one just outside (0.31), the rest spread up to the cutoff
+    near = np.array([[0.12, -0.1, 0.12], [0.2, 0.2, -0.126]])
+    assert abs(np.linalg.norm(near[0]) - 0.197) < 1e-3 and 0.3 < np.linalg.norm(near[1]) < 0.32
+    pos = np.concatenate([pts[0] + near, pts[0] + cluster(rng, 9, 3.0)])
+    types = [0, 1] + [int(t) for t in rng.integers(0, 2, 9)]
+    r = oracle.bispectrum_points(pts, pos, types, BIG, pbc=(0, 0, 0), rcutfac=rcutfac, wself=wself, radelem=radelem, wj=wj,
+                                 rmin0=rmin0)
+    tr = r["triples"]
+    idx = [int(np.where((tr[:, 0] == j) & (tr[:, 1] == 0) & (tr[:, 2] == j))[0][0]) for j in range(11)]
+    for p, B, nn in zip(pts, r["B"], r["nnbr"]):
+        nb = brute_neighbors(p, pos, types, BIG, np.zeros(3), (0, 0, 0), rcut_t)
+        assert nn == len(nb) >= 6
+        s = wself + sum(wj[t] * fc_theta(np.linalg.norm(d), rcut_t[t], rmin0)[0] for d, t in nb)
+        np.testing.assert_allclose(B[0], s ** 3, rtol=1e-13)
+        ref, _ = chebyshev_bj0j(p, pos, types, BIG, np.zeros(3), (0, 0, 0), rcut_t, wj, wself, 10, rmin0)
+        np.testing.assert_allclose(B[idx], ref, rtol=1e-11)
+    # the test can tell the readings apart: clamping theta0 at 0 inside rmin0 changes B_{j,0,j} of the first point
+    nb = brute_neighbors(pts[0], pos, types, BIG, np.zeros(3), (0, 0, 0), rcut_t)
+    cs, qs = [wself], [np.array([1.0, 0, 0, 0])]
+    for d, t in nb:
+        rr = np.linalg.norm(d)
+        fc, th0 = fc_theta(rr, rcut_t[t], rmin0)
+        th0 = max(th0, 0.0)
+        cs.append(wj[t] * fc)
+        qs.append(np.concatenate([[np.cos(th0)], np.sin(th0) * d / rr]))
+    cs, qs = np.array(cs), np.array(qs)
+    clamped = np.array([cs.sum() * (cs @ eval_chebyu(j, np.clip(qs @ qs.T, -1, 1)) @ cs) for j in range(11)])
+    assert np.abs(clamped - r["B"][0][idx]).max() > 1e-3 * np.abs(clamped).max()
+    # a neighbor at r < rmin0 with wself = 0 and nothing else: (w * 1)^3 (j + 1), any direction (single-neighbor closed form)
+    one = oracle.bispectrum_points([[0, 0, 0]], [[0.1, 0.05, -0.12]], [0], BIG, pbc=(0, 0, 0), wself=0.0, wj=(0.8,), rmin0=rmin0)
+    np.testing.assert_allclose(one["B"][0], 0.8 ** 3 * (one["triples"][:, 2] + 1), rtol=2e-12)
 
 
 def test_chebyshev_grid_oracle_agrees_with_the_wigner_cg_path():
