@@ -37,15 +37,15 @@ extern "C" {
 #define MALA_SNAP_ECUDA (-2)
 #define MALA_SNAP_ENOMEM (-3)
 
-/* largest supported twojmax (32 grid points x all U levels must fit one SM's shared memory) */
-#define MALA_SNAP_MAX_TWOJMAX 10
+/* largest supported twojmax.  Up to 10 a 32-point tile of U_tot fits one SM's shared memory; 11..14 run on half tiles. */
+#define MALA_SNAP_MAX_TWOJMAX 14
 
 typedef struct mala_snap mala_snap_t; /* opaque; owns device tables and a lazily grown workspace */
 
 /*
  * Create a descriptor calculator (descriptor_type "Bispectrum", twojmax, rcutfac).
  *   handle   [out] HOST
- *   twojmax  0..MALA_SNAP_MAX_TWOJMAX, even or odd (10 in the paper)
+ *   twojmax  0..MALA_SNAP_MAX_TWOJMAX (14), even or odd (10 in the paper's configurations; a hyperparameter)
  *   rcutfac  > 0; cutoff of type t is rcut_t = 2 * rcutfac * radelem[t]  (reading #10)
  *   rfac0    in (0, 1]: theta0 = rfac0 * pi * (r - rmin0) / (rcut_t - rmin0)      (north_star: 0.99363)
  *   rmin0    in [0, min rcut_t)                                                     (north_star: 0)
@@ -116,10 +116,9 @@ int mala_gaussian_grid(mala_snap_t *h, double sigma, int natoms, const double *p
 /*
  * Tuning / test knobs.  Unknown names give MALA_SNAP_EINVAL.
  *   "zi_impl"          0 = automatic (per-triple specialised kernel when twojmax == 10, anti-diagonal kernel
- *                      otherwise), 1 = generic table-driven kernel, 2 = per-triple specialised kernel (EINVAL if
- *                      twojmax != 10), 3 = anti-diagonal kernel (code specialised on j1 only, any twojmax).
- *                      The anti-diagonal kernel keeps its tables in __constant__ memory, one image per process:
- *                      handles with different twojmax must not run it concurrently on different streams.
+ *                      otherwise), 1 = generic table-driven kernel (twojmax <= 10), 2 = per-triple specialised kernel
+ *                      (EINVAL if twojmax != 10), 3 = anti-diagonal kernel (code specialised on j1 only, any twojmax;
+ *                      its tables are per-handle arrays in global memory, so handles of different twojmax coexist).
  *   "timing"           1 = record a CUDA-event pair on the caller's stream around every kernel launch of the
  *                      following calls (read back with mala_snap_kernel_times); 0 = off (default)
  *   "workspace_mb"     cap, in MiB, of the U_tot + candidate workspace (default 4096)

@@ -94,11 +94,13 @@ struct mala_snap {
     int device = 0, num_sms = 0;
     // options
     int zi_impl = 0;
-    // constant-memory images of the diag kernel (uploaded again when another handle used the constants last)
+    // tables of the anti-diagonal kernels (per handle, global memory)
     std::vector<double> k_dcg;
     std::vector<DiagTriple> k_dtriple;
-    std::vector<unsigned short> k_dsched;
-    int k_duoff[kMaxTwoJ + 2] = {0};
+    std::vector<unsigned short> k_dsched, k_ditems;
+    DevBuf<double> d_dcg;
+    DevBuf<DiagTriple> d_dtriple;
+    DevBuf<unsigned short> d_dsched, d_ditems;
     long long workspace_mb = 4096;
     long long host_chunk_mb = 256;
     // device tables
@@ -142,6 +144,13 @@ struct mala_snap {
         t.type_rcut = d_rcut.p; t.type_w = d_w.p; t.bconst = d_bconst.p;
         return t;
     }
+    DiagTables diag_tables() const {
+        DiagTables t;
+        t.cg2 = reinterpret_cast<const double2 *>(d_dcg.p); t.triple = d_dtriple.p; t.sched = d_dsched.p; t.items = d_ditems.p;
+        return t;
+    }
+    // twojmax above kFullTileTwoJ: U_tot of 32 points does not fit one SM's shared memory; half-tile layout and kernel
+    bool half_tiles() const { return twojmax > kFullTileTwoJ; }
     // 0 = automatic: the per-triple specialised kernel at twojmax = 10, the anti-diagonal kernel otherwise
     bool use_spec() const { return zi_impl == 2 || (zi_impl == 0 && twojmax == kSpecTJ); }
     bool use_diag() const { return zi_impl == 3 || (zi_impl == 0 && twojmax != kSpecTJ); }
@@ -158,14 +167,18 @@ int upload(DevBuf<T> &b, const std::vector<T> &v) {
 }
 
 int set_kernel_attributes(mala_snap *h) {
-    const int ui_smem = (int)compute_ui_smem_bytes(kMaxTwoJ);
-    CUDA_TRY(cudaFuncSetAttribute(compute_ui_kernel<kMaxTwoJ, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, ui_smem));
-    CUDA_TRY(cudaFuncSetAttribute(compute_ui_kernel<kMaxTwoJ, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ui_smem));
-    const int zi_smem = (int)compute_zi_smem_bytes(uhalf_size(kMaxTwoJ), triple_count(kMaxTwoJ));
+    const int ui_smem = (int)compute_ui_smem_bytes(kFullTileTwoJ);
+    CUDA_TRY(cudaFuncSetAttribute(compute_ui_kernel<kFullTileTwoJ, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, ui_smem));
+    CUDA_TRY(cudaFuncSetAttribute(compute_ui_kernel<kFullTileTwoJ, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ui_smem));
+    CUDA_TRY(cudaFuncSetAttribute(compute_ui_kernel<kMaxTwoJ, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)compute_ui_smem_bytes(kMaxTwoJ)));
+    const int zi_smem = (int)compute_zi_smem_bytes(uhalf_size(kFullTileTwoJ), triple_count(kFullTileTwoJ));
     CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, zi_smem));
     CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_coop_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)compute_zi_coop_smem_bytes()));
     CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_diag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)compute_zi_diag_smem_bytes(uhalf_size(kMaxTwoJ), triple_count(kMaxTwoJ))));
+                                  (int)compute_zi_diag_smem_bytes(uhalf_size(kFullTileTwoJ), triple_count(kFullTileTwoJ))));
+    CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_diag_half_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)compute_zi_diag_half_smem_bytes(uhalf_size(kMaxTwoJ), triple_count(kMaxTwoJ))));
     (void)h;
     return 0;
 }
@@ -197,25 +210,11 @@ struct TimedSpan {
     }
 };
 
-// The diag kernel reads its tables from __constant__ memory, which is one image per process: the handle that used it
-// last is remembered and another handle uploads its own image (stream-ordered) before launching.
-const mala_snap *g_diag_owner = nullptr;
-
-int bind_diag_constants(mala_snap *h, cudaStream_t st) {
-    if (g_diag_owner == h) return 0;
-    CUDA_TRY(cudaMemcpyToSymbolAsync(c_dcg2, h->k_dcg.data(), h->k_dcg.size() * sizeof(double), 0, cudaMemcpyHostToDevice, st));
-    CUDA_TRY(cudaMemcpyToSymbolAsync(c_dtriple, h->k_dtriple.data(), h->k_dtriple.size() * sizeof(DiagTriple), 0, cudaMemcpyHostToDevice, st));
-    CUDA_TRY(cudaMemcpyToSymbolAsync(c_dsched, h->k_dsched.data(), h->k_dsched.size() * sizeof(unsigned short), 0, cudaMemcpyHostToDevice, st));
-    CUDA_TRY(cudaMemcpyToSymbolAsync(c_duoff, h->k_duoff, sizeof(h->k_duoff), 0, cudaMemcpyHostToDevice, st));
-    g_diag_owner = h;
-    return 0;
-}
-
 // processing order (J1 descending, then cost), padded CG blocks and the per-warp item schedule of the diag kernel
-void build_diag_schedule(mala_snap *h) {
+int build_diag_schedule(mala_snap *h) {
     const SnapTables &T = h->tab;
     const int nt = T.ntriples;
-    for (int J = 0; J <= kMaxTwoJ + 1; J++) h->k_duoff[J] = uhalf_off(J);
+    const int NWD = h->half_tiles() ? kDiagHalfWarps : kDiagWarps;  // warps of the kernel this handle will launch
     // CG blocks with an even row stride (16-byte rows: two coefficients per uniform load)
     std::vector<int> cgoff(nt, 0);
     h->k_dcg.clear();
@@ -247,6 +246,20 @@ void build_diag_schedule(mala_snap *h) {
         }
         for (double c : icost[t]) tcost[t] += c;
     }
+    // item descriptors (16-point kernel): item -> last-of-column flag | mb << 8 | mb1, items numbered column by column
+    std::vector<int> itemoff(nt, 0);
+    h->k_ditems.clear();
+    for (int t = 0; t < nt; t++) {
+        const int J1 = T.triples[4 * t], J2 = T.triples[4 * t + 1], J = T.triples[4 * t + 2];
+        itemoff[t] = (int)h->k_ditems.size();
+        for (int mb = 0; mb <= J / 2; mb++) {
+            int lo, hi;
+            diag_item_range(J1, J2, J, mb, lo, hi);
+            for (int i = lo; i <= hi; i++)
+                h->k_ditems.push_back((unsigned short)((i == hi ? 0x8000u : 0u) | ((unsigned)mb << 8) | (unsigned)i));
+        }
+    }
+    h->k_ditems.push_back(0);
     std::vector<int> order(nt);
     for (int i = 0; i < nt; i++) order[i] = i;
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) {
@@ -254,9 +267,9 @@ void build_diag_schedule(mala_snap *h) {
         return tcost[a] > tcost[b];
     });
     h->k_dtriple.assign(nt, DiagTriple{});
-    h->k_dsched.assign((size_t)kDiagMaxNT * kDiagWarps * 2, 0);
-    const int teams = (kDiagWarps % kDiagTeams == 0) ? kDiagTeams : 1;
-    const int tw = kDiagWarps / teams;
+    h->k_dsched.assign((size_t)nt * NWD * 2, 0);
+    const int teams = (NWD % kDiagTeams == 0) ? kDiagTeams : 1;
+    const int tw = NWD / teams;
     // balanced per reduction group, like the per-triple kernel: team split by exhaustive search, per-group running loads
     std::vector<int> pos_team(nt, 0);
     for (int g0 = 0; g0 < nt; g0 += kDiagGroup) {
@@ -282,12 +295,12 @@ void build_diag_schedule(mala_snap *h) {
                 pos_team[g0 + i] = team;
             }
         }
-        std::vector<double> load(kDiagWarps, 0.0);
+        std::vector<double> load(NWD, 0.0);
         for (int pos = g0; pos < g0 + gn; pos++) {
             const int t = order[pos], team = pos_team[pos];
             DiagTriple &d = h->k_dtriple[pos];
             d.J1 = (short)T.triples[4 * t]; d.J2 = (short)T.triples[4 * t + 1]; d.J = (short)T.triples[4 * t + 2];
-            d.index = (short)t; d.cgoff = cgoff[t]; d.pad = 0;
+            d.index = (short)t; d.cgoff = cgoff[t]; d.itemoff = itemoff[t];
             const std::vector<double> &cost = icost[t];
             const int n = (int)cost.size();
             double sum_load = tcost[t] + 0.5 * tw * kCallCost;
@@ -308,28 +321,33 @@ void build_diag_schedule(mala_snap *h) {
                     i++;
                 }
                 load[w] += acc;
-                h->k_dsched[((size_t)pos * kDiagWarps + w) * 2] = (unsigned short)begin;
-                h->k_dsched[((size_t)pos * kDiagWarps + w) * 2 + 1] = (unsigned short)i;
+                h->k_dsched[((size_t)pos * NWD + w) * 2] = (unsigned short)begin;
+                h->k_dsched[((size_t)pos * NWD + w) * 2 + 1] = (unsigned short)i;
             }
         }
     }
+    int rc = 0;
+    if ((rc = upload(h->d_dcg, h->k_dcg))) return rc;
+    if ((rc = upload(h->d_dtriple, h->k_dtriple))) return rc;
+    if ((rc = upload(h->d_dsched, h->k_dsched))) return rc;
+    if ((rc = upload(h->d_ditems, h->k_ditems))) return rc;
+    return 0;
 }
 
 // enqueue compute_zi_bi for one chunk
 int launch_zi(mala_snap *h, const ChunkBuffers &cb, double *out, cudaStream_t st) {
-    const int grid = std::max(1, std::min(h->num_sms, cb.ntiles));
-    const size_t smem = compute_zi_smem_bytes(h->sc.nelem, h->sc.ntriples);
-    if (h->use_diag()) {
-        int rc = bind_diag_constants(h, st);
-        if (rc) return rc;
-    }
+    const int grid = std::max(1, std::min(h->num_sms, h->half_tiles() ? 2 * cb.ntiles : cb.ntiles));
     TimedSpan span(h, st, kKindZi);
-    if (h->use_diag())
-        compute_zi_bi_diag_kernel<<<grid, kDiagWarps * 32, compute_zi_diag_smem_bytes(h->sc.nelem, h->sc.ntriples), st>>>(h->geom, h->sc, h->tables(), cb, out);
+    if (h->half_tiles())
+        compute_zi_bi_diag_half_kernel<<<grid, kDiagHalfWarps * 32, compute_zi_diag_half_smem_bytes(h->sc.nelem, h->sc.ntriples), st>>>(
+            h->geom, h->sc, h->tables(), h->diag_tables(), cb, out);
+    else if (h->use_diag())
+        compute_zi_bi_diag_kernel<<<grid, kDiagWarps * 32, compute_zi_diag_smem_bytes(h->sc.nelem, h->sc.ntriples), st>>>(
+            h->geom, h->sc, h->tables(), h->diag_tables(), cb, out);
     else if (h->use_spec())
         compute_zi_bi_coop_kernel<<<grid, kCoopWarps * 32, compute_zi_coop_smem_bytes(), st>>>(h->geom, h->sc, h->tables(), cb, out);
     else
-        compute_zi_bi_generic_kernel<<<grid, kZiWarps * 32, smem, st>>>(h->geom, h->sc, h->tables(), cb, out);
+        compute_zi_bi_generic_kernel<<<grid, kZiWarps * 32, compute_zi_smem_bytes(h->sc.nelem, h->sc.ntriples), st>>>(h->geom, h->sc, h->tables(), cb, out);
     CUDA_TRY(cudaGetLastError());
     h->stats[0]++;
     return 0;
@@ -340,9 +358,12 @@ int launch_zi(mala_snap *h, const ChunkBuffers &cb, double *out, cudaStream_t st
 int compute_bconst(mala_snap *h) {
     const int nelem = h->sc.nelem, nt = h->sc.ntriples, P = kTilePoints;
     CUDA_TRY(cudaDeviceSynchronize());
-    std::vector<double2> u((size_t)nelem * P);
+    std::vector<double2> u((size_t)nelem * P);  // [nelem][32], or [2][nelem][16] in the half-tile layout
     for (int e = 0; e < nelem; e++)
-        for (int l = 0; l < P; l++) u[(size_t)e * P + l] = make_double2(h->tab.udiag[e] ? h->wself : 0.0, 0.0);
+        for (int l = 0; l < P; l++) {
+            const size_t at = h->half_tiles() ? ((size_t)(l >> 4) * nelem + e) * 16 + (l & 15) : (size_t)e * P + l;
+            u[at] = make_double2(h->tab.udiag[e] ? h->wself : 0.0, 0.0);
+        }
     DevBuf<double2> t_utot;
     DevBuf<int> t_active, t_counters;
     DevBuf<double> tmp;
@@ -367,6 +388,7 @@ int compute_bconst(mala_snap *h) {
     h->geom = g;
     ChunkBuffers cb{};
     cb.active = t_active.p; cb.counters = t_counters.p; cb.status = h->d_status.p; cb.utot = t_utot.p; cb.tile_begin = 0; cb.ntiles = 1;
+    cb.utot_half = h->half_tiles() ? 1 : 0;
     int rc = launch_zi(h, cb, tmp.p, nullptr);
     h->geom = saved;
     if (rc) { cleanup(); return rc; }
@@ -696,6 +718,7 @@ int run_slab(mala_snap *h, int z0, int z1, double *out, double2 *u_out, cudaStre
         cb.cand = h->d_cand.p; cb.ncand = h->d_ncand.p; cb.active = h->d_active.p; cb.counters = h->d_counters.p;
         cb.status = h->d_status.p;
         cb.utot = h->d_utot.p; cb.cand_cap = h->cand_cap;
+        cb.utot_half = h->half_tiles() ? 1 : 0;
         cb.tile_begin = (int)t0;
         cb.ntiles = (int)std::min(chunk_tiles, total_tiles - t0);
         CUDA_TRY(cudaMemsetAsync(cb.counters, 0, 4 * sizeof(int), st));
@@ -706,13 +729,18 @@ int run_slab(mala_snap *h, int z0, int z1, double *out, double2 *u_out, cudaStre
         }
         CUDA_TRY(cudaGetLastError());
         const int grid = std::max(1, std::min(h->num_sms, cb.ntiles));
-        const int ui_grid = std::max(1, std::min(2 * h->num_sms, 2 * cb.ntiles));  // half-tile items, two CTAs per SM
         {
             TimedSpan span(h, st, kKindUi);
-            if (h->twojmax == kMaxTwoJ)
-                compute_ui_kernel<kMaxTwoJ, true><<<ui_grid, (kMaxTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kMaxTwoJ), st>>>(g, h->sc, tb, cb);
-            else  // smaller twojmax: same code with run-time guards on the levels
+            if (h->half_tiles()) {  // twojmax 11..14: eight column warps, one CTA per SM
+                const int ui_grid = std::max(1, std::min(h->num_sms, 2 * cb.ntiles));
                 compute_ui_kernel<kMaxTwoJ, false><<<ui_grid, (kMaxTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kMaxTwoJ), st>>>(g, h->sc, tb, cb);
+            } else {
+                const int ui_grid = std::max(1, std::min(2 * h->num_sms, 2 * cb.ntiles));  // half-tile items, two CTAs per SM
+                if (h->twojmax == kFullTileTwoJ)
+                    compute_ui_kernel<kFullTileTwoJ, true><<<ui_grid, (kFullTileTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kFullTileTwoJ), st>>>(g, h->sc, tb, cb);
+                else  // smaller twojmax: same code with run-time guards on the levels
+                    compute_ui_kernel<kFullTileTwoJ, false><<<ui_grid, (kFullTileTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kFullTileTwoJ), st>>>(g, h->sc, tb, cb);
+            }
         }
         CUDA_TRY(cudaGetLastError());
         h->stats[0] += 2;
@@ -836,7 +864,8 @@ int mala_snap_create(mala_snap_t **handle, int twojmax, double rcutfac, double r
                      const double *radelem, const double *wj) {
     if (!handle) return fail(MALA_SNAP_EINVAL, "handle is NULL");
     *handle = nullptr;
-    if (twojmax < 0 || twojmax > MALA_SNAP_MAX_TWOJMAX) return fail(MALA_SNAP_EINVAL, "twojmax outside [0, 10]");
+    if (twojmax < 0 || twojmax > MALA_SNAP_MAX_TWOJMAX) return fail(MALA_SNAP_EINVAL, "twojmax outside [0, 14]");
+    static_assert(MALA_SNAP_MAX_TWOJMAX == kMaxTwoJ, "header and kernels disagree on the largest twojmax");
     if (!(rcutfac > 0.0) || !std::isfinite(rcutfac)) return fail(MALA_SNAP_EINVAL, "rcutfac must be positive");
     if (!(rfac0 > 0.0) || !(rfac0 <= 1.0)) return fail(MALA_SNAP_EINVAL, "rfac0 must lie in (0, 1]");
     if (!std::isfinite(wself)) return fail(MALA_SNAP_EINVAL, "wself is not finite");
@@ -996,7 +1025,7 @@ int mala_snap_create(mala_snap_t **handle, int twojmax, double rcutfac, double r
             }
             CUDA_TRY(cudaMemcpyToSymbol(c_wlist, wlist, sizeof(wlist)));
         }
-        build_diag_schedule(h);
+        if ((rc = build_diag_schedule(h))) return rc;
         if ((rc = set_kernel_attributes(h))) return rc;
         if (h->d_status.reserve(1)) return fail(MALA_SNAP_ENOMEM, "cudaMalloc (status) failed");
         CUDA_TRY(cudaMemset(h->d_status.p, 0, sizeof(int)));
@@ -1049,6 +1078,8 @@ int mala_snap_set_option(mala_snap_t *h, const char *name, long long value) {
     if (n == "zi_impl") {
         if (value < 0 || value > 3) return fail(MALA_SNAP_EINVAL, "zi_impl must be 0, 1, 2 or 3");
         if (value == 2 && h->twojmax != kSpecTJ) return fail(MALA_SNAP_EINVAL, "the specialised kernel exists for twojmax = 10 only");
+        if (value != 0 && value != 3 && h->half_tiles())
+            return fail(MALA_SNAP_EINVAL, "twojmax > 10 runs on half tiles: only the anti-diagonal kernel (zi_impl 0 or 3) supports them");
         h->zi_impl = (int)value;
         return compute_bconst(h);
     }
@@ -1097,6 +1128,7 @@ int mala_snap_kernel_times(mala_snap_t *h, double ms[4], long long launches[4]) 
 
 const char *mala_snap_zi_kernel(const mala_snap_t *h) {
     if (!h) return "";
+    if (h->half_tiles()) return "compute_zi_bi_diag_half_kernel";
     return h->use_diag() ? "compute_zi_bi_diag_kernel" : (h->use_spec() ? "compute_zi_bi_coop_kernel" : "compute_zi_bi_generic_kernel");
 }
 
@@ -1226,7 +1258,6 @@ int mala_snap_debug_utot(mala_snap_t *h, int natoms, const double *pos, const in
 
 void mala_snap_destroy(mala_snap_t *h) {
     if (!h) return;
-    if (g_diag_owner == h) g_diag_owner = nullptr;
     cudaDeviceSynchronize();
     h->d_triples.release(); h->d_udiag.release(); h->d_order.release();
     h->d_cg.release(); h->d_unorm.release(); h->d_rcut.release(); h->d_w.release(); h->d_bconst.release();
@@ -1238,6 +1269,7 @@ void mala_snap_destroy(mala_snap_t *h) {
     }
     h->d_cand.release(); h->d_ncand.release(); h->d_active.release(); h->d_counters.release(); h->d_utot.release();
     h->d_status.release();
+    h->d_dcg.release(); h->d_dtriple.release(); h->d_dsched.release(); h->d_ditems.release();
     if (h->h_status) cudaFreeHost(h->h_status);
     for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
     if (h->ev_upload) cudaEventDestroy(h->ev_upload);

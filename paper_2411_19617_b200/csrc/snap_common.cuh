@@ -8,7 +8,9 @@
 namespace mala {
 
 constexpr int kTilePoints = 32;  // grid points per tile = lanes of a warp ("lanes as points")
-constexpr int kMaxTwoJ = 10;
+constexpr int kMaxTwoJ = 14;      // largest supported twojmax
+constexpr int kFullTileTwoJ = 10;  // up to here U_tot of a whole 32-point tile fits one SM's shared memory; above it the
+                                   // contraction works on half tiles (16 points) and U_tot is stored half tile by half tile
 
 // Geometry of one slab call, passed by value to every kernel.
 struct GridGeom {
@@ -68,7 +70,8 @@ struct ChunkBuffers {
     int *active;             // [chunk_tiles] compacted list of non-empty tiles (local tile ids)
     int *counters;           // [0] number of active tiles, [1] ui work counter, [2] zi work counter (zeroed per chunk)
     int *status;             // handle-wide status word, never cleared by a chunk: kStatus* bits
-    double2 *utot;           // [chunk_tiles][nelem][32]
+    double2 *utot;           // [chunk_tiles][nelem][32], or [chunk_tiles][2][nelem][16] when utot_half is set
+    int utot_half;           // 1: half-tile layout (twojmax > kFullTileTwoJ)
     int cand_cap;
     int tile_begin;          // first global tile id of the chunk
     int ntiles;              // tiles in the chunk

@@ -222,8 +222,11 @@ __device__ __forceinline__ void pair_geometry(const double dx, const double dy, 
 // Work item = half a tile (16 grid points).  Lane = (point p = lane & 15, half h = lane >> 4): both halves see the same
 // points and split each point's neighbors (entries of even / odd index), so a CTA needs shared-memory accumulators for
 // 16 points only (69 KB) and two CTAs share an SM -- twice the warps to hide the FP64 latency with.
+// Instances: <10, true> (twojmax = 10, the configs of the paper), <10, false> (twojmax < 10, run-time guards on the levels),
+// both with 6 column warps and two CTAs per SM; <14, false> (twojmax 11..14): 8 column warps, one CTA per SM (the accumulators
+// of 16 points take 167 KB at twojmax = 14).
 template <int TJMAX, bool EXACT>
-__global__ void __launch_bounds__((TJMAX / 2 + 1) * 32, 2)
+__global__ void __launch_bounds__((TJMAX / 2 + 1) * 32, (TJMAX <= kFullTileTwoJ ? 2 : 1))
 compute_ui_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers cb) {
     constexpr int NW = TJMAX / 2 + 1;
     constexpr int NP = kUiPoints;
@@ -321,13 +324,14 @@ compute_ui_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers cb) {
         __syncthreads();
         // binomial normalisation, self term (delta(0) of Eq. (24)), store of the half tile: lanes hh*16 .. hh*16+15 of
         // every element; each half-warp takes an element of its own
-        double2 *dst = cb.utot + (size_t)slot * nelem * 32 + hh * NP;
+        double2 *dst = cb.utot_half ? cb.utot + (size_t)item * nelem * NP : cb.utot + (size_t)slot * nelem * 32 + hh * NP;
+        const int estride = cb.utot_half ? NP : 32;
         for (int e = warp * 2 + (upper ? 1 : 0); e < nelem; e += NW * 2) {
             double2 v = uacc[e * NP + p];
             const double sN = tb.unorm[e];
             v.x = v.x * sN + (tb.udiag[e] ? sc.wself : 0.0);
             v.y = v.y * sN;
-            dst[e * 32 + p] = v;
+            dst[e * estride + p] = v;
         }
     }
 }
@@ -355,7 +359,9 @@ __global__ void utot_scatter_kernel(GridGeom g, SnapConst sc, DeviceTables tb, C
     double2 *dst = u_out + ((size_t)((size_t)(iz - g.z0) * g.ny + iy) * g.nx + ix) * sc.nelem;
     for (int e = 0; e < sc.nelem; e++) {
         double2 v;
-        if (slot >= 0) v = cb.utot[((size_t)slot * sc.nelem + e) * 32 + lane];
+        if (slot >= 0)
+            v = cb.utot_half ? cb.utot[((size_t)(2 * slot + (lane >> 4)) * sc.nelem + e) * 16 + (lane & 15)]
+                             : cb.utot[((size_t)slot * sc.nelem + e) * 32 + lane];
         else v = make_double2(tb.udiag[e] ? sc.wself : 0.0, 0.0);
         dst[e] = v;
     }

@@ -48,6 +48,17 @@ __device__ __forceinline__ void tma_load_1d(void *dst_smem, const void *src_gmem
                  : "memory");
 }
 
+// issue a bulk load of `total` bytes (a multiple of 16) in pieces of at most 32 KB, all completing on one mbarrier phase
+__device__ __forceinline__ void tma_load_bytes(void *dst, const void *src, uint32_t total, uint64_t *bar) {
+    mbar_expect_tx(bar, total);
+    uint32_t done = 0;
+    while (done < total) {
+        const uint32_t n = min(total - done, 32768u);
+        tma_load_1d(reinterpret_cast<unsigned char *>(dst) + done, reinterpret_cast<const unsigned char *>(src) + done, n, bar);
+        done += n;
+    }
+}
+
 // issue the bulk load of one U_tot tile (nelem*512 bytes) in pieces of at most 32 KB
 __device__ __forceinline__ void tma_load_tile(double2 *dst, const double2 *src, int nelem, uint64_t *bar) {
     const uint32_t total = (uint32_t)nelem * 32u * (uint32_t)sizeof(double2);

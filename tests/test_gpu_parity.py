@@ -150,8 +150,9 @@ def _small_case(seed, twojmax, natoms, pbc, triclinic, two_types, ngrid=(7, 5, 6
     return pos, types, box, origin, pbc, ngrid, params
 
 
-@pytest.mark.parametrize("twojmax", [0, 1, 2, 3, 4, 5, 7, 8, 9, 10])
+@pytest.mark.parametrize("twojmax", [0, 1, 2, 3, 4, 5, 7, 8, 9, 10, 11, 12, 13, 14])
 def test_small_cases_every_twojmax(twojmax):
+    """twojmax 11..14 run on half tiles (16 points per CTA, two items per warp): SURVEY.md 8(f) row f4"""
     torch = _torch()
     for seed, (natoms, pbc, tri, two) in enumerate([(0, (1, 1, 1), False, False), (1, (0, 0, 0), False, False),
                                                     (3, (1, 1, 1), True, True), (5, (1, 0, 1), True, True),
@@ -188,7 +189,7 @@ def test_random_small_systems_all_kernels():
     rng = np.random.default_rng(2024)
     n = 0
     for it in range(60):
-        tj = int(rng.integers(0, 11))
+        tj = int(rng.integers(0, 15 if it % 5 == 0 else 11))
         box = np.diag(rng.uniform(2.5, 6.0, 3))
         if rng.random() < 0.5:
             box = box + np.tril(rng.uniform(-1, 1, (3, 3)), -1)
@@ -207,7 +208,7 @@ def test_random_small_systems_all_kernels():
         origin = tuple(rng.uniform(-0.3, 0.3, 3))
         ref = oracle.bispectrum_grid(pos, types, box, origin, pbc, ngrid, z0, z1, **params)
         with MalaSnap(**params) as snap:
-            for zi in ([1, 3] if tj != 10 else [1, 2, 3]):
+            for zi in ([3, 0] if tj > 10 else ([1, 3] if tj != 10 else [1, 2, 3])):
                 snap.set_option("zi_impl", zi)
                 if rng.random() < 0.3:
                     snap.set_option("workspace_mb", 1)

@@ -57,7 +57,7 @@ def test_create_argument_errors_come_before_device_use():
     lib = pkg.load_library()
     h = ctypes.c_void_p()
     one = (ctypes.c_double * 1)(0.5)
-    bad = [dict(twojmax=-1), dict(twojmax=11), dict(rcutfac=0.0), dict(rfac0=0.0), dict(rfac0=1.5), dict(rmin0=5.0), dict(ntypes=0)]
+    bad = [dict(twojmax=-1), dict(twojmax=15), dict(rcutfac=0.0), dict(rfac0=0.0), dict(rfac0=1.5), dict(rmin0=5.0), dict(ntypes=0)]
     for kw in bad:
         a = dict(twojmax=10, rcutfac=4.676, rfac0=0.99363, rmin0=0.0, wself=1.0, ntypes=1)
         a.update(kw)
@@ -68,7 +68,7 @@ def test_create_argument_errors_come_before_device_use():
     lib.mala_snap_destroy(None)  # NULL-safe
 
 
-@pytest.mark.parametrize("tj", [0, 1, 2, 3, 5, 10])
+@pytest.mark.parametrize("tj", [0, 1, 2, 3, 5, 10, 14])
 def test_library_cg_table_matches_oracle_racah(tj):
     """two independent implementations (long-double factorial table vs the oracle's) of the same closed form"""
     worst = 0.0
