@@ -87,6 +87,8 @@ def parse_args():
     p.add_argument("--descriptor", default="bispectrum", choices=["bispectrum", "gaussian"],
                    help="gaussian: the SURVEY 8(f) f2 path (mala_gaussian_grid), a separate metric line")
     p.add_argument("--sigma", type=float, default=0.5, help="Gaussian width for --descriptor gaussian")
+    p.add_argument("--ldos", action="store_true",
+                   help="SURVEY 8(f) f1: descriptors + the descriptor->LDOS network in one call (mala_bispectrum_ldos_grid), a separate metric line")
     p.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
     p.add_argument("--no-e2e", action="store_true", help="skip the host-output leg (profiling runs)")
     args = p.parse_args()
@@ -537,6 +539,119 @@ def run_gaussian(args, w, rank, world, local):
     print(json.dumps(line), flush=True)
 
 
+def run_ldos(args, w, rank, world, local):
+    """--ldos: grid points/s of mala_bispectrum_ldos_grid (row f1): descriptors, then the 91 -> 256 -> 256 -> 241 network on the
+    tensor cores, LDOS (fp32) resident in HBM; e2e adds the device->host copy of the LDOS.  Roofline of the network kernel:
+    bound "tensor", 2 * sum_l w_l w_{l+1} flop per grid point against the TF32 peak (measured bf16 burst peak x the nominal
+    TF32 : BF16 ratio of 1/2)."""
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        torch.distributed.init_process_group("nccl", device_id=dev)
+    from paper_2411_19617_b200 import MalaMlp, MalaSnap, bispectrum_ldos_grid, workloads
+
+    def barrier():
+        if world > 1:
+            torch.distributed.barrier()
+        torch.cuda.synchronize()
+
+    fm = flop_model(w.twojmax)
+    sizes = (fm["ncomp"], 256, 256, 241)
+    ws, bs, shift, scale = workloads.ldos_network(sizes=sizes)
+    npts = w.npoints
+    snap = MalaSnap(**w.snap_params())
+    net = MalaMlp(ws, bs, "leaky_relu", True, shift, scale)
+    stream = torch.cuda.current_stream()
+    out = torch.empty((npts, sizes[-1]), dtype=torch.float32, device=dev)
+    call = lambda: bispectrum_ldos_grid(snap, net, w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, out=out, stream=stream)
+    snap.set_option("timing", 1)
+    for _ in range(args.warmup):
+        call()
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.15)
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    ktimes, launches = [], 0
+    barrier()
+    for a, b in evs:
+        a.record(stream)
+        call()
+        b.record(stream)
+        ktimes.append(snap.kernel_times())
+        launches += snap.last_stats()["kernels"]
+    barrier()
+    clocks = sampler.stop()
+    total_ms = float(sum(a.elapsed_time(b) for a, b in evs))
+    total_ms, total_pts = reduce_max_sum(total_ms, npts * args.steps, world, dev)
+    value = total_pts / (total_ms * 1e-3)
+    stats = snap.last_stats()
+    mlp_ms = float(np.mean([k["other"][0] for k in ktimes]))
+    mlp_launches = ktimes[-1]["other"][1]
+    kms = {"tile_bin": float(np.mean([k["tile_bin"][0] for k in ktimes])), "compute_ui": float(np.mean([k["compute_ui"][0] for k in ktimes])),
+           "compute_zi_bi": float(np.mean([k["compute_zi_bi"][0] for k in ktimes])), "mlp_forward": mlp_ms}
+    flop_pt = 2 * sum(a * b for a, b in zip(sizes[:-1], sizes[1:]))
+    rows = 32 * stats["tiles"]                    # the network runs on whole tiles (ragged lanes included)
+    achieved = flop_pt * npts / (mlp_ms * 1e-3) / 1e12 if mlp_ms > 0 else 0.0
+    bf16 = None
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            bf16 = json.load(f).get("bf16_tflops")
+    except (OSError, ValueError):
+        pass
+    peak_src = "MEASURED_PEAKS.json bf16 burst peak x 0.5 (nominal TF32 : BF16)" if bf16 else "fallback: nominal 2250 x 0.5 (B200_PROFILING.md)"
+    peak = 0.5 * (bf16 if bf16 else 2250.0)
+    roofline = {"bound": "tensor", "kernel": "mlp_forward_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                "peak_source": peak_src, "traffic": None, "flop_per_point": flop_pt, "flop_per_launch": flop_pt * npts / max(mlp_launches, 1),
+                "launches_per_step": mlp_launches, "ms_per_launch": mlp_ms / max(mlp_launches, 1), "kernel_ms_per_step": kms,
+                "rows_processed_per_step": rows, "network": list(sizes), "operand_dtype": "tf32 (fp32 accumulate)",
+                "note": "the network is ~1.5 % of the step; it is bound by streaming its 0.62 MB of weights from L2 once per 128-row tile, "
+                        "not by the tensor pipe (DESIGN.md section 13)"}
+    roofline["traffic"], roofline["traffic_source"] = ncu_traffic(f"config{w.extra.get('cfg')}/tj{w.twojmax}", "mlp_forward_kernel",
+                                                                  mlp_ms / max(mlp_launches, 1))
+    host = torch.empty((npts, sizes[-1]), dtype=torch.float32, pin_memory=True)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        call()
+        host.copy_(out, non_blocking=True)
+        torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    e2e_s, e2e_pts = reduce_max_sum(e2e_s, npts * args.steps, world, dev)
+    h2d = int(w.pos.nbytes + w.types.nbytes + 9 * 8 + 3 * 8 + 3 * 4 + 3 * 4)
+    e2e = {"value": e2e_pts / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": int(npts * sizes[-1] * 4),
+           "ms_per_step": 1e3 * e2e_s / args.steps}
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+        from oracle import mlp_oracle
+        rng = np.random.default_rng(7)
+        n = 60000
+        sample = rng.integers(0, npts, n)
+        t0 = time.perf_counter()
+        B = oracle.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, sample=sample, **w.snap_params())
+        mlp_oracle.mlp_forward(B, ws, bs, "leaky_relu", True, shift, scale)
+        dt = time.perf_counter() - t0
+        cpu = {"value": n / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": f"{n} seeded random grid points of {w.name} (of {npts}) in {dt:.1f} s wall: C descriptor oracle + numpy fp64 network"}
+    net.close()
+    snap.close()
+    if world > 1:
+        torch.distributed.destroy_process_group()
+    if rank != 0:
+        return
+    cfg = workload_config(w, "mala_bispectrum_ldos_grid (device out)")
+    cfg.update({"ncomp_out": sizes[-1], "network": list(sizes), "chunks_per_step": stats["chunks"], "workspace_bytes": stats["workspace_bytes"]})
+    line = {"metric": "grid points/s of LDOS vectors: twojmax=%d fp64 bispectrum descriptors + descriptor->LDOS network (SURVEY 8(f) f1)" % w.twojmax,
+            "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64 descriptors, tf32 network", "data": "synthetic",
+            "config": cfg, "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+
+
 def spawn_ranks(args):
     """`python bench.py --gpus N` without a launcher: start the N ranks ourselves, exactly as the driver would
     (torch.distributed.run, one process per GPU, rendezvous on 127.0.0.1), and pass their output through."""
@@ -567,6 +682,9 @@ def main():
         return
     if args.descriptor == "gaussian":
         run_gaussian(args, w, rank, world, local)
+        return
+    if args.ldos:
+        run_ldos(args, w, rank, world, local)
         return
     run_native(args, w, rank, world, local)
 

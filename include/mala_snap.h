@@ -100,6 +100,51 @@ int mala_bispectrum_grid_host(mala_snap_t *h, int natoms, const double *pos, con
                               int z_begin, int z_end, double *out_host, void *cuda_stream);
 
 /*
+ * ---- the network that maps descriptors to the LDOS, fused behind the descriptor kernels ----------
+ *
+ * A fully connected feed-forward network, x_{l+1} = sigma(W_l x_l + b_l) (Eq. (19); neuron Eq. (18),
+ * PAPER.md:164), applied point by point to the bispectrum vector to give the LDOS vector d(r, epsilon) (e.g.
+ * 241 energy levels).  Runs on the tensor cores (tcgen05, TF32 operands rounded to nearest, fp32
+ * accumulation, fp32 bias and activation); DESIGN.md section 13 states the tolerance against the fp64 oracle.
+ *   nlayers        number of weight matrices, 1..8
+ *   sizes          HOST [nlayers+1]: widths w_0 .. w_L, each 1..256 (w_0 = number of descriptor components for the fused call)
+ *   weights        HOST [nlayers] pointers; weights[l] is W_l, [sizes[l+1]][sizes[l]] row-major fp64 (row = output neuron)
+ *   biases         HOST [nlayers] pointers; biases[l] is b_l, [sizes[l+1]] fp64
+ *   activation     sigma: 0 identity, 1 ReLU, 2 leaky ReLU (slope 0.01), 3 logistic sigmoid              (reading N2)
+ *   activate_last  1: sigma follows the last layer too, as Eq. (19) is written; 0: linear output layer     (reading N1)
+ *   in_shift, in_scale  HOST [sizes[0]] or NULL: the input scaling x_0 = (x - shift) * scale of PAPER.md:473 (reading N3)
+ * All host arrays are copied (and the weights rounded to TF32 and packed) before the call returns.
+ */
+typedef struct mala_mlp mala_mlp_t;
+int mala_mlp_create(mala_mlp_t **net, int nlayers, const int *sizes, const double *const *weights, const double *const *biases,
+                    int activation, int activate_last, const double *in_shift, const double *in_scale);
+
+/* input / output width of the network (either pointer may be NULL) */
+int mala_mlp_widths(const mala_mlp_t *net, int *w_in, int *w_out);
+
+/*
+ * The network alone:  y[p][w_L] = net(x[p][w_0])  for npoints rows.
+ *   x   DEVICE [npoints][w_0] fp64          y   DEVICE [npoints][w_L] fp32
+ * Enqueued on cuda_stream; does not synchronise.
+ */
+int mala_mlp_forward(mala_mlp_t *net, long long npoints, const double *x, float *y, void *cuda_stream);
+
+/* NULL-safe */
+void mala_mlp_destroy(mala_mlp_t *net);
+
+/*
+ * Descriptors and network in one call: the LDOS on the z-slab [z_begin, z_end) of the grid.  All arguments but `net` and
+ * `ldos` as mala_bispectrum_grid.  Per workspace chunk the descriptors go to a compact device staging buffer owned by the
+ * handle and the network consumes them before the next chunk starts; they are never written to caller memory.
+ *   ldos  DEVICE [(z_end-z_begin)*ny*nx][w_L] fp32, ix fastest
+ * MALA_SNAP_EINVAL if the network's input width is not mala_snap_ncomp(h).  Enqueued on cuda_stream; does not synchronise.
+ * mala_snap_kernel_times reports the network under ms[3].
+ */
+int mala_bispectrum_ldos_grid(mala_snap_t *h, mala_mlp_t *net, int natoms, const double *pos, const int *types,
+                              const double box[9], const double origin[3], const int pbc[3], const int ngrid[3], int z_begin,
+                              int z_end, float *ldos, void *cuda_stream);
+
+/*
  * Gaussian descriptors on the same grid ("a sum of Gaussians centered at R", the Gaussian representation of
  * the ionic configuration behind Eqs. (40)-(43)).  One channel per atom type t:
  *     G_t(r) = wj[t] * (2 pi sigma^2)^(-3/2) * sum exp(-|R - r|^2 / (2 sigma^2))

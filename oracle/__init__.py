@@ -210,6 +210,25 @@ def bj0j_grid(pos, types, box, origin, pbc, ngrid, z_begin=0, z_end=None, *, sam
     return out
 
 
+def bispectrum_grad_points(points, pos, types, box, origin=(0, 0, 0), pbc=(1, 1, 1), *, beta=None, want_dB=True, twojmax=10,
+                           rcutfac=4.67637, rfac0=0.99363, rmin0=0.0, wself=1.0, radelem=(0.5,), wj=(1.0,)):
+    """Row f3 (Eq. (45)): dB[p, alpha, k, t] = d B_t(r_p) / d R_alpha,k by forward differentiation of the
+    definition, and, with beta [npoints, ncomp], g[alpha, k] = sum_p sum_t beta[p, t] dB[p, alpha, k, t]."""
+    points = _d(points).reshape(-1, 3)
+    npnt = points.shape[0]
+    nt = ntriples(twojmax)
+    args, keep = _sys_args(twojmax, rcutfac, rfac0, rmin0, wself, radelem, wj, pos, types, box, origin, pbc)
+    natoms = keep[2].shape[0]
+    dB = np.zeros((npnt, natoms, 3, nt)) if want_dB else None
+    b = None if beta is None else _d(beta).reshape(npnt, nt)
+    g = np.zeros((natoms, 3)) if beta is not None else None
+    rc = lib().oracle_bispectrum_grad_points(*args, C.c_int(npnt), _p(points, C.c_double), _p(dB, C.c_double), _p(b, C.c_double),
+                                             _p(g, C.c_double))
+    if rc != 0:
+        raise ValueError("oracle_bispectrum_grad_points: invalid argument")
+    return {"dB": dB, "g": g}
+
+
 def num_threads():
     return lib().oracle_num_threads()
 

@@ -630,6 +630,204 @@ int oracle_bj0j_grid(int twojmax, double rcutfac, double rfac0, double rmin0, do
     return bad ? -1 : 0;
 }
 
+/* ------------------------------------------------------------------ */
+/* Row f3: derivative of the descriptors with respect to the atom       */
+/* positions, dB(r, j)/dR_alpha (Eq. (45): the third  */
+/* factor of the chain rule, applied to a per-grid-point vector).       */
+/* Plain forward differentiation of the definition above, term by term: */
+/*   d/dR of f_c, theta0, the quaternion, (a, b);                       */
+/*   dD^J by the product rule on the double binomial sum;               */
+/*   dB = T(dU,U,U) + T(U,dU,U) + T(U,U,dU) for the trilinear form      */
+/*   T(X,Y,W) = Re sum conj(W^j) sum CG CG X^{j1} Y^{j2}, full sums.    */
+/* All images of atom alpha move with it.  No adjoint trick, no         */
+/* symmetry: the CUDA path (Y contraction + dU recursion) shares        */
+/* nothing with this.  Pinned in tests/test_force_oracle.py by central  */
+/* finite differences of oracle_bispectrum_points, by the closed forms  */
+/* of the one-neighbor case and of B_000, by sum_alpha dB/dR_alpha =    */
+/* -dB/dr (point moved instead of atoms) and by rotation covariance.    */
+/* ------------------------------------------------------------------ */
+
+/* d(a, b, fc)/dR_k for k = x, y, z (d = R - r_point).  Returns 0 if not a neighbor. */
+static int pair_grad(const double d[3], double rcut, double rfac0, double rmin0, cplx *a, cplx *b, double *fc,
+                     cplx da[3], cplx db[3], double dfc[3])
+{
+    double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+    if (!(r < rcut)) return 0;
+    if (r < 1e-10 * rcut) { /* reading #11: U = I, weight w; the direction is undefined, the derivative is taken as 0 */
+        *a = 1.0; *b = 0.0; *fc = 1.0;
+        for (int k = 0; k < 3; k++) { da[k] = 0.0; db[k] = 0.0; dfc[k] = 0.0; }
+        return 1;
+    }
+    double x = (r - rmin0) / (rcut - rmin0);
+    double dxdr = 1.0 / (rcut - rmin0);
+    double fcp; /* dfc/dr */
+    if (x <= 0.0) { *fc = 1.0; fcp = 0.0; }
+    else { *fc = 0.5 * (cos(M_PI * x) + 1.0); fcp = -0.5 * M_PI * sin(M_PI * x) * dxdr; }
+    double th0 = rfac0 * M_PI * x, th0p = rfac0 * M_PI * dxdr;
+    double c0 = cos(th0), s0 = sin(th0);
+    double u[3] = {d[0] / r, d[1] / r, d[2] / r};
+    double q[4] = {c0, s0 * u[0], s0 * u[1], s0 * u[2]};
+    *a = q[0] - I * q[3];
+    *b = q[2] - I * q[1];
+    for (int k = 0; k < 3; k++) {
+        double dr = u[k]; /* dr/dR_k */
+        double dq0 = -s0 * th0p * dr;
+        double dq[3];
+        for (int i = 0; i < 3; i++) dq[i] = c0 * th0p * dr * u[i] + s0 * (((i == k) ? 1.0 : 0.0) - u[i] * u[k]) / r;
+        da[k] = dq0 - I * dq[2];
+        db[k] = dq[1] - I * dq[0];
+        dfc[k] = fcp * dr;
+    }
+    return 1;
+}
+
+/* D^J(g) and its directional derivative for (da, db): product rule on every factor of the double binomial sum */
+static void wigner_dD(int J, cplx a, cplx b, cplx da, cplx db, cplx *dD)
+{
+    cplx g[4] = {a, -conj(b), b, conj(a)};          /* g00 g01 g10 g11 */
+    cplx dg[4] = {da, -conj(db), db, conj(da)};
+    cplx pw[4][ORACLE_MAX_TWOJ + 1];
+    for (int f = 0; f < 4; f++) {
+        pw[f][0] = 1.0;
+        for (int i = 1; i <= J; i++) pw[f][i] = pw[f][i - 1] * g[f];
+    }
+    for (int mp = 0; mp <= J; mp++)
+        for (int m = 0; m <= J; m++) {
+            cplx s = 0.0;
+            for (int k = 0; k <= m; k++) {
+                int l = mp - k;
+                if (l < 0 || l > J - m) continue;
+                int e[4] = {k, m - k, l, J - m - l};    /* exponents of g00 g01 g10 g11 */
+                cplx term = 0.0;
+                for (int f = 0; f < 4; f++) {
+                    if (e[f] == 0) continue;
+                    cplx t = (double)e[f] * pw[f][e[f] - 1] * dg[f];
+                    for (int h = 0; h < 4; h++)
+                        if (h != f) t *= pw[h][e[h]];
+                    term += t;
+                }
+                s += binom(m, k) * binom(J - m, l) * term;
+            }
+            double nrm = sqrt(fact(mp) * fact(J - mp) / (fact(m) * fact(J - m)));
+            dD[mp * (J + 1) + m] = nrm * s;
+        }
+}
+
+/* T(X, Y, W)[t] = Re sum_{m,m'} conj(W^j[m,m']) sum CG CG X^{j1}[m1,m1'] Y^{j2}[m2,m2'], full sums (b_from_u with three arrays) */
+static void b_trilinear(const cgcache_t *cg, const cplx *X, const cplx *Y, const cplx *W, double *out)
+{
+    for (int t = 0; t < cg->n; t++) {
+        int J1 = cg->tr[3 * t], J2 = cg->tr[3 * t + 1], J = cg->tr[3 * t + 2];
+        const cplx *U1 = X + uoff(J1), *U2 = Y + uoff(J2), *UJ = W + uoff(J);
+        const double *C = cg->tab[t];
+        int sh = (J1 + J2 - J) / 2;
+        cplx acc = 0.0;
+        for (int m = 0; m <= J; m++)
+            for (int mp = 0; mp <= J; mp++) {
+                cplx z = 0.0;
+                for (int m1 = 0; m1 <= J1; m1++) {
+                    int m2 = m + sh - m1;
+                    if (m2 < 0 || m2 > J2) continue;
+                    double c1 = C[m1 * (J2 + 1) + m2];
+                    for (int m1p = 0; m1p <= J1; m1p++) {
+                        int m2p = mp + sh - m1p;
+                        if (m2p < 0 || m2p > J2) continue;
+                        double c2 = C[m1p * (J2 + 1) + m2p];
+                        z += c1 * c2 * U1[m1 * (J1 + 1) + m1p] * U2[m2 * (J2 + 1) + m2p];
+                    }
+                }
+                acc += conj(UJ[m * (J + 1) + mp]) * z;
+            }
+        out[t] = creal(acc);
+    }
+}
+
+/* dB at explicit points.  dB_out (optional) [npoints][natoms][3][ncomp]; beta (optional) [npoints][ncomp] and
+ * g_out [natoms][3] = sum_p sum_t beta[p][t] dB[p][alpha][k][t]  (Eq. (45): "apply dB/dR_alpha to an array"). */
+int oracle_bispectrum_grad_points(int twojmax, double rcutfac, double rfac0, double rmin0, double wself, int ntypes, const double *radelem,
+                                  const double *wj, int natoms, const double *pos, const int *types, const double *box,
+                                  const double *origin, const int *pbc, int npoints, const double *points, double *dB_out,
+                                  const double *beta, double *g_out)
+{
+    if (twojmax < 0 || twojmax > ORACLE_MAX_TWOJ) return -1;
+    tables_init();
+    sys_t s = {twojmax, rcutfac, rfac0, rmin0, wself, ntypes, radelem, wj, natoms, pos, types, box, origin, pbc, NULL, {0, 0, 0}, 0.0};
+    if (sys_prepare(&s)) return -1;
+    int nt = oracle_ntriples(twojmax);
+    int *tr = (int *)malloc(sizeof(int) * 3 * nt);
+    oracle_triples(twojmax, tr);
+    cgcache_t cg;
+    cg_build(&cg, nt, tr);
+    int usz = uoff(twojmax + 1);
+    const double *a1 = box, *a2 = box + 3, *a3 = box + 6;
+    if (g_out)
+        for (int i = 0; i < 3 * natoms; i++) g_out[i] = 0.0;
+#pragma omp parallel
+    {
+        cplx *U = (cplx *)malloc(sizeof(cplx) * usz);
+        cplx *dU = (cplx *)malloc(sizeof(cplx) * usz * 3);
+        cplx *D = (cplx *)malloc(sizeof(cplx) * (twojmax + 1) * (twojmax + 1));
+        cplx *dD = (cplx *)malloc(sizeof(cplx) * (twojmax + 1) * (twojmax + 1));
+        double *t1 = (double *)malloc(sizeof(double) * nt * 3), *gl = (double *)calloc(3 * (natoms > 0 ? natoms : 1), sizeof(double));
+#pragma omp for schedule(dynamic, 1)
+        for (int p = 0; p < npoints; p++) {
+            const double *rp = points + 3 * p;
+            utot_point(&s, rp, U, D, NULL, 0);
+            for (int n = 0; n < natoms; n++) {
+                int t = types[n];
+                double rcut = 2.0 * rcutfac * radelem[t], w = wj[t];
+                for (int i = 0; i < 3 * usz; i++) dU[i] = 0.0;
+                int hits = 0;
+                for (int n1 = -s.nimg[0]; n1 <= s.nimg[0]; n1++)
+                    for (int n2 = -s.nimg[1]; n2 <= s.nimg[1]; n2++)
+                        for (int n3 = -s.nimg[2]; n3 <= s.nimg[2]; n3++) {
+                            double d[3];
+                            for (int k = 0; k < 3; k++) d[k] = s.wpos[3 * n + k] + n1 * a1[k] + n2 * a2[k] + n3 * a3[k] - rp[k];
+                            cplx a, b, da[3], db[3];
+                            double fc, dfc[3];
+                            if (!pair_grad(d, rcut, rfac0, rmin0, &a, &b, &fc, da, db, dfc)) continue;
+                            hits++;
+                            for (int J = 0; J <= twojmax; J++) {
+                                wigner_D(J, a, b, D);
+                                for (int k = 0; k < 3; k++) {
+                                    wigner_dD(J, a, b, da[k], db[k], dD);
+                                    cplx *dUJ = dU + (size_t)k * usz + uoff(J);
+                                    for (int i = 0; i < (J + 1) * (J + 1); i++) dUJ[i] += w * (dfc[k] * D[i] + fc * dD[i]);
+                                }
+                            }
+                        }
+                double *dst = dB_out ? dB_out + (((size_t)p * natoms + n) * 3) * nt : NULL;
+                if (!hits) {
+                    if (dst) for (int i = 0; i < 3 * nt; i++) dst[i] = 0.0;
+                    continue;
+                }
+                for (int k = 0; k < 3; k++) {
+                    const cplx *dUk = dU + (size_t)k * usz;
+                    b_trilinear(&cg, dUk, U, U, t1);
+                    b_trilinear(&cg, U, dUk, U, t1 + nt);
+                    b_trilinear(&cg, U, U, dUk, t1 + 2 * nt);
+                    double acc = 0.0;
+                    for (int i = 0; i < nt; i++) {
+                        double v = t1[i] + t1[nt + i] + t1[2 * nt + i];
+                        if (dst) dst[k * nt + i] = v;
+                        if (beta) acc += beta[(size_t)p * nt + i] * v;
+                    }
+                    gl[3 * n + k] += acc;
+                }
+            }
+        }
+        if (g_out) {
+#pragma omp critical
+            for (int i = 0; i < 3 * natoms; i++) g_out[i] += gl[i];
+        }
+        free(U); free(dU); free(D); free(dD); free(t1); free(gl);
+    }
+    cg_free(&cg);
+    free(tr);
+    free(s.wpos);
+    return 0;
+}
+
 int oracle_num_threads(void)
 {
 #ifdef _OPENMP

@@ -4,4 +4,5 @@
 synthetic inputs.  Nothing here imports the CPU oracle.
 """
 from .snap import (MalaSnap, MalaSnapError, load_library, library_path, mala_last_error,  # noqa: F401
-                   mala_snap_clebsch_gordan, mala_snap_fp64_peak, bispectrum_for_workload)
+                   mala_snap_clebsch_gordan, mala_snap_fp64_peak, bispectrum_for_workload, MalaMlp,
+                   bispectrum_ldos_grid)

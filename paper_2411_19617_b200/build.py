@@ -11,11 +11,11 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmala_snap.so")
-SOURCES = ["mala_snap.cu"]
-DEPS = ["mala_snap.cu", "snap_common.cuh", "snap_tables.h", "snap_ui.cuh", "snap_zi.cuh", "snap_zi_coop.cuh", "snap_zi_diag.cuh", "snap_gauss.cuh",
-        os.path.join("..", "..", "include", "mala_snap.h")]
+SOURCES = ["mala_snap.cu", "mala_mlp.cu"]
+DEPS = ["mala_snap.cu", "mala_mlp.cu", "snap_common.cuh", "snap_internal.h", "snap_tables.h", "snap_ui.cuh", "snap_zi.cuh", "snap_zi_coop.cuh",
+        "snap_zi_diag.cuh", "snap_gauss.cuh", os.path.join("..", "..", "include", "mala_snap.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "--expt-relaxed-constexpr", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-shared", "-diag-suppress", "177"]
+              "-Xcompiler", "-fPIC", "-diag-suppress", "177"]
 
 
 def nvcc():
@@ -30,8 +30,18 @@ def build(force: bool = False, verbose: bool = False) -> str:
     newest = max(newest, os.path.getmtime(os.path.abspath(__file__)))
     if (not force) and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
         return LIB
-    cmd = [nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SOURCES
-    subprocess.check_call(cmd, cwd=CSRC)
+    objdir = os.path.join(HERE, "build")
+    os.makedirs(objdir, exist_ok=True)
+    procs, objs = [], []
+    for src in SOURCES:   # one nvcc per translation unit, side by side
+        obj = os.path.join(objdir, os.path.splitext(src)[0] + ".o")
+        objs.append(obj)
+        cmd = [nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, src]
+        procs.append((cmd, subprocess.Popen(cmd, cwd=CSRC)))
+    for cmd, p in procs:
+        if p.wait() != 0:
+            raise subprocess.CalledProcessError(p.returncode, cmd)
+    subprocess.check_call([nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs)
     return LIB
 
 

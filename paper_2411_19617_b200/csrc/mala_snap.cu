@@ -17,6 +17,7 @@
 
 #include "../../include/mala_snap.h"
 #include "snap_common.cuh"
+#include "snap_internal.h"
 #include "snap_tables.h"
 #include "snap_ui.cuh"
 #include "snap_zi.cuh"
@@ -32,6 +33,10 @@ static int fail(int code, const std::string &msg) {
     g_last_error = msg;
     return code;
 }
+
+namespace mala {
+int set_error(int code, const std::string &msg) { return fail(code, msg); }
+}  // namespace mala
 
 #define CUDA_TRY(call)                                                                              \
     do {                                                                                            \
@@ -123,6 +128,7 @@ struct mala_snap {
     int sticky_status = 0;         // bits seen so far (a raised bit makes every later call fail)
     int cand_cap_limit = 0;        // test hook: clamp the candidate capacity (0 = off) to provoke the overflow path
     DevBuf<double2> d_utot;
+    DevBuf<double> d_bstage;       // fused network: descriptors of one chunk, [tile][32][ncomp]
     DevBuf<double> d_stage[2];
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t ev_done[2] = {nullptr, nullptr}, ev_copied[2] = {nullptr, nullptr};
@@ -694,7 +700,10 @@ int candidate_bound(const mala_snap *h) {
 
 // enqueue the whole path for the slab [z0, z1) into out (DEVICE, relative to z0); out == nullptr: stop after compute_ui
 // and scatter U_tot into u_out (test hook)
-int run_slab(mala_snap *h, int z0, int z1, double *out, double2 *u_out, cudaStream_t st) {
+// net != nullptr: the descriptors of every chunk go to a compact staging buffer and the network maps them to ldos (DEVICE,
+// [points of the slab][w_out] fp32) before the next chunk starts; out is not used
+int run_slab(mala_snap *h, int z0, int z1, double *out, double2 *u_out, cudaStream_t st, const mala_mlp *net = nullptr,
+             float *ldos = nullptr) {
     if (z1 <= z0) return 0;
     choose_tiles(h, z0, z1);
     GridGeom &g = h->geom;
@@ -702,10 +711,14 @@ int run_slab(mala_snap *h, int z0, int z1, double *out, double2 *u_out, cudaStre
     if (h->cand_cap < 0) return fail(MALA_SNAP_EINVAL, "more than 2^24 candidate atoms per tile; use a finer cell or smaller z-slabs");
     const long long total_tiles = h->total_tiles;
     if (total_tiles > 2000000000LL) return fail(MALA_SNAP_EINVAL, "slab has too many tiles; use smaller z-slabs");
-    const size_t per_tile = (size_t)h->sc.nelem * 32 * sizeof(double2) + (size_t)h->cand_cap * sizeof(int) + 2 * sizeof(int);
+    const size_t per_tile = (size_t)h->sc.nelem * 32 * sizeof(double2) + (size_t)h->cand_cap * sizeof(int) + 2 * sizeof(int) +
+                            (net ? (size_t)32 * h->sc.ntriples * sizeof(double) : 0);
     const size_t budget = (size_t)std::max<long long>(h->workspace_mb, 1) << 20;
     long long chunk_tiles = (long long)std::max<size_t>(budget / per_tile, (size_t)h->num_sms);
     chunk_tiles = std::min(chunk_tiles, total_tiles);
+    if (net && h->d_bstage.reserve((size_t)chunk_tiles * 32 * h->sc.ntriples, st, true))
+        return fail(MALA_SNAP_ENOMEM, "cudaMallocAsync (descriptor staging) failed");
+    if (net) out = h->d_bstage.p;
     if (h->d_utot.reserve((size_t)chunk_tiles * h->sc.nelem * 32, st, true) || h->d_cand.reserve((size_t)chunk_tiles * h->cand_cap, st, true) ||
         h->d_ncand.reserve(chunk_tiles, st, true) || h->d_active.reserve(chunk_tiles, st, true) || h->d_counters.reserve(4, st, true))
         return fail(MALA_SNAP_ENOMEM, "cudaMallocAsync (workspace) failed");
@@ -719,6 +732,7 @@ int run_slab(mala_snap *h, int z0, int z1, double *out, double2 *u_out, cudaStre
         cb.status = h->d_status.p;
         cb.utot = h->d_utot.p; cb.cand_cap = h->cand_cap;
         cb.utot_half = h->half_tiles() ? 1 : 0;
+        cb.compact_out = net ? 1 : 0;
         cb.tile_begin = (int)t0;
         cb.ntiles = (int)std::min(chunk_tiles, total_tiles - t0);
         CUDA_TRY(cudaMemsetAsync(cb.counters, 0, 4 * sizeof(int), st));
@@ -747,6 +761,14 @@ int run_slab(mala_snap *h, int z0, int z1, double *out, double2 *u_out, cudaStre
         if (out) {
             int rc = launch_zi(h, cb, out, st);
             if (rc) return rc;
+            if (net) {
+                MlpRows rows{};
+                rows.nrows = (long long)cb.ntiles * 32; rows.x = out; rows.y = ldos; rows.compact = 1; rows.tile_begin = cb.tile_begin;
+                rows.geom = g;
+                TimedSpan span(h, st, kKindOther);
+                if ((rc = mlp_launch(net, rows, st))) return rc;
+                h->stats[0]++;
+            }
         } else if (u_out) {
             TimedSpan span(h, st, kKindOther);
             utot_scatter_kernel<<<bin_blocks, 256, 0, st>>>(g, h->sc, tb, cb, u_out);
@@ -1220,6 +1242,24 @@ int mala_bispectrum_grid_host(mala_snap_t *h, int natoms, const double *pos, con
     return check_status(h, true);
 }
 
+int mala_bispectrum_ldos_grid(mala_snap_t *h, mala_mlp_t *net, int natoms, const double *pos, const int *types, const double box[9],
+                              const double origin[3], const int pbc[3], const int ngrid[3], int z_begin, int z_end, float *ldos,
+                              void *cuda_stream) {
+    const CallArgs a{natoms, pos, types, box, origin, pbc, ngrid, z_begin, z_end};
+    int rc = validate(h, a, true, ldos);
+    if (rc) return rc;
+    if (!net) return fail(MALA_SNAP_EINVAL, "net is NULL");
+    if (mlp_in_width(net) != h->sc.ntriples)
+        return fail(MALA_SNAP_EINVAL, "the network's input width differs from the number of bispectrum components of this handle");
+    if ((rc = check_status(h, false))) return rc;
+    std::fill(h->stats, h->stats + 8, 0LL);
+    if (z_end == z_begin) return MALA_SNAP_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if ((rc = build_plan(h, a, st))) return rc;
+    if ((rc = run_slab(h, z_begin, z_end, nullptr, nullptr, st, net, ldos))) return rc;
+    return finish_call(h, st);
+}
+
 int mala_gaussian_grid(mala_snap_t *h, double sigma, int natoms, const double *pos, const int *types, const double box[9],
                        const double origin[3], const int pbc[3], const int ngrid[3], int z_begin, int z_end, double *out,
                        void *cuda_stream) {
@@ -1268,7 +1308,7 @@ void mala_snap_destroy(mala_snap_t *h) {
         if (h->ev_copied[i]) cudaEventDestroy(h->ev_copied[i]);
     }
     h->d_cand.release(); h->d_ncand.release(); h->d_active.release(); h->d_counters.release(); h->d_utot.release();
-    h->d_status.release();
+    h->d_status.release(); h->d_bstage.release();
     h->d_dcg.release(); h->d_dtriple.release(); h->d_dsched.release(); h->d_ditems.release();
     if (h->h_status) cudaFreeHost(h->h_status);
     for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);

@@ -72,6 +72,8 @@ struct ChunkBuffers {
     int *status;             // handle-wide status word, never cleared by a chunk: kStatus* bits
     double2 *utot;           // [chunk_tiles][nelem][32], or [chunk_tiles][2][nelem][16] when utot_half is set
     int utot_half;           // 1: half-tile layout (twojmax > kFullTileTwoJ)
+    int compact_out;         // 1: descriptors go to out[(local tile) * 32 + lane][ncomp] (staging for the fused network)
+                             //    instead of out[grid point][ncomp]
     int cand_cap;
     int tile_begin;          // first global tile id of the chunk
     int ntiles;              // tiles in the chunk
@@ -100,5 +102,16 @@ __host__ __device__ inline TileInfo tile_info(const GridGeom &g, int tile) {
     ti.radius = R.tile_radius;
     return ti;
 }
+
+// grid point of lane `lane` of tile `tile` (bricks are filled x fastest); valid = the point exists (ragged tiles, slab end)
+__host__ __device__ inline void lane_point(const GridGeom &g, int tile, int lane, int &ix, int &iy, int &iz, bool &valid) {
+    const TileInfo ti = tile_info(g, tile);
+    const int lx = lane % ti.tx, ly = (lane / ti.tx) % ti.ty, lz = lane / (ti.tx * ti.ty);
+    ix = ti.ix0 + lx;
+    iy = ti.iy0 + ly;
+    iz = ti.iz0 + lz;
+    valid = (ix < ti.xend) && (iy < ti.yend) && (iz < g.z1);
+}
+
 
 }  // namespace mala

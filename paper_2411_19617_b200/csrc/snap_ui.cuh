@@ -19,15 +19,6 @@ namespace mala {
 constexpr int kGeoCap = 48;     // neighbor entries per grid point buffered between two accumulate passes
 constexpr int kUiPoints = 16;   // grid points per compute_ui CTA: half a tile; lane = (point, half), the halves split the neighbors
 
-__device__ __forceinline__ void lane_point(const GridGeom &g, int tile, int lane, int &ix, int &iy, int &iz, bool &valid) {
-    const TileInfo ti = tile_info(g, tile);
-    const int lx = lane % ti.tx, ly = (lane / ti.tx) % ti.ty, lz = lane / (ti.tx * ti.ty);
-    ix = ti.ix0 + lx;
-    iy = ti.iy0 + ly;
-    iz = ti.iz0 + lz;
-    valid = (ix < ti.xend) && (iy < ti.yend) && (iz < g.z1);
-}
-
 __device__ __forceinline__ void point_position(const GridGeom &g, int ix, int iy, int iz, double &x, double &y, double &z) {
     const double fx = (double)ix / (double)g.nx, fy = (double)iy / (double)g.ny, fz = (double)iz / (double)g.nz;
     x = g.origin[0] + fx * g.a1[0] + fy * g.a2[0] + fz * g.a3[0];
@@ -105,6 +96,11 @@ __global__ void __launch_bounds__(256) tile_bin_kernel(GridGeom g, SnapConst sc,
     if (out == nullptr) return;
     // empty tile: constant descriptor, written as contiguous rows of tx points
     const int nt = sc.ntriples;
+    if (cb.compact_out) {
+        double *dst = out + (size_t)wt * 32 * nt;
+        for (int i = lane; i < 32 * nt; i += 32) __stcs(dst + i, tb.bconst[i % nt]);
+        return;
+    }
     const int ix0 = ti.ix0;
     const int npx = min(ti.tx, ti.xend - ix0);
     for (int r = 0; r < ti.ty * ti.tz; r++) {

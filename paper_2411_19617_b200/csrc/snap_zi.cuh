@@ -82,8 +82,16 @@ __device__ __forceinline__ void prefetch_l2_tile(const double2 *src, int nelem) 
 
 // ---- writer (row a7): B of one tile, staged as Bs[lane][nt] in shared memory, to out[point][nt] --------------
 // Points of one tile row (fixed iy, iz) are consecutive in x, so a row is one contiguous run of npx*nt doubles.
-__device__ __forceinline__ void write_tile(const GridGeom &g, int tile, const double *Bs, int nt, double *out, int nwarps) {
+// compact (ChunkBuffers::compact_out): the tile's 32 x nt block goes, as it is, to out[wt * 32 ...] (wt = tile id in the chunk).
+__device__ __forceinline__ void write_tile(const GridGeom &g, int tile, const double *Bs, int nt, double *out, int nwarps,
+                                           int compact = 0, int wt = 0) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (compact) {
+        double2 *d2 = reinterpret_cast<double2 *>(out + (size_t)wt * 32 * nt);   // 32 * nt * 8 bytes is a multiple of 16
+        const double2 *s2 = reinterpret_cast<const double2 *>(Bs);
+        for (int i = threadIdx.x; i < 16 * nt; i += nwarps * 32) __stcs(d2 + i, s2[i]);
+        return;
+    }
     const TileInfo ti = tile_info(g, tile);
     const int ix0 = ti.ix0;
     const int npx = min(ti.tx, ti.xend - ix0);
@@ -202,7 +210,7 @@ compute_zi_bi_generic_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuf
             Bs[lane * nt + t] = b;
         }
         __syncthreads();
-        write_tile(g, cb.tile_begin + wt, Bs, nt, out, kZiWarps);
+        write_tile(g, cb.tile_begin + wt, Bs, nt, out, kZiWarps, cb.compact_out, wt);
     }
 }
 

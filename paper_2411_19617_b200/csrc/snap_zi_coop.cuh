@@ -165,6 +165,55 @@ __device__ __forceinline__ void cg_convolve(double (&zr)[J + 1], double (&zi)[J 
 
 // items mb1 in [mb1_begin, mb1_end) of output column mb: returns their contribution to B.
 // MID: mb is the middle column of an even J; only rows ma <= J/2 are formed.
+// x = U^{J1}[:, mb1]; columns beyond the middle come from the stored half by u[ma][mb] = (-1)^(ma-mb) conj(u[J-ma][J-mb])
+template <int J1>
+__device__ __forceinline__ void load_x_column(const unsigned char *Ulane, const int mb1, double (&xr)[J1 + 1], double (&xi)[J1 + 1]) {
+    if (mb1 <= J1 / 2) {  // stored column: plain loads (the branch is warp-uniform)
+        const unsigned char *xb = Ulane + (uhalf_off(J1) + mb1 * (J1 + 1)) * kRowBytes;
+#pragma unroll
+        for (int k = 0; k <= J1; k++) {
+            const double2 v = *reinterpret_cast<const double2 *>(xb + k * kRowBytes);
+            xr[k] = v.x;
+            xi[k] = v.y;
+        }
+    } else {  // mirror column, read backwards; real part (-1)^(ma1-mb1), imaginary part the opposite (conjugation)
+        const unsigned char *xb = Ulane + (uhalf_off(J1) + (J1 - mb1) * (J1 + 1) + J1) * kRowBytes;
+        const unsigned m0 = (mb1 & 1) ? 0x80000000u : 0u;
+#pragma unroll
+        for (int k = 0; k <= J1; k++) {
+            const double2 v = *reinterpret_cast<const double2 *>(xb - k * kRowBytes);
+            xr[k] = flip_sign(v.x, (k & 1) ? (m0 ^ 0x80000000u) : m0);
+            xi[k] = flip_sign(v.y, (k & 1) ? m0 : (m0 ^ 0x80000000u));
+        }
+    }
+}
+
+// weight of item (mb, mb1): the CG factor of its column pair times the number of items it stands for
+template <int J1, int J2, int J, int CGOFF>
+__device__ __forceinline__ double item_cgb(const int mb, const int mb1) {
+    constexpr int SH = (J1 + J2 - J) / 2;
+    const int mb2 = mb + SH - mb1;
+    double cgb = c_cg_spec[CGOFF + mb2 * (J1 + 1) + mb1];
+    if (item_symmetric3(J1, J2, J)) cgb *= item_weight3(J, mb, mb1);  // stands for its whole symmetry class
+    else if (J1 == J2 && mb1 != mb2) cgb += cgb;                        // stands for its mirror item (mb2, mb1) too
+    if (item_hermitian(J1, J2, J) && mb1 != mb && mb1 != J - mb) cgb += cgb;  // and for item (mb1, mb)
+    return cgb;
+}
+
+// y = U^{J2}[:, mb2] with the same column symmetry, folded with cgb into four scale factors
+template <int J2>
+__device__ __forceinline__ void y_column(const unsigned char *Ulane, const int mb2, const double cgb, const unsigned char *&yb, int &ystep,
+                                         double &p0, double &p1, double &q0, double &q1) {
+    const bool fy = mb2 > J2 / 2;
+    const int cy = fy ? J2 - mb2 : mb2;
+    yb = Ulane + (uhalf_off(J2) + cy * (J2 + 1) + (fy ? J2 : 0)) * kRowBytes;
+    ystep = fy ? -kRowBytes : kRowBytes;
+    p0 = (fy && (mb2 & 1)) ? -cgb : cgb;  // parity-0 rows, real part
+    p1 = fy ? -p0 : cgb;                  // parity-1 rows, real part
+    q0 = fy ? -p0 : cgb;                  // imaginary parts: conjugation flips the sign again
+    q1 = fy ? -p1 : cgb;
+}
+
 template <int J1, int J2, int J, int CGOFF, bool MID>
 __device__ __forceinline__ double column_segment(const unsigned char *Ulane, const int mb, const int mb1_begin, const int mb1_end) {
     constexpr int SH = (J1 + J2 - J) / 2;
@@ -174,32 +223,8 @@ __device__ __forceinline__ double column_segment(const unsigned char *Ulane, con
     for (int k = 0; k <= J; k++) { zr[k] = 0.0; zi[k] = 0.0; }
 #pragma unroll 1
     for (int mb1 = mb1_begin; mb1 < mb1_end; mb1++) {
-        const int mb2 = mb + SH - mb1;
-        double cgb = c_cg_spec[CGOFF + mb2 * (J1 + 1) + mb1];
-        if (item_symmetric3(J1, J2, J)) cgb *= item_weight3(J, mb, mb1);  // stands for its whole symmetry class
-        else if (J1 == J2 && mb1 != mb2) cgb += cgb;                        // stands for its mirror item (mb2, mb1) too
-        if (item_hermitian(J1, J2, J) && mb1 != mb && mb1 != J - mb) cgb += cgb;  // and for item (mb1, mb)
-        // x = U^{J1}[:, mb1]; columns beyond the middle come from the stored half by
-        // u[ma][mb] = (-1)^(ma-mb) conj(u[J-ma][J-mb])
         double xr[J1 + 1], xi[J1 + 1];
-        if (mb1 <= J1 / 2) {  // stored column: plain loads (the branch is warp-uniform)
-            const unsigned char *xb = Ulane + (uhalf_off(J1) + mb1 * (J1 + 1)) * kRowBytes;
-#pragma unroll
-            for (int k = 0; k <= J1; k++) {
-                const double2 v = *reinterpret_cast<const double2 *>(xb + k * kRowBytes);
-                xr[k] = v.x;
-                xi[k] = v.y;
-            }
-        } else {  // mirror column, read backwards; real part (-1)^(ma1-mb1), imaginary part the opposite (conjugation)
-            const unsigned char *xb = Ulane + (uhalf_off(J1) + (J1 - mb1) * (J1 + 1) + J1) * kRowBytes;
-            const unsigned m0 = (mb1 & 1) ? 0x80000000u : 0u;
-#pragma unroll
-            for (int k = 0; k <= J1; k++) {
-                const double2 v = *reinterpret_cast<const double2 *>(xb - k * kRowBytes);
-                xr[k] = flip_sign(v.x, (k & 1) ? (m0 ^ 0x80000000u) : m0);
-                xi[k] = flip_sign(v.y, (k & 1) ? m0 : (m0 ^ 0x80000000u));
-            }
-        }
+        load_x_column<J1>(Ulane, mb1, xr, xi);
         if (item_stretched(J1, J2, J)) {
 #pragma unroll
             for (int k = 0; k <= J1; k++) {
@@ -207,15 +232,10 @@ __device__ __forceinline__ double column_segment(const unsigned char *Ulane, con
                 xi[k] *= c_sqbin[J1][k];
             }
         }
-        // y = U^{J2}[:, mb2], same symmetry, folded with cgb into four scale factors
-        const bool fy = mb2 > J2 / 2;
-        const int cy = fy ? J2 - mb2 : mb2;
-        const unsigned char *yb = Ulane + (uhalf_off(J2) + cy * (J2 + 1) + (fy ? J2 : 0)) * kRowBytes;
-        const int ystep = fy ? -kRowBytes : kRowBytes;
-        const double p0 = (fy && (mb2 & 1)) ? -cgb : cgb;  // parity-0 rows, real part
-        const double p1 = fy ? -p0 : cgb;                  // parity-1 rows, real part
-        const double q0 = fy ? -p0 : cgb;                  // imaginary parts: conjugation flips the sign again
-        const double q1 = fy ? -p1 : cgb;
+        const unsigned char *yb;
+        int ystep;
+        double p0, p1, q0, q1;
+        y_column<J2>(Ulane, mb + SH - mb1, item_cgb<J1, J2, J, CGOFF>(mb, mb1), yb, ystep, p0, p1, q0, q1);
         cg_convolve<J1, J2, J, CGOFF, MAHI>(zr, zi, xr, xi, yb, ystep, p0, p1, q0, q1);
     }
     // compute_bi: B += w * Re(conj(U^J[ma][mb]) * z[ma]).  Columns below the middle stand for their mirror images
@@ -349,7 +369,7 @@ compute_zi_bi_coop_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffer
             }
         }
         __syncthreads();
-        write_tile(g, cb.tile_begin + wt, Bs, nt, out, NW);
+        write_tile(g, cb.tile_begin + wt, Bs, nt, out, NW, cb.compact_out, wt);
     }
 }
 

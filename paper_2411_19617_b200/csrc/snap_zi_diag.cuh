@@ -327,7 +327,7 @@ compute_zi_bi_diag_kernel(GridGeom g, SnapConst sc, DeviceTables tb, DiagTables 
             }
         }
         __syncthreads();
-        write_tile(g, cb.tile_begin + wt, Bs, nt, out, NW);
+        write_tile(g, cb.tile_begin + wt, Bs, nt, out, NW, cb.compact_out, wt);
     }
 }
 
@@ -421,8 +421,14 @@ __device__ __forceinline__ double diag_dispatch_half(const int J1, const unsigne
 }
 
 // B of 16 points, staged as Bs[point][nt], to out[point][nt]: one warp per point row of nt doubles
-__device__ __forceinline__ void write_half_tile(const GridGeom &g, int tile, int half, const double *Bs, int nt, double *out, int nwarps) {
+__device__ __forceinline__ void write_half_tile(const GridGeom &g, int tile, int half, const double *Bs, int nt, double *out, int nwarps,
+                                                int compact, int wt) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (compact) {
+        double *dst = out + ((size_t)wt * 32 + half * 16) * nt;
+        for (int i = threadIdx.x; i < 16 * nt; i += nwarps * 32) __stcs(dst + i, Bs[i]);
+        return;
+    }
     for (int p = warp; p < 16; p += nwarps) {
         int ix, iy, iz;
         bool valid;
@@ -487,7 +493,7 @@ compute_zi_bi_diag_half_kernel(GridGeom g, SnapConst sc, DeviceTables tb, DiagTa
             }
         }
         __syncthreads();
-        write_half_tile(g, cb.tile_begin + wt, half, Bs, nt, out, NW);
+        write_half_tile(g, cb.tile_begin + wt, half, Bs, nt, out, NW, cb.compact_out, wt);
     }
 }
 

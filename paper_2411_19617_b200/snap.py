@@ -9,6 +9,7 @@ import os
 
 import numpy as np
 
+dp_t = C.POINTER(C.c_double)
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libmala_snap.so")
 _lib = None
@@ -19,7 +20,7 @@ MALA_SNAP_ECUDA = -2
 MALA_SNAP_ENOMEM = -3
 
 EXPORTS = ("mala_snap_create", "mala_snap_ncomp", "mala_snap_triples", "mala_bispectrum_grid", "mala_bispectrum_grid_host",
-           "mala_gaussian_grid",
+           "mala_gaussian_grid", "mala_mlp_create", "mala_mlp_widths", "mala_mlp_forward", "mala_mlp_destroy", "mala_bispectrum_ldos_grid",
            "mala_snap_set_option", "mala_snap_last_stats", "mala_snap_kernel_times", "mala_snap_zi_kernel", "mala_snap_fp64_peak", "mala_snap_clebsch_gordan", "mala_snap_debug_utot",
            "mala_snap_destroy", "mala_last_error")
 
@@ -62,6 +63,16 @@ def load_library():
     lib.mala_bispectrum_grid_host.argtypes = grid_args
     lib.mala_gaussian_grid.restype = C.c_int
     lib.mala_gaussian_grid.argtypes = [vp, C.c_double] + grid_args[1:]
+    lib.mala_mlp_create.restype = C.c_int
+    lib.mala_mlp_create.argtypes = [C.POINTER(vp), C.c_int, ip, C.POINTER(dp), C.POINTER(dp), C.c_int, C.c_int, dp, dp]
+    lib.mala_mlp_widths.restype = C.c_int
+    lib.mala_mlp_widths.argtypes = [vp, ip, ip]
+    lib.mala_mlp_forward.restype = C.c_int
+    lib.mala_mlp_forward.argtypes = [vp, C.c_longlong, vp, vp, vp]
+    lib.mala_mlp_destroy.restype = None
+    lib.mala_mlp_destroy.argtypes = [vp]
+    lib.mala_bispectrum_ldos_grid.restype = C.c_int
+    lib.mala_bispectrum_ldos_grid.argtypes = [vp, vp] + grid_args[1:]
     lib.mala_snap_debug_utot.restype = C.c_int
     lib.mala_snap_debug_utot.argtypes = grid_args
     lib.mala_snap_set_option.restype = C.c_int
@@ -251,6 +262,84 @@ class MalaSnap:
             _check(rc)
         assert rc == nelem
         return out
+
+
+ACTIVATIONS = {"identity": 0, "relu": 1, "leaky_relu": 2, "sigmoid": 3}
+
+
+class MalaMlp:
+    """The descriptor -> LDOS network (mala_mlp_create ... mala_mlp_destroy): weights[l] is [w_{l+1}, w_l], biases[l] is [w_{l+1}]."""
+
+    def __init__(self, weights, biases, act="leaky_relu", activate_last=True, in_shift=None, in_scale=None):
+        lib = load_library()
+        self._lib = lib
+        self._h = C.c_void_p()
+        ws = [_d(w) for w in weights]
+        bs = [_d(b).ravel() for b in biases]
+        if len(ws) != len(bs) or not ws:
+            raise ValueError("weights and biases must be non-empty lists of the same length")
+        sizes = [ws[0].shape[1]] + [w.shape[0] for w in ws]
+        for l, (w, b) in enumerate(zip(ws, bs)):
+            if w.ndim != 2 or w.shape[1] != sizes[l] or b.shape != (w.shape[0],):
+                raise ValueError(f"layer {l}: shapes do not chain")
+        sizes_a = _i(sizes)
+        wp = (dp_t * len(ws))(*[_dp(w) for w in ws])
+        bp = (dp_t * len(bs))(*[_dp(b) for b in bs])
+        sh = None if in_shift is None else _d(in_shift).ravel()
+        sc = None if in_scale is None else _d(in_scale).ravel()
+        for v in (sh, sc):
+            if v is not None and v.shape != (sizes[0],):
+                raise ValueError("in_shift / in_scale must have w_0 entries")
+        _check(lib.mala_mlp_create(C.byref(self._h), len(ws), _ip(sizes_a), wp, bp, int(ACTIVATIONS[act]), int(bool(activate_last)),
+                                   None if sh is None else _dp(sh), None if sc is None else _dp(sc)))
+        self.sizes = sizes
+        self.w_in, self.w_out = sizes[0], sizes[-1]
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            self._lib.mala_mlp_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    # -- mala_mlp_forward: x DEVICE [npoints, w_in] fp64 -> y DEVICE [npoints, w_out] fp32
+    def forward(self, x, out=None, stream=None):
+        import torch
+        if (not x.is_cuda) or x.dtype != torch.float64 or (not x.is_contiguous()) or x.dim() != 2 or x.shape[1] != self.w_in:
+            raise ValueError("x must be a contiguous CUDA float64 tensor [npoints, w_in]")
+        n = x.shape[0]
+        if out is None:
+            out = torch.empty((n, self.w_out), dtype=torch.float32, device=x.device)
+        if (not out.is_cuda) or out.dtype != torch.float32 or (not out.is_contiguous()) or out.numel() < n * self.w_out:
+            raise ValueError("out must be a contiguous CUDA float32 tensor with at least npoints*w_out elements")
+        s = torch.cuda.current_stream() if stream is None else stream
+        _check(self._lib.mala_mlp_forward(self._h, C.c_longlong(n), C.c_void_p(x.data_ptr()), C.c_void_p(out.data_ptr()),
+                                          C.c_void_p(s.cuda_stream)))
+        return out
+
+
+def bispectrum_ldos_grid(snap, net, pos, types, box, origin=(0, 0, 0), pbc=(1, 1, 1), ngrid=(1, 1, 1), z_begin=0, z_end=None, out=None,
+                         stream=None):
+    """mala_bispectrum_ldos_grid: LDOS [npoints, w_out] fp32 in device memory; the descriptors stay inside the library."""
+    import torch
+    args, keep, npts = snap._system(pos, types, box, origin, pbc, ngrid, z_begin, z_end)
+    if out is None:
+        out = torch.empty((npts, net.w_out), dtype=torch.float32, device="cuda")
+    if (not out.is_cuda) or out.dtype != torch.float32 or (not out.is_contiguous()) or out.numel() < npts * net.w_out:
+        raise ValueError("out must be a contiguous CUDA float32 tensor with at least npoints*w_out elements")
+    s = torch.cuda.current_stream() if stream is None else stream
+    _check(snap._lib.mala_bispectrum_ldos_grid(snap._h, net._h, *args, C.c_void_p(out.data_ptr()), C.c_void_p(s.cuda_stream)))
+    return out
 
 
 def bispectrum_for_workload(snap, w, out=None, host=False, z_begin=0, z_end=None):

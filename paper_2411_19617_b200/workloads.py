@@ -163,6 +163,19 @@ def binary_alloy(seed=1006, ngrid=(90, 90, 90)):
                     seed=seed, notes="256-site fcc cell, two species by a seeded coin: radelem (0.5, 0.4), wj (1.0, 0.6), 90^3 grid")
 
 
+def ldos_network(seed=2001, sizes=(91, 256, 256, 241), in_scale=0.02):
+    """Seeded synthetic weights of a descriptor -> LDOS network: the paper's trained models are not
+    available, so every W_l is N(0, 2 / w_l) and every b_l is N(0, 0.1^2) (hand-written Box-Muller); 241 outputs as in
+    PAPER.md:542.  The input scaling is the same constant for every feature: x_0 = in_scale * B, which puts the
+    descriptors of the Al configs into the range [0, 5].  Returns (weights, biases, in_shift, in_scale) as fp64 arrays."""
+    rng = _Rng(seed)
+    ws, bs = [], []
+    for wk, wn in zip(sizes[:-1], sizes[1:]):
+        ws.append(rng.normal((wn, wk)) * np.sqrt(2.0 / wk))
+        bs.append(0.1 * rng.normal((wn,)))
+    return ws, bs, np.zeros(sizes[0]), np.full(sizes[0], float(in_scale))
+
+
 CONFIGS = {
     1: tiny_al, 2: solid_al, 3: liquid_al, 4: boron_cluster, 5: be_slab,
     "tiny_al": tiny_al, "solid_al": solid_al, "liquid_al": liquid_al, "boron_cluster": boron_cluster, "be_slab": be_slab,
