@@ -37,16 +37,17 @@ constexpr int kMlpMaxWidth = 256;   // one MMA covers N <= 256; the A operand of
 constexpr int kMlpRows = 128;       // rows per tile = MMA M = TMEM lanes
 constexpr int kMlpBK = 16;          // K elements per ring stage (two MMA K-steps of 8)
 constexpr int kMlpStages = 4;
-constexpr int kMlpThreads = 192;    // warps 0-3: rows (loader + epilogue), warp 4: weight producer, warp 5: TMEM + MMA issue
+constexpr int kMlpRowWarps = 8;     // warps 0-7: loader + epilogue; warp w works on rows 32 (w & 3) .. + 31 (its TMEM subpartition) and
+                                    // on the column half w >> 2 of every accumulator
+constexpr int kMlpThreads = (kMlpRowWarps + 2) * 32;  // + warp 8: weight producer, warp 9: TMEM allocation + MMA issue
 constexpr int kMlpTmemCols = 256;
-constexpr int kXPerLane = kMlpMaxWidth / 32;  // input features per lane when a warp reads one row
 constexpr int kMlpABytes = kMlpRows * (kMlpMaxWidth + 1) * 4;  // A operand (128 KB); as output staging [128][w_out | 1] fp32 it needs 514 B more
 
 struct MlpParams {
     int nlayers;
     int act, activate_last;
     int w_in, w_out;
-    int K[kMlpMaxLayers], N[kMlpMaxLayers];   // padded: K to 16, N to 16
+    int K[kMlpMaxLayers], N[kMlpMaxLayers];   // padded: K to 16, N to 32 (two column halves of whole 16-column TMEM loads)
     int woff[kMlpMaxLayers];                  // float offset of layer l in the packed weight image
     int boff[kMlpMaxLayers];                  // float offset of layer l in the bias array
     const float *wpacked;                     // [layer][K block][chunk 0..3][n][4] TF32-rounded, zero padded
@@ -132,17 +133,17 @@ __device__ __forceinline__ float to_tf32(float v) {
     asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(v));
     return __uint_as_float(r);
 }
-__device__ __forceinline__ float activate(int act, float v) {
-    switch (act) {
-        case 1: return v > 0.f ? v : 0.f;
-        case 2: return v > 0.f ? v : 0.01f * v;
-        case 3: return 1.f / (1.f + __expf(-v));
-        default: return v;
-    }
+template <int ACT>
+__device__ __forceinline__ float activate(float v) {
+    if (ACT == 1) return fmaxf(v, 0.f);
+    if (ACT == 2) return v > 0.f ? v : 0.01f * v;
+    if (ACT == 3) return 1.f / (1.f + __expf(-v));
+    return v;
 }
 
 // ---- the kernel -----------------------------------------------------------------------------------------------
 // dynamic shared memory: A operand [Kmax/4][128][16 B] | ring [stages][16 KB] | biases | barriers
+template <int ACT>
 __global__ void __launch_bounds__(kMlpThreads, 1) mlp_forward_kernel(MlpParams P, MlpRows R) {
     extern __shared__ __align__(128) unsigned char smem[];
     unsigned char *Abuf = smem;                                   // kMlpMaxWidth / 4 chunks x 2048 B = 128 KB (+ staging slack)
@@ -156,7 +157,7 @@ __global__ void __launch_bounds__(kMlpThreads, 1) mlp_forward_kernel(MlpParams P
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < kMlpStages; s++) { mb_init(&full[s], 1); mb_init(&empty[s], 1); }
-        mb_init(a_ready, kMlpRows);
+        mb_init(a_ready, kMlpRowWarps * 32);
         mb_init(d_full, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -164,7 +165,7 @@ __global__ void __launch_bounds__(kMlpThreads, 1) mlp_forward_kernel(MlpParams P
         const int l = i / kMlpMaxWidth, n = i % kMlpMaxWidth;
         bias_s[i] = (n < P.N[l]) ? P.bias[P.boff[l] + n] : 0.f;
     }
-    if (warp == 5) {  // TMEM: one warp allocates (and frees at the end)
+    if (warp == kMlpRowWarps + 1) {  // TMEM: one warp allocates (and frees at the end)
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(s32(tmem_slot)), "n"(kMlpTmemCols));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
@@ -173,7 +174,7 @@ __global__ void __launch_bounds__(kMlpThreads, 1) mlp_forward_kernel(MlpParams P
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
 
-    if (warp == 4) {
+    if (warp == kMlpRowWarps) {
         // ===== weight producer: the same sequence of K-blocks for every tile =====
         if (lane == 0) {
             uint32_t it = 0;
@@ -189,7 +190,7 @@ __global__ void __launch_bounds__(kMlpThreads, 1) mlp_forward_kernel(MlpParams P
                     }
                 }
         }
-    } else if (warp == 5) {
+    } else if (warp == kMlpRowWarps + 1) {
         // ===== MMA issuer =====
         if (lane == 0) {
             uint32_t it = 0, step = 0;
@@ -217,42 +218,31 @@ __global__ void __launch_bounds__(kMlpThreads, 1) mlp_forward_kernel(MlpParams P
         }
     } else {
         // ===== rows: load the descriptors, then one epilogue per layer =====
-        const int row = threadIdx.x;  // 0..127 = TMEM lane
+        const int sub = warp & 3, half = warp >> 2;
+        const int row = sub * 32 + lane;  // the TMEM lane (= tile row) this thread reads
         uint32_t step = 0;
         float *stage_out = reinterpret_cast<float *>(Abuf);  // last layer: [row][ostride] fp32
         const int ostride = P.w_out | 1;                     // odd stride: conflict-free row-per-thread writes
-        double xsh[kXPerLane], xsc[kXPerLane];               // input scaling of the features this lane owns
-#pragma unroll
-        for (int q = 0; q < kXPerLane; q++) {
-            const int k = lane + 32 * q;
-            xsh[q] = k < P.w_in ? P.in_shift[k] : 0.0;
-            xsc[q] = k < P.w_in ? P.in_scale[k] : 0.0;       // padded features become exact zeros
-        }
         for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
             const long long row0 = tile * kMlpRows;
-            // ---- layer-0 operand: x = (descriptor - shift) * scale, rounded to TF32.  Warp w takes rows w, w + 4, ...; a lane owns
+            // ---- layer-0 operand: x = (descriptor - shift) * scale, rounded to TF32.  Warp w takes rows w, w + 8, ...; a lane owns
             // the features k = lane, lane + 32, ... of every row (coalesced 8-byte loads), eight rows of loads in flight at a time
-            for (int rb = 0; rb < kMlpRows / 4; rb += 8) {
-                double xv[8][kXPerLane];
+#pragma unroll 1
+            for (int k = lane; k < P.K[0]; k += 32) {
+                const bool kin = k < P.w_in;
+                const double sh = kin ? P.in_shift[k] : 0.0, sc = kin ? P.in_scale[k] : 0.0;  // padded features become exact zeros
+                unsigned char *dstk = Abuf + (size_t)(k >> 2) * (kMlpRows * 16) + (k & 3) * 4;
+#pragma unroll 1
+                for (int rb = 0; rb < kMlpRows / kMlpRowWarps; rb += 8) {
+                    double xv[8];
 #pragma unroll
-                for (int i = 0; i < 8; i++) {
-                    const long long gr = row0 + warp + 4 * (rb + i);
-#pragma unroll
-                    for (int q = 0; q < kXPerLane; q++) {
-                        const int k = lane + 32 * q;
-                        xv[i][q] = (gr < R.nrows && k < P.w_in) ? __ldcs(R.x + gr * P.w_in + k) : 0.0;
+                    for (int i = 0; i < 8; i++) {
+                        const long long gr = row0 + warp + kMlpRowWarps * (rb + i);
+                        xv[i] = (kin && gr < R.nrows) ? __ldcs(R.x + gr * P.w_in + k) : 0.0;
                     }
-                }
 #pragma unroll
-                for (int i = 0; i < 8; i++) {
-                    const int r = warp + 4 * (rb + i);
-#pragma unroll
-                    for (int q = 0; q < kXPerLane; q++) {
-                        const int k = lane + 32 * q;
-                        if (k < P.K[0])
-                            *reinterpret_cast<float *>(Abuf + (size_t)(k >> 2) * (kMlpRows * 16) + r * 16 + (k & 3) * 4) =
-                                to_tf32((float)((xv[i][q] - xsh[q]) * xsc[q]));
-                    }
+                    for (int i = 0; i < 8; i++)
+                        *reinterpret_cast<float *>(dstk + (warp + kMlpRowWarps * (rb + i)) * 16) = to_tf32((float)((xv[i] - sh) * sc));
                 }
             }
             fence_async_smem();
@@ -262,25 +252,35 @@ __global__ void __launch_bounds__(kMlpThreads, 1) mlp_forward_kernel(MlpParams P
                 tc_fence_after();
                 const bool last = (l == P.nlayers - 1);
                 const bool act_on = !last || P.activate_last;
-                const uint32_t taddr = tmem_base + ((uint32_t)(warp * 32) << 16);
-                for (int n0 = 0; n0 < P.N[l]; n0 += 16) {
-                    float v[16];
-                    tmem_ld16(taddr + (uint32_t)n0, v);
-#pragma unroll
-                    for (int j = 0; j < 16; j++) {
-                        v[j] += bias_s[l * kMlpMaxWidth + n0 + j];
-                        if (act_on) v[j] = activate(P.act, v[j]);
-                    }
-                    if (!last) {
+                const int nh = P.N[l] >> 1;               // this warp's column half: [half * nh, half * nh + nh)
+                const uint32_t taddr = tmem_base + ((uint32_t)(sub * 32) << 16) + (uint32_t)(half * nh);
+                const float *bl = bias_s + l * kMlpMaxWidth + half * nh;
+                if (!last) {
+                    unsigned char *arow = Abuf + (size_t)((half * nh) >> 2) * (kMlpRows * 16) + row * 16;
+                    for (int n0 = 0; n0 < nh; n0 += 16) {
+                        float v[16];
+                        tmem_ld16(taddr + (uint32_t)n0, v);
 #pragma unroll
                         for (int c = 0; c < 4; c++) {
-                            const float4 q = make_float4(to_tf32(v[4 * c]), to_tf32(v[4 * c + 1]), to_tf32(v[4 * c + 2]), to_tf32(v[4 * c + 3]));
-                            *reinterpret_cast<float4 *>(Abuf + (size_t)((n0 >> 2) + c) * (kMlpRows * 16) + row * 16) = q;
+                            const float4 b4 = *reinterpret_cast<const float4 *>(bl + n0 + 4 * c);
+                            float4 q = make_float4(v[4 * c] + b4.x, v[4 * c + 1] + b4.y, v[4 * c + 2] + b4.z, v[4 * c + 3] + b4.w);
+                            if (act_on) q = make_float4(activate<ACT>(q.x), activate<ACT>(q.y), activate<ACT>(q.z), activate<ACT>(q.w));
+                            q = make_float4(to_tf32(q.x), to_tf32(q.y), to_tf32(q.z), to_tf32(q.w));
+                            *reinterpret_cast<float4 *>(arow + (size_t)((n0 >> 2) + c) * (kMlpRows * 16)) = q;
                         }
-                    } else {
+                    }
+                } else {
+                    float *orow = stage_out + row * ostride + half * nh;
+                    const int nvalid = P.w_out - half * nh;   // columns of this half that exist
+                    for (int n0 = 0; n0 < nh && n0 < nvalid; n0 += 16) {
+                        float v[16];
+                        tmem_ld16(taddr + (uint32_t)n0, v);
 #pragma unroll
-                        for (int j = 0; j < 16; j++)
-                            if (n0 + j < P.w_out) stage_out[row * ostride + n0 + j] = v[j];
+                        for (int j = 0; j < 16; j++) {
+                            float q = v[j] + bl[n0 + j];
+                            if (act_on) q = activate<ACT>(q);
+                            if (n0 + j < nvalid) orow[n0 + j] = q;
+                        }
                     }
                 }
                 tc_fence_before();  // the accumulator reads above are ordered before the next layer's MMAs
@@ -290,8 +290,8 @@ __global__ void __launch_bounds__(kMlpThreads, 1) mlp_forward_kernel(MlpParams P
                 }
             }
             // ---- write the tile: one warp per row, w_out contiguous floats
-            asm volatile("bar.sync 1, 128;" ::: "memory");
-            for (int r = warp; r < kMlpRows; r += 4) {
+            asm volatile("bar.sync 1, %0;" ::"n"(kMlpRowWarps * 32) : "memory");
+            for (int r = warp; r < kMlpRows; r += kMlpRowWarps) {
                 const long long gr = row0 + r;
                 if (gr >= R.nrows) break;
                 long long orow = gr;
@@ -305,12 +305,12 @@ __global__ void __launch_bounds__(kMlpThreads, 1) mlp_forward_kernel(MlpParams P
                 float *dst = R.y + orow * P.w_out;
                 for (int n = lane; n < P.w_out; n += 32) __stcs(dst + n, stage_out[r * ostride + n]);
             }
-            asm volatile("bar.sync 1, 128;" ::: "memory");  // staging area is the next tile's A operand
+            asm volatile("bar.sync 1, %0;" ::"n"(kMlpRowWarps * 32) : "memory");  // staging area is the next tile's A operand
         }
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 5) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kMlpTmemCols));
+    if (warp == kMlpRowWarps + 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kMlpTmemCols));
 }
 
 constexpr size_t kMlpSmemBytes = (size_t)kMlpABytes + (size_t)kMlpStages * (kMlpBK / 4) * kMlpMaxWidth * 16 +
@@ -349,7 +349,12 @@ int mlp_launch(const mala_mlp *net, const MlpRows &rows, cudaStream_t st) {
     if (rows.nrows <= 0) return 0;
     const long long ntiles = (rows.nrows + kMlpRows - 1) / kMlpRows;
     const int grid = (int)std::min<long long>(ntiles, net->num_sms);
-    mlp_forward_kernel<<<grid, kMlpThreads, kMlpSmemBytes, st>>>(net->P, rows);
+    switch (net->P.act) {
+        case 1: mlp_forward_kernel<1><<<grid, kMlpThreads, kMlpSmemBytes, st>>>(net->P, rows); break;
+        case 2: mlp_forward_kernel<2><<<grid, kMlpThreads, kMlpSmemBytes, st>>>(net->P, rows); break;
+        case 3: mlp_forward_kernel<3><<<grid, kMlpThreads, kMlpSmemBytes, st>>>(net->P, rows); break;
+        default: mlp_forward_kernel<0><<<grid, kMlpThreads, kMlpSmemBytes, st>>>(net->P, rows); break;
+    }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return set_error(MALA_SNAP_ECUDA, std::string("mlp_forward_kernel: ") + cudaGetErrorString(e));
     return 0;
@@ -384,7 +389,8 @@ int mala_mlp_create(mala_mlp_t **net, int nlayers, const int *sizes, const doubl
     std::vector<float> wp, bp;
     for (int l = 0; l < nlayers; l++) {
         const int wk = sizes[l], wn = sizes[l + 1];
-        const int K = (wk + 15) / 16 * 16, N = (wn + 15) / 16 * 16;
+        const int K = (l == 0) ? (wk + 15) / 16 * 16 : P.N[l - 1];   // = the padded width of the layer before
+        const int N = (wn + 31) / 32 * 32;
         P.K[l] = K; P.N[l] = N;
         P.woff[l] = (int)wp.size(); P.boff[l] = (int)bp.size();
         m->flop_per_row += 2LL * wk * wn;
@@ -428,7 +434,10 @@ int mala_mlp_create(mala_mlp_t **net, int nlayers, const int *sizes, const doubl
     if (e == cudaSuccess) e = cudaMemcpy(m->d_b, bp.data(), bp.size() * sizeof(float), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(m->d_shift, sh.data(), sh.size() * sizeof(double), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(m->d_scale, sc.data(), sc.size() * sizeof(double), cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(mlp_forward_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMlpSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(mlp_forward_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMlpSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(mlp_forward_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMlpSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(mlp_forward_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMlpSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(mlp_forward_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMlpSmemBytes);
     if (e != cudaSuccess) return cleanup(MALA_SNAP_ECUDA, std::string("network upload: ") + cudaGetErrorString(e));
     P.wpacked = m->d_w; P.bias = m->d_b; P.in_shift = m->d_shift; P.in_scale = m->d_scale;
     *net = m;
