@@ -145,6 +145,24 @@ int mala_bispectrum_ldos_grid(mala_snap_t *h, mala_mlp_t *net, int natoms, const
                               int z_end, float *ldos, void *cuda_stream);
 
 /*
+ * ---- the adjoint of the descriptor map (forces) --------------------------------------------------
+ *
+ * "Apply dB(r, j; R)/dR_alpha to an array" -- the third factor of the chain rule for the force on ion alpha, Eqs. (44)-(45),
+ * PAPER.md:418-428.  With beta(r, j) = dE/dB(r, j) supplied by the caller (the result of back-propagating through the
+ * network),
+ *     g[alpha][k] += sum_{grid points r of the slab} sum_j beta[r][j] * dB(r, j)/dR_{alpha,k},     k = x, y, z,
+ * where all periodic images of atom alpha move with it.  The force contribution is f_alpha = -g[alpha].
+ *   beta   DEVICE [(z_end-z_begin)*ny*nx][ncomp] fp64, ix fastest (the layout of mala_bispectrum_grid's out)
+ *   g      DEVICE [natoms*3] fp64; the call ADDS the slab's contribution (zero it before the first slab; slabs and GPUs sum)
+ * All other arguments as mala_bispectrum_grid.  twojmax <= 10 (MALA_SNAP_EINVAL above).  Enqueued on cuda_stream; does not
+ * synchronise.  The per-atom sums use floating-point atomics: results are reproducible to rounding, not bit for bit.
+ * mala_snap_kernel_times reports compute_yi under ms[2] and compute_dedr under ms[3].
+ */
+int mala_bispectrum_force_adjoint(mala_snap_t *h, int natoms, const double *pos, const int *types, const double box[9],
+                                  const double origin[3], const int pbc[3], const int ngrid[3], int z_begin, int z_end,
+                                  const double *beta, double *g, void *cuda_stream);
+
+/*
  * Gaussian descriptors on the same grid ("a sum of Gaussians centered at R", the Gaussian representation of
  * the ionic configuration behind Eqs. (40)-(43)).  One channel per atom type t:
  *     G_t(r) = wj[t] * (2 pi sigma^2)^(-3/2) * sum exp(-|R - r|^2 / (2 sigma^2))

@@ -24,6 +24,7 @@
 #include "snap_zi_coop.cuh"
 #include "snap_zi_diag.cuh"
 #include "snap_gauss.cuh"
+#include "snap_force.cuh"
 
 using namespace mala;
 
@@ -129,6 +130,17 @@ struct mala_snap {
     int cand_cap_limit = 0;        // test hook: clamp the candidate capacity (0 = off) to provoke the overflow path
     DevBuf<double2> d_utot;
     DevBuf<double> d_bstage;       // fused network: descriptors of one chunk, [tile][32][ncomp]
+    // row f3 (force adjoint): tables of compute_yi and the Y workspace
+    DevBuf<YTerm> d_yterms;
+    DevBuf<int> d_ylevel, d_yorder;
+    DevBuf<double> d_ycg, d_yweight;
+    DevBuf<double2> d_ytot;
+    bool force_ready = false;
+    ForceTables force_tables() const {
+        ForceTables f;
+        f.terms = d_yterms.p; f.level_begin = d_ylevel.p; f.cg = d_ycg.p; f.eorder = d_yorder.p; f.yweight = d_yweight.p;
+        return f;
+    }
     DevBuf<double> d_stage[2];
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t ev_done[2] = {nullptr, nullptr}, ev_copied[2] = {nullptr, nullptr};
@@ -510,7 +522,7 @@ int build_plan(mala_snap *h, const CallArgs &a, cudaStream_t st) {
                     gh.y = g.origin[1] + ff[0] * rows[0][1] + ff[1] * rows[1][1] + ff[2] * rows[2][1];
                     gh.z = g.origin[2] + ff[0] * rows[0][2] + ff[1] * rows[1][2] + ff[2] * rows[2][2];
                     gh.type = a.types[n];
-                    gh.pad = 0;
+                    gh.pad = n;  // the atom this image belongs to
                     ghosts.push_back(gh);
                     if (ghosts.size() > 400000000u) return fail(MALA_SNAP_ENOMEM, "too many periodic images");
                 }
@@ -826,6 +838,132 @@ int run_slab_gauss(mala_snap *h, int z0, int z1, double sigma, double *out, cuda
     }
     h->stats[2] += total_tiles;
     h->stats[4] = h->cand_cap;
+    h->stats[6] += (long long)g.nx * g.ny * (z1 - z0);
+    return 0;
+}
+
+// tables of compute_yi (snap_force.cuh): three Z-type contributions per bispectrum component, grouped by target level
+int build_force_tables(mala_snap *h) {
+    if (h->force_ready) return 0;
+    const SnapTables &T = h->tab;
+    const int tj = h->twojmax, nt = T.ntriples;
+    struct Raw { int A, B, C, index; double coef; };
+    std::vector<Raw> raw;
+    for (int t = 0; t < nt; t++) {
+        const int j1 = T.triples[4 * t], j2 = T.triples[4 * t + 1], j = T.triples[4 * t + 2];
+        raw.push_back({j1, j2, j, t, 1.0});
+        raw.push_back({j, j2, j1, t, (double)(j + 1) / (double)(j1 + 1)});
+        raw.push_back({j, j1, j2, t, (double)(j + 1) / (double)(j2 + 1)});
+    }
+    std::stable_sort(raw.begin(), raw.end(), [](const Raw &a, const Raw &b) { return a.C < b.C; });
+    std::vector<YTerm> terms;
+    std::vector<double> cg;
+    std::vector<int> level(tj + 2, 0);
+    for (const Raw &r : raw) {
+        YTerm y{};
+        y.A = (short)r.A; y.B = (short)r.B; y.C = (short)r.C; y.index = (short)r.index; y.coef = r.coef;
+        y.cgoff = (int)cg.size();
+        const int sh = (r.A + r.B - r.C) / 2;
+        for (int m2 = 0; m2 <= r.B; m2++)
+            for (int m1 = 0; m1 <= r.A; m1++) {
+                const int m = m1 + m2 - sh;
+                cg.push_back((m >= 0 && m <= r.C) ? clebsch_gordan(r.A, 2 * m1 - r.A, r.B, 2 * m2 - r.B, r.C, 2 * m - r.C) : 0.0);
+            }
+        level[r.C + 1]++;
+        terms.push_back(y);
+    }
+    for (int C = 0; C <= tj; C++) level[C + 1] += level[C];
+    // cost of a Y element = product terms over its contributions; processing order by decreasing cost
+    std::vector<double> cost(T.nelem, 0.0), yweight(T.nelem, 0.0);
+    for (int C = 0; C <= tj; C++)
+        for (int mb = 0; mb <= C / 2; mb++)
+            for (int ma = 0; ma <= C; ma++) {
+                const int e = uhalf_off(C) + mb * (C + 1) + ma;
+                for (int k = level[C]; k < level[C + 1]; k++) {
+                    const int A = terms[k].A, B = terms[k].B, sh = (A + B - C) / 2;
+                    const int nb = std::min(A, mb + sh) - std::max(0, mb + sh - B) + 1, na = std::min(A, ma + sh) - std::max(0, ma + sh - B) + 1;
+                    cost[e] += (double)std::max(nb, 0) * std::max(na, 0) + 4.0;
+                }
+                const bool mid = (C % 2 == 0) && (mb == C / 2);
+                yweight[e] = T.unorm[e] * (mid ? 1.0 : 2.0);
+            }
+    std::vector<int> order(T.nelem);
+    for (int e = 0; e < T.nelem; e++) order[e] = e;
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return cost[a] > cost[b]; });
+    int rc = 0;
+    if ((rc = upload(h->d_yterms, terms))) return rc;
+    if ((rc = upload(h->d_ylevel, level))) return rc;
+    if ((rc = upload(h->d_ycg, cg))) return rc;
+    if ((rc = upload(h->d_yorder, order))) return rc;
+    if ((rc = upload(h->d_yweight, yweight))) return rc;
+    CUDA_TRY(cudaFuncSetAttribute(compute_yi_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)compute_yi_smem_bytes(uhalf_size(kFullTileTwoJ), triple_count(kFullTileTwoJ))));
+    CUDA_TRY(cudaFuncSetAttribute(compute_dedr_kernel<kFullTileTwoJ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)compute_dedr_smem_bytes(kFullTileTwoJ)));
+    h->force_ready = true;
+    return 0;
+}
+
+// row f3 for the slab [z0, z1): tile binning -> compute_ui -> compute_yi (beta in, Y out) -> compute_dedr (adds into gout)
+int run_slab_force(mala_snap *h, int z0, int z1, const double *beta, double *gout, cudaStream_t st) {
+    if (z1 <= z0) return 0;
+    choose_tiles(h, z0, z1);
+    GridGeom &g = h->geom;
+    h->cand_cap = candidate_bound(h);
+    if (h->cand_cap < 0) return fail(MALA_SNAP_EINVAL, "more than 2^24 candidate atoms per tile; use a finer cell or smaller z-slabs");
+    const long long total_tiles = h->total_tiles;
+    if (total_tiles > 2000000000LL) return fail(MALA_SNAP_EINVAL, "slab has too many tiles; use smaller z-slabs");
+    const size_t per_tile = (size_t)2 * h->sc.nelem * 32 * sizeof(double2) + (size_t)h->cand_cap * sizeof(int) + 2 * sizeof(int);
+    const size_t budget = (size_t)std::max<long long>(h->workspace_mb, 1) << 20;
+    long long chunk_tiles = (long long)std::max<size_t>(budget / per_tile, (size_t)h->num_sms);
+    chunk_tiles = std::min(chunk_tiles, total_tiles);
+    if (h->d_utot.reserve((size_t)chunk_tiles * h->sc.nelem * 32, st, true) || h->d_ytot.reserve((size_t)chunk_tiles * h->sc.nelem * 32, st, true) ||
+        h->d_cand.reserve((size_t)chunk_tiles * h->cand_cap, st, true) || h->d_ncand.reserve(chunk_tiles, st, true) ||
+        h->d_active.reserve(chunk_tiles, st, true) || h->d_counters.reserve(4, st, true))
+        return fail(MALA_SNAP_ENOMEM, "cudaMallocAsync (workspace) failed");
+    h->stats[4] = h->cand_cap;
+    h->stats[5] = (long long)(per_tile * (size_t)chunk_tiles);
+    const DeviceTables tb = h->tables();
+    for (long long t0 = 0; t0 < total_tiles; t0 += chunk_tiles) {
+        ChunkBuffers cb{};
+        cb.ghosts = h->d_ghosts[h->cur].p; cb.cell_start = h->d_cell_start[h->cur].p;
+        cb.cand = h->d_cand.p; cb.ncand = h->d_ncand.p; cb.active = h->d_active.p; cb.counters = h->d_counters.p;
+        cb.status = h->d_status.p; cb.utot = h->d_utot.p; cb.cand_cap = h->cand_cap;
+        cb.tile_begin = (int)t0;
+        cb.ntiles = (int)std::min(chunk_tiles, total_tiles - t0);
+        CUDA_TRY(cudaMemsetAsync(cb.counters, 0, 4 * sizeof(int), st));
+        const int bin_blocks = (cb.ntiles + 7) / 8;
+        {
+            TimedSpan span(h, st, kKindBin);
+            tile_bin_kernel<<<bin_blocks, 256, 0, st>>>(g, h->sc, tb, cb, nullptr);
+        }
+        CUDA_TRY(cudaGetLastError());
+        const int grid2 = std::max(1, std::min(2 * h->num_sms, 2 * cb.ntiles));
+        {
+            TimedSpan span(h, st, kKindUi);
+            if (h->twojmax == kFullTileTwoJ)
+                compute_ui_kernel<kFullTileTwoJ, true><<<grid2, (kFullTileTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kFullTileTwoJ), st>>>(g, h->sc, tb, cb);
+            else
+                compute_ui_kernel<kFullTileTwoJ, false><<<grid2, (kFullTileTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kFullTileTwoJ), st>>>(g, h->sc, tb, cb);
+        }
+        CUDA_TRY(cudaGetLastError());
+        {
+            TimedSpan span(h, st, kKindZi);   // reported in the compute_zi_bi slot: the same kind of contraction
+            const int grid = std::max(1, std::min(h->num_sms, cb.ntiles));
+            compute_yi_kernel<<<grid, kYiWarps * 32, compute_yi_smem_bytes(h->sc.nelem, h->sc.ntriples), st>>>(g, h->sc, h->force_tables(), cb, beta,
+                                                                                                                h->d_ytot.p);
+        }
+        CUDA_TRY(cudaGetLastError());
+        {
+            TimedSpan span(h, st, kKindOther);
+            compute_dedr_kernel<kFullTileTwoJ><<<grid2, (kFullTileTwoJ / 2 + 1) * 32, compute_dedr_smem_bytes(kFullTileTwoJ), st>>>(g, h->sc, tb, cb,
+                                                                                                                                 h->d_ytot.p, gout);
+        }
+        CUDA_TRY(cudaGetLastError());
+        h->stats[0] += 4;
+        h->stats[1]++;
+    }
+    h->stats[2] += total_tiles;
     h->stats[6] += (long long)g.nx * g.ny * (z1 - z0);
     return 0;
 }
@@ -1260,6 +1398,24 @@ int mala_bispectrum_ldos_grid(mala_snap_t *h, mala_mlp_t *net, int natoms, const
     return finish_call(h, st);
 }
 
+int mala_bispectrum_force_adjoint(mala_snap_t *h, int natoms, const double *pos, const int *types, const double box[9],
+                                  const double origin[3], const int pbc[3], const int ngrid[3], int z_begin, int z_end, const double *beta,
+                                  double *g, void *cuda_stream) {
+    const CallArgs a{natoms, pos, types, box, origin, pbc, ngrid, z_begin, z_end};
+    int rc = validate(h, a, true, beta);
+    if (rc) return rc;
+    if (natoms > 0 && !g) return fail(MALA_SNAP_EINVAL, "g is NULL");
+    if (h->half_tiles()) return fail(MALA_SNAP_EINVAL, "mala_bispectrum_force_adjoint supports twojmax <= 10");
+    if ((rc = check_status(h, false))) return rc;
+    std::fill(h->stats, h->stats + 8, 0LL);
+    if (z_end == z_begin || natoms == 0) return MALA_SNAP_OK;
+    if ((rc = build_force_tables(h))) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if ((rc = build_plan(h, a, st))) return rc;
+    if ((rc = run_slab_force(h, z_begin, z_end, beta, g, st))) return rc;
+    return finish_call(h, st);
+}
+
 int mala_gaussian_grid(mala_snap_t *h, double sigma, int natoms, const double *pos, const int *types, const double box[9],
                        const double origin[3], const int pbc[3], const int ngrid[3], int z_begin, int z_end, double *out,
                        void *cuda_stream) {
@@ -1309,6 +1465,7 @@ void mala_snap_destroy(mala_snap_t *h) {
     }
     h->d_cand.release(); h->d_ncand.release(); h->d_active.release(); h->d_counters.release(); h->d_utot.release();
     h->d_status.release(); h->d_bstage.release();
+    h->d_yterms.release(); h->d_ylevel.release(); h->d_yorder.release(); h->d_ycg.release(); h->d_yweight.release(); h->d_ytot.release();
     h->d_dcg.release(); h->d_dtriple.release(); h->d_dsched.release(); h->d_ditems.release();
     if (h->h_status) cudaFreeHost(h->h_status);
     for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);

@@ -46,7 +46,7 @@ struct SnapConst {
 struct __align__(16) Ghost {
     double x, y, z;
     int type;
-    int pad;
+    int pad;   // index of the atom this ghost is an image of (row f3 scatters the adjoint back to atoms)
 };
 
 // device pointers of one handle
@@ -68,7 +68,8 @@ struct ChunkBuffers {
     int *cand;               // [chunk_tiles * cand_cap] ghost indices per tile
     int *ncand;              // [chunk_tiles]
     int *active;             // [chunk_tiles] compacted list of non-empty tiles (local tile ids)
-    int *counters;           // [0] number of active tiles, [1] ui work counter, [2] zi work counter (zeroed per chunk)
+    int *counters;           // [0] number of active tiles, [1] ui work counter, [2] zi / yi work counter, [3] dedr work counter
+                             // (zeroed per chunk)
     int *status;             // handle-wide status word, never cleared by a chunk: kStatus* bits
     double2 *utot;           // [chunk_tiles][nelem][32], or [chunk_tiles][2][nelem][16] when utot_half is set
     int utot_half;           // 1: half-tile layout (twojmax > kFullTileTwoJ)

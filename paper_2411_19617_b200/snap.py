@@ -20,7 +20,7 @@ MALA_SNAP_ECUDA = -2
 MALA_SNAP_ENOMEM = -3
 
 EXPORTS = ("mala_snap_create", "mala_snap_ncomp", "mala_snap_triples", "mala_bispectrum_grid", "mala_bispectrum_grid_host",
-           "mala_gaussian_grid", "mala_mlp_create", "mala_mlp_widths", "mala_mlp_forward", "mala_mlp_destroy", "mala_bispectrum_ldos_grid",
+           "mala_gaussian_grid", "mala_mlp_create", "mala_mlp_widths", "mala_mlp_forward", "mala_mlp_destroy", "mala_bispectrum_ldos_grid", "mala_bispectrum_force_adjoint",
            "mala_snap_set_option", "mala_snap_last_stats", "mala_snap_kernel_times", "mala_snap_zi_kernel", "mala_snap_fp64_peak", "mala_snap_clebsch_gordan", "mala_snap_debug_utot",
            "mala_snap_destroy", "mala_last_error")
 
@@ -73,6 +73,8 @@ def load_library():
     lib.mala_mlp_destroy.argtypes = [vp]
     lib.mala_bispectrum_ldos_grid.restype = C.c_int
     lib.mala_bispectrum_ldos_grid.argtypes = [vp, vp] + grid_args[1:]
+    lib.mala_bispectrum_force_adjoint.restype = C.c_int
+    lib.mala_bispectrum_force_adjoint.argtypes = grid_args[:10] + [vp, vp, vp]
     lib.mala_snap_debug_utot.restype = C.c_int
     lib.mala_snap_debug_utot.argtypes = grid_args
     lib.mala_snap_set_option.restype = C.c_int
@@ -248,6 +250,23 @@ class MalaSnap:
         s = torch.cuda.current_stream() if stream is None else stream
         _check(self._lib.mala_gaussian_grid(self._h, C.c_double(float(sigma)), *args, C.c_void_p(out.data_ptr()),
                                             C.c_void_p(s.cuda_stream)))
+        return out
+
+    # -- mala_bispectrum_force_adjoint: g[atom, k] += sum_points sum_j beta[point, j] dB_j(point)/dR_{atom,k}
+    def force_adjoint(self, beta, pos, types, box, origin=(0, 0, 0), pbc=(1, 1, 1), ngrid=(1, 1, 1), z_begin=0, z_end=None, out=None,
+                      stream=None):
+        import torch
+        args, keep, npts = self._system(pos, types, box, origin, pbc, ngrid, z_begin, z_end)
+        natoms = keep[0].shape[0]
+        if (not beta.is_cuda) or beta.dtype != torch.float64 or (not beta.is_contiguous()) or beta.numel() < npts * self.ncomp:
+            raise ValueError("beta must be a contiguous CUDA float64 tensor with at least npoints*ncomp elements")
+        if out is None:
+            out = torch.zeros((natoms, 3), dtype=torch.float64, device="cuda")
+        if (not out.is_cuda) or out.dtype != torch.float64 or (not out.is_contiguous()) or out.numel() < natoms * 3:
+            raise ValueError("out must be a contiguous CUDA float64 tensor [natoms, 3]")
+        s = torch.cuda.current_stream() if stream is None else stream
+        _check(self._lib.mala_bispectrum_force_adjoint(self._h, *args, C.c_void_p(beta.data_ptr()), C.c_void_p(out.data_ptr()),
+                                                       C.c_void_p(s.cuda_stream)))
         return out
 
     # -- mala_snap_debug_utot (test hook)
