@@ -89,6 +89,8 @@ def parse_args():
     p.add_argument("--sigma", type=float, default=0.5, help="Gaussian width for --descriptor gaussian")
     p.add_argument("--ldos", action="store_true",
                    help="SURVEY 8(f) f1: descriptors + the descriptor->LDOS network in one call (mala_bispectrum_ldos_grid), a separate metric line")
+    p.add_argument("--force", action="store_true",
+                   help="SURVEY 8(f) f3: the adjoint of the descriptor map (mala_bispectrum_force_adjoint), a separate metric line")
     p.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
     p.add_argument("--no-e2e", action="store_true", help="skip the host-output leg (profiling runs)")
     args = p.parse_args()
@@ -652,6 +654,143 @@ def run_ldos(args, w, rank, world, local):
     print(json.dumps(line), flush=True)
 
 
+def force_flop_model(twojmax):
+    """Algorithmic flops of row f3 per non-empty grid point (compute_yi) and per (grid point, neighbor) pair (compute_dedr),
+    counted from the index ranges.  Y^C[ma][mb] over half columns receives, for every bispectrum
+    component (j1, j2, j), the three Z-type contributions (j1, j2) -> j, (j, j2) -> j1 and (j, j1) -> j2: 10 flop per
+    product term and 4 per outer step, as for compute_zi.  compute_dedr repeats the U recursion of the pair (F_PAIR) and
+    dots every coefficient of levels 0 .. twojmax-1 with two Y columns for the four Cayley-Klein derivatives (4 complex
+    multiply-adds = 32 flop) plus the weight sum (8 flop per element of U)."""
+    tj = int(twojmax)
+    fm = flop_model(tj)
+    triples = [(j1, j2, j) for j1 in range(tj + 1) for j2 in range(j1 + 1) for j in range(j1 - j2, min(tj, j1 + j2) + 1, 2) if j >= j1]
+    terms = outer = 0
+    for j1, j2, j in triples:
+        for A, B, C in ((j1, j2, j), (j, j2, j1), (j, j1, j2)):
+            sh = (A + B - C) // 2
+            for mb in range(C // 2 + 1):
+                mid = (C % 2 == 0) and (mb == C // 2)
+                nb = min(A, mb + sh) - max(0, mb + sh - B) + 1
+                for ma in range((C // 2 if mid else C) + 1):
+                    na = min(A, ma + sh) - max(0, ma + sh - B) + 1
+                    terms += na * nb
+                    outer += nb
+    nelem_lower = sum((J + 1) * (J // 2 + 1) for J in range(tj))   # coefficients of levels 0 .. tj-1
+    return {"F_Y": 10 * terms + 4 * outer, "Y_terms": terms, "F_DEDR_PAIR": fm["F_PAIR"] + 32 * nelem_lower + 8 * fm["nelem"]}
+
+
+def run_force(args, w, rank, world, local):
+    """--force: grid points/s of mala_bispectrum_force_adjoint (row f3, Eqs. (44)-(45) PAPER.md:418-428): beta[point][ncomp]
+    resident in HBM -> g[natoms][3].  e2e adds the host->device copy of beta from pinned memory and the device->host read of g."""
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        torch.distributed.init_process_group("nccl", device_id=dev)
+    from paper_2411_19617_b200 import MalaSnap, mala_snap_fp64_peak
+
+    def barrier():
+        if world > 1:
+            torch.distributed.barrier()
+        torch.cuda.synchronize()
+
+    fm, ffm = flop_model(w.twojmax), force_flop_model(w.twojmax)
+    nt, npts, natoms = fm["ncomp"], w.npoints, int(w.pos.shape[0])
+    snap = MalaSnap(**w.snap_params())
+    stream = torch.cuda.current_stream()
+    gen = torch.Generator(device="cpu").manual_seed(7)
+    beta_host = torch.randn((npts, nt), dtype=torch.float64, generator=gen).pin_memory()
+    beta = beta_host.to(dev)
+    g = torch.zeros((natoms, 3), dtype=torch.float64, device=dev)
+
+    def call():
+        g.zero_()
+        snap.force_adjoint(beta, w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, out=g, stream=stream)
+
+    snap.set_option("timing", 1)
+    for _ in range(args.warmup):
+        call()
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.15)
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    ktimes, launches = [], 0
+    barrier()
+    for a, b in evs:
+        a.record(stream)
+        call()
+        b.record(stream)
+        ktimes.append(snap.kernel_times())
+        launches += snap.last_stats()["kernels"]
+    barrier()
+    clocks = sampler.stop()
+    total_ms = float(sum(a.elapsed_time(b) for a, b in evs))
+    total_ms, total_pts = reduce_max_sum(total_ms, npts * args.steps, world, dev)
+    value = total_pts / (total_ms * 1e-3)
+    stats = snap.last_stats()
+    kms = {"tile_bin": float(np.mean([k["tile_bin"][0] for k in ktimes])), "compute_ui": float(np.mean([k["compute_ui"][0] for k in ktimes])),
+           "compute_yi": float(np.mean([k["compute_zi_bi"][0] for k in ktimes])), "compute_dedr": float(np.mean([k["other"][0] for k in ktimes]))}
+    pairs, nonempty = workload_counts(w)
+    yi_launches = ktimes[-1]["compute_zi_bi"][1]
+    yi_flop = nonempty * ffm["F_Y"]
+    achieved = yi_flop / (kms["compute_yi"] * 1e-3) / 1e12 if kms["compute_yi"] > 0 else 0.0
+    peak_meas, mhz_eff = mala_snap_fp64_peak(stream)
+    step_flop = yi_flop + pairs * (fm["F_PAIR"] + ffm["F_DEDR_PAIR"])
+    roofline = {"bound": "alu", "kernel": "compute_yi_kernel", "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS, "unit": "TFLOP/s",
+                "frac": achieved / FP64_NOMINAL_TFLOPS,
+                "peak_source": "nominal FP64 FMA pipe: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md 'FP64 roofline')",
+                "peak_measured_dfma": peak_meas, "frac_of_measured_dfma": achieved / peak_meas if peak_meas > 0 else None, "traffic": None,
+                "flop_per_point": {"yi": ffm["F_Y"], "dedr_per_pair": ffm["F_DEDR_PAIR"], "ui_per_pair": fm["F_PAIR"]},
+                "flop_per_launch": yi_flop / max(yi_launches, 1), "launches_per_step": yi_launches,
+                "ms_per_launch": kms["compute_yi"] / max(yi_launches, 1), "kernel_ms_per_step": kms,
+                "compute_dedr_tflops": pairs * ffm["F_DEDR_PAIR"] / (kms["compute_dedr"] * 1e-3) / 1e12 if kms["compute_dedr"] > 0 else None,
+                "step_model_tflops": step_flop / (total_ms / args.steps * 1e-3) / 1e12 if world == 1 else None}
+    roofline["traffic"], roofline["traffic_source"] = ncu_traffic(f"config{w.extra.get('cfg')}/tj{w.twojmax}", "compute_yi_kernel",
+                                                                  kms["compute_yi"] / max(yi_launches, 1))
+    # end to end: beta from pinned host memory, g back to the host, every step
+    g_host = torch.empty((natoms, 3), dtype=torch.float64, pin_memory=True)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        beta.copy_(beta_host, non_blocking=True)
+        call()
+        g_host.copy_(g, non_blocking=True)
+        torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    e2e_s, e2e_pts = reduce_max_sum(e2e_s, npts * args.steps, world, dev)
+    h2d = int(beta_host.numel() * 8 + w.pos.nbytes + w.types.nbytes + 9 * 8 + 3 * 8 + 3 * 4 + 3 * 4)
+    e2e = {"value": e2e_pts / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": int(natoms * 3 * 8),
+           "ms_per_step": 1e3 * e2e_s / args.steps}
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+        rng = np.random.default_rng(7)
+        n = 256 * max(oracle.num_threads(), 1)
+        sample = rng.integers(0, npts, n)
+        pts = oracle.grid_points(w.box, w.origin, w.ngrid, sample=sample)
+        b = rng.normal(size=(n, nt))
+        t0 = time.perf_counter()
+        oracle.bispectrum_grad_points(pts, w.pos, w.types, w.box, w.origin, w.pbc, beta=b, want_dB=False, **w.snap_params())
+        dt = time.perf_counter() - t0
+        cpu = {"value": n / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": f"{n} seeded random grid points of {w.name} (of {npts}) in {dt:.1f} s wall: forward-mode dB/dR of the C oracle"}
+    snap.close()
+    if world > 1:
+        torch.distributed.destroy_process_group()
+    if rank != 0:
+        return
+    cfg = workload_config(w, "mala_bispectrum_force_adjoint (beta and g resident in HBM)")
+    cfg.update({"chunks_per_step": stats["chunks"], "workspace_bytes": stats["workspace_bytes"]})
+    line = {"metric": "grid points/s of the descriptor adjoint g = sum beta dB/dR (SURVEY 8(f) f3), twojmax=%d fp64" % w.twojmax,
+            "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": cfg,
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+
+
 def spawn_ranks(args):
     """`python bench.py --gpus N` without a launcher: start the N ranks ourselves, exactly as the driver would
     (torch.distributed.run, one process per GPU, rendezvous on 127.0.0.1), and pass their output through."""
@@ -685,6 +824,9 @@ def main():
         return
     if args.ldos:
         run_ldos(args, w, rank, world, local)
+        return
+    if args.force:
+        run_force(args, w, rank, world, local)
         return
     run_native(args, w, rank, world, local)
 

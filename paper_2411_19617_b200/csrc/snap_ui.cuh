@@ -96,9 +96,21 @@ __global__ void __launch_bounds__(256) tile_bin_kernel(GridGeom g, SnapConst sc,
     if (out == nullptr) return;
     // empty tile: constant descriptor, written as contiguous rows of tx points
     const int nt = sc.ntriples;
+    // a run of n doubles repeating the nt constants: 16-byte streaming stores where the run is 16-byte aligned
+    auto fill_run = [&](double *dst, const int n) {
+        if ((((uintptr_t)dst) & 15) == 0) {
+            double2 *d2 = reinterpret_cast<double2 *>(dst);
+            for (int i = lane; i < (n >> 1); i += 32) {
+                const int k = (2 * i) % nt;
+                __stcs(d2 + i, make_double2(__ldg(tb.bconst + k), __ldg(tb.bconst + (k + 1 == nt ? 0 : k + 1))));
+            }
+            if ((n & 1) && lane == 0) __stcs(dst + n - 1, __ldg(tb.bconst + (n - 1) % nt));
+        } else {
+            for (int i = lane; i < n; i += 32) __stcs(dst + i, __ldg(tb.bconst + i % nt));
+        }
+    };
     if (cb.compact_out) {
-        double *dst = out + (size_t)wt * 32 * nt;
-        for (int i = lane; i < 32 * nt; i += 32) __stcs(dst + i, tb.bconst[i % nt]);
+        fill_run(out + (size_t)wt * 32 * nt, 32 * nt);
         return;
     }
     const int ix0 = ti.ix0;
@@ -107,8 +119,7 @@ __global__ void __launch_bounds__(256) tile_bin_kernel(GridGeom g, SnapConst sc,
         const int iy = ti.iy0 + (r % ti.ty);
         const int iz = ti.iz0 + (r / ti.ty);
         if (iy >= ti.yend || iz >= g.z1) continue;
-        double *dst = out + ((size_t)((size_t)(iz - g.z0) * g.ny + iy) * g.nx + ix0) * nt;
-        for (int i = lane; i < npx * nt; i += 32) __stcs(dst + i, tb.bconst[i % nt]);
+        fill_run(out + ((size_t)((size_t)(iz - g.z0) * g.ny + iy) * g.nx + ix0) * nt, npx * nt);
     }
 }
 
