@@ -91,6 +91,8 @@ def parse_args():
                    help="SURVEY 8(f) f1: descriptors + the descriptor->LDOS network in one call (mala_bispectrum_ldos_grid), a separate metric line")
     p.add_argument("--force", action="store_true",
                    help="SURVEY 8(f) f3: the adjoint of the descriptor map (mala_bispectrum_force_adjoint), a separate metric line")
+    p.add_argument("--zi-impl", type=int, default=0,
+                   help="compute_zi kernel: 0 automatic, 1 table-driven, 2 per-triple (twojmax 10), 3 anti-diagonal, 4 register-tiled blocks")
     p.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
     p.add_argument("--no-e2e", action="store_true", help="skip the host-output leg (profiling runs)")
     args = p.parse_args()
@@ -336,6 +338,8 @@ def run_native(args, w, rank, world, local):
     npts = (z1 - z0) * ny * nx
     snap = MalaSnap(**w.snap_params())
     assert snap.ncomp == nt
+    if args.zi_impl:
+        snap.set_option("zi_impl", args.zi_impl)
     stream = torch.cuda.current_stream()
     out = torch.empty((max(npts, 1), nt), dtype=torch.float64, device=dev)
     call = lambda: snap.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, z0, z1, out=out, stream=stream)

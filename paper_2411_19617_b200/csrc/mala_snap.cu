@@ -23,6 +23,7 @@
 #include "snap_zi.cuh"
 #include "snap_zi_coop.cuh"
 #include "snap_zi_diag.cuh"
+#include "snap_zi_block.cuh"
 #include "snap_gauss.cuh"
 #include "snap_force.cuh"
 
@@ -107,6 +108,18 @@ struct mala_snap {
     DevBuf<double> d_dcg;
     DevBuf<DiagTriple> d_dtriple;
     DevBuf<unsigned short> d_dsched, d_ditems;
+    // tables of the block kernel (snap_zi_block.cuh)
+    DevBuf<BlkItem> d_bitems;
+    DevBuf<BlkUnit> d_bunits;
+    DevBuf<double> d_bcoef;
+    DevBuf<int> d_bwrange, d_btslot;
+    int blk_nslots = 0;
+    bool blk_ready = false;
+    BlkTables blk_tables() const {
+        BlkTables t;
+        t.items = d_bitems.p; t.units = d_bunits.p; t.coef = d_bcoef.p; t.wrange = d_bwrange.p; t.tslot = d_btslot.p; t.nslots = blk_nslots;
+        return t;
+    }
     long long workspace_mb = 4096;
     long long host_chunk_mb = 256;
     // device tables
@@ -172,6 +185,7 @@ struct mala_snap {
     // 0 = automatic: the per-triple specialised kernel at twojmax = 10, the anti-diagonal kernel otherwise
     bool use_spec() const { return zi_impl == 2 || (zi_impl == 0 && twojmax == kSpecTJ); }
     bool use_diag() const { return zi_impl == 3 || (zi_impl == 0 && twojmax != kSpecTJ); }
+    bool use_block() const { return zi_impl == 4 && !half_tiles(); }
 };
 
 namespace {
@@ -197,6 +211,8 @@ int set_kernel_attributes(mala_snap *h) {
                                   (int)compute_zi_diag_smem_bytes(uhalf_size(kFullTileTwoJ), triple_count(kFullTileTwoJ))));
     CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_diag_half_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   (int)compute_zi_diag_half_smem_bytes(uhalf_size(kMaxTwoJ), triple_count(kMaxTwoJ))));
+    CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_block_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)compute_zi_block_smem_bytes(uhalf_size(kFullTileTwoJ), triple_count(kFullTileTwoJ), kBlkMaxSlots)));
     (void)h;
     return 0;
 }
@@ -352,11 +368,162 @@ int build_diag_schedule(mala_snap *h) {
     return 0;
 }
 
+// Tables of the block kernel (snap_zi_block.cuh): items per (triple, column), units = blocks of the (ma1, ma2) rectangle with
+// their packed coefficients, the deal of the units to the warps and the partial-sum slots.
+int build_block_schedule(mala_snap *h) {
+    const SnapTables &T = h->tab;
+    const int nt = T.ntriples, NW = kBlkWarps;
+    std::vector<BlkItem> items;
+    std::vector<double> coef;
+    struct HostUnit { BlkUnit u; int triple; double cost; };
+    std::vector<std::vector<HostUnit>> tunits(nt);
+    std::vector<double> tcost(nt, 0.0);
+    auto chunks = [](int len, int mx) {
+        std::vector<std::pair<int, int>> out;
+        const int k = (len + mx - 1) / mx, base = len / k, rem = len % k;
+        int s = 0;
+        for (int i = 0; i < k; i++) { const int c = base + (i < rem ? 1 : 0); out.push_back({s, c}); s += c; }
+        return out;
+    };
+    for (int t = 0; t < nt; t++) {
+        const int J1 = T.triples[4 * t], J2 = T.triples[4 * t + 1], J = T.triples[4 * t + 2], cg0 = T.triples[4 * t + 3];
+        const int sh = (J1 + J2 - J) / 2;
+        for (int mb = 0; mb <= J / 2; mb++) {
+            int lo, hi;
+            diag_item_range(J1, J2, J, mb, lo, hi);
+            if (hi < lo) continue;
+            const bool mid = (J % 2 == 0) && (mb == J / 2);
+            const int item_first = (int)items.size();
+            for (int mb1 = lo; mb1 <= hi; mb1++) {
+                const int mb2 = mb + sh - mb1;
+                double w = T.cg[cg0 + mb2 * (J1 + 1) + mb1];
+                if (J == J1 && J1 == J2) {   // one item per S3 x Z2 class (diag_weight3)
+                    const int mu1 = mb1 - J / 2, mu3 = J / 2 - mb, mu2 = -mu1 - mu3;
+                    const int perms = (mu1 == mu2 && mu2 == mu3) ? 1 : ((mu1 == mu2 || mu2 == mu3) ? 3 : 6);
+                    w *= (double)(perms * ((mu2 == 0) ? 1 : 2)) / (mid ? 1.0 : 2.0);
+                } else if (J1 == J2 && mb1 != mb2) w += w;
+                if (J == J1 && J1 != J2 && mb1 != mb && mb1 != J - mb) w += w;
+                BlkItem it;
+                const bool fx = mb1 > J1 / 2, fy = mb2 > J2 / 2;
+                const int ex = fx ? uhalf_off(J1) + (J1 - mb1) * (J1 + 1) + J1 : uhalf_off(J1) + mb1 * (J1 + 1);
+                const int ey = fy ? uhalf_off(J2) + (J2 - mb2) * (J2 + 1) + J2 : uhalf_off(J2) + mb2 * (J2 + 1);
+                it.xo = (ex << 2) | (fx ? 2 : 0) | (mb1 & 1);
+                it.yo = (ey << 2) | (fy ? 2 : 0) | (mb2 & 1);
+                it.w = w;
+                items.push_back(it);
+            }
+            const int n = hi - lo + 1;
+            // coefficient of (ma1, ma2): CG x weight of row ma in the fold (2; in the middle column 2 below the centre, 1 on it, 0 above)
+            auto cf = [&](int m1, int m2) {
+                const int ma = m1 + m2 - sh;
+                if (ma < 0 || ma > J) return 0.0;
+                const double wf = mid ? (ma < J / 2 ? 2.0 : (ma == J / 2 ? 1.0 : 0.0)) : 2.0;
+                return wf * T.cg[cg0 + m2 * (J1 + 1) + m1];
+            };
+            for (auto cx : chunks(J1 + 1, kBlkBX))
+                for (auto cy : chunks(J2 + 1, kBlkBY)) {
+                    int a_lo = 1 << 30, a_hi = -1, b_lo = 1 << 30, b_hi = -1;   // bounding box of the non-zero coefficients
+                    for (int a = cx.first; a < cx.first + cx.second; a++)
+                        for (int b = cy.first; b < cy.first + cy.second; b++)
+                            if (cf(a, b) != 0.0) { a_lo = std::min(a_lo, a); a_hi = std::max(a_hi, a); b_lo = std::min(b_lo, b); b_hi = std::max(b_hi, b); }
+                    if (a_hi < 0) continue;
+                    const int bx = a_hi - a_lo + 1, by = b_hi - b_lo + 1;
+                    HostUnit hu{};
+                    hu.triple = t;
+                    hu.u.item_first = item_first; hu.u.nitems = (short)n;
+                    hu.u.a0 = (short)a_lo; hu.u.b0 = (short)b_lo; hu.u.ma0 = (short)(a_lo + b_lo - sh);
+                    hu.u.uo = uhalf_off(J) + mb * (J + 1);
+                    hu.u.shape = (short)((bx - 1) * kBlkBY + (by - 1));
+                    if (coef.size() & 1) coef.push_back(0.0);
+                    hu.u.cgoff = (int)coef.size();
+                    for (int a = 0; a < bx; a++)
+                        for (int b = 0; b < by; b++) coef.push_back(cf(a_lo + a, b_lo + b));
+                    // issue cycles: an FP64 instruction holds the port for two, anything else for one
+                    hu.cost = n * (2.0 * (4 * bx * by + 2 * by) + 3.0 * bx + 2.0 * by + 30.0) + 2.0 * (2 * bx * by + 2 * (bx + by - 1)) + 0.5 * bx * by + bx + by + 60.0;
+                    tcost[t] += hu.cost;
+                    tunits[t].push_back(hu);
+                }
+        }
+    }
+    if (coef.size() & 1) coef.push_back(0.0);
+    coef.resize(coef.size() + 2, 0.0);
+    // pieces: whole triples, the heaviest ones cut into parts of at most half a warp's share
+    double total = 0.0;
+    for (double c : tcost) total += c;
+    const double share = total / NW;
+    struct Piece { int triple, begin, end; double cost; };
+    std::vector<Piece> pieces;
+    for (int t = 0; t < nt; t++) {
+        const int nu = (int)tunits[t].size();
+        if (nu == 0) continue;
+        const int parts = std::max(1, std::min(nu, (int)std::ceil(tcost[t] / (0.5 * share))));
+        int i = 0;
+        for (int k = 0; k < parts; k++) {
+            const double want = tcost[t] * (k + 1) / parts;
+            Piece pc{t, i, i, 0.0};
+            double run = 0.0;
+            for (int q = 0; q < i; q++) run += tunits[t][q].cost;
+            while (i < nu && (k == parts - 1 || run + 0.5 * tunits[t][i].cost <= want)) { run += tunits[t][i].cost; pc.cost += tunits[t][i].cost; i++; }
+            pc.end = i;
+            if (pc.end > pc.begin) pieces.push_back(pc);
+        }
+    }
+    std::stable_sort(pieces.begin(), pieces.end(), [](const Piece &a, const Piece &b) { return a.cost > b.cost; });
+    std::vector<double> load(NW, 0.0);
+    std::vector<int> piece_warp(pieces.size(), 0);
+    for (size_t i = 0; i < pieces.size(); i++) {
+        int w = 0;
+        for (int k = 1; k < NW; k++)
+            if (load[k] < load[w]) w = k;
+        load[w] += pieces[i].cost;
+        piece_warp[i] = w;
+    }
+    // slots: the pieces of a triple, in piece order; triples without work keep an empty range
+    std::vector<int> tslot(nt + 1, 0), piece_slot(pieces.size(), 0);
+    int nslots = 0;
+    for (int t = 0; t < nt; t++) {
+        tslot[t] = nslots;
+        for (size_t i = 0; i < pieces.size(); i++)
+            if (pieces[i].triple == t) piece_slot[i] = nslots++;
+    }
+    tslot[nt] = nslots;
+    if (nslots > kBlkMaxSlots) return fail(MALA_SNAP_ECUDA, "internal: too many partial-sum slots");
+    // units sorted by (warp, shape)
+    std::vector<std::vector<std::vector<BlkUnit>>> byws(NW, std::vector<std::vector<BlkUnit>>(kBlkShapes));
+    for (size_t i = 0; i < pieces.size(); i++)
+        for (int q = pieces[i].begin; q < pieces[i].end; q++) {
+            BlkUnit u = tunits[pieces[i].triple][q].u;
+            u.slot = (short)piece_slot[i];
+            byws[piece_warp[i]][u.shape].push_back(u);
+        }
+    std::vector<BlkUnit> units;
+    std::vector<int> wrange((size_t)NW * (kBlkShapes + 1), 0);
+    for (int w = 0; w < NW; w++) {
+        for (int sI = 0; sI < kBlkShapes; sI++) {
+            wrange[(size_t)w * (kBlkShapes + 1) + sI] = (int)units.size();
+            for (const BlkUnit &u : byws[w][sI]) units.push_back(u);
+        }
+        wrange[(size_t)w * (kBlkShapes + 1) + kBlkShapes] = (int)units.size();
+    }
+    int rc = 0;
+    if ((rc = upload(h->d_bitems, items))) return rc;
+    if ((rc = upload(h->d_bunits, units))) return rc;
+    if ((rc = upload(h->d_bcoef, coef))) return rc;
+    if ((rc = upload(h->d_bwrange, wrange))) return rc;
+    if ((rc = upload(h->d_btslot, tslot))) return rc;
+    h->blk_nslots = nslots;
+    h->blk_ready = true;
+    return 0;
+}
+
 // enqueue compute_zi_bi for one chunk
 int launch_zi(mala_snap *h, const ChunkBuffers &cb, double *out, cudaStream_t st) {
     const int grid = std::max(1, std::min(h->num_sms, h->half_tiles() ? 2 * cb.ntiles : cb.ntiles));
     TimedSpan span(h, st, kKindZi);
-    if (h->half_tiles())
+    if (h->use_block())
+        compute_zi_bi_block_kernel<<<grid, kBlkWarps * 32, compute_zi_block_smem_bytes(h->sc.nelem, h->sc.ntriples, h->blk_nslots), st>>>(
+            h->geom, h->sc, h->tables(), h->blk_tables(), cb, out);
+    else if (h->half_tiles())
         compute_zi_bi_diag_half_kernel<<<grid, kDiagHalfWarps * 32, compute_zi_diag_half_smem_bytes(h->sc.nelem, h->sc.ntriples), st>>>(
             h->geom, h->sc, h->tables(), h->diag_tables(), cb, out);
     else if (h->use_diag())
@@ -1186,6 +1353,7 @@ int mala_snap_create(mala_snap_t **handle, int twojmax, double rcutfac, double r
             CUDA_TRY(cudaMemcpyToSymbol(c_wlist, wlist, sizeof(wlist)));
         }
         if ((rc = build_diag_schedule(h))) return rc;
+        if (!h->half_tiles() && (rc = build_block_schedule(h))) return rc;
         if ((rc = set_kernel_attributes(h))) return rc;
         if (h->d_status.reserve(1)) return fail(MALA_SNAP_ENOMEM, "cudaMalloc (status) failed");
         CUDA_TRY(cudaMemset(h->d_status.p, 0, sizeof(int)));
@@ -1236,10 +1404,11 @@ int mala_snap_set_option(mala_snap_t *h, const char *name, long long value) {
     if (!h || !name) return fail(MALA_SNAP_EINVAL, "handle or name is NULL");
     const std::string n(name);
     if (n == "zi_impl") {
-        if (value < 0 || value > 3) return fail(MALA_SNAP_EINVAL, "zi_impl must be 0, 1, 2 or 3");
+        if (value < 0 || value > 4) return fail(MALA_SNAP_EINVAL, "zi_impl must be 0 .. 4");
         if (value == 2 && h->twojmax != kSpecTJ) return fail(MALA_SNAP_EINVAL, "the specialised kernel exists for twojmax = 10 only");
         if (value != 0 && value != 3 && h->half_tiles())
             return fail(MALA_SNAP_EINVAL, "twojmax > 10 runs on half tiles: only the anti-diagonal kernel (zi_impl 0 or 3) supports them");
+        if (value == 4 && !h->blk_ready) return fail(MALA_SNAP_EINVAL, "the block kernel has no tables for this handle");
         h->zi_impl = (int)value;
         return compute_bconst(h);
     }
@@ -1288,6 +1457,7 @@ int mala_snap_kernel_times(mala_snap_t *h, double ms[4], long long launches[4]) 
 
 const char *mala_snap_zi_kernel(const mala_snap_t *h) {
     if (!h) return "";
+    if (h->use_block()) return "compute_zi_bi_block_kernel";
     if (h->half_tiles()) return "compute_zi_bi_diag_half_kernel";
     return h->use_diag() ? "compute_zi_bi_diag_kernel" : (h->use_spec() ? "compute_zi_bi_coop_kernel" : "compute_zi_bi_generic_kernel");
 }

@@ -1,0 +1,203 @@
+// snap_zi_block.cuh -- compute_zi / compute_bi as register-tiled outer products (rows a5 + a6 + a7), any twojmax <= 10.
+//
+// For a triple (J1,J2,J) and an output column mb, the Z column is
+//     z[ma] = sum_{ma1 + ma2 - sh = ma} CG(ma1, ma2) * T[ma1][ma2],     T[ma1][ma2] = sum_items w_i x_i[ma1] y_i[ma2],
+// where the items i are the (mb1, mb2 = mb + sh - mb1) column pairs, x_i = U^{J1}[:, mb1], y_i = U^{J2}[:, mb2] and w_i the
+// Clebsch-Gordan factor of the column pair times the size of the symmetry class the item stands for (snap_zi_coop.cuh).
+// The per-triple and the anti-diagonal kernel apply CG(ma1, ma2) inside the item loop (6 FP64 instructions per product
+// term) and unroll the whole (ma1, ma2) rectangle, which makes their code long and walked once per item.  Here the item
+// loop is the INNER loop: a BX x BY block of T lives in registers, an item adds the outer product of BX elements of x and
+// BY elements of y (4 FP64 instructions per term), and the CG coefficients -- with the weights of the compute_bi fold
+// already multiplied in -- are applied once per block and column afterwards.  The body depends on the block shape only:
+// every triple, column and block runs through the same 24 small loops, which stay in the instruction caches.
+//
+// Work unit = (triple, column, block); the host cuts every rectangle into blocks of at most 4 x 6, trims each block to the
+// bounding box of its non-zero coefficients (the band 0 <= ma <= J, or ma <= J/2 in the middle column of an even J), packs
+// the coefficients per unit and deals the units of whole triples to the warps (the heaviest triples are split).  A unit adds
+// its share of B to a partial-sum slot owned by one warp; the slots of a triple are summed in a fixed order at the end of
+// the tile: bit-reproducible, no atomics, one CTA-wide barrier per tile.
+#pragma once
+#include "snap_zi.cuh"
+
+namespace mala {
+
+constexpr int kBlkWarps = 16;        // 128 registers per thread: a 4 x 6 complex block takes 96 of them
+constexpr int kBlkBX = 4, kBlkBY = 6;
+constexpr int kBlkShapes = kBlkBX * kBlkBY;
+constexpr int kBlkPadBytes = 5120;   // zeros in front of U: the fold may read up to 5 rows before a column (times an exact zero)
+constexpr int kBlkMaxSlots = 160;    // partial-sum slots (one per (warp, triple) pair that has work)
+
+struct __align__(16) BlkItem {       // one (mb1, mb2) column pair of an output column
+    int xo, yo;                      // (element index of row 0 of the column as it is read) << 2 | mirrored << 1 | (mb & 1)
+    double w;                        // CG factor of the column pair times its multiplicity
+};
+struct __align__(16) BlkUnit {
+    int item_first;                  // first item of the column in BlkTables::items
+    int cgoff;                       // offset (in doubles, even) of the packed coefficients [BX][BY] in BlkTables::coef
+    int uo;                          // element index of U^J[0][mb]
+    short nitems, a0, b0, ma0;       // block origin (ma1, ma2) and the row ma of its first anti-diagonal (may be negative)
+    short slot, shape, pad0, pad1;   // partial-sum slot; shape = (BX-1) * kBlkBY + (BY-1)
+};
+struct BlkTables {
+    const BlkItem *items;
+    const BlkUnit *units;            // sorted by (warp, shape)
+    const double *coef;
+    const int *wrange;               // [warps][kBlkShapes + 1] unit ranges per warp and shape
+    const int *tslot;                // [nt + 1] slots of triple t are tslot[t] .. tslot[t+1]-1
+    int nslots;
+};
+
+__device__ __forceinline__ double blk_flip(double v, unsigned mask) {
+    return __hiloint2double(__double2hiint(v) ^ (int)mask, __double2loint(v));
+}
+
+// one unit: returns its contribution to B of its triple (per lane = grid point)
+template <int BX, int BY>
+__device__ __forceinline__ double blk_unit(const unsigned char *Ulane, const BlkTables &T, const BlkUnit &u) {
+    constexpr int RB = 32 * (int)sizeof(double2);
+    double tr[BX][BY], ti[BX][BY];
+#pragma unroll
+    for (int a = 0; a < BX; a++)
+#pragma unroll
+        for (int b = 0; b < BY; b++) { tr[a][b] = 0.0; ti[a][b] = 0.0; }
+    const int a0 = u.a0, b0 = u.b0;
+    const BlkItem *it = T.items + u.item_first;
+#pragma unroll 1
+    for (int i = 0; i < u.nitems; i++) {
+        const int4 raw = __ldg(reinterpret_cast<const int4 *>(it + i));
+        const int xo = raw.x, yo = raw.y;
+        const double w = __hiloint2double(raw.w, raw.z);
+        const bool fx = xo & 2, fy = yo & 2;
+        const unsigned char *xp = Ulane + ((xo >> 2) + (fx ? -a0 : a0)) * RB;
+        const unsigned char *yp = Ulane + ((yo >> 2) + (fy ? -b0 : b0)) * RB;
+        const int xstep = fx ? -RB : RB, ystep = fy ? -RB : RB;
+        // mirrored column: u[ma][mb] = (-1)^(ma-mb) conj(u[J-ma][J-mb]); x by sign flips, y folded into four scale factors
+        const unsigned mx0 = (fx && ((a0 + xo) & 1)) ? 0x80000000u : 0u;   // local row 0 (and every even local row), real part
+        const unsigned mx1 = fx ? (mx0 ^ 0x80000000u) : 0u;                // odd local rows, real part
+        const double p0 = (fy && ((b0 + yo) & 1)) ? -w : w, p1 = fy ? -p0 : w, q0 = fy ? -p0 : w, q1 = fy ? -p1 : w;
+        double yr[BY], yi[BY];
+#pragma unroll
+        for (int b = 0; b < BY; b++) {
+            const double2 v = *reinterpret_cast<const double2 *>(yp + b * ystep);
+            yr[b] = v.x * ((b & 1) ? p1 : p0);
+            yi[b] = v.y * ((b & 1) ? q1 : q0);
+        }
+#pragma unroll
+        for (int a = 0; a < BX; a++) {
+            const double2 v = *reinterpret_cast<const double2 *>(xp + a * xstep);
+            const double xr = blk_flip(v.x, (a & 1) ? mx1 : mx0);
+            const double xi = blk_flip(v.y, fx ? ((a & 1) ? mx0 : mx1) : 0u);
+#pragma unroll
+            for (int b = 0; b < BY; b++) {
+                tr[a][b] = fma(xr, yr[b], tr[a][b]);
+                tr[a][b] = fma(-xi, yi[b], tr[a][b]);
+                ti[a][b] = fma(xr, yi[b], ti[a][b]);
+                ti[a][b] = fma(xi, yr[b], ti[a][b]);
+            }
+        }
+    }
+    // z on the anti-diagonals of the block (coefficients = CG x fold weight), dotted with conj(U^J[:, mb]) at once
+    const double2 *cp = reinterpret_cast<const double2 *>(T.coef + u.cgoff);
+    double cf[(BX * BY + 1) / 2 * 2];
+#pragma unroll
+    for (int k = 0; k < (BX * BY + 1) / 2; k++) {
+        const double2 c2 = __ldg(cp + k);
+        cf[2 * k] = c2.x;
+        cf[2 * k + 1] = c2.y;
+    }
+    const unsigned char *ub = Ulane + (u.uo + u.ma0) * RB;
+    double bs0 = 0.0, bs1 = 0.0;
+#pragma unroll
+    for (int d = 0; d < BX + BY - 1; d++) {
+        double zr = 0.0, zi = 0.0;
+#pragma unroll
+        for (int a = 0; a < BX; a++) {
+            const int b = d - a;
+            if (b >= 0 && b < BY) {
+                zr = fma(cf[a * BY + b], tr[a][b], zr);
+                zi = fma(cf[a * BY + b], ti[a][b], zi);
+            }
+        }
+        const double2 uu = *reinterpret_cast<const double2 *>(ub + d * RB);
+        bs0 = fma(uu.x, zr, bs0);
+        bs1 = fma(uu.y, zi, bs1);
+    }
+    return bs0 + bs1;
+}
+
+template <int BX, int BY>
+__device__ __forceinline__ void blk_run_shape(const unsigned char *Ulane, const BlkTables &T, const int warp, const int lane, double *P) {
+    constexpr int shape = (BX - 1) * kBlkBY + (BY - 1);
+    const int begin = __ldg(T.wrange + warp * (kBlkShapes + 1) + shape), end = __ldg(T.wrange + warp * (kBlkShapes + 1) + shape + 1);
+#pragma unroll 1
+    for (int k = begin; k < end; k++) {
+        // the unit record is warp-uniform: a broadcast tells the compiler so (uniform branches, uniform table addresses)
+        const int4 r0 = __ldg(reinterpret_cast<const int4 *>(T.units + k)), r1 = __ldg(reinterpret_cast<const int4 *>(T.units + k) + 1);
+        BlkUnit u;
+        u.item_first = __shfl_sync(0xffffffffu, r0.x, 0);
+        u.cgoff = __shfl_sync(0xffffffffu, r0.y, 0);
+        u.uo = __shfl_sync(0xffffffffu, r0.z, 0);
+        const int na = __shfl_sync(0xffffffffu, r0.w, 0), bm = __shfl_sync(0xffffffffu, r1.x, 0), ss = __shfl_sync(0xffffffffu, r1.y, 0);
+        u.nitems = (short)(na & 0xffff); u.a0 = (short)(na >> 16);
+        u.b0 = (short)(bm & 0xffff); u.ma0 = (short)(bm >> 16);
+        u.slot = (short)(ss & 0xffff);
+        const double b = blk_unit<BX, BY>(Ulane, T, u);
+        P[u.slot * 32 + lane] += b;
+    }
+}
+
+__global__ void __launch_bounds__(kBlkWarps * 32, 1)
+compute_zi_bi_block_kernel(GridGeom g, SnapConst sc, DeviceTables tb, BlkTables T, ChunkBuffers cb, double *out) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int NW = kBlkWarps;
+    const int nelem = sc.nelem, nt = sc.ntriples;
+    double2 *U = reinterpret_cast<double2 *>(smem_raw + kBlkPadBytes);
+    double *Bs = reinterpret_cast<double *>(U + (size_t)nelem * 32);
+    double *P = Bs + 32 * nt;   // [nslots][32]
+    __shared__ uint64_t bar;
+    __shared__ int s_slot;
+    const int lane = threadIdx.x & 31, warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
+    if (threadIdx.x == 0) mbar_init(&bar, 1);
+    for (int i = threadIdx.x; i < kBlkPadBytes / 8; i += NW * 32) reinterpret_cast<double *>(smem_raw)[i] = 0.0;
+    for (int i = threadIdx.x; i < 32 * nt; i += NW * 32) Bs[i] = 0.0;   // the fold may read (times zero) past the last column
+    uint32_t parity = 0;
+    const int nactive = cb.counters[0];
+    if (threadIdx.x == 0) s_slot = atomicAdd(&cb.counters[2], 1);
+    for (;;) {
+        __syncthreads();  // previous tile written out: Bs, P and U are free; s_slot is visible
+        const int slot = s_slot;
+        if (slot >= nactive) break;
+        const int wt = cb.active[slot];
+        __syncthreads();  // everybody has read s_slot
+        if (threadIdx.x == 0) {
+            tma_load_tile(U, cb.utot + (size_t)slot * nelem * 32, nelem, &bar);
+            const int next = atomicAdd(&cb.counters[2], 1);   // claim the next tile now and pull its U_tot into L2
+            s_slot = next;
+            if (next < nactive) prefetch_l2_tile(cb.utot + (size_t)next * nelem * 32, nelem);
+        }
+        for (int i = threadIdx.x; i < T.nslots * 32; i += NW * 32) P[i] = 0.0;
+        mbar_wait(&bar, parity);
+        parity ^= 1u;
+        __syncthreads();  // P zeroed
+        const unsigned char *Ulane = reinterpret_cast<const unsigned char *>(U + lane);
+#define MALA_BLK_ROW(BX) \
+    blk_run_shape<BX, 1>(Ulane, T, warp, lane, P); blk_run_shape<BX, 2>(Ulane, T, warp, lane, P); blk_run_shape<BX, 3>(Ulane, T, warp, lane, P); \
+    blk_run_shape<BX, 4>(Ulane, T, warp, lane, P); blk_run_shape<BX, 5>(Ulane, T, warp, lane, P); blk_run_shape<BX, 6>(Ulane, T, warp, lane, P);
+        MALA_BLK_ROW(4) MALA_BLK_ROW(3) MALA_BLK_ROW(2) MALA_BLK_ROW(1)
+#undef MALA_BLK_ROW
+        __syncthreads();
+        for (int t = warp; t < nt; t += NW) {   // fixed-order sum of the slots of triple t
+            double s = 0.0;
+            for (int k = __ldg(T.tslot + t); k < __ldg(T.tslot + t + 1); k++) s += P[k * 32 + lane];
+            Bs[lane * nt + t] = s;
+        }
+        __syncthreads();
+        write_tile(g, cb.tile_begin + wt, Bs, nt, out, NW, cb.compact_out, wt);
+    }
+}
+
+inline size_t compute_zi_block_smem_bytes(int nelem, int nt, int nslots) {
+    return (size_t)kBlkPadBytes + (size_t)nelem * 32 * sizeof(double2) + (size_t)32 * nt * sizeof(double) + (size_t)nslots * 32 * sizeof(double) + 16;
+}
+
+}  // namespace mala

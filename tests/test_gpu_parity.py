@@ -52,7 +52,7 @@ def tiny_ref():
     return w, oracle_grid(w)
 
 
-@pytest.mark.parametrize("zi_impl", [1, 2, 3])
+@pytest.mark.parametrize("zi_impl", [1, 2, 3, 4])
 def test_config1_tiny_al_full_grid(tiny_ref, zi_impl):
     w, ref = tiny_ref
     got = gpu_grid(w, zi_impl=zi_impl)
@@ -208,7 +208,7 @@ def test_random_small_systems_all_kernels():
         origin = tuple(rng.uniform(-0.3, 0.3, 3))
         ref = oracle.bispectrum_grid(pos, types, box, origin, pbc, ngrid, z0, z1, **params)
         with MalaSnap(**params) as snap:
-            for zi in ([3, 0] if tj > 10 else ([1, 3] if tj != 10 else [1, 2, 3])):
+            for zi in ([3, 0] if tj > 10 else ([1, 3, 4] if tj != 10 else [1, 2, 3, 4])):
                 snap.set_option("zi_impl", zi)
                 if rng.random() < 0.3:
                     snap.set_option("workspace_mb", 1)
@@ -216,7 +216,7 @@ def test_random_small_systems_all_kernels():
                 torch.cuda.synchronize()
                 assert_parity(got.cpu().numpy(), ref)
                 n += 1
-    assert n >= 120
+    assert n >= 160
 
 
 def test_zero_atoms_gives_self_term_everywhere():
