@@ -109,15 +109,13 @@ struct mala_snap {
     DevBuf<DiagTriple> d_dtriple;
     DevBuf<unsigned short> d_dsched, d_ditems;
     // tables of the block kernel (snap_zi_block.cuh)
-    DevBuf<BlkItem> d_bitems;
-    DevBuf<BlkUnit> d_bunits;
-    DevBuf<double> d_bcoef;
+    DevBuf<int4> d_bstream;
     DevBuf<int> d_bwrange, d_btslot;
     int blk_nslots = 0;
     bool blk_ready = false;
     BlkTables blk_tables() const {
         BlkTables t;
-        t.items = d_bitems.p; t.units = d_bunits.p; t.coef = d_bcoef.p; t.wrange = d_bwrange.p; t.tslot = d_btslot.p; t.nslots = blk_nslots;
+        t.stream = d_bstream.p; t.wrange = d_bwrange.p; t.tslot = d_btslot.p; t.nslots = blk_nslots;
         return t;
     }
     long long workspace_mb = 4096;
@@ -368,14 +366,15 @@ int build_diag_schedule(mala_snap *h) {
     return 0;
 }
 
-// Tables of the block kernel (snap_zi_block.cuh): items per (triple, column), units = blocks of the (ma1, ma2) rectangle with
-// their packed coefficients, the deal of the units to the warps and the partial-sum slots.
+// Tables of the block kernel (snap_zi_block.cuh): the units (blocks of the (ma1, ma2) rectangle of a triple and column, with
+// their items and packed coefficients), their deal to the warps, one record stream per warp and the partial-sum slots.
 int build_block_schedule(mala_snap *h) {
     const SnapTables &T = h->tab;
     const int nt = T.ntriples, NW = kBlkWarps;
-    std::vector<BlkItem> items;
-    std::vector<double> coef;
-    struct HostUnit { BlkUnit u; int triple; double cost; };
+    constexpr int RB = 32 * (int)sizeof(double2);
+    struct HostItem { int ex, ey; bool fx, fy; int mb1, mb2; double w; };   // element index of row 0 of each column as it is read
+    struct HostUnit { int triple, items_first, nitems, a0, b0, bx, by, ub_elem; std::vector<double> coef; double cost; };
+    std::vector<HostItem> items;
     std::vector<std::vector<HostUnit>> tunits(nt);
     std::vector<double> tcost(nt, 0.0);
     auto chunks = [](int len, int mx) {
@@ -393,7 +392,7 @@ int build_block_schedule(mala_snap *h) {
             diag_item_range(J1, J2, J, mb, lo, hi);
             if (hi < lo) continue;
             const bool mid = (J % 2 == 0) && (mb == J / 2);
-            const int item_first = (int)items.size();
+            const int items_first = (int)items.size();
             for (int mb1 = lo; mb1 <= hi; mb1++) {
                 const int mb2 = mb + sh - mb1;
                 double w = T.cg[cg0 + mb2 * (J1 + 1) + mb1];
@@ -403,13 +402,10 @@ int build_block_schedule(mala_snap *h) {
                     w *= (double)(perms * ((mu2 == 0) ? 1 : 2)) / (mid ? 1.0 : 2.0);
                 } else if (J1 == J2 && mb1 != mb2) w += w;
                 if (J == J1 && J1 != J2 && mb1 != mb && mb1 != J - mb) w += w;
-                BlkItem it;
-                const bool fx = mb1 > J1 / 2, fy = mb2 > J2 / 2;
-                const int ex = fx ? uhalf_off(J1) + (J1 - mb1) * (J1 + 1) + J1 : uhalf_off(J1) + mb1 * (J1 + 1);
-                const int ey = fy ? uhalf_off(J2) + (J2 - mb2) * (J2 + 1) + J2 : uhalf_off(J2) + mb2 * (J2 + 1);
-                it.xo = (ex << 2) | (fx ? 2 : 0) | (mb1 & 1);
-                it.yo = (ey << 2) | (fy ? 2 : 0) | (mb2 & 1);
-                it.w = w;
+                HostItem it;
+                it.fx = mb1 > J1 / 2; it.fy = mb2 > J2 / 2; it.mb1 = mb1; it.mb2 = mb2; it.w = w;
+                it.ex = it.fx ? uhalf_off(J1) + (J1 - mb1) * (J1 + 1) + J1 : uhalf_off(J1) + mb1 * (J1 + 1);
+                it.ey = it.fy ? uhalf_off(J2) + (J2 - mb2) * (J2 + 1) + J2 : uhalf_off(J2) + mb2 * (J2 + 1);
                 items.push_back(it);
             }
             const int n = hi - lo + 1;
@@ -427,26 +423,21 @@ int build_block_schedule(mala_snap *h) {
                         for (int b = cy.first; b < cy.first + cy.second; b++)
                             if (cf(a, b) != 0.0) { a_lo = std::min(a_lo, a); a_hi = std::max(a_hi, a); b_lo = std::min(b_lo, b); b_hi = std::max(b_hi, b); }
                     if (a_hi < 0) continue;
-                    const int bx = a_hi - a_lo + 1, by = b_hi - b_lo + 1;
-                    HostUnit hu{};
-                    hu.triple = t;
-                    hu.u.item_first = item_first; hu.u.nitems = (short)n;
-                    hu.u.a0 = (short)a_lo; hu.u.b0 = (short)b_lo; hu.u.ma0 = (short)(a_lo + b_lo - sh);
-                    hu.u.uo = uhalf_off(J) + mb * (J + 1);
-                    hu.u.shape = (short)((bx - 1) * kBlkBY + (by - 1));
-                    if (coef.size() & 1) coef.push_back(0.0);
-                    hu.u.cgoff = (int)coef.size();
-                    for (int a = 0; a < bx; a++)
-                        for (int b = 0; b < by; b++) coef.push_back(cf(a_lo + a, b_lo + b));
+                    HostUnit hu;
+                    hu.triple = t; hu.items_first = items_first; hu.nitems = n;
+                    hu.a0 = a_lo; hu.b0 = b_lo; hu.bx = a_hi - a_lo + 1; hu.by = b_hi - b_lo + 1;
+                    hu.ub_elem = uhalf_off(J) + mb * (J + 1) + (a_lo + b_lo - sh);   // row of the first anti-diagonal (may lie before the column)
+                    for (int a = 0; a < hu.bx; a++)
+                        for (int b = 0; b < hu.by; b++) hu.coef.push_back(cf(a_lo + a, b_lo + b));
                     // issue cycles: an FP64 instruction holds the port for two, anything else for one
-                    hu.cost = n * (2.0 * (4 * bx * by + 2 * by) + 3.0 * bx + 2.0 * by + 30.0) + 2.0 * (2 * bx * by + 2 * (bx + by - 1)) + 0.5 * bx * by + bx + by + 60.0;
+                    const int bx = hu.bx, by = hu.by;
+                    hu.cost = n * (2.0 * (4 * bx * by + 2 * by) + 3.0 * bx + 2.0 * by + 14.0) + 2.0 * (2 * bx * by + 2 * (bx + by - 1)) + 0.5 * bx * by +
+                              bx + by + 2.0 * bx * by + 40.0;
                     tcost[t] += hu.cost;
-                    tunits[t].push_back(hu);
+                    tunits[t].push_back(std::move(hu));
                 }
         }
     }
-    if (coef.size() & 1) coef.push_back(0.0);
-    coef.resize(coef.size() + 2, 0.0);
     // pieces: whole triples, the heaviest ones cut into parts of at most half a warp's share
     double total = 0.0;
     for (double c : tcost) total += c;
@@ -458,11 +449,10 @@ int build_block_schedule(mala_snap *h) {
         if (nu == 0) continue;
         const int parts = std::max(1, std::min(nu, (int)std::ceil(tcost[t] / (0.5 * share))));
         int i = 0;
+        double run = 0.0;
         for (int k = 0; k < parts; k++) {
             const double want = tcost[t] * (k + 1) / parts;
             Piece pc{t, i, i, 0.0};
-            double run = 0.0;
-            for (int q = 0; q < i; q++) run += tunits[t][q].cost;
             while (i < nu && (k == parts - 1 || run + 0.5 * tunits[t][i].cost <= want)) { run += tunits[t][i].cost; pc.cost += tunits[t][i].cost; i++; }
             pc.end = i;
             if (pc.end > pc.begin) pieces.push_back(pc);
@@ -488,27 +478,47 @@ int build_block_schedule(mala_snap *h) {
     }
     tslot[nt] = nslots;
     if (nslots > kBlkMaxSlots) return fail(MALA_SNAP_ECUDA, "internal: too many partial-sum slots");
-    // units sorted by (warp, shape)
-    std::vector<std::vector<std::vector<BlkUnit>>> byws(NW, std::vector<std::vector<BlkUnit>>(kBlkShapes));
-    for (size_t i = 0; i < pieces.size(); i++)
-        for (int q = pieces[i].begin; q < pieces[i].end; q++) {
-            BlkUnit u = tunits[pieces[i].triple][q].u;
-            u.slot = (short)piece_slot[i];
-            byws[piece_warp[i]][u.shape].push_back(u);
-        }
-    std::vector<BlkUnit> units;
-    std::vector<int> wrange((size_t)NW * (kBlkShapes + 1), 0);
+    // one record stream per warp, units by decreasing shape (the order in which the kernel runs its shape loops)
+    std::vector<int4> stream;
+    std::vector<int> wrange((size_t)NW * (kBlkShapes + 2), 0);
+    auto push_d2 = [&](double a, double b) {
+        int4 v;
+        std::memcpy(&v.x, &a, 8);
+        std::memcpy(&v.z, &b, 8);
+        stream.push_back(v);
+    };
     for (int w = 0; w < NW; w++) {
-        for (int sI = 0; sI < kBlkShapes; sI++) {
-            wrange[(size_t)w * (kBlkShapes + 1) + sI] = (int)units.size();
-            for (const BlkUnit &u : byws[w][sI]) units.push_back(u);
-        }
-        wrange[(size_t)w * (kBlkShapes + 1) + kBlkShapes] = (int)units.size();
+        wrange[(size_t)w * (kBlkShapes + 2) + kBlkShapes] = (int)stream.size();
+        for (int bx = kBlkBX; bx >= 1; bx--)
+            for (int by = kBlkBY; by >= 1; by--) {
+                int count = 0;
+                for (size_t i = 0; i < pieces.size(); i++) {
+                    if (piece_warp[i] != w) continue;
+                    for (int q = pieces[i].begin; q < pieces[i].end; q++) {
+                        const HostUnit &u = tunits[pieces[i].triple][q];
+                        if (u.bx != bx || u.by != by) continue;
+                        count++;
+                        stream.push_back(make_int4(u.nitems, u.ub_elem * RB, piece_slot[i], 0));
+                        for (int k = 0; k < u.nitems; k++) {
+                            const HostItem &it = items[u.items_first + k];
+                            const int xe = it.fx ? it.ex - u.a0 : it.ex + u.a0, ye = it.fy ? it.ey - u.b0 : it.ey + u.b0;
+                            // x = (-1)^(ma1 - mb1) conj(v) on a mirrored column: sign masks of the real part by the parity of the local row
+                            const unsigned sgn = 0x80000000u;
+                            const unsigned me = it.fx ? (((u.a0 + it.mb1) & 1) ? sgn : 0u) : 0u, mo = it.fx ? (me ^ sgn) : 0u;
+                            stream.push_back(make_int4(xe * RB | (it.fx ? 1 : 0), ye * RB | (it.fy ? 1 : 0), (int)me, (int)mo));
+                            const double pe = (it.fy && ((u.b0 + it.mb2) & 1)) ? -it.w : it.w, po = it.fy ? -pe : it.w;
+                            push_d2(pe, po);
+                        }
+                        for (size_t k = 0; k < u.coef.size(); k += 2) push_d2(u.coef[k], k + 1 < u.coef.size() ? u.coef[k + 1] : 0.0);
+                    }
+                }
+                wrange[(size_t)w * (kBlkShapes + 2) + (bx - 1) * kBlkBY + (by - 1)] = count;
+            }
+        wrange[(size_t)w * (kBlkShapes + 2) + kBlkShapes + 1] = (int)stream.size() - wrange[(size_t)w * (kBlkShapes + 2) + kBlkShapes];
     }
+    for (int k = 0; k < 128; k++) stream.push_back(make_int4(0, 0, 0, 0));   // the kernel prefetches up to 1 KB ahead
     int rc = 0;
-    if ((rc = upload(h->d_bitems, items))) return rc;
-    if ((rc = upload(h->d_bunits, units))) return rc;
-    if ((rc = upload(h->d_bcoef, coef))) return rc;
+    if ((rc = upload(h->d_bstream, stream))) return rc;
     if ((rc = upload(h->d_bwrange, wrange))) return rc;
     if ((rc = upload(h->d_btslot, tslot))) return rc;
     h->blk_nslots = nslots;

@@ -27,22 +27,18 @@ constexpr int kBlkShapes = kBlkBX * kBlkBY;
 constexpr int kBlkPadBytes = 5120;   // zeros in front of U: the fold may read up to 5 rows before a column (times an exact zero)
 constexpr int kBlkMaxSlots = 160;    // partial-sum slots (one per (warp, triple) pair that has work)
 
-struct __align__(16) BlkItem {       // one (mb1, mb2) column pair of an output column
-    int xo, yo;                      // (element index of row 0 of the column as it is read) << 2 | mirrored << 1 | (mb & 1)
-    double w;                        // CG factor of the column pair times its multiplicity
-};
-struct __align__(16) BlkUnit {
-    int item_first;                  // first item of the column in BlkTables::items
-    int cgoff;                       // offset (in doubles, even) of the packed coefficients [BX][BY] in BlkTables::coef
-    int uo;                          // element index of U^J[0][mb]
-    short nitems, a0, b0, ma0;       // block origin (ma1, ma2) and the row ma of its first anti-diagonal (may be negative)
-    short slot, shape, pad0, pad1;   // partial-sum slot; shape = (BX-1) * kBlkBY + (BY-1)
-};
+// Every warp reads ONE contiguous stream of 16-byte words, in the order it consumes them (units sorted by shape):
+//   unit header   int4   { nitems, byte offset of U^J[ma0][mb] (row of the block's first anti-diagonal; may be negative), slot, 0 }
+//   nitems x      int4   { x offset | reversed, y offset | reversed, sign mask of even rows, sign mask of odd rows }
+//                 double2{ scale of even y rows, scale of odd y rows }
+//   coefficients  double2 x ceil(BX BY / 2)      CG x fold weight, [a][b]
+// Offsets are bytes from the first element of the tile's U_tot to the element the block reads first, for lane 0; a column
+// beyond the middle is read backwards from its mirror image (u[ma][mb] = (-1)^(ma-mb) conj(u[J-ma][J-mb])): x gets its signs
+// by flipping sign bits (real part: mask of the row parity; imaginary part: the mask of the other parity), y has them folded
+// into its two scale factors (real part of an even row and imaginary part of an odd row take the first, the others the second).
 struct BlkTables {
-    const BlkItem *items;
-    const BlkUnit *units;            // sorted by (warp, shape)
-    const double *coef;
-    const int *wrange;               // [warps][kBlkShapes + 1] unit ranges per warp and shape
+    const int4 *stream;              // all warps, one after the other
+    const int *wrange;               // [warps][kBlkShapes + 2]: number of units per shape, then the warp's first word and word count
     const int *tslot;                // [nt + 1] slots of triple t are tslot[t] .. tslot[t+1]-1
     int nslots;
 };
@@ -50,43 +46,44 @@ struct BlkTables {
 __device__ __forceinline__ double blk_flip(double v, unsigned mask) {
     return __hiloint2double(__double2hiint(v) ^ (int)mask, __double2loint(v));
 }
+__device__ __forceinline__ void blk_prefetch(const void *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
-// one unit: returns its contribution to B of its triple (per lane = grid point)
+// one unit: reads its records at `ptr` (advanced past them) and returns its contribution to B of its triple, per lane
 template <int BX, int BY>
-__device__ __forceinline__ double blk_unit(const unsigned char *Ulane, const BlkTables &T, const BlkUnit &u) {
+__device__ __forceinline__ double blk_unit(const unsigned char *Ulane, const int4 *&ptr, int &slot) {
     constexpr int RB = 32 * (int)sizeof(double2);
     double tr[BX][BY], ti[BX][BY];
 #pragma unroll
     for (int a = 0; a < BX; a++)
 #pragma unroll
         for (int b = 0; b < BY; b++) { tr[a][b] = 0.0; ti[a][b] = 0.0; }
-    const int a0 = u.a0, b0 = u.b0;
-    const BlkItem *it = T.items + u.item_first;
+    const int4 hd = __ldg(ptr);
+    const int nitems = __shfl_sync(0xffffffffu, hd.x, 0), uboff = __shfl_sync(0xffffffffu, hd.y, 0);
+    slot = __shfl_sync(0xffffffffu, hd.z, 0);
+    ptr += 1;
+    blk_prefetch(ptr + 40);   // 640 .. 896 bytes ahead: the records of the next unit or two
+    blk_prefetch(ptr + 48);
+    blk_prefetch(ptr + 56);
 #pragma unroll 1
-    for (int i = 0; i < u.nitems; i++) {
-        const int4 raw = __ldg(reinterpret_cast<const int4 *>(it + i));
-        const int xo = raw.x, yo = raw.y;
-        const double w = __hiloint2double(raw.w, raw.z);
-        const bool fx = xo & 2, fy = yo & 2;
-        const unsigned char *xp = Ulane + ((xo >> 2) + (fx ? -a0 : a0)) * RB;
-        const unsigned char *yp = Ulane + ((yo >> 2) + (fy ? -b0 : b0)) * RB;
-        const int xstep = fx ? -RB : RB, ystep = fy ? -RB : RB;
-        // mirrored column: u[ma][mb] = (-1)^(ma-mb) conj(u[J-ma][J-mb]); x by sign flips, y folded into four scale factors
-        const unsigned mx0 = (fx && ((a0 + xo) & 1)) ? 0x80000000u : 0u;   // local row 0 (and every even local row), real part
-        const unsigned mx1 = fx ? (mx0 ^ 0x80000000u) : 0u;                // odd local rows, real part
-        const double p0 = (fy && ((b0 + yo) & 1)) ? -w : w, p1 = fy ? -p0 : w, q0 = fy ? -p0 : w, q1 = fy ? -p1 : w;
+    for (int i = 0; i < nitems; i++) {
+        const int4 r = __ldg(ptr);
+        const double2 sc = __ldg(reinterpret_cast<const double2 *>(ptr + 1));
+        ptr += 2;
+        const unsigned char *xp = Ulane + (r.x & ~1), *yp = Ulane + (r.y & ~1);
+        const int xstep = (r.x & 1) ? -RB : RB, ystep = (r.y & 1) ? -RB : RB;
+        const unsigned me = (unsigned)r.z, mo = (unsigned)r.w;
         double yr[BY], yi[BY];
 #pragma unroll
         for (int b = 0; b < BY; b++) {
             const double2 v = *reinterpret_cast<const double2 *>(yp + b * ystep);
-            yr[b] = v.x * ((b & 1) ? p1 : p0);
-            yi[b] = v.y * ((b & 1) ? q1 : q0);
+            yr[b] = v.x * ((b & 1) ? sc.y : sc.x);
+            yi[b] = v.y * ((b & 1) ? sc.x : sc.y);
         }
 #pragma unroll
         for (int a = 0; a < BX; a++) {
             const double2 v = *reinterpret_cast<const double2 *>(xp + a * xstep);
-            const double xr = blk_flip(v.x, (a & 1) ? mx1 : mx0);
-            const double xi = blk_flip(v.y, fx ? ((a & 1) ? mx0 : mx1) : 0u);
+            const double xr = blk_flip(v.x, (a & 1) ? mo : me);
+            const double xi = blk_flip(v.y, (a & 1) ? me : mo);
 #pragma unroll
             for (int b = 0; b < BY; b++) {
                 tr[a][b] = fma(xr, yr[b], tr[a][b]);
@@ -97,7 +94,8 @@ __device__ __forceinline__ double blk_unit(const unsigned char *Ulane, const Blk
         }
     }
     // z on the anti-diagonals of the block (coefficients = CG x fold weight), dotted with conj(U^J[:, mb]) at once
-    const double2 *cp = reinterpret_cast<const double2 *>(T.coef + u.cgoff);
+    const double2 *cp = reinterpret_cast<const double2 *>(ptr);
+    ptr += (BX * BY + 1) / 2;
     double cf[(BX * BY + 1) / 2 * 2];
 #pragma unroll
     for (int k = 0; k < (BX * BY + 1) / 2; k++) {
@@ -105,7 +103,7 @@ __device__ __forceinline__ double blk_unit(const unsigned char *Ulane, const Blk
         cf[2 * k] = c2.x;
         cf[2 * k + 1] = c2.y;
     }
-    const unsigned char *ub = Ulane + (u.uo + u.ma0) * RB;
+    const unsigned char *ub = Ulane + uboff;
     double bs0 = 0.0, bs1 = 0.0;
 #pragma unroll
     for (int d = 0; d < BX + BY - 1; d++) {
@@ -126,23 +124,15 @@ __device__ __forceinline__ double blk_unit(const unsigned char *Ulane, const Blk
 }
 
 template <int BX, int BY>
-__device__ __forceinline__ void blk_run_shape(const unsigned char *Ulane, const BlkTables &T, const int warp, const int lane, double *P) {
+__device__ __forceinline__ void blk_run_shape(const unsigned char *Ulane, const BlkTables &T, const int warp, const int lane, const int4 *&ptr,
+                                              double *P) {
     constexpr int shape = (BX - 1) * kBlkBY + (BY - 1);
-    const int begin = __ldg(T.wrange + warp * (kBlkShapes + 1) + shape), end = __ldg(T.wrange + warp * (kBlkShapes + 1) + shape + 1);
+    const int n = __ldg(T.wrange + warp * (kBlkShapes + 2) + shape);
 #pragma unroll 1
-    for (int k = begin; k < end; k++) {
-        // the unit record is warp-uniform: a broadcast tells the compiler so (uniform branches, uniform table addresses)
-        const int4 r0 = __ldg(reinterpret_cast<const int4 *>(T.units + k)), r1 = __ldg(reinterpret_cast<const int4 *>(T.units + k) + 1);
-        BlkUnit u;
-        u.item_first = __shfl_sync(0xffffffffu, r0.x, 0);
-        u.cgoff = __shfl_sync(0xffffffffu, r0.y, 0);
-        u.uo = __shfl_sync(0xffffffffu, r0.z, 0);
-        const int na = __shfl_sync(0xffffffffu, r0.w, 0), bm = __shfl_sync(0xffffffffu, r1.x, 0), ss = __shfl_sync(0xffffffffu, r1.y, 0);
-        u.nitems = (short)(na & 0xffff); u.a0 = (short)(na >> 16);
-        u.b0 = (short)(bm & 0xffff); u.ma0 = (short)(bm >> 16);
-        u.slot = (short)(ss & 0xffff);
-        const double b = blk_unit<BX, BY>(Ulane, T, u);
-        P[u.slot * 32 + lane] += b;
+    for (int k = 0; k < n; k++) {
+        int slot;
+        const double b = blk_unit<BX, BY>(Ulane, ptr, slot);
+        P[slot * 32 + lane] += b;
     }
 }
 
@@ -180,9 +170,11 @@ compute_zi_bi_block_kernel(GridGeom g, SnapConst sc, DeviceTables tb, BlkTables 
         parity ^= 1u;
         __syncthreads();  // P zeroed
         const unsigned char *Ulane = reinterpret_cast<const unsigned char *>(U + lane);
+        const int4 *ptr = T.stream + __ldg(T.wrange + warp * (kBlkShapes + 2) + kBlkShapes);
+        // shapes in decreasing size: the order of the stream
 #define MALA_BLK_ROW(BX) \
-    blk_run_shape<BX, 1>(Ulane, T, warp, lane, P); blk_run_shape<BX, 2>(Ulane, T, warp, lane, P); blk_run_shape<BX, 3>(Ulane, T, warp, lane, P); \
-    blk_run_shape<BX, 4>(Ulane, T, warp, lane, P); blk_run_shape<BX, 5>(Ulane, T, warp, lane, P); blk_run_shape<BX, 6>(Ulane, T, warp, lane, P);
+    blk_run_shape<BX, 6>(Ulane, T, warp, lane, ptr, P); blk_run_shape<BX, 5>(Ulane, T, warp, lane, ptr, P); blk_run_shape<BX, 4>(Ulane, T, warp, lane, ptr, P); \
+    blk_run_shape<BX, 3>(Ulane, T, warp, lane, ptr, P); blk_run_shape<BX, 2>(Ulane, T, warp, lane, ptr, P); blk_run_shape<BX, 1>(Ulane, T, warp, lane, ptr, P);
         MALA_BLK_ROW(4) MALA_BLK_ROW(3) MALA_BLK_ROW(2) MALA_BLK_ROW(1)
 #undef MALA_BLK_ROW
         __syncthreads();
