@@ -514,9 +514,9 @@ int build_block_schedule(mala_snap *h) {
                 }
                 wrange[(size_t)w * (kBlkShapes + 2) + (bx - 1) * kBlkBY + (by - 1)] = count;
             }
+        while ((stream.size() - (size_t)wrange[(size_t)w * (kBlkShapes + 2) + kBlkShapes]) % 32) stream.push_back(make_int4(0, 0, 0, 0));  // whole 512-byte chunks
         wrange[(size_t)w * (kBlkShapes + 2) + kBlkShapes + 1] = (int)stream.size() - wrange[(size_t)w * (kBlkShapes + 2) + kBlkShapes];
     }
-    for (int k = 0; k < 128; k++) stream.push_back(make_int4(0, 0, 0, 0));   // the kernel prefetches up to 1 KB ahead
     int rc = 0;
     if ((rc = upload(h->d_bstream, stream))) return rc;
     if ((rc = upload(h->d_bwrange, wrange))) return rc;

@@ -24,8 +24,8 @@ namespace mala {
 constexpr int kBlkWarps = 16;        // 128 registers per thread: a 4 x 6 complex block takes 96 of them
 constexpr int kBlkBX = 4, kBlkBY = 6;
 constexpr int kBlkShapes = kBlkBX * kBlkBY;
-constexpr int kBlkPadBytes = 5120;   // zeros in front of U: the fold may read up to 5 rows before a column (times an exact zero)
-constexpr int kBlkMaxSlots = 160;    // partial-sum slots (one per (warp, triple) pair that has work)
+constexpr int kBlkPadBytes = 3072;   // zeros in front of U: the fold may read up to 5 rows before a column (times an exact zero)
+constexpr int kBlkMaxSlots = 120;    // partial-sum slots (one per (warp, triple) pair that has work)
 
 // Every warp reads ONE contiguous stream of 16-byte words, in the order it consumes them (units sorted by shape):
 //   unit header   int4   { nitems, byte offset of U^J[ma0][mb] (row of the block's first anti-diagonal; may be negative), slot, 0 }
@@ -46,29 +46,65 @@ struct BlkTables {
 __device__ __forceinline__ double blk_flip(double v, unsigned mask) {
     return __hiloint2double(__double2hiint(v) ^ (int)mask, __double2loint(v));
 }
-__device__ __forceinline__ void blk_prefetch(const void *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+// The warp's record stream comes through a private ring in shared memory, filled 512 bytes at a time by one cp.async per lane:
+// requests run up to four chunks ahead of the word being consumed, so the records are on chip long before they are needed
+// (read straight from L2 they cost a quarter of the kernel's time in long-scoreboard stalls).
+constexpr int kBlkRingWords = 128;   // 16-byte words per warp (2 KB)
+struct BlkReader {
+    const int4 *src;     // the warp's stream
+    uint32_t ring;       // shared-memory address of the warp's ring
+    int lane;
+    int wpos, wreq, wready, wtotal;   // words consumed / requested / known to have arrived (multiples of 32) / in the stream
+    __device__ __forceinline__ void fill() {
+        // chunk [wreq, wreq + 32) takes the place of [wreq - 128, wreq - 96): free once wpos has passed it
+        while (wreq - (kBlkRingWords - 32) <= wpos && wreq < wtotal) {
+            const uint32_t dst = ring + (uint32_t)(((wreq + lane) & (kBlkRingWords - 1)) * 16);
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src + wreq + lane) : "memory");
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            wreq += 32;
+        }
+    }
+    __device__ __forceinline__ void ensure(const int wend) {   // words below wend must be readable
+        if (wend > wready) {
+            asm volatile("cp.async.wait_all;" ::: "memory");
+            __syncwarp();
+            wready = wreq;
+        }
+    }
+    __device__ __forceinline__ int4 word(const int w) const {
+        int4 v;
+        asm volatile("ld.shared.v4.s32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(ring + (uint32_t)((w & (kBlkRingWords - 1)) * 16)));
+        return v;
+    }
+    __device__ __forceinline__ double2 dword(const int w) const {
+        double2 v;
+        asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(ring + (uint32_t)((w & (kBlkRingWords - 1)) * 16)));
+        return v;
+    }
+};
 
-// one unit: reads its records at `ptr` (advanced past them) and returns its contribution to B of its triple, per lane
+// one unit: consumes its records from the reader and returns its contribution to B of its triple, per lane
 template <int BX, int BY>
-__device__ __forceinline__ double blk_unit(const unsigned char *Ulane, const int4 *&ptr, int &slot) {
+__device__ __forceinline__ double blk_unit(const unsigned char *Ulane, BlkReader &rd, int &slot) {
     constexpr int RB = 32 * (int)sizeof(double2);
+    constexpr int NCW = (BX * BY + 1) / 2;
     double tr[BX][BY], ti[BX][BY];
 #pragma unroll
     for (int a = 0; a < BX; a++)
 #pragma unroll
         for (int b = 0; b < BY; b++) { tr[a][b] = 0.0; ti[a][b] = 0.0; }
-    const int4 hd = __ldg(ptr);
-    const int nitems = __shfl_sync(0xffffffffu, hd.x, 0), uboff = __shfl_sync(0xffffffffu, hd.y, 0);
-    slot = __shfl_sync(0xffffffffu, hd.z, 0);
-    ptr += 1;
-    blk_prefetch(ptr + 40);   // 640 .. 896 bytes ahead: the records of the next unit or two
-    blk_prefetch(ptr + 48);
-    blk_prefetch(ptr + 56);
+    rd.ensure(rd.wpos + 1);
+    const int4 hd = rd.word(rd.wpos);
+    const int nitems = hd.x, uboff = hd.y;
+    slot = hd.z;
+    rd.ensure(rd.wpos + 1 + 2 * nitems + NCW);
+    rd.fill();
+    int w = rd.wpos + 1;
 #pragma unroll 1
     for (int i = 0; i < nitems; i++) {
-        const int4 r = __ldg(ptr);
-        const double2 sc = __ldg(reinterpret_cast<const double2 *>(ptr + 1));
-        ptr += 2;
+        const int4 r = rd.word(w);
+        const double2 sc = rd.dword(w + 1);
+        w += 2;
         const unsigned char *xp = Ulane + (r.x & ~1), *yp = Ulane + (r.y & ~1);
         const int xstep = (r.x & 1) ? -RB : RB, ystep = (r.y & 1) ? -RB : RB;
         const unsigned me = (unsigned)r.z, mo = (unsigned)r.w;
@@ -94,15 +130,14 @@ __device__ __forceinline__ double blk_unit(const unsigned char *Ulane, const int
         }
     }
     // z on the anti-diagonals of the block (coefficients = CG x fold weight), dotted with conj(U^J[:, mb]) at once
-    const double2 *cp = reinterpret_cast<const double2 *>(ptr);
-    ptr += (BX * BY + 1) / 2;
-    double cf[(BX * BY + 1) / 2 * 2];
+    double cf[NCW * 2];
 #pragma unroll
-    for (int k = 0; k < (BX * BY + 1) / 2; k++) {
-        const double2 c2 = __ldg(cp + k);
+    for (int k = 0; k < NCW; k++) {
+        const double2 c2 = rd.dword(w + k);
         cf[2 * k] = c2.x;
         cf[2 * k + 1] = c2.y;
     }
+    rd.wpos = w + NCW;
     const unsigned char *ub = Ulane + uboff;
     double bs0 = 0.0, bs1 = 0.0;
 #pragma unroll
@@ -124,14 +159,14 @@ __device__ __forceinline__ double blk_unit(const unsigned char *Ulane, const int
 }
 
 template <int BX, int BY>
-__device__ __forceinline__ void blk_run_shape(const unsigned char *Ulane, const BlkTables &T, const int warp, const int lane, const int4 *&ptr,
+__device__ __forceinline__ void blk_run_shape(const unsigned char *Ulane, const BlkTables &T, const int warp, const int lane, BlkReader &rd,
                                               double *P) {
     constexpr int shape = (BX - 1) * kBlkBY + (BY - 1);
     const int n = __ldg(T.wrange + warp * (kBlkShapes + 2) + shape);
 #pragma unroll 1
     for (int k = 0; k < n; k++) {
         int slot;
-        const double b = blk_unit<BX, BY>(Ulane, ptr, slot);
+        const double b = blk_unit<BX, BY>(Ulane, rd, slot);
         P[slot * 32 + lane] += b;
     }
 }
@@ -144,6 +179,7 @@ compute_zi_bi_block_kernel(GridGeom g, SnapConst sc, DeviceTables tb, BlkTables 
     double2 *U = reinterpret_cast<double2 *>(smem_raw + kBlkPadBytes);
     double *Bs = reinterpret_cast<double *>(U + (size_t)nelem * 32);
     double *P = Bs + 32 * nt;   // [nslots][32]
+    int4 *rings = reinterpret_cast<int4 *>(P + (size_t)T.nslots * 32);   // [NW][kBlkRingWords]
     __shared__ uint64_t bar;
     __shared__ int s_slot;
     const int lane = threadIdx.x & 31, warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
@@ -166,15 +202,20 @@ compute_zi_bi_block_kernel(GridGeom g, SnapConst sc, DeviceTables tb, BlkTables 
             if (next < nactive) prefetch_l2_tile(cb.utot + (size_t)next * nelem * 32, nelem);
         }
         for (int i = threadIdx.x; i < T.nslots * 32; i += NW * 32) P[i] = 0.0;
+        BlkReader rd;
+        rd.src = T.stream + __ldg(T.wrange + warp * (kBlkShapes + 2) + kBlkShapes);
+        rd.wtotal = __ldg(T.wrange + warp * (kBlkShapes + 2) + kBlkShapes + 1);
+        rd.ring = smem_u32(rings + warp * kBlkRingWords);
+        rd.lane = lane; rd.wpos = 0; rd.wreq = 0; rd.wready = 0;
+        rd.fill();   // the first four chunks travel while the U_tot tile does
         mbar_wait(&bar, parity);
         parity ^= 1u;
         __syncthreads();  // P zeroed
         const unsigned char *Ulane = reinterpret_cast<const unsigned char *>(U + lane);
-        const int4 *ptr = T.stream + __ldg(T.wrange + warp * (kBlkShapes + 2) + kBlkShapes);
         // shapes in decreasing size: the order of the stream
 #define MALA_BLK_ROW(BX) \
-    blk_run_shape<BX, 6>(Ulane, T, warp, lane, ptr, P); blk_run_shape<BX, 5>(Ulane, T, warp, lane, ptr, P); blk_run_shape<BX, 4>(Ulane, T, warp, lane, ptr, P); \
-    blk_run_shape<BX, 3>(Ulane, T, warp, lane, ptr, P); blk_run_shape<BX, 2>(Ulane, T, warp, lane, ptr, P); blk_run_shape<BX, 1>(Ulane, T, warp, lane, ptr, P);
+    blk_run_shape<BX, 6>(Ulane, T, warp, lane, rd, P); blk_run_shape<BX, 5>(Ulane, T, warp, lane, rd, P); blk_run_shape<BX, 4>(Ulane, T, warp, lane, rd, P); \
+    blk_run_shape<BX, 3>(Ulane, T, warp, lane, rd, P); blk_run_shape<BX, 2>(Ulane, T, warp, lane, rd, P); blk_run_shape<BX, 1>(Ulane, T, warp, lane, rd, P);
         MALA_BLK_ROW(4) MALA_BLK_ROW(3) MALA_BLK_ROW(2) MALA_BLK_ROW(1)
 #undef MALA_BLK_ROW
         __syncthreads();
@@ -189,7 +230,8 @@ compute_zi_bi_block_kernel(GridGeom g, SnapConst sc, DeviceTables tb, BlkTables 
 }
 
 inline size_t compute_zi_block_smem_bytes(int nelem, int nt, int nslots) {
-    return (size_t)kBlkPadBytes + (size_t)nelem * 32 * sizeof(double2) + (size_t)32 * nt * sizeof(double) + (size_t)nslots * 32 * sizeof(double) + 16;
+    return (size_t)kBlkPadBytes + (size_t)nelem * 32 * sizeof(double2) + (size_t)32 * nt * sizeof(double) + (size_t)nslots * 32 * sizeof(double) +
+           (size_t)kBlkWarps * kBlkRingWords * 16 + 16;
 }
 
 }  // namespace mala
