@@ -488,7 +488,10 @@ int build_block_schedule(mala_snap *h) {
         stream.push_back(v);
     };
     for (int w = 0; w < NW; w++) {
-        wrange[(size_t)w * (kBlkShapes + 2) + kBlkShapes] = (int)stream.size();
+        const size_t w0 = stream.size();
+        wrange[(size_t)w * (kBlkShapes + 2) + kBlkShapes] = (int)w0;
+        size_t last_header = 0;
+        bool have_header = false;
         for (int bx = kBlkBX; bx >= 1; bx--)
             for (int by = kBlkBY; by >= 1; by--) {
                 int count = 0;
@@ -498,6 +501,17 @@ int build_block_schedule(mala_snap *h) {
                         const HostUnit &u = tunits[pieces[i].triple][q];
                         if (u.bx != bx || u.by != by) continue;
                         count++;
+                        // a unit must not straddle the end of the ring: the unit before it skips the words up to the boundary
+                        const int words = 1 + 3 * u.nitems + (bx * by + 1) / 2;
+                        const size_t pos = stream.size() - w0;
+                        if (pos / kBlkRingWords != (pos + words - 1) / kBlkRingWords) {
+                            const int skip = (int)(kBlkRingWords - pos % kBlkRingWords);
+                            if (!have_header) return fail(MALA_SNAP_ECUDA, "internal: block stream starts with an oversized unit");
+                            stream[last_header].w += skip;
+                            for (int k = 0; k < skip; k++) stream.push_back(make_int4(0, 0, 0, 0));
+                        }
+                        last_header = stream.size();
+                        have_header = true;
                         stream.push_back(make_int4(u.nitems, u.ub_elem * RB, piece_slot[i], 0));
                         for (int k = 0; k < u.nitems; k++) {
                             const HostItem &it = items[u.items_first + k];
@@ -505,7 +519,8 @@ int build_block_schedule(mala_snap *h) {
                             // x = (-1)^(ma1 - mb1) conj(v) on a mirrored column: sign masks of the real part by the parity of the local row
                             const unsigned sgn = 0x80000000u;
                             const unsigned me = it.fx ? (((u.a0 + it.mb1) & 1) ? sgn : 0u) : 0u, mo = it.fx ? (me ^ sgn) : 0u;
-                            stream.push_back(make_int4(xe * RB | (it.fx ? 1 : 0), ye * RB | (it.fy ? 1 : 0), (int)me, (int)mo));
+                            stream.push_back(make_int4(xe * RB, it.fx ? -RB : RB, ye * RB, it.fy ? -RB : RB));
+                            stream.push_back(make_int4((int)me, (int)mo, it.fx ? 1 : 0, 0));
                             const double pe = (it.fy && ((u.b0 + it.mb2) & 1)) ? -it.w : it.w, po = it.fy ? -pe : it.w;
                             push_d2(pe, po);
                         }
@@ -514,8 +529,8 @@ int build_block_schedule(mala_snap *h) {
                 }
                 wrange[(size_t)w * (kBlkShapes + 2) + (bx - 1) * kBlkBY + (by - 1)] = count;
             }
-        while ((stream.size() - (size_t)wrange[(size_t)w * (kBlkShapes + 2) + kBlkShapes]) % 32) stream.push_back(make_int4(0, 0, 0, 0));  // whole 512-byte chunks
-        wrange[(size_t)w * (kBlkShapes + 2) + kBlkShapes + 1] = (int)stream.size() - wrange[(size_t)w * (kBlkShapes + 2) + kBlkShapes];
+        while ((stream.size() - w0) % 32) stream.push_back(make_int4(0, 0, 0, 0));  // whole 512-byte chunks
+        wrange[(size_t)w * (kBlkShapes + 2) + kBlkShapes + 1] = (int)(stream.size() - w0);
     }
     int rc = 0;
     if ((rc = upload(h->d_bstream, stream))) return rc;

@@ -28,8 +28,10 @@ constexpr int kBlkPadBytes = 3072;   // zeros in front of U: the fold may read u
 constexpr int kBlkMaxSlots = 120;    // partial-sum slots (one per (warp, triple) pair that has work)
 
 // Every warp reads ONE contiguous stream of 16-byte words, in the order it consumes them (units sorted by shape):
-//   unit header   int4   { nitems, byte offset of U^J[ma0][mb] (row of the block's first anti-diagonal; may be negative), slot, 0 }
-//   nitems x      int4   { x offset | reversed, y offset | reversed, sign mask of even rows, sign mask of odd rows }
+//   unit header   int4   { nitems, byte offset of U^J[ma0][mb] (row of the block's first anti-diagonal; may be negative), slot,
+//                          words to skip behind the unit (the host keeps a unit from straddling the end of the ring) }
+//   nitems x      int4   { x offset, x step, y offset, y step }                (bytes; a step is +-512)
+//                 int4   { sign mask of even x rows, of odd x rows, x reversed, 0 }
 //                 double2{ scale of even y rows, scale of odd y rows }
 //   coefficients  double2 x ceil(BX BY / 2)      CG x fold weight, [a][b]
 // Offsets are bytes from the first element of the tile's U_tot to the element the block reads first, for lane 0; a column
@@ -50,6 +52,21 @@ __device__ __forceinline__ double blk_flip(double v, unsigned mask) {
 // requests run up to four chunks ahead of the word being consumed, so the records are on chip long before they are needed
 // (read straight from L2 they cost a quarter of the kernel's time in long-scoreboard stalls).
 constexpr int kBlkRingWords = 128;   // 16-byte words per warp (2 KB)
+__device__ __forceinline__ int4 blk_lds4(const uint32_t addr) {
+    int4 v;
+    asm volatile("ld.shared.v4.s32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ double blk_lds1(const uint32_t addr) {
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ double2 blk_lds2(const uint32_t addr) {
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
 struct BlkReader {
     const int4 *src;     // the warp's stream
     uint32_t ring;       // shared-memory address of the warp's ring
@@ -94,20 +111,23 @@ __device__ __forceinline__ double blk_unit(const unsigned char *Ulane, BlkReader
 #pragma unroll
         for (int b = 0; b < BY; b++) { tr[a][b] = 0.0; ti[a][b] = 0.0; }
     rd.ensure(rd.wpos + 1);
-    const int4 hd = rd.word(rd.wpos);
+    // a unit never wraps around the ring: its words are read at fixed offsets from `base`
+    uint32_t base = rd.ring + (uint32_t)((rd.wpos & (kBlkRingWords - 1)) * 16);
+    const int4 hd = blk_lds4(base);
     const int nitems = hd.x, uboff = hd.y;
     slot = hd.z;
-    rd.ensure(rd.wpos + 1 + 2 * nitems + NCW);
-    rd.fill();
-    int w = rd.wpos + 1;
+    const int wend = rd.wpos + 1 + 3 * nitems + NCW;
+    rd.ensure(wend);
+    rd.wpos = wend + hd.w;
+    base += 16;
 #pragma unroll 1
     for (int i = 0; i < nitems; i++) {
-        const int4 r = rd.word(w);
-        const double2 sc = rd.dword(w + 1);
-        w += 2;
-        const unsigned char *xp = Ulane + (r.x & ~1), *yp = Ulane + (r.y & ~1);
-        const int xstep = (r.x & 1) ? -RB : RB, ystep = (r.y & 1) ? -RB : RB;
-        const unsigned me = (unsigned)r.z, mo = (unsigned)r.w;
+        const int4 r = blk_lds4(base);
+        const int4 m = blk_lds4(base + 16);
+        const double2 sc = blk_lds2(base + 32);
+        base += 48;
+        const unsigned char *xp = Ulane + r.x, *yp = Ulane + r.z;
+        const int xstep = r.y, ystep = r.w;
         double yr[BY], yi[BY];
 #pragma unroll
         for (int b = 0; b < BY; b++) {
@@ -115,6 +135,7 @@ __device__ __forceinline__ double blk_unit(const unsigned char *Ulane, BlkReader
             yr[b] = v.x * ((b & 1) ? sc.y : sc.x);
             yi[b] = v.y * ((b & 1) ? sc.x : sc.y);
         }
+        const unsigned me = (unsigned)m.x, mo = (unsigned)m.y;   // mirrored x column: (-1)^(ma1 - mb1) conj (zero masks otherwise)
 #pragma unroll
         for (int a = 0; a < BX; a++) {
             const double2 v = *reinterpret_cast<const double2 *>(xp + a * xstep);
@@ -129,15 +150,8 @@ __device__ __forceinline__ double blk_unit(const unsigned char *Ulane, BlkReader
             }
         }
     }
-    // z on the anti-diagonals of the block (coefficients = CG x fold weight), dotted with conj(U^J[:, mb]) at once
-    double cf[NCW * 2];
-#pragma unroll
-    for (int k = 0; k < NCW; k++) {
-        const double2 c2 = rd.dword(w + k);
-        cf[2 * k] = c2.x;
-        cf[2 * k + 1] = c2.y;
-    }
-    rd.wpos = w + NCW;
+    // z on the anti-diagonals of the block (coefficients = CG x fold weight, read where they are used: T dies element by
+    // element, so the registers never hold the block and its coefficients together), dotted with conj(U^J[:, mb]) at once
     const unsigned char *ub = Ulane + uboff;
     double bs0 = 0.0, bs1 = 0.0;
 #pragma unroll
@@ -147,14 +161,16 @@ __device__ __forceinline__ double blk_unit(const unsigned char *Ulane, BlkReader
         for (int a = 0; a < BX; a++) {
             const int b = d - a;
             if (b >= 0 && b < BY) {
-                zr = fma(cf[a * BY + b], tr[a][b], zr);
-                zi = fma(cf[a * BY + b], ti[a][b], zi);
+                const double c = blk_lds1(base + 8 * (a * BY + b));
+                zr = fma(c, tr[a][b], zr);
+                zi = fma(c, ti[a][b], zi);
             }
         }
         const double2 uu = *reinterpret_cast<const double2 *>(ub + d * RB);
         bs0 = fma(uu.x, zr, bs0);
         bs1 = fma(uu.y, zi, bs1);
     }
+    rd.fill();   // only now: the requests overwrite ring words up to wpos, i.e. this unit's
     return bs0 + bs1;
 }
 
