@@ -178,10 +178,11 @@ int mala_gaussian_grid(mala_snap_t *h, double sigma, int natoms, const double *p
 
 /*
  * Tuning / test knobs.  Unknown names give MALA_SNAP_EINVAL.
- *   "zi_impl"          0 = automatic (per-triple specialised kernel when twojmax == 10, anti-diagonal kernel
- *                      otherwise), 1 = generic table-driven kernel (twojmax <= 10), 2 = per-triple specialised kernel
- *                      (EINVAL if twojmax != 10), 3 = anti-diagonal kernel (code specialised on j1 only, any twojmax;
- *                      its tables are per-handle arrays in global memory, so handles of different twojmax coexist).
+ *   "zi_impl"          0 = automatic (register-tiled block kernel up to twojmax 10, anti-diagonal kernel on half tiles above),
+ *                      1 = generic table-driven kernel (twojmax <= 10), 2 = per-triple specialised kernel (EINVAL if
+ *                      twojmax != 10), 3 = anti-diagonal kernel (code specialised on j1 only, any twojmax), 4 = block kernel
+ *                      (twojmax <= 10).  All tables but the per-triple kernel's are per-handle arrays in global memory, so
+ *                      handles of different twojmax coexist.  Every kernel gives the same B up to rounding (summation order).
  *   "timing"           1 = record a CUDA-event pair on the caller's stream around every kernel launch of the
  *                      following calls (read back with mala_snap_kernel_times); 0 = off (default)
  *   "workspace_mb"     cap, in MiB, of the U_tot + candidate workspace (default 4096)

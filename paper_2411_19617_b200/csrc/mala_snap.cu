@@ -180,10 +180,10 @@ struct mala_snap {
     }
     // twojmax above kFullTileTwoJ: U_tot of 32 points does not fit one SM's shared memory; half-tile layout and kernel
     bool half_tiles() const { return twojmax > kFullTileTwoJ; }
-    // 0 = automatic: the per-triple specialised kernel at twojmax = 10, the anti-diagonal kernel otherwise
-    bool use_spec() const { return zi_impl == 2 || (zi_impl == 0 && twojmax == kSpecTJ); }
-    bool use_diag() const { return zi_impl == 3 || (zi_impl == 0 && twojmax != kSpecTJ); }
-    bool use_block() const { return zi_impl == 4 && !half_tiles(); }
+    // 0 = automatic: the block kernel up to twojmax = 10, the anti-diagonal kernel on half tiles above
+    bool use_block() const { return (zi_impl == 4 || zi_impl == 0) && !half_tiles() && blk_ready; }
+    bool use_spec() const { return zi_impl == 2; }
+    bool use_diag() const { return zi_impl == 3 || (zi_impl == 0 && !use_block()); }
 };
 
 namespace {
