@@ -209,7 +209,9 @@ int set_kernel_attributes(mala_snap *h) {
                                   (int)compute_zi_diag_smem_bytes(uhalf_size(kFullTileTwoJ), triple_count(kFullTileTwoJ))));
     CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_diag_half_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   (int)compute_zi_diag_half_smem_bytes(uhalf_size(kMaxTwoJ), triple_count(kMaxTwoJ))));
-    CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_block_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_block_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)compute_zi_block_smem_bytes(uhalf_size(kFullTileTwoJ), triple_count(kFullTileTwoJ), kBlkMaxSlots)));
+    CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_block_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   (int)compute_zi_block_smem_bytes(uhalf_size(kFullTileTwoJ), triple_count(kFullTileTwoJ), kBlkMaxSlots)));
     (void)h;
     return 0;
@@ -425,12 +427,18 @@ int build_block_schedule(mala_snap *h) {
                     if (a_hi < 0) continue;
                     HostUnit hu;
                     hu.triple = t; hu.items_first = items_first; hu.nitems = n;
-                    hu.a0 = a_lo; hu.b0 = b_lo; hu.bx = a_hi - a_lo + 1; hu.by = b_hi - b_lo + 1;
+                    // pad to the smallest shape the kernel has a body for: shift the origin back where the column is long enough,
+                    // else run past its end (those reads hit other finite words of the tile and meet zero coefficients)
+                    int bx = a_hi - a_lo + 1, by = b_hi - b_lo + 1;
+                    if (bx < kBlkBXMin) { a_lo = std::max(0, std::min(a_lo, J1 + 1 - kBlkBXMin)); bx = kBlkBXMin; }
+                    if (by < kBlkBYMin) { b_lo = std::max(0, std::min(b_lo, J2 + 1 - kBlkBYMin)); by = kBlkBYMin; }
+                    hu.a0 = a_lo; hu.b0 = b_lo; hu.bx = bx; hu.by = by;
                     hu.ub_elem = uhalf_off(J) + mb * (J + 1) + (a_lo + b_lo - sh);   // row of the first anti-diagonal (may lie before the column)
                     for (int a = 0; a < hu.bx; a++)
-                        for (int b = 0; b < hu.by; b++) hu.coef.push_back(cf(a_lo + a, b_lo + b));
+                        for (int b = 0; b < hu.by; b++)
+                            hu.coef.push_back((a_lo + a >= cx.first && a_lo + a < cx.first + cx.second && b_lo + b >= cy.first && b_lo + b < cy.first + cy.second)
+                                                  ? cf(a_lo + a, b_lo + b) : 0.0);
                     // issue cycles: an FP64 instruction holds the port for two, anything else for one
-                    const int bx = hu.bx, by = hu.by;
                     hu.cost = n * (2.0 * (4 * bx * by + 2 * by) + 3.0 * bx + 2.0 * by + 14.0) + 2.0 * (2 * bx * by + 2 * (bx + by - 1)) + 0.5 * bx * by +
                               bx + by + 2.0 * bx * by + 40.0;
                     tcost[t] += hu.cost;
@@ -467,6 +475,12 @@ int build_block_schedule(mala_snap *h) {
             if (load[k] < load[w]) w = k;
         load[w] += pieces[i].cost;
         piece_warp[i] = w;
+    }
+    if (std::getenv("MALA_BLK_DEBUG")) {
+        double mx = 0.0;
+        for (double l : load) mx = std::max(mx, l);
+        std::fprintf(stderr, "block schedule: twojmax %d, %zu pieces, total %.0f, mean load %.0f, max load %.0f (%.3f)\n", h->twojmax, pieces.size(), total, total / NW, mx, mx / (total / NW));
+        for (int t = 0; t < nt; t++) if (tcost[t] > 0.3 * share) std::fprintf(stderr, "  triple %d (%d,%d,%d) cost %.0f units %zu\n", t, T.triples[4*t], T.triples[4*t+1], T.triples[4*t+2], tcost[t], tunits[t].size());
     }
     // slots: the pieces of a triple, in piece order; triples without work keep an empty range
     std::vector<int> tslot(nt + 1, 0), piece_slot(pieces.size(), 0);
@@ -545,9 +559,11 @@ int build_block_schedule(mala_snap *h) {
 int launch_zi(mala_snap *h, const ChunkBuffers &cb, double *out, cudaStream_t st) {
     const int grid = std::max(1, std::min(h->num_sms, h->half_tiles() ? 2 * cb.ntiles : cb.ntiles));
     TimedSpan span(h, st, kKindZi);
-    if (h->use_block())
-        compute_zi_bi_block_kernel<<<grid, kBlkWarps * 32, compute_zi_block_smem_bytes(h->sc.nelem, h->sc.ntriples, h->blk_nslots), st>>>(
-            h->geom, h->sc, h->tables(), h->blk_tables(), cb, out);
+    if (h->use_block()) {
+        const size_t smem = compute_zi_block_smem_bytes(h->sc.nelem, h->sc.ntriples, h->blk_nslots);
+        if (h->twojmax >= 8) compute_zi_bi_block_kernel<true><<<grid, kBlkWarps * 32, smem, st>>>(h->geom, h->sc, h->tables(), h->blk_tables(), cb, out);
+        else compute_zi_bi_block_kernel<false><<<grid, kBlkWarps * 32, smem, st>>>(h->geom, h->sc, h->tables(), h->blk_tables(), cb, out);
+    }
     else if (h->half_tiles())
         compute_zi_bi_diag_half_kernel<<<grid, kDiagHalfWarps * 32, compute_zi_diag_half_smem_bytes(h->sc.nelem, h->sc.ntriples), st>>>(
             h->geom, h->sc, h->tables(), h->diag_tables(), cb, out);

@@ -9,9 +9,9 @@
 // loop is the INNER loop: a BX x BY block of T lives in registers, an item adds the outer product of BX elements of x and
 // BY elements of y (4 FP64 instructions per term), and the CG coefficients -- with the weights of the compute_bi fold
 // already multiplied in -- are applied once per block and column afterwards.  The body depends on the block shape only:
-// every triple, column and block runs through the same 24 small loops, which stay in the instruction caches.
+// every triple, column and block runs through the same 30 small loops, which stay in the instruction caches.
 //
-// Work unit = (triple, column, block); the host cuts every rectangle into blocks of at most 4 x 6, trims each block to the
+// Work unit = (triple, column, block); the host cuts every rectangle into blocks of at most 6 x 5, trims each block to the
 // bounding box of its non-zero coefficients (the band 0 <= ma <= J, or ma <= J/2 in the middle column of an even J), packs
 // the coefficients per unit and deals the units of whole triples to the warps (the heaviest triples are split).  A unit adds
 // its share of B to a partial-sum slot owned by one warp; the slots of a triple are summed in a fixed order at the end of
@@ -21,8 +21,26 @@
 
 namespace mala {
 
-constexpr int kBlkWarps = 16;        // 128 registers per thread: a 4 x 6 complex block takes 96 of them
-constexpr int kBlkBX = 4, kBlkBY = 6;
+#ifndef MALA_BLK_WARPS
+#define MALA_BLK_WARPS 12
+#endif
+#ifndef MALA_BLK_BX
+#define MALA_BLK_BX 6
+#endif
+#ifndef MALA_BLK_BY
+#define MALA_BLK_BY 5
+#endif
+constexpr int kBlkWarps = MALA_BLK_WARPS;   // 12 warps = 168 registers per thread: a 6 x 5 complex block takes 120 of them
+constexpr int kBlkBX = MALA_BLK_BX, kBlkBY = MALA_BLK_BY;
+#ifndef MALA_BLK_BXMIN
+#define MALA_BLK_BXMIN 3
+#endif
+#ifndef MALA_BLK_BYMIN
+#define MALA_BLK_BYMIN 3
+#endif
+// smaller blocks are padded to the minimum shape with zero coefficients (2-3 % more FP64 work): 12 loop bodies instead of 30,
+// which is what the instruction caches reward (twojmax 6: 3.0 ms with all 30 shapes and the first item peeled, 1.8 ms with 12 and none)
+constexpr int kBlkBXMin = MALA_BLK_BXMIN, kBlkBYMin = MALA_BLK_BYMIN;
 constexpr int kBlkShapes = kBlkBX * kBlkBY;
 constexpr int kBlkPadBytes = 3072;   // zeros in front of U: the fold may read up to 5 rows before a column (times an exact zero)
 constexpr int kBlkMaxSlots = 120;    // partial-sum slots (one per (warp, triple) pair that has work)
@@ -100,55 +118,74 @@ struct BlkReader {
     }
 };
 
-// one unit: consumes its records from the reader and returns its contribution to B of its triple, per lane
-template <int BX, int BY>
-__device__ __forceinline__ double blk_unit(const unsigned char *Ulane, BlkReader &rd, int &slot) {
-    constexpr int RB = 32 * (int)sizeof(double2);
-    constexpr int NCW = (BX * BY + 1) / 2;
-    double tr[BX][BY], ti[BX][BY];
+// one item of a unit: T (+)= x (x) y.  FIRST: the block starts from this item's products (no zeroing pass)
+template <int BX, int BY, bool FIRST>
+__device__ __forceinline__ void blk_item(const unsigned char *Ulane, const uint32_t base, double (&tr)[BX][BY], double (&ti)[BX][BY]) {
+    const int4 r = blk_lds4(base);
+    const int4 m = blk_lds4(base + 16);
+    const double2 sc = blk_lds2(base + 32);
+    const unsigned char *xp = Ulane + r.x, *yp = Ulane + r.z;
+    const int xstep = r.y, ystep = r.w;
+    double yr[BY], yi[BY];
 #pragma unroll
-    for (int a = 0; a < BX; a++)
+    for (int b = 0; b < BY; b++) {
+        const double2 v = *reinterpret_cast<const double2 *>(yp + b * ystep);
+        yr[b] = v.x * ((b & 1) ? sc.y : sc.x);
+        yi[b] = v.y * ((b & 1) ? sc.x : sc.y);
+    }
+    const unsigned me = (unsigned)m.x, mo = (unsigned)m.y;   // mirrored x column: (-1)^(ma1 - mb1) conj (zero masks otherwise)
 #pragma unroll
-        for (int b = 0; b < BY; b++) { tr[a][b] = 0.0; ti[a][b] = 0.0; }
-    rd.ensure(rd.wpos + 1);
-    // a unit never wraps around the ring: its words are read at fixed offsets from `base`
-    uint32_t base = rd.ring + (uint32_t)((rd.wpos & (kBlkRingWords - 1)) * 16);
-    const int4 hd = blk_lds4(base);
-    const int nitems = hd.x, uboff = hd.y;
-    slot = hd.z;
-    const int wend = rd.wpos + 1 + 3 * nitems + NCW;
-    rd.ensure(wend);
-    rd.wpos = wend + hd.w;
-    base += 16;
-#pragma unroll 1
-    for (int i = 0; i < nitems; i++) {
-        const int4 r = blk_lds4(base);
-        const int4 m = blk_lds4(base + 16);
-        const double2 sc = blk_lds2(base + 32);
-        base += 48;
-        const unsigned char *xp = Ulane + r.x, *yp = Ulane + r.z;
-        const int xstep = r.y, ystep = r.w;
-        double yr[BY], yi[BY];
+    for (int a = 0; a < BX; a++) {
+        const double2 v = *reinterpret_cast<const double2 *>(xp + a * xstep);
+        const double xr = blk_flip(v.x, (a & 1) ? mo : me);
+        const double xi = blk_flip(v.y, (a & 1) ? me : mo);
 #pragma unroll
         for (int b = 0; b < BY; b++) {
-            const double2 v = *reinterpret_cast<const double2 *>(yp + b * ystep);
-            yr[b] = v.x * ((b & 1) ? sc.y : sc.x);
-            yi[b] = v.y * ((b & 1) ? sc.x : sc.y);
-        }
-        const unsigned me = (unsigned)m.x, mo = (unsigned)m.y;   // mirrored x column: (-1)^(ma1 - mb1) conj (zero masks otherwise)
-#pragma unroll
-        for (int a = 0; a < BX; a++) {
-            const double2 v = *reinterpret_cast<const double2 *>(xp + a * xstep);
-            const double xr = blk_flip(v.x, (a & 1) ? mo : me);
-            const double xi = blk_flip(v.y, (a & 1) ? me : mo);
-#pragma unroll
-            for (int b = 0; b < BY; b++) {
+            if (FIRST) {
+                tr[a][b] = fma(-xi, yi[b], xr * yr[b]);
+                ti[a][b] = fma(xi, yr[b], xr * yi[b]);
+            } else {
                 tr[a][b] = fma(xr, yr[b], tr[a][b]);
                 tr[a][b] = fma(-xi, yi[b], tr[a][b]);
                 ti[a][b] = fma(xr, yi[b], ti[a][b]);
                 ti[a][b] = fma(xi, yr[b], ti[a][b]);
             }
         }
+    }
+}
+
+// one unit: consumes its records from the reader and returns its contribution to B of its triple, per lane
+template <int BX, int BY, bool PEEL>
+__device__ __forceinline__ double blk_unit(const unsigned char *Ulane, BlkReader &rd, int &slot) {
+    constexpr int RB = 32 * (int)sizeof(double2);
+    constexpr int NCW = (BX * BY + 1) / 2;
+    double tr[BX][BY], ti[BX][BY];
+    rd.ensure(rd.wpos + 1);
+    // a unit never wraps around the ring: its words are read at fixed offsets from `base`
+    uint32_t base = rd.ring + (uint32_t)((rd.wpos & (kBlkRingWords - 1)) * 16);
+    const int4 hd = blk_lds4(base);
+    const int nitems = hd.x, uboff = hd.y;   // nitems >= 1
+    slot = hd.z;
+    const int wend = rd.wpos + 1 + 3 * nitems + NCW;
+    rd.ensure(wend);
+    rd.wpos = wend + hd.w;
+    base += 16;
+    // PEEL: the first item initialises the block (no zeroing pass, -4 % instructions) at the price of a second copy of the
+    // item body; pays from twojmax 8 up, where a tile has enough work per fetched instruction
+    if constexpr (PEEL) {
+        blk_item<BX, BY, true>(Ulane, base, tr, ti);
+        base += 48;
+    } else {
+#pragma unroll
+        for (int a = 0; a < BX; a++)
+#pragma unroll
+            for (int b = 0; b < BY; b++) { tr[a][b] = 0.0; ti[a][b] = 0.0; }
+    }
+    const int ifirst = PEEL ? 1 : 0;
+#pragma unroll 1
+    for (int i = ifirst; i < nitems; i++) {
+        blk_item<BX, BY, false>(Ulane, base, tr, ti);
+        base += 48;
     }
     // z on the anti-diagonals of the block (coefficients = CG x fold weight, read where they are used: T dies element by
     // element, so the registers never hold the block and its coefficients together), dotted with conj(U^J[:, mb]) at once
@@ -174,7 +211,7 @@ __device__ __forceinline__ double blk_unit(const unsigned char *Ulane, BlkReader
     return bs0 + bs1;
 }
 
-template <int BX, int BY>
+template <int BX, int BY, bool PEEL>
 __device__ __forceinline__ void blk_run_shape(const unsigned char *Ulane, const BlkTables &T, const int warp, const int lane, BlkReader &rd,
                                               double *P) {
     constexpr int shape = (BX - 1) * kBlkBY + (BY - 1);
@@ -182,11 +219,19 @@ __device__ __forceinline__ void blk_run_shape(const unsigned char *Ulane, const 
 #pragma unroll 1
     for (int k = 0; k < n; k++) {
         int slot;
-        const double b = blk_unit<BX, BY>(Ulane, rd, slot);
+        const double b = blk_unit<BX, BY, PEEL>(Ulane, rd, slot);
         P[slot * 32 + lane] += b;
     }
 }
 
+template <int BX, int BY, bool PEEL>
+__device__ __forceinline__ void blk_run_all(const unsigned char *Ulane, const BlkTables &T, const int warp, const int lane, BlkReader &rd, double *P) {
+    if constexpr (BX >= kBlkBXMin && BY >= kBlkBYMin) blk_run_shape<BX, BY, PEEL>(Ulane, T, warp, lane, rd, P);
+    if constexpr (BY > 1) blk_run_all<BX, BY - 1, PEEL>(Ulane, T, warp, lane, rd, P);
+    else if constexpr (BX > 1) blk_run_all<BX - 1, kBlkBY, PEEL>(Ulane, T, warp, lane, rd, P);
+}
+
+template <bool PEEL>
 __global__ void __launch_bounds__(kBlkWarps * 32, 1)
 compute_zi_bi_block_kernel(GridGeom g, SnapConst sc, DeviceTables tb, BlkTables T, ChunkBuffers cb, double *out) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -228,12 +273,7 @@ compute_zi_bi_block_kernel(GridGeom g, SnapConst sc, DeviceTables tb, BlkTables 
         parity ^= 1u;
         __syncthreads();  // P zeroed
         const unsigned char *Ulane = reinterpret_cast<const unsigned char *>(U + lane);
-        // shapes in decreasing size: the order of the stream
-#define MALA_BLK_ROW(BX) \
-    blk_run_shape<BX, 6>(Ulane, T, warp, lane, rd, P); blk_run_shape<BX, 5>(Ulane, T, warp, lane, rd, P); blk_run_shape<BX, 4>(Ulane, T, warp, lane, rd, P); \
-    blk_run_shape<BX, 3>(Ulane, T, warp, lane, rd, P); blk_run_shape<BX, 2>(Ulane, T, warp, lane, rd, P); blk_run_shape<BX, 1>(Ulane, T, warp, lane, rd, P);
-        MALA_BLK_ROW(4) MALA_BLK_ROW(3) MALA_BLK_ROW(2) MALA_BLK_ROW(1)
-#undef MALA_BLK_ROW
+        blk_run_all<kBlkBX, kBlkBY, PEEL>(Ulane, T, warp, lane, rd, P);   // shapes in decreasing size: the order of the stream
         __syncthreads();
         for (int t = warp; t < nt; t += NW) {   // fixed-order sum of the slots of triple t
             double s = 0.0;
