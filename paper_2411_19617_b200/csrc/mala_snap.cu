@@ -20,6 +20,7 @@
 #include "snap_internal.h"
 #include "snap_tables.h"
 #include "snap_ui.cuh"
+#include "snap_ui_dft.cuh"
 #include "snap_zi.cuh"
 #include "snap_zi_coop.cuh"
 #include "snap_zi_diag.cuh"
@@ -101,6 +102,7 @@ struct mala_snap {
     int device = 0, num_sms = 0;
     // options
     int zi_impl = 0;
+    int ui_impl = 0;   // 0 automatic (sampling kernel when twojmax == 10), 1 column kernel, 2 sampling kernel
     // tables of the anti-diagonal kernels (per handle, global memory)
     std::vector<double> k_dcg;
     std::vector<DiagTriple> k_dtriple;
@@ -182,6 +184,7 @@ struct mala_snap {
     bool half_tiles() const { return twojmax > kFullTileTwoJ; }
     // 0 = automatic: the block kernel up to twojmax = 10, the anti-diagonal kernel on half tiles above
     bool use_block() const { return (zi_impl == 4 || zi_impl == 0) && !half_tiles() && blk_ready; }
+    bool use_ui_dft() const { return twojmax == kFullTileTwoJ && ui_impl != 1; }
     bool use_spec() const { return zi_impl == 2; }
     bool use_diag() const { return zi_impl == 3 || (zi_impl == 0 && !use_block()); }
 };
@@ -202,6 +205,8 @@ int set_kernel_attributes(mala_snap *h) {
     CUDA_TRY(cudaFuncSetAttribute(compute_ui_kernel<kFullTileTwoJ, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ui_smem));
     CUDA_TRY(cudaFuncSetAttribute(compute_ui_kernel<kMaxTwoJ, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   (int)compute_ui_smem_bytes(kMaxTwoJ)));
+    CUDA_TRY(cudaFuncSetAttribute(compute_ui_dft_kernel<kFullTileTwoJ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)compute_ui_dft_smem_bytes<kFullTileTwoJ>()));
     const int zi_smem = (int)compute_zi_smem_bytes(uhalf_size(kFullTileTwoJ), triple_count(kFullTileTwoJ));
     CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, zi_smem));
     CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_coop_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)compute_zi_coop_smem_bytes()));
@@ -970,7 +975,10 @@ int run_slab(mala_snap *h, int z0, int z1, double *out, double2 *u_out, cudaStre
                 compute_ui_kernel<kMaxTwoJ, false><<<ui_grid, (kMaxTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kMaxTwoJ), st>>>(g, h->sc, tb, cb);
             } else {
                 const int ui_grid = std::max(1, std::min(2 * h->num_sms, 2 * cb.ntiles));  // half-tile items, two CTAs per SM
-                if (h->twojmax == kFullTileTwoJ)
+                if (h->use_ui_dft())   // twojmax = 10: column polynomials sampled at the 11th roots of unity (snap_ui_dft.cuh), whole tiles
+                    compute_ui_dft_kernel<kFullTileTwoJ><<<std::max(1, std::min(h->num_sms, cb.ntiles)), (kFullTileTwoJ + 1) * 32,
+                                                           compute_ui_dft_smem_bytes<kFullTileTwoJ>(), st>>>(g, h->sc, tb, cb);
+                else if (h->twojmax == kFullTileTwoJ)
                     compute_ui_kernel<kFullTileTwoJ, true><<<ui_grid, (kFullTileTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kFullTileTwoJ), st>>>(g, h->sc, tb, cb);
                 else  // smaller twojmax: same code with run-time guards on the levels
                     compute_ui_kernel<kFullTileTwoJ, false><<<ui_grid, (kFullTileTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kFullTileTwoJ), st>>>(g, h->sc, tb, cb);
@@ -1149,7 +1157,10 @@ int run_slab_force(mala_snap *h, int z0, int z1, const double *beta, double *gou
         const int grid2 = std::max(1, std::min(2 * h->num_sms, 2 * cb.ntiles));
         {
             TimedSpan span(h, st, kKindUi);
-            if (h->twojmax == kFullTileTwoJ)
+            if (h->use_ui_dft())
+                compute_ui_dft_kernel<kFullTileTwoJ><<<std::max(1, std::min(h->num_sms, cb.ntiles)), (kFullTileTwoJ + 1) * 32,
+                                                       compute_ui_dft_smem_bytes<kFullTileTwoJ>(), st>>>(g, h->sc, tb, cb);
+            else if (h->twojmax == kFullTileTwoJ)
                 compute_ui_kernel<kFullTileTwoJ, true><<<grid2, (kFullTileTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kFullTileTwoJ), st>>>(g, h->sc, tb, cb);
             else
                 compute_ui_kernel<kFullTileTwoJ, false><<<grid2, (kFullTileTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kFullTileTwoJ), st>>>(g, h->sc, tb, cb);
@@ -1444,6 +1455,12 @@ int mala_snap_triples(const mala_snap_t *h, int *j1j2j) {
 int mala_snap_set_option(mala_snap_t *h, const char *name, long long value) {
     if (!h || !name) return fail(MALA_SNAP_EINVAL, "handle or name is NULL");
     const std::string n(name);
+    if (n == "ui_impl") {
+        if (value < 0 || value > 2) return fail(MALA_SNAP_EINVAL, "ui_impl must be 0, 1 or 2");
+        if (value == 2 && h->twojmax != kFullTileTwoJ) return fail(MALA_SNAP_EINVAL, "the sampling compute_ui kernel is built for twojmax = 10");
+        h->ui_impl = (int)value;
+        return MALA_SNAP_OK;
+    }
     if (n == "zi_impl") {
         if (value < 0 || value > 4) return fail(MALA_SNAP_EINVAL, "zi_impl must be 0 .. 4");
         if (value == 2 && h->twojmax != kSpecTJ) return fail(MALA_SNAP_EINVAL, "the specialised kernel exists for twojmax = 10 only");

@@ -1,0 +1,189 @@
+// snap_ui_dft.cuh -- compute_ui by sampling the column polynomials (rows a3 + a4 of SURVEY.md 8(a)), twojmax = 10.
+//
+// Same quantity and the same storage as snap_ui.cuh: U_tot^J = wself*I + sum_neighbors c * U^J(neighbor) in half columns,
+// where column mb of level J is the coefficient list of the polynomial Q_{J,mb}(x) = (b + a x)^mb (conj(a) - conj(b) x)^(J-mb),
+// a and b the Cayley-Klein parameters of the neighbor (Eq. (24)-(25)).
+//
+// A polynomial of degree <= 10 is fixed by its values at the 11th roots of unity x_s, and there its value is a product of
+// powers:  Q_{J,mb}(x_s) = u_s^mb v_s^(J-mb),  u_s = b + a x_s,  v_s = conj(a) - conj(b) x_s.  So instead of carrying
+// coefficient lists through a recursion and adding them to accumulators in shared memory neighbor by neighbor (snap_ui.cuh:
+// 4,300 FP64 instructions per pair, half of the issue slots lost to barriers, shared-memory round trips and bookkeeping),
+//   * warp s owns sample point x_s, lane = grid point (a whole 32-point tile), and keeps the 36 sums
+//     S_{J,mb}(x_s) = sum_neighbors c u_s^mb v_s^(J-mb) in REGISTERS over all neighbors of the point: per neighbor one complex
+//     multiplication and one complex addition per (J, mb) -- 224 FP64 instructions, nothing else but five loads;
+//   * once per tile the coefficients come back by the inverse DFT of length 11, q_k = (1/11) sum_s S(x_s) x_s^(-k)
+//     (unitary, hence well conditioned: 1.6e-14 absolute on sums of 30 neighbors), followed by the binomial normalisation
+//     and the self term as before.
+// 2,460 + 470 (DFT, amortised over ~26 neighbors) FP64 instructions per pair, one instruction stream for all eleven warps,
+// no atomics, fixed summation order (bit-reproducible).
+// Everything in front of the accumulation (candidate windows, distance tests, dealing the hits to all warps for the pair
+// geometry) is that of compute_ui_kernel, on whole tiles.
+#pragma once
+#include "snap_ui.cuh"
+
+namespace mala {
+
+constexpr int kDftCap = 48;   // neighbor entries per grid point buffered between two accumulate passes
+
+constexpr int dft_njm(int tj) {   // number of (J, mb <= J/2) columns
+    int n = 0;
+    for (int J = 0; J <= tj; J++) n += J / 2 + 1;
+    return n;
+}
+// accumulator index of column (mb, n = J - mb), n >= mb: mb-major, the order in which the kernel produces them
+constexpr int dft_index(int tj, int mb, int n) {
+    int idx = 0;
+    for (int m = 0; m < mb; m++) idx += tj - 2 * m + 1;
+    return idx + (n - mb);
+}
+
+template <int TJ>
+__global__ void __launch_bounds__((TJ + 1) * 32, 1)
+compute_ui_dft_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers cb) {
+    constexpr int NW = TJ + 1;          // warps = sample points
+    constexpr int NJM = dft_njm(TJ);
+    constexpr int nelem = uhalf_size(TJ);
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    // phase 1: geo [kDftCap][5][32], crec [kDftCap][6], hitk [32][kDftCap];  phase 2 (same bytes): S [NW][NJM][32] double2
+    double *geo = reinterpret_cast<double *>(smem_raw);
+    double *crec = geo + kDftCap * 5 * 32;
+    unsigned char *hitk = reinterpret_cast<unsigned char *>(crec + kDftCap * 6);
+    double2 *S = reinterpret_cast<double2 *>(smem_raw);
+    __shared__ int s_item;
+    __shared__ double2 s_tw[NW * NW];   // [k][s] = x_s^(-k) = e^{-2 pi i s k / NW}
+    __shared__ unsigned short s_elem[nelem];   // element -> column index << 4 | k
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x < NW * NW) {
+        double sn, cs;
+        sincospi(2.0 * (double)(((threadIdx.x / NW) * (threadIdx.x % NW)) % NW) / (double)NW, &sn, &cs);
+        s_tw[threadIdx.x] = make_double2(cs, -sn);
+    }
+    if (threadIdx.x == 0) {
+        int e = 0;
+        for (int J = 0; J <= TJ; J++)
+            for (int mb = 0; mb <= J / 2; mb++)
+                for (int k = 0; k <= J; k++, e++) s_elem[e] = (unsigned short)((dft_index(TJ, mb, J - mb) << 4) | k);
+    }
+    double xsr, xsi;                    // this warp's sample point x_s = e^{2 pi i s / NW}
+    {
+        double sn, cs;
+        sincospi(2.0 * (double)warp / (double)NW, &sn, &cs);
+        xsr = cs; xsi = sn;
+    }
+
+    for (;;) {
+        __syncthreads();  // everybody is done with the previous tile (S reads, s_item)
+        if (threadIdx.x == 0) s_item = atomicAdd(&cb.counters[1], 1);
+        __syncthreads();
+        const int slot = s_item;
+        if (slot >= cb.counters[0]) break;
+        const int wt = cb.active[slot];
+        const int tile = cb.tile_begin + wt;
+        int ix, iy, iz;
+        bool valid;
+        lane_point(g, tile, lane, ix, iy, iz, valid);
+        ix = min(ix, g.nx - 1); iy = min(iy, g.ny - 1); iz = min(iz, g.z1 - 1);  // ragged tiles: a valid point whose result is never used
+        double px, py, pz;
+        point_position(g, ix, iy, iz, px, py, pz);
+
+        double accr[NJM], acci[NJM];
+#pragma unroll
+        for (int k = 0; k < NJM; k++) { accr[k] = 0.0; acci[k] = 0.0; }
+
+        const int nc = cb.ncand[wt];
+        const int *mycand = cb.cand + (size_t)wt * cb.cand_cap;
+        for (int wbase = 0; wbase < nc; wbase += kDftCap) {
+            const int nw = min(kDftCap, nc - wbase);
+            __syncthreads();  // crec, hitk and geo free again
+            if ((int)threadIdx.x < nw) {
+                const Ghost gh = cb.ghosts[mycand[wbase + threadIdx.x]];
+                const double rc = tb.type_rcut[gh.type];
+                double *q = crec + threadIdx.x * 6;
+                q[0] = gh.x; q[1] = gh.y; q[2] = gh.z; q[3] = rc; q[4] = tb.type_w[gh.type]; q[5] = rc * rc;
+            }
+            __syncthreads();
+            int cnt = 0;  // neighbors of this lane's point in the window (identical in every warp)
+            for (int k = 0; k < nw; k++) {
+                const double *q = crec + k * 6;
+                const double dx = q[0] - px, dy = q[1] - py, dz = q[2] - pz;
+                if (dx * dx + dy * dy + dz * dz < q[5]) {
+                    if (warp == 0) hitk[lane * kDftCap + cnt] = (unsigned char)k;
+                    cnt++;
+                }
+            }
+            __syncthreads();
+            // the hits of a point are dealt to the NW lanes of that point: pair geometry once per (point, neighbor)
+            for (int e = warp; e < cnt; e += NW) {
+                const double *q = crec + (int)hitk[lane * kDftCap + e] * 6;
+                const double dx = q[0] - px, dy = q[1] - py, dz = q[2] - pz;
+                const double r2 = dx * dx + dy * dy + dz * dz;
+                double c, ar, ai, br, bi;
+                pair_geometry(dx, dy, dz, r2, q[3], q[4], sc.rfac0, sc.rmin0, c, ar, ai, br, bi);
+                double *o = geo + (size_t)e * 5 * 32 + lane;
+                o[0] = c; o[32] = ar; o[64] = ai; o[96] = br; o[128] = bi;
+            }
+            __syncthreads();
+            const int nmax = __reduce_max_sync(0xffffffffu, cnt);
+#pragma unroll 1
+            for (int i = 0; i < nmax; i++) {
+                double c = 0.0, ar = 1.0, ai = 0.0, br = 0.0, bi = 0.0;   // lanes past their count add zeros
+                if (i < cnt) {
+                    const double *q = geo + (size_t)i * 5 * 32 + lane;
+                    c = q[0]; ar = q[32]; ai = q[64]; br = q[96]; bi = q[128];
+                }
+                // u = b + a x_s,  v = conj(a) - conj(b) x_s,  w = u v
+                const double ur = fma(-ai, xsi, fma(ar, xsr, br)), ui = fma(ai, xsr, fma(ar, xsi, bi));
+                const double vr = ar - fma(bi, xsi, br * xsr), vi = -ai - fma(-bi, xsr, br * xsi);
+                const double wr = fma(-ui, vi, ur * vr), wi = fma(ui, vr, ur * vi);
+                double pr = c, pi = 0.0;   // c w^mb
+#pragma unroll
+                for (int mb = 0; mb <= TJ / 2; mb++) {
+                    double zr = pr, zi = pi;   // c u^mb v^n, n = mb .. TJ - mb
+                    accr[dft_index(TJ, mb, mb)] += zr;
+                    acci[dft_index(TJ, mb, mb)] += zi;
+#pragma unroll
+                    for (int n = mb + 1; n <= TJ - mb; n++) {
+                        const double tr = fma(-zi, vi, zr * vr), ti = fma(zi, vr, zr * vi);
+                        zr = tr; zi = ti;
+                        accr[dft_index(TJ, mb, n)] += zr;
+                        acci[dft_index(TJ, mb, n)] += zi;
+                    }
+                    if (mb < TJ / 2) {
+                        const double tr = fma(-pi, wi, pr * wr), ti = fma(pi, wr, pr * wi);
+                        pr = tr; pi = ti;
+                    }
+                }
+            }
+        }
+        __syncthreads();  // geo is dead: its bytes become S
+#pragma unroll
+        for (int k = 0; k < NJM; k++) S[((size_t)warp * NJM + k) * 32 + lane] = make_double2(accr[k], acci[k]);
+        __syncthreads();
+        // inverse DFT per column: q_k = (1/NW) sum_s S_s x_s^(-k); then the binomial normalisation and the self term
+        double2 *dst = cb.utot + (size_t)slot * nelem * 32;
+        for (int e = warp; e < nelem; e += NW) {
+            const int jm = s_elem[e] >> 4, k = s_elem[e] & 15;
+            const double2 *Sp = S + (size_t)jm * 32 + lane;
+            const double2 *tw = s_tw + k * NW;
+            double sr = 0.0, si = 0.0;
+#pragma unroll
+            for (int sI = 0; sI < NW; sI++) {
+                const double2 v = Sp[(size_t)sI * NJM * 32];
+                const double2 t = tw[sI];
+                sr = fma(v.x, t.x, sr); sr = fma(-v.y, t.y, sr);
+                si = fma(v.x, t.y, si); si = fma(v.y, t.x, si);
+            }
+            const double sN = tb.unorm[e] * (1.0 / (double)NW);
+            dst[(size_t)e * 32 + lane] = make_double2(sr * sN + (tb.udiag[e] ? sc.wself : 0.0), si * sN);
+        }
+    }
+}
+
+template <int TJ>
+inline size_t compute_ui_dft_smem_bytes() {
+    const size_t phase1 = (size_t)kDftCap * 5 * 32 * sizeof(double) + (size_t)kDftCap * 6 * sizeof(double) + (size_t)32 * kDftCap;
+    const size_t phase2 = (size_t)(TJ + 1) * dft_njm(TJ) * 32 * sizeof(double2);
+    return (phase1 > phase2 ? phase1 : phase2) + 16;
+}
+
+}  // namespace mala
