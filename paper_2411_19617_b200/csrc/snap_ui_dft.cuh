@@ -23,6 +23,10 @@
 
 namespace mala {
 
+#ifndef MALA_DFT_UNROLL
+#define MALA_DFT_UNROLL 1
+#endif
+constexpr int kDftUnroll = MALA_DFT_UNROLL;   // neighbors per trip of the accumulation loop
 constexpr int kDftCap = 48;   // neighbor entries per grid point buffered between two accumulate passes
 
 constexpr int dft_njm(int tj) {   // number of (J, mb <= J/2) columns
@@ -124,7 +128,7 @@ compute_ui_dft_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers cb
             }
             __syncthreads();
             const int nmax = __reduce_max_sync(0xffffffffu, cnt);
-#pragma unroll 1
+#pragma unroll kDftUnroll
             for (int i = 0; i < nmax; i++) {
                 double c = 0.0, ar = 1.0, ai = 0.0, br = 0.0, bi = 0.0;   // lanes past their count add zeros
                 if (i < cnt) {
