@@ -184,7 +184,7 @@ struct mala_snap {
     bool half_tiles() const { return twojmax > kFullTileTwoJ; }
     // 0 = automatic: the block kernel up to twojmax = 10, the anti-diagonal kernel on half tiles above
     bool use_block() const { return (zi_impl == 4 || zi_impl == 0) && !half_tiles() && blk_ready; }
-    bool use_ui_dft() const { return twojmax == kFullTileTwoJ && ui_impl != 1; }
+    bool use_ui_dft() const { return twojmax >= 1 && twojmax <= kFullTileTwoJ && ui_impl != 1; }
     bool use_spec() const { return zi_impl == 2; }
     bool use_diag() const { return zi_impl == 3 || (zi_impl == 0 && !use_block()); }
 };
@@ -205,8 +205,11 @@ int set_kernel_attributes(mala_snap *h) {
     CUDA_TRY(cudaFuncSetAttribute(compute_ui_kernel<kFullTileTwoJ, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ui_smem));
     CUDA_TRY(cudaFuncSetAttribute(compute_ui_kernel<kMaxTwoJ, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   (int)compute_ui_smem_bytes(kMaxTwoJ)));
-    CUDA_TRY(cudaFuncSetAttribute(compute_ui_dft_kernel<kFullTileTwoJ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)compute_ui_dft_smem_bytes<kFullTileTwoJ>()));
+#define MALA_DFT_ATTR(TJ) \
+    CUDA_TRY(cudaFuncSetAttribute(compute_ui_dft_kernel<TJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)compute_ui_dft_smem_bytes<TJ>()));
+    MALA_DFT_ATTR(1) MALA_DFT_ATTR(2) MALA_DFT_ATTR(3) MALA_DFT_ATTR(4) MALA_DFT_ATTR(5)
+    MALA_DFT_ATTR(6) MALA_DFT_ATTR(7) MALA_DFT_ATTR(8) MALA_DFT_ATTR(9) MALA_DFT_ATTR(10)
+#undef MALA_DFT_ATTR
     const int zi_smem = (int)compute_zi_smem_bytes(uhalf_size(kFullTileTwoJ), triple_count(kFullTileTwoJ));
     CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, zi_smem));
     CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_coop_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)compute_zi_coop_smem_bytes()));
@@ -558,6 +561,20 @@ int build_block_schedule(mala_snap *h) {
     h->blk_nslots = nslots;
     h->blk_ready = true;
     return 0;
+}
+
+// enqueue the sampling compute_ui (snap_ui_dft.cuh) for one chunk: whole tiles, twojmax + 1 warps
+void launch_ui_dft(mala_snap *h, const GridGeom &g, const DeviceTables &tb, const ChunkBuffers &cb, cudaStream_t st) {
+    switch (h->twojmax) {
+#define MALA_DFT_CASE(TJ) \
+    case TJ: \
+        compute_ui_dft_kernel<TJ><<<std::max(1, std::min(dft_ctas(TJ) * h->num_sms, cb.ntiles)), (TJ + 1) * 32, compute_ui_dft_smem_bytes<TJ>(), st>>>(g, h->sc, tb, cb); \
+        break;
+        MALA_DFT_CASE(1) MALA_DFT_CASE(2) MALA_DFT_CASE(3) MALA_DFT_CASE(4) MALA_DFT_CASE(5)
+        MALA_DFT_CASE(6) MALA_DFT_CASE(7) MALA_DFT_CASE(8) MALA_DFT_CASE(9) MALA_DFT_CASE(10)
+#undef MALA_DFT_CASE
+        default: break;
+    }
 }
 
 // enqueue compute_zi_bi for one chunk
@@ -975,9 +992,8 @@ int run_slab(mala_snap *h, int z0, int z1, double *out, double2 *u_out, cudaStre
                 compute_ui_kernel<kMaxTwoJ, false><<<ui_grid, (kMaxTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kMaxTwoJ), st>>>(g, h->sc, tb, cb);
             } else {
                 const int ui_grid = std::max(1, std::min(2 * h->num_sms, 2 * cb.ntiles));  // half-tile items, two CTAs per SM
-                if (h->use_ui_dft())   // twojmax = 10: column polynomials sampled at the 11th roots of unity (snap_ui_dft.cuh), whole tiles
-                    compute_ui_dft_kernel<kFullTileTwoJ><<<std::max(1, std::min(h->num_sms, cb.ntiles)), (kFullTileTwoJ + 1) * 32,
-                                                           compute_ui_dft_smem_bytes<kFullTileTwoJ>(), st>>>(g, h->sc, tb, cb);
+                if (h->use_ui_dft())   // twojmax 1..10: column polynomials sampled at the roots of unity (snap_ui_dft.cuh), whole tiles
+                    launch_ui_dft(h, g, tb, cb, st);
                 else if (h->twojmax == kFullTileTwoJ)
                     compute_ui_kernel<kFullTileTwoJ, true><<<ui_grid, (kFullTileTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kFullTileTwoJ), st>>>(g, h->sc, tb, cb);
                 else  // smaller twojmax: same code with run-time guards on the levels
@@ -1158,8 +1174,7 @@ int run_slab_force(mala_snap *h, int z0, int z1, const double *beta, double *gou
         {
             TimedSpan span(h, st, kKindUi);
             if (h->use_ui_dft())
-                compute_ui_dft_kernel<kFullTileTwoJ><<<std::max(1, std::min(h->num_sms, cb.ntiles)), (kFullTileTwoJ + 1) * 32,
-                                                       compute_ui_dft_smem_bytes<kFullTileTwoJ>(), st>>>(g, h->sc, tb, cb);
+                launch_ui_dft(h, g, tb, cb, st);
             else if (h->twojmax == kFullTileTwoJ)
                 compute_ui_kernel<kFullTileTwoJ, true><<<grid2, (kFullTileTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kFullTileTwoJ), st>>>(g, h->sc, tb, cb);
             else
@@ -1457,7 +1472,7 @@ int mala_snap_set_option(mala_snap_t *h, const char *name, long long value) {
     const std::string n(name);
     if (n == "ui_impl") {
         if (value < 0 || value > 2) return fail(MALA_SNAP_EINVAL, "ui_impl must be 0, 1 or 2");
-        if (value == 2 && h->twojmax != kFullTileTwoJ) return fail(MALA_SNAP_EINVAL, "the sampling compute_ui kernel is built for twojmax = 10");
+        if (value == 2 && (h->twojmax < 1 || h->twojmax > kFullTileTwoJ)) return fail(MALA_SNAP_EINVAL, "the sampling compute_ui kernel covers twojmax 1..10");
         h->ui_impl = (int)value;
         return MALA_SNAP_OK;
     }

@@ -1,9 +1,10 @@
-// snap_ui_dft.cuh -- compute_ui by sampling the column polynomials (rows a3 + a4 of SURVEY.md 8(a)), twojmax = 10.
+// snap_ui_dft.cuh -- compute_ui by sampling the column polynomials (rows a3 + a4 of SURVEY.md 8(a)), twojmax 1..10.
 //
 // Same quantity and the same storage as snap_ui.cuh: U_tot^J = wself*I + sum_neighbors c * U^J(neighbor) in half columns,
 // where column mb of level J is the coefficient list of the polynomial Q_{J,mb}(x) = (b + a x)^mb (conj(a) - conj(b) x)^(J-mb),
 // a and b the Cayley-Klein parameters of the neighbor (Eq. (24)-(25)).
 //
+// (Written for twojmax = 10; the kernel is a template on twojmax with twojmax + 1 sample points and warps.)
 // A polynomial of degree <= 10 is fixed by its values at the 11th roots of unity x_s, and there its value is a product of
 // powers:  Q_{J,mb}(x_s) = u_s^mb v_s^(J-mb),  u_s = b + a x_s,  v_s = conj(a) - conj(b) x_s.  So instead of carrying
 // coefficient lists through a recursion and adding them to accumulators in shared memory neighbor by neighbor (snap_ui.cuh:
@@ -41,8 +42,11 @@ constexpr int dft_index(int tj, int mb, int n) {
     return idx + (n - mb);
 }
 
+// resident CTAs per SM: the 4 * dft_njm accumulator registers per thread decide
+constexpr int dft_ctas(int tj) { return tj >= 8 ? 1 : (tj >= 6 ? 2 : 3); }
+
 template <int TJ>
-__global__ void __launch_bounds__((TJ + 1) * 32, 1)
+__global__ void __launch_bounds__((TJ + 1) * 32, dft_ctas(TJ))
 compute_ui_dft_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers cb) {
     constexpr int NW = TJ + 1;          // warps = sample points
     constexpr int NJM = dft_njm(TJ);
