@@ -183,6 +183,9 @@ int mala_gaussian_grid(mala_snap_t *h, double sigma, int natoms, const double *p
  *                      twojmax != 10), 3 = anti-diagonal kernel (code specialised on j1 only, any twojmax), 4 = block kernel
  *                      (twojmax <= 10).  All tables but the per-triple kernel's are per-handle arrays in global memory, so
  *                      handles of different twojmax coexist.  Every kernel gives the same B up to rounding (summation order).
+ *   "ui_impl"          0 = automatic (sampling kernel for twojmax 1..10: column polynomials evaluated at the roots of unity,
+ *                      sums in registers, inverse DFT per tile; column kernel otherwise), 1 = column kernel (polynomial
+ *                      recursion, accumulators in shared memory; any twojmax), 2 = sampling kernel (EINVAL outside 1..10)
  *   "timing"           1 = record a CUDA-event pair on the caller's stream around every kernel launch of the
  *                      following calls (read back with mala_snap_kernel_times); 0 = off (default)
  *   "workspace_mb"     cap, in MiB, of the U_tot + candidate workspace (default 4096)

@@ -59,6 +59,29 @@ def test_config1_tiny_al_full_grid(tiny_ref, zi_impl):
     assert_parity(got, ref)
 
 
+@pytest.mark.parametrize("ui_impl", [1, 2])
+def test_config1_both_compute_ui_kernels(tiny_ref, ui_impl):
+    """the column kernel (polynomial recursion) and the sampling kernel (roots of unity + inverse DFT) against the oracle"""
+    w, ref = tiny_ref
+    got = gpu_grid(w, ui_impl=ui_impl)
+    assert_parity(got, ref)
+
+
+@pytest.mark.parametrize("twojmax", [1, 3, 6, 9])
+def test_compute_ui_kernels_other_twojmax(twojmax):
+    torch = _torch()
+    pos, types, box, origin, pbc, ngrid, params = _small_case(7000 + twojmax, twojmax, 5, (1, 0, 1), True, True)
+    ref = oracle.bispectrum_grid(pos, types, box, origin, pbc, ngrid, **params)
+    for ui in (1, 2):
+        with MalaSnap(**params) as snap:
+            snap.set_option("ui_impl", ui)
+            got = snap.bispectrum_grid(pos, types, box, origin, pbc, ngrid)
+            torch.cuda.synchronize()
+        assert_parity(got.cpu().numpy(), ref)
+    with MalaSnap(twojmax=12) as snap, pytest.raises(MalaSnapError):
+        snap.set_option("ui_impl", 2)
+
+
 def test_triples_match_oracle_order():
     with MalaSnap(twojmax=10) as s:
         assert s.ncomp == 91
