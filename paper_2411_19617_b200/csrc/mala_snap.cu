@@ -484,12 +484,6 @@ int build_block_schedule(mala_snap *h) {
         load[w] += pieces[i].cost;
         piece_warp[i] = w;
     }
-    if (std::getenv("MALA_BLK_DEBUG")) {
-        double mx = 0.0;
-        for (double l : load) mx = std::max(mx, l);
-        std::fprintf(stderr, "block schedule: twojmax %d, %zu pieces, total %.0f, mean load %.0f, max load %.0f (%.3f)\n", h->twojmax, pieces.size(), total, total / NW, mx, mx / (total / NW));
-        for (int t = 0; t < nt; t++) if (tcost[t] > 0.3 * share) std::fprintf(stderr, "  triple %d (%d,%d,%d) cost %.0f units %zu\n", t, T.triples[4*t], T.triples[4*t+1], T.triples[4*t+2], tcost[t], tunits[t].size());
-    }
     // slots: the pieces of a triple, in piece order; triples without work keep an empty range
     std::vector<int> tslot(nt + 1, 0), piece_slot(pieces.size(), 0);
     int nslots = 0;
@@ -1710,6 +1704,7 @@ void mala_snap_destroy(mala_snap_t *h) {
     h->d_status.release(); h->d_bstage.release();
     h->d_yterms.release(); h->d_ylevel.release(); h->d_yorder.release(); h->d_ycg.release(); h->d_yweight.release(); h->d_ytot.release();
     h->d_dcg.release(); h->d_dtriple.release(); h->d_dsched.release(); h->d_ditems.release();
+    h->d_bstream.release(); h->d_bwrange.release(); h->d_btslot.release();
     if (h->h_status) cudaFreeHost(h->h_status);
     for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
     if (h->ev_upload) cudaEventDestroy(h->ev_upload);
