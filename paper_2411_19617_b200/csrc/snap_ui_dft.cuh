@@ -59,18 +59,17 @@ compute_ui_dft_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers cb
     double2 *S = reinterpret_cast<double2 *>(smem_raw);
     __shared__ int s_item;
     __shared__ double2 s_tw[NW * NW];   // [k][s] = x_s^(-k) = e^{-2 pi i s k / NW}
-    __shared__ unsigned short s_elem[nelem];   // element -> column index << 4 | k
+    __shared__ unsigned short s_col[NJM];      // work order of the inverse DFT: column (J << 4 | mb), longest columns first
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     if (threadIdx.x < NW * NW) {
         double sn, cs;
         sincospi(2.0 * (double)(((threadIdx.x / NW) * (threadIdx.x % NW)) % NW) / (double)NW, &sn, &cs);
         s_tw[threadIdx.x] = make_double2(cs, -sn);
     }
-    if (threadIdx.x == 0) {
-        int e = 0;
-        for (int J = 0; J <= TJ; J++)
-            for (int mb = 0; mb <= J / 2; mb++)
-                for (int k = 0; k <= J; k++, e++) s_elem[e] = (unsigned short)((dft_index(TJ, mb, J - mb) << 4) | k);
+    if (threadIdx.x == 0) {   // columns by decreasing length, dealt to the warps round-robin
+        int n = 0;
+        for (int J = TJ; J >= 0; J--)
+            for (int mb = 0; mb <= J / 2; mb++) s_col[n++] = (unsigned short)((J << 4) | mb);
     }
     double xsr, xsi;                    // this warp's sample point x_s = e^{2 pi i s / NW}
     {
@@ -169,20 +168,30 @@ compute_ui_dft_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers cb
         __syncthreads();
         // inverse DFT per column: q_k = (1/NW) sum_s S_s x_s^(-k); then the binomial normalisation and the self term
         double2 *dst = cb.utot + (size_t)slot * nelem * 32;
-        for (int e = warp; e < nelem; e += NW) {
-            const int jm = s_elem[e] >> 4, k = s_elem[e] & 15;
-            const double2 *Sp = S + (size_t)jm * 32 + lane;
-            const double2 *tw = s_tw + k * NW;
-            double sr = 0.0, si = 0.0;
+        for (int c = warp; c < NJM; c += NW) {   // one column per trip: its NW samples in registers, all of its J + 1 coefficients
+            const int J = s_col[c] >> 4, mb = s_col[c] & 15;
+            const double2 *Sp = S + (size_t)dft_index(TJ, mb, J - mb) * 32 + lane;
+            double vr[NW], vi[NW];
 #pragma unroll
             for (int sI = 0; sI < NW; sI++) {
                 const double2 v = Sp[(size_t)sI * NJM * 32];
-                const double2 t = tw[sI];
-                sr = fma(v.x, t.x, sr); sr = fma(-v.y, t.y, sr);
-                si = fma(v.x, t.y, si); si = fma(v.y, t.x, si);
+                vr[sI] = v.x; vi[sI] = v.y;
             }
-            const double sN = tb.unorm[e] * (1.0 / (double)NW);
-            dst[(size_t)e * 32 + lane] = make_double2(sr * sN + (tb.udiag[e] ? sc.wself : 0.0), si * sN);
+            const int e0 = uhalf_off(J) + mb * (J + 1);
+#pragma unroll 2
+            for (int k = 0; k <= J; k++) {
+                const double2 *tw = s_tw + k * NW;
+                double sr = 0.0, si = 0.0;
+#pragma unroll
+                for (int sI = 0; sI < NW; sI++) {
+                    const double2 t = tw[sI];
+                    sr = fma(vr[sI], t.x, sr); sr = fma(-vi[sI], t.y, sr);
+                    si = fma(vr[sI], t.y, si); si = fma(vi[sI], t.x, si);
+                }
+                const int e = e0 + k;
+                const double sN = tb.unorm[e] * (1.0 / (double)NW);
+                dst[(size_t)e * 32 + lane] = make_double2(sr * sN + (tb.udiag[e] ? sc.wself : 0.0), si * sN);
+            }
         }
     }
 }
