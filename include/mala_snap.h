@@ -155,7 +155,8 @@ int mala_bispectrum_ldos_grid(mala_snap_t *h, mala_mlp_t *net, int natoms, const
  *   beta   DEVICE [(z_end-z_begin)*ny*nx][ncomp] fp64, ix fastest (the layout of mala_bispectrum_grid's out)
  *   g      DEVICE [natoms*3] fp64; the call ADDS the slab's contribution (zero it before the first slab; slabs and GPUs sum)
  * All other arguments as mala_bispectrum_grid.  twojmax <= 10 (MALA_SNAP_EINVAL above).  Enqueued on cuda_stream; does not
- * synchronise.  The per-atom sums use floating-point atomics: results are reproducible to rounding, not bit for bit.
+ * synchronise.  The per-atom sums (and the accumulation of Y in shared memory) use floating-point atomics: results are
+ * reproducible to rounding, not bit for bit.
  * mala_snap_kernel_times reports compute_yi under ms[2] and compute_dedr under ms[3].
  */
 int mala_bispectrum_force_adjoint(mala_snap_t *h, int natoms, const double *pos, const int *types, const double box[9],
@@ -186,6 +187,8 @@ int mala_gaussian_grid(mala_snap_t *h, double sigma, int natoms, const double *p
  *   "ui_impl"          0 = automatic (sampling kernel for twojmax 1..10: column polynomials evaluated at the roots of unity,
  *                      sums in registers, inverse DFT per tile; column kernel otherwise), 1 = column kernel (polynomial
  *                      recursion, accumulators in shared memory; any twojmax), 2 = sampling kernel (EINVAL outside 1..10)
+ *   "yi_impl"          compute_yi of mala_bispectrum_force_adjoint: 0 = register-tiled block kernel (default), 1 = table-driven
+ *                      kernel (element by element)
  *   "timing"           1 = record a CUDA-event pair on the caller's stream around every kernel launch of the
  *                      following calls (read back with mala_snap_kernel_times); 0 = off (default)
  *   "workspace_mb"     cap, in MiB, of the U_tot + candidate workspace (default 4096)

@@ -27,6 +27,7 @@
 #include "snap_zi_block.cuh"
 #include "snap_gauss.cuh"
 #include "snap_force.cuh"
+#include "snap_yi_block.cuh"
 
 using namespace mala;
 
@@ -148,6 +149,16 @@ struct mala_snap {
     DevBuf<int> d_ylevel, d_yorder;
     DevBuf<double> d_ycg, d_yweight;
     DevBuf<double2> d_ytot;
+    DevBuf<int4> d_ybstream;          // compute_yi on the block machinery (snap_yi_block.cuh)
+    DevBuf<int> d_ybwrange, d_ybpass;
+    int yb_npasses = 0, yb_yacc = 0;
+    int yi_impl = 0;                  // 0 automatic (block kernel), 1 table-driven kernel
+    YBlkTables yblk_tables() const {
+        YBlkTables t;
+        t.stream = d_ybstream.p; t.wrange = d_ybwrange.p; t.pass_elem = d_ybpass.p; t.yweight = d_yweight.p;
+        t.npasses = yb_npasses; t.yacc_elems = yb_yacc;
+        return t;
+    }
     bool force_ready = false;
     ForceTables force_tables() const {
         ForceTables f;
@@ -1068,6 +1079,9 @@ int run_slab_gauss(mala_snap *h, int z0, int z1, double sigma, double *out, cuda
     return 0;
 }
 
+struct YHostTerm { int A, B, C, index; double coef; int cgoff; };
+int build_yi_block_schedule(mala_snap *h, const std::vector<YHostTerm> &terms, const std::vector<double> &cg);
+
 // tables of compute_yi (snap_force.cuh): three Z-type contributions per bispectrum component, grouped by target level
 int build_force_tables(mala_snap *h) {
     if (h->force_ready) return 0;
@@ -1126,7 +1140,182 @@ int build_force_tables(mala_snap *h) {
                                   (int)compute_yi_smem_bytes(uhalf_size(kFullTileTwoJ), triple_count(kFullTileTwoJ))));
     CUDA_TRY(cudaFuncSetAttribute(compute_dedr_kernel<kFullTileTwoJ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   (int)compute_dedr_smem_bytes(kFullTileTwoJ)));
+    {
+        std::vector<YHostTerm> ht;
+        for (const YTerm &y : terms) ht.push_back({y.A, y.B, y.C, y.index, y.coef, y.cgoff});
+        if ((rc = build_yi_block_schedule(h, ht, cg))) return rc;
+    }
     h->force_ready = true;
+    return 0;
+}
+
+// Record streams of compute_yi_block_kernel (snap_yi_block.cuh): every term (A, B -> C) of Y is cut into units exactly as
+// the triples of compute_zi are (build_block_schedule), without the symmetries that belong to B (only the swap of equal
+// factors, A == B, halves the items) and without fold weights; the units of a pass (a group of target levels) are dealt to
+// the warps by decreasing cost, pass by pass, because a barrier ends every pass.
+int build_yi_block_schedule(mala_snap *h, const std::vector<YHostTerm> &terms, const std::vector<double> &cg) {
+    const int tj = h->twojmax, NW = kBlkWarps;
+    constexpr int RB = 32 * (int)sizeof(double2);
+    // passes: consecutive levels from the top, as many as fit the accumulator (at least the top level alone)
+    const int cap = std::max(64, (tj + 1) * (tj / 2 + 1));
+    std::vector<int> pass_of_level(tj + 1, 0);
+    std::vector<std::pair<int, int>> pass_levels;            // [lo level, hi level]
+    for (int hi = tj; hi >= 0;) {
+        int lo = hi, size = (hi + 1) * (hi / 2 + 1);
+        while (lo - 1 >= 0 && size + lo * ((lo - 1) / 2 + 1) <= cap) { lo--; size += (lo + 1) * (lo / 2 + 1); }
+        pass_levels.push_back({lo, hi});
+        hi = lo - 1;
+    }
+    const int npasses = (int)pass_levels.size();
+    if (npasses > kYBlkMaxPasses) return fail(MALA_SNAP_ECUDA, "internal: too many passes in compute_yi");
+    for (int p = 0; p < npasses; p++)
+        for (int L = pass_levels[p].first; L <= pass_levels[p].second; L++) pass_of_level[L] = p;
+    struct HostItem { int ex, ey; bool fx, fy; int mb1, mb2; double w; };
+    struct HostUnit { int items_first, nitems, a0, b0, bx, by, yelem, dlo, dhi, index; double coef; std::vector<double> c; double cost; };
+    std::vector<HostItem> items;
+    std::vector<std::vector<HostUnit>> punits(npasses);
+    auto chunks = [](int len, int mx) {
+        std::vector<std::pair<int, int>> out;
+        const int k = (len + mx - 1) / mx, base = len / k, rem = len % k;
+        int s = 0;
+        for (int i = 0; i < k; i++) { const int c = base + (i < rem ? 1 : 0); out.push_back({s, c}); s += c; }
+        return out;
+    };
+    for (const YHostTerm &t : terms) {
+        const int A = t.A, B = t.B, C = t.C, sh = (A + B - C) / 2, pass = pass_of_level[C];
+        const int e_pass = uhalf_off(pass_levels[pass].first);
+        for (int mb = 0; mb <= C / 2; mb++) {
+            int lo = std::max(0, mb + sh - B), hi = std::min(A, mb + sh);
+            if (A == B && (mb + sh) / 2 < hi) hi = (mb + sh) / 2;   // items (mb1, mb2) and (mb2, mb1) contribute the same column
+            if (hi < lo) continue;
+            const int items_first = (int)items.size();
+            for (int mb1 = lo; mb1 <= hi; mb1++) {
+                const int mb2 = mb + sh - mb1;
+                double w = cg[t.cgoff + mb2 * (A + 1) + mb1];
+                if (A == B && mb1 != mb2) w += w;
+                HostItem it;
+                it.fx = mb1 > A / 2; it.fy = mb2 > B / 2; it.mb1 = mb1; it.mb2 = mb2; it.w = w;
+                it.ex = it.fx ? uhalf_off(A) + (A - mb1) * (A + 1) + A : uhalf_off(A) + mb1 * (A + 1);
+                it.ey = it.fy ? uhalf_off(B) + (B - mb2) * (B + 1) + B : uhalf_off(B) + mb2 * (B + 1);
+                items.push_back(it);
+            }
+            const int n = hi - lo + 1;
+            auto cf = [&](int m1, int m2) {
+                const int ma = m1 + m2 - sh;
+                return (ma < 0 || ma > C) ? 0.0 : cg[t.cgoff + m2 * (A + 1) + m1];
+            };
+            for (auto cx : chunks(A + 1, kBlkBX))
+                for (auto cy : chunks(B + 1, kBlkBY)) {
+                    int a_lo = 1 << 30, a_hi = -1, b_lo = 1 << 30, b_hi = -1;
+                    for (int a = cx.first; a < cx.first + cx.second; a++)
+                        for (int b = cy.first; b < cy.first + cy.second; b++)
+                            if (cf(a, b) != 0.0) { a_lo = std::min(a_lo, a); a_hi = std::max(a_hi, a); b_lo = std::min(b_lo, b); b_hi = std::max(b_hi, b); }
+                    if (a_hi < 0) continue;
+                    HostUnit u;
+                    u.items_first = items_first; u.nitems = n; u.index = t.index; u.coef = t.coef;
+                    int bx = a_hi - a_lo + 1, by = b_hi - b_lo + 1;
+                    if (bx < kBlkBXMin) { a_lo = std::max(0, std::min(a_lo, A + 1 - kBlkBXMin)); bx = kBlkBXMin; }
+                    if (by < kBlkBYMin) { b_lo = std::max(0, std::min(b_lo, B + 1 - kBlkBYMin)); by = kBlkBYMin; }
+                    u.a0 = a_lo; u.b0 = b_lo; u.bx = bx; u.by = by;
+                    const int ma0 = a_lo + b_lo - sh;
+                    u.yelem = uhalf_off(C) + mb * (C + 1) + ma0 - e_pass;   // element of row ma0 in the pass's accumulator (may be negative)
+                    u.dlo = std::max(0, -ma0); u.dhi = std::min(bx + by - 2, C - ma0);
+                    for (int a = 0; a < bx; a++)
+                        for (int b = 0; b < by; b++)
+                            u.c.push_back((a_lo + a >= cx.first && a_lo + a < cx.first + cx.second && b_lo + b >= cy.first && b_lo + b < cy.first + cy.second)
+                                              ? cf(a_lo + a, b_lo + b) : 0.0);
+                    u.cost = n * (2.0 * (4 * bx * by + 2 * by) + 3.0 * bx + 2.0 * by + 14.0) + 2.0 * (2 * bx * by) + 12.0 * (bx + by - 1) + 2.0 * bx * by + 50.0;
+                    punits[pass].push_back(std::move(u));
+                }
+        }
+    }
+    // deal: per pass, units by decreasing cost to the least loaded warp
+    std::vector<std::vector<std::vector<const HostUnit *>>> mine(NW, std::vector<std::vector<const HostUnit *>>(npasses));
+    for (int p = 0; p < npasses; p++) {
+        std::vector<const HostUnit *> order;
+        for (const HostUnit &u : punits[p]) order.push_back(&u);
+        std::stable_sort(order.begin(), order.end(), [](const HostUnit *a, const HostUnit *b) { return a->cost > b->cost; });
+        std::vector<double> load(NW, 0.0);
+        for (const HostUnit *u : order) {
+            int w = 0;
+            for (int k = 1; k < NW; k++)
+                if (load[k] < load[w]) w = k;
+            load[w] += u->cost;
+            mine[w][p].push_back(u);
+        }
+    }
+    std::vector<int4> stream;
+    std::vector<int> wrange((size_t)NW * npasses * kBlkShapes + 2 * NW, 0);
+    auto push_d2 = [&](double a, double b) {
+        int4 v;
+        std::memcpy(&v.x, &a, 8);
+        std::memcpy(&v.z, &b, 8);
+        stream.push_back(v);
+    };
+    for (int w = 0; w < NW; w++) {
+        const size_t w0 = stream.size();
+        wrange[yblk_wrange_first(w, npasses)] = (int)w0;
+        size_t last_header = 0;
+        bool have_header = false;
+        for (int p = 0; p < npasses; p++)
+            for (int bx = kBlkBX; bx >= 1; bx--)
+                for (int by = kBlkBY; by >= 1; by--) {
+                    int count = 0;
+                    for (const HostUnit *up : mine[w][p]) {
+                        const HostUnit &u = *up;
+                        if (u.bx != bx || u.by != by) continue;
+                        count++;
+                        const int words = 2 + 3 * u.nitems + (bx * by + 1) / 2;
+                        const size_t pos = stream.size() - w0;
+                        if (pos / kBlkRingWords != (pos + words - 1) / kBlkRingWords) {
+                            const int skip = (int)(kBlkRingWords - pos % kBlkRingWords);
+                            if (!have_header) return fail(MALA_SNAP_ECUDA, "internal: Y stream starts with an oversized unit");
+                            stream[last_header].w += skip;
+                            for (int k = 0; k < skip; k++) stream.push_back(make_int4(0, 0, 0, 0));
+                        }
+                        last_header = stream.size();
+                        have_header = true;
+                        stream.push_back(make_int4(u.nitems, u.yelem * RB, u.index, 0));
+                        {
+                            int4 h1;
+                            h1.x = u.dlo; h1.y = u.dhi;
+                            std::memcpy(&h1.z, &u.coef, 8);
+                            stream.push_back(h1);
+                        }
+                        for (int k = 0; k < u.nitems; k++) {
+                            const HostItem &it = items[u.items_first + k];
+                            const int xe = it.fx ? it.ex - u.a0 : it.ex + u.a0, ye = it.fy ? it.ey - u.b0 : it.ey + u.b0;
+                            const unsigned sgn = 0x80000000u;
+                            const unsigned me = it.fx ? (((u.a0 + it.mb1) & 1) ? sgn : 0u) : 0u, mo = it.fx ? (me ^ sgn) : 0u;
+                            stream.push_back(make_int4(xe * RB, it.fx ? -RB : RB, ye * RB, it.fy ? -RB : RB));
+                            stream.push_back(make_int4((int)me, (int)mo, it.fx ? 1 : 0, 0));
+                            const double pe = (it.fy && ((u.b0 + it.mb2) & 1)) ? -it.w : it.w, po = it.fy ? -pe : it.w;
+                            push_d2(pe, po);
+                        }
+                        for (size_t k = 0; k < u.c.size(); k += 2) push_d2(u.c[k], k + 1 < u.c.size() ? u.c[k + 1] : 0.0);
+                    }
+                    wrange[yblk_wrange_count(w, p, (bx - 1) * kBlkBY + (by - 1), npasses)] = count;
+                }
+        while ((stream.size() - w0) % 32) stream.push_back(make_int4(0, 0, 0, 0));
+        wrange[yblk_wrange_first(w, npasses) + 1] = (int)(stream.size() - w0);
+    }
+    std::vector<int> pe(npasses + 1, 0);
+    int yacc = 0;
+    for (int p = 0; p < npasses; p++) {
+        pe[p] = uhalf_off(pass_levels[p].first);
+        yacc = std::max(yacc, uhalf_off(pass_levels[p].second + 1) - uhalf_off(pass_levels[p].first));
+    }
+    // pass_elem[p+1] must be the END of pass p: passes run from the top level down, so ends are stored beside the starts
+    std::vector<int> pass_elem(2 * npasses, 0);
+    for (int p = 0; p < npasses; p++) { pass_elem[2 * p] = pe[p]; pass_elem[2 * p + 1] = uhalf_off(pass_levels[p].second + 1); }
+    int rc = 0;
+    if ((rc = upload(h->d_ybstream, stream))) return rc;
+    if ((rc = upload(h->d_ybwrange, wrange))) return rc;
+    if ((rc = upload(h->d_ybpass, pass_elem))) return rc;
+    h->yb_npasses = npasses;
+    h->yb_yacc = yacc;
+    CUDA_TRY(cudaFuncSetAttribute(compute_yi_block_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)compute_yi_block_smem_bytes(uhalf_size(kFullTileTwoJ), triple_count(kFullTileTwoJ), std::max(64, uhalf_off(kFullTileTwoJ + 1) - uhalf_off(kFullTileTwoJ)))));
     return 0;
 }
 
@@ -1178,8 +1367,12 @@ int run_slab_force(mala_snap *h, int z0, int z1, const double *beta, double *gou
         {
             TimedSpan span(h, st, kKindZi);   // reported in the compute_zi_bi slot: the same kind of contraction
             const int grid = std::max(1, std::min(h->num_sms, cb.ntiles));
-            compute_yi_kernel<<<grid, kYiWarps * 32, compute_yi_smem_bytes(h->sc.nelem, h->sc.ntriples), st>>>(g, h->sc, h->force_tables(), cb, beta,
-                                                                                                                h->d_ytot.p);
+            if (h->yi_impl == 1)
+                compute_yi_kernel<<<grid, kYiWarps * 32, compute_yi_smem_bytes(h->sc.nelem, h->sc.ntriples), st>>>(g, h->sc, h->force_tables(), cb, beta,
+                                                                                                                    h->d_ytot.p);
+            else   // the same contraction on the register-tiled block machinery (snap_yi_block.cuh)
+                compute_yi_block_kernel<<<grid, kBlkWarps * 32, compute_yi_block_smem_bytes(h->sc.nelem, h->sc.ntriples, h->yb_yacc), st>>>(
+                    g, h->sc, h->yblk_tables(), cb, beta, h->d_ytot.p);
         }
         CUDA_TRY(cudaGetLastError());
         {
@@ -1464,6 +1657,11 @@ int mala_snap_triples(const mala_snap_t *h, int *j1j2j) {
 int mala_snap_set_option(mala_snap_t *h, const char *name, long long value) {
     if (!h || !name) return fail(MALA_SNAP_EINVAL, "handle or name is NULL");
     const std::string n(name);
+    if (n == "yi_impl") {
+        if (value < 0 || value > 1) return fail(MALA_SNAP_EINVAL, "yi_impl must be 0 or 1");
+        h->yi_impl = (int)value;
+        return MALA_SNAP_OK;
+    }
     if (n == "ui_impl") {
         if (value < 0 || value > 2) return fail(MALA_SNAP_EINVAL, "ui_impl must be 0, 1 or 2");
         if (value == 2 && (h->twojmax < 1 || h->twojmax > kFullTileTwoJ)) return fail(MALA_SNAP_EINVAL, "the sampling compute_ui kernel covers twojmax 1..10");
@@ -1705,6 +1903,7 @@ void mala_snap_destroy(mala_snap_t *h) {
     h->d_yterms.release(); h->d_ylevel.release(); h->d_yorder.release(); h->d_ycg.release(); h->d_yweight.release(); h->d_ytot.release();
     h->d_dcg.release(); h->d_dtriple.release(); h->d_dsched.release(); h->d_ditems.release();
     h->d_bstream.release(); h->d_bwrange.release(); h->d_btslot.release();
+    h->d_ybstream.release(); h->d_ybwrange.release(); h->d_ybpass.release();
     if (h->h_status) cudaFreeHost(h->h_status);
     for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
     if (h->ev_upload) cudaEventDestroy(h->ev_upload);

@@ -23,7 +23,7 @@ def _grid_points(box, origin, ngrid, z0, z1):
     return frac @ np.asarray(box, float).reshape(3, 3) + np.asarray(origin, float)
 
 
-def _compare(pos, types, box, origin, pbc, ngrid, z0, z1, params, seed, tol=1e-9):
+def _compare(pos, types, box, origin, pbc, ngrid, z0, z1, params, seed, tol=1e-9, yi_impl=0):
     torch = _torch()
     rng = np.random.default_rng(seed)
     pts = _grid_points(box, origin, ngrid, z0, z1)
@@ -31,6 +31,7 @@ def _compare(pos, types, box, origin, pbc, ngrid, z0, z1, params, seed, tol=1e-9
     beta = rng.normal(size=(pts.shape[0], nt))
     ref = oracle.bispectrum_grad_points(pts, pos, types, box, origin, pbc, beta=beta, want_dB=False, **params)["g"]
     with MalaSnap(**params) as snap:
+        snap.set_option("yi_impl", yi_impl)   # 0: register-tiled block kernel, 1: table-driven kernel
         g = snap.force_adjoint(torch.as_tensor(beta, device="cuda"), pos, types, box, origin, pbc, ngrid, z0, z1)
         torch.cuda.synchronize()
         got = g.cpu().numpy()
@@ -40,10 +41,11 @@ def _compare(pos, types, box, origin, pbc, ngrid, z0, z1, params, seed, tol=1e-9
     return got, beta
 
 
-def test_cluster_in_a_box_twojmax6():
+@pytest.mark.parametrize("yi_impl", [0, 1])
+def test_cluster_in_a_box_twojmax6(yi_impl):
     rng = np.random.default_rng(41)
     pos = rng.uniform(3.0, 7.0, size=(6, 3))
-    _compare(pos, np.zeros(6, np.int32), np.eye(3) * 10.0, (0, 0, 0), (0, 0, 0), (9, 8, 7), 0, 7, dict(twojmax=6, rcutfac=3.0), 1)
+    _compare(pos, np.zeros(6, np.int32), np.eye(3) * 10.0, (0, 0, 0), (0, 0, 0), (9, 8, 7), 0, 7, dict(twojmax=6, rcutfac=3.0), 1, yi_impl=yi_impl)
 
 
 def test_periodic_triclinic_box_smaller_than_the_cutoff_two_types():
