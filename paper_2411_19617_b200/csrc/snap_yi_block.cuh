@@ -72,9 +72,9 @@ __device__ __forceinline__ void yblk_unit(const unsigned char *Ulane, BlkReader 
             }
         }
         if (d >= dlo && d <= dhi) {   // rows outside the column carry exact zeros: skipped (warp-uniform)
-            double *y = reinterpret_cast<double *>(yb + d * RB);
+            double *y = reinterpret_cast<double *>(yb + d * RB);   // real parts of the 32 lanes, then the imaginary parts: conflict-free
             yblk_atomic_add(y, wl * zr);
-            yblk_atomic_add(y + 1, wl * zi);
+            yblk_atomic_add(y + 32, wl * zi);
         }
     }
     rd.fill();
@@ -99,8 +99,8 @@ compute_yi_block_kernel(GridGeom g, SnapConst sc, YBlkTables T, ChunkBuffers cb,
     const int nelem = sc.nelem, nt = sc.ntriples;
     double2 *U = reinterpret_cast<double2 *>(smem_raw + kBlkPadBytes);
     double *Bt = reinterpret_cast<double *>(U + (size_t)nelem * 32);                 // [nt][32] beta of the tile, lane fastest
-    double2 *Yacc = reinterpret_cast<double2 *>(Bt + (size_t)32 * nt);               // [yacc_elems][32]
-    int4 *rings = reinterpret_cast<int4 *>(Yacc + (size_t)T.yacc_elems * 32);        // [NW][kBlkRingWords]
+    double *Yacc = Bt + (size_t)32 * nt;                                             // [yacc_elems][re | im][32]
+    int4 *rings = reinterpret_cast<int4 *>(Yacc + (size_t)T.yacc_elems * 64);        // [NW][kBlkRingWords]
     __shared__ uint64_t bar;
     __shared__ int s_slot;
     const int lane = threadIdx.x & 31, warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
@@ -129,7 +129,7 @@ compute_yi_block_kernel(GridGeom g, SnapConst sc, YBlkTables T, ChunkBuffers cb,
             lane_point(g, cb.tile_begin + wt, l, ix, iy, iz, valid);
             Bt[t * 32 + l] = valid ? beta[((size_t)((size_t)(iz - g.z0) * g.ny + iy) * g.nx + ix) * nt + t] : 0.0;
         }
-        for (int i = threadIdx.x; i < T.yacc_elems * 32; i += NW * 32) Yacc[i] = make_double2(0.0, 0.0);
+        for (int i = threadIdx.x; i < T.yacc_elems * 64; i += NW * 32) Yacc[i] = 0.0;
         BlkReader rd;
         rd.src = T.stream + __ldg(T.wrange + yblk_wrange_first(warp, T.npasses));
         rd.wtotal = __ldg(T.wrange + yblk_wrange_first(warp, T.npasses) + 1);
@@ -150,9 +150,10 @@ compute_yi_block_kernel(GridGeom g, SnapConst sc, YBlkTables T, ChunkBuffers cb,
             for (int i = threadIdx.x; i < (e1 - e0) * 32; i += NW * 32) {
                 const int e = e0 + (i >> 5);
                 const double yw = __ldg(T.yweight + e);
-                const double2 v = Yacc[i];
-                Yt[(size_t)e * 32 + (i & 31)] = make_double2(yw * v.x, yw * v.y);
-                Yacc[i] = make_double2(0.0, 0.0);
+                const int at = (i >> 5) * 64 + (i & 31);
+                Yt[(size_t)e * 32 + (i & 31)] = make_double2(yw * Yacc[at], yw * Yacc[at + 32]);
+                Yacc[at] = 0.0;
+                Yacc[at + 32] = 0.0;
             }
             __syncthreads();
         }
