@@ -453,10 +453,13 @@ int build_block_schedule(mala_snap *h) {
                     if (by < kBlkBYMin) { b_lo = std::max(0, std::min(b_lo, J2 + 1 - kBlkBYMin)); by = kBlkBYMin; }
                     hu.a0 = a_lo; hu.b0 = b_lo; hu.bx = bx; hu.by = by;
                     hu.ub_elem = uhalf_off(J) + mb * (J + 1) + (a_lo + b_lo - sh);   // row of the first anti-diagonal (may lie before the column)
-                    for (int a = 0; a < hu.bx; a++)
-                        for (int b = 0; b < hu.by; b++)
+                    for (int d = 0; d <= hu.bx + hu.by - 2; d++)   // in the order the kernel consumes them (blk_coef_index)
+                        for (int a = 0; a < hu.bx; a++) {
+                            const int b = d - a;
+                            if (b < 0 || b >= hu.by) continue;
                             hu.coef.push_back((a_lo + a >= cx.first && a_lo + a < cx.first + cx.second && b_lo + b >= cy.first && b_lo + b < cy.first + cy.second)
                                                   ? cf(a_lo + a, b_lo + b) : 0.0);
+                        }
                     // issue cycles: an FP64 instruction holds the port for two, anything else for one
                     hu.cost = n * (2.0 * (4 * bx * by + 2 * by) + 3.0 * bx + 2.0 * by + 14.0) + 2.0 * (2 * bx * by + 2 * (bx + by - 1)) + 0.5 * bx * by +
                               bx + by + 2.0 * bx * by + 40.0;
@@ -1220,10 +1223,13 @@ int build_yi_block_schedule(mala_snap *h, const std::vector<YHostTerm> &terms, c
                     const int ma0 = a_lo + b_lo - sh;
                     u.yelem = uhalf_off(C) + mb * (C + 1) + ma0 - e_pass;   // element of row ma0 in the pass's accumulator (may be negative)
                     u.dlo = std::max(0, -ma0); u.dhi = std::min(bx + by - 2, C - ma0);
-                    for (int a = 0; a < bx; a++)
-                        for (int b = 0; b < by; b++)
+                    for (int d = 0; d <= bx + by - 2; d++)   // in the order the kernel consumes them (blk_coef_index)
+                        for (int a = 0; a < bx; a++) {
+                            const int b = d - a;
+                            if (b < 0 || b >= by) continue;
                             u.c.push_back((a_lo + a >= cx.first && a_lo + a < cx.first + cx.second && b_lo + b >= cy.first && b_lo + b < cy.first + cy.second)
                                               ? cf(a_lo + a, b_lo + b) : 0.0);
+                        }
                     u.cost = n * (2.0 * (4 * bx * by + 2 * by) + 3.0 * bx + 2.0 * by + 14.0) + 2.0 * (2 * bx * by) + 12.0 * (bx + by - 1) + 2.0 * bx * by + 50.0;
                     punits[pass].push_back(std::move(u));
                 }

@@ -59,6 +59,7 @@ __device__ __forceinline__ void yblk_unit(const unsigned char *Ulane, BlkReader 
         base += 48;
     }
     unsigned char *yb = Yl + yoff;
+    double2 cpair = make_double2(0.0, 0.0);
 #pragma unroll
     for (int d = 0; d < BX + BY - 1; d++) {
         double zr = 0.0, zi = 0.0;
@@ -66,7 +67,9 @@ __device__ __forceinline__ void yblk_unit(const unsigned char *Ulane, BlkReader 
         for (int a = 0; a < BX; a++) {
             const int b = d - a;
             if (b >= 0 && b < BY) {
-                const double c = blk_lds1(base + 8 * (a * BY + b));
+                const int k = blk_coef_index(BX, BY, d, a);   // a compile-time constant once the loops are unrolled
+                if ((k & 1) == 0) cpair = blk_lds2(base + 8 * k);   // two coefficients per 16-byte load, in consumption order
+                const double c = (k & 1) ? cpair.y : cpair.x;
                 zr = fma(c, tr[a][b], zr);
                 zi = fma(c, ti[a][b], zi);
             }

@@ -118,6 +118,19 @@ struct BlkReader {
     }
 };
 
+// position of coefficient (a, b = d - a) in the order the projection consumes them: anti-diagonal by anti-diagonal, a ascending
+__host__ __device__ constexpr int blk_coef_index(int BX, int BY, int d, int a) {
+    int k = 0;
+    for (int dd = 0; dd <= d; dd++)
+        for (int aa = 0; aa < BX; aa++) {
+            const int bb = dd - aa;
+            if (bb < 0 || bb >= BY) continue;
+            if (dd == d && aa == a) return k;
+            k++;
+        }
+    return k;
+}
+
 // one item of a unit: T (+)= x (x) y.  FIRST: the block starts from this item's products (no zeroing pass)
 template <int BX, int BY, bool FIRST>
 __device__ __forceinline__ void blk_item(const unsigned char *Ulane, const uint32_t base, double (&tr)[BX][BY], double (&ti)[BX][BY]) {
@@ -191,6 +204,7 @@ __device__ __forceinline__ double blk_unit(const unsigned char *Ulane, BlkReader
     // element, so the registers never hold the block and its coefficients together), dotted with conj(U^J[:, mb]) at once
     const unsigned char *ub = Ulane + uboff;
     double bs0 = 0.0, bs1 = 0.0;
+    double2 cpair = make_double2(0.0, 0.0);
 #pragma unroll
     for (int d = 0; d < BX + BY - 1; d++) {
         double zr = 0.0, zi = 0.0;
@@ -198,7 +212,9 @@ __device__ __forceinline__ double blk_unit(const unsigned char *Ulane, BlkReader
         for (int a = 0; a < BX; a++) {
             const int b = d - a;
             if (b >= 0 && b < BY) {
-                const double c = blk_lds1(base + 8 * (a * BY + b));
+                const int k = blk_coef_index(BX, BY, d, a);   // a compile-time constant once the loops are unrolled
+                if ((k & 1) == 0) cpair = blk_lds2(base + 8 * k);   // two coefficients per 16-byte load, in consumption order
+                const double c = (k & 1) ? cpair.y : cpair.x;
                 zr = fma(c, tr[a][b], zr);
                 zi = fma(c, ti[a][b], zi);
             }
