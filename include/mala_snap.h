@@ -196,7 +196,7 @@ int mala_gaussian_grid(mala_snap_t *h, double sigma, int natoms, const double *p
  *                      the true bound makes tile_bin_kernel overflow, which must surface as MALA_SNAP_ECUDA (see
  *                      mala_snap_last_stats); never set it in production
  *   "host_chunk_mb"    cap, in MiB, of each of the two staging buffers of mala_bispectrum_grid_host (default 256;
- *                      outputs above 96 MiB are split into at least three chunks so the copies overlap the kernels)
+ *                      outputs above 96 MiB are split into about ten chunks of at least eight planes so the copies overlap the kernels)
  */
 int mala_snap_set_option(mala_snap_t *h, const char *name, long long value);
 

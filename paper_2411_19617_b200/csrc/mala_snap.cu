@@ -1794,10 +1794,11 @@ int mala_bispectrum_grid_host(mala_snap_t *h, int natoms, const double *pos, con
     const size_t plane = (size_t)ngrid[0] * ngrid[1] * h->sc.ntriples;  // doubles per z-plane
     const size_t budget = ((size_t)h->host_chunk_mb << 20) / sizeof(double);
     int planes = (int)std::max<size_t>(1, std::min<size_t>(budget / std::max<size_t>(plane, 1), (size_t)(z_end - z_begin)));
-    // at least three chunks once the output is large enough for the copy to matter: the device->host copy of a chunk
-    // overlaps the kernels of the next one, so only the last chunk's copy is exposed
+    // about ten chunks once the output is large enough for the copy to matter: the device->host copy of a chunk overlaps
+    // the kernels of the next one, so only the last chunk's copy is exposed (config 2: 25.9 ms with 4 chunks, 25.2 with 12;
+    // 18 chunks of 5 planes: 26.3 -- the persistent kernels want a dozen tiles per SM)
     const size_t total = plane * (size_t)(z_end - z_begin);
-    if (total * sizeof(double) > ((size_t)96 << 20)) planes = std::min(planes, (z_end - z_begin + 2) / 3);
+    if (total * sizeof(double) > ((size_t)96 << 20)) planes = std::min(planes, std::max(8, (z_end - z_begin + 9) / 10));
     if (planes >= 8) planes = planes / 8 * 8;  // whole tiles for every tile shape
     for (int b = 0; b < 2; b++)
         if (h->d_stage[b].reserve(plane * planes, st, true)) return fail(MALA_SNAP_ENOMEM, "cudaMallocAsync (staging) failed");
