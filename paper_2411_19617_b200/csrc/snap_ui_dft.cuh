@@ -28,7 +28,7 @@ namespace mala {
 #define MALA_DFT_UNROLL 1
 #endif
 constexpr int kDftUnroll = MALA_DFT_UNROLL;   // neighbors per trip of the accumulation loop
-constexpr int kDftCap = 48;   // neighbor entries per grid point buffered between two accumulate passes
+constexpr int kDftCap = 48;   // neighbor entries per grid point buffered between two accumulate passes (<= 64: hit masks)
 
 constexpr int dft_njm(int tj) {   // number of (J, mb <= J/2) columns
     int n = 0;
@@ -52,10 +52,10 @@ compute_ui_dft_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers cb
     constexpr int NJM = dft_njm(TJ);
     constexpr int nelem = uhalf_size(TJ);
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    // phase 1: geo [kDftCap][5][32], crec [kDftCap][6], hitk [32][kDftCap];  phase 2 (same bytes): S [NW][NJM][32] double2
+    // phase 1: geo [kDftCap][5][32], crec [kDftCap][6], hmask [NW][32];  phase 2 (same bytes): S [NW][NJM][32] double2
     double *geo = reinterpret_cast<double *>(smem_raw);
     double *crec = geo + kDftCap * 5 * 32;
-    unsigned char *hitk = reinterpret_cast<unsigned char *>(crec + kDftCap * 6);
+    unsigned long long *hmask = reinterpret_cast<unsigned long long *>(crec + kDftCap * 6);   // [NW][32] hit masks of the warps
     double2 *S = reinterpret_cast<double2 *>(smem_raw);
     __shared__ int s_item;
     __shared__ double2 s_tw[NW * NW];   // [k][s] = x_s^(-k) = e^{-2 pi i s k / NW}
@@ -109,25 +109,34 @@ compute_ui_dft_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers cb
                 q[0] = gh.x; q[1] = gh.y; q[2] = gh.z; q[3] = rc; q[4] = tb.type_w[gh.type]; q[5] = rc * rc;
             }
             __syncthreads();
-            int cnt = 0;  // neighbors of this lane's point in the window (identical in every warp)
-            for (int k = 0; k < nw; k++) {
+            // distance tests: warp w takes candidates w, w + NW, ... for the 32 points and publishes its hits as a bit mask
+            unsigned long long mine = 0ull;
+            for (int k = warp; k < nw; k += NW) {
                 const double *q = crec + k * 6;
                 const double dx = q[0] - px, dy = q[1] - py, dz = q[2] - pz;
-                if (dx * dx + dy * dy + dz * dz < q[5]) {
-                    if (warp == 0) hitk[lane * kDftCap + cnt] = (unsigned char)k;
-                    cnt++;
-                }
+                if (dx * dx + dy * dy + dz * dz < q[5]) mine |= 1ull << k;
             }
+            hmask[warp * 32 + lane] = mine;
             __syncthreads();
-            // the hits of a point are dealt to the NW lanes of that point: pair geometry once per (point, neighbor)
-            for (int e = warp; e < cnt; e += NW) {
-                const double *q = crec + (int)hitk[lane * kDftCap + e] * 6;
-                const double dx = q[0] - px, dy = q[1] - py, dz = q[2] - pz;
-                const double r2 = dx * dx + dy * dy + dz * dz;
-                double c, ar, ai, br, bi;
-                pair_geometry(dx, dy, dz, r2, q[3], q[4], sc.rfac0, sc.rmin0, c, ar, ai, br, bi);
-                double *o = geo + (size_t)e * 5 * 32 + lane;
-                o[0] = c; o[32] = ar; o[64] = ai; o[96] = br; o[128] = bi;
+            unsigned long long hits = 0ull;   // neighbors of this lane's point in the window, identical in every warp
+#pragma unroll
+            for (int w2 = 0; w2 < NW; w2++) hits |= hmask[w2 * 32 + lane];
+            const int cnt = __popcll(hits);
+            // the hits of a point (in candidate order) are dealt to the NW lanes of that point: pair geometry once per pair
+            {
+                int e = 0, turn = 0;   // turn = e mod NW
+                for (unsigned long long r = hits; r != 0ull; r &= r - 1ull, e++) {
+                    if (turn == warp) {
+                        const double *q = crec + (__ffsll((long long)r) - 1) * 6;
+                        const double dx = q[0] - px, dy = q[1] - py, dz = q[2] - pz;
+                        const double r2 = dx * dx + dy * dy + dz * dz;
+                        double c, ar, ai, br, bi;
+                        pair_geometry(dx, dy, dz, r2, q[3], q[4], sc.rfac0, sc.rmin0, c, ar, ai, br, bi);
+                        double *o = geo + (size_t)e * 5 * 32 + lane;
+                        o[0] = c; o[32] = ar; o[64] = ai; o[96] = br; o[128] = bi;
+                    }
+                    turn = (turn + 1 == NW) ? 0 : turn + 1;
+                }
             }
             __syncthreads();
             const int nmax = __reduce_max_sync(0xffffffffu, cnt);
@@ -198,7 +207,7 @@ compute_ui_dft_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers cb
 
 template <int TJ>
 inline size_t compute_ui_dft_smem_bytes() {
-    const size_t phase1 = (size_t)kDftCap * 5 * 32 * sizeof(double) + (size_t)kDftCap * 6 * sizeof(double) + (size_t)32 * kDftCap;
+    const size_t phase1 = (size_t)kDftCap * 5 * 32 * sizeof(double) + (size_t)kDftCap * 6 * sizeof(double) + (size_t)(TJ + 1) * 32 * sizeof(unsigned long long);
     const size_t phase2 = (size_t)(TJ + 1) * dft_njm(TJ) * 32 * sizeof(double2);
     return (phase1 > phase2 ? phase1 : phase2) + 16;
 }
