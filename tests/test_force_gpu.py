@@ -84,6 +84,30 @@ def test_config1_twojmax10_slab_and_slab_additivity():
         assert np.abs(g2.cpu().numpy() - got).max() <= 1e-11 * np.abs(got).max()
 
 
+def test_config2_full_grid_sparse_beta_in_bench_configuration():
+    """the whole 90^3 grid of config 2 in the configuration bench.py --force times (two workspace chunks, every SM walking many
+    tiles): beta is non-zero at 160 seeded grid points only, so the oracle's forward-mode derivative at those points is the
+    complete answer"""
+    torch = _torch()
+    w = workloads.make(2)
+    rng = np.random.default_rng(77)
+    sample = np.sort(rng.choice(w.npoints, 160, replace=False))
+    nt = 91
+    bs = rng.normal(size=(sample.size, nt))
+    pts = oracle.grid_points(w.box, w.origin, w.ngrid, sample=sample)
+    ref = oracle.bispectrum_grad_points(pts, w.pos, w.types, w.box, w.origin, w.pbc, beta=bs, want_dB=False, **w.snap_params())["g"]
+    beta = torch.zeros((w.npoints, nt), dtype=torch.float64, device="cuda")
+    beta[torch.as_tensor(sample, device="cuda")] = torch.as_tensor(bs, device="cuda")
+    with MalaSnap(**w.snap_params()) as snap:
+        g = snap.force_adjoint(beta, w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid)
+        torch.cuda.synchronize()
+        assert snap.last_stats()["chunks"] >= 2
+    got = g.cpu().numpy()
+    scale = np.abs(ref).max()
+    assert scale > 0 and np.isfinite(got).all()
+    assert np.abs(got - ref).max() <= 1e-9 * scale, f"max |dg| / max |g| = {np.abs(got - ref).max() / scale:.3e}"
+
+
 def test_uniform_beta_on_a_full_periodic_grid_gives_a_small_net_translation_force():
     """moving all atoms together equals moving the grid the other way: with the same beta at every point of a full periodic grid
     the sum over atoms of g is the beta-weighted grid sum of -dB/dr, which converges to zero as the grid resolves B (a sanity
