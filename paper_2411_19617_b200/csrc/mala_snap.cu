@@ -193,8 +193,8 @@ struct mala_snap {
     }
     // twojmax above kFullTileTwoJ: U_tot of 32 points does not fit one SM's shared memory; half-tile layout and kernel
     bool half_tiles() const { return twojmax > kFullTileTwoJ; }
-    // 0 = automatic: the block kernel up to twojmax = 10, the anti-diagonal kernel on half tiles above
-    bool use_block() const { return (zi_impl == 4 || zi_impl == 0) && !half_tiles() && blk_ready; }
+    // 0 = automatic: the block kernel (on half tiles above twojmax = 10)
+    bool use_block() const { return (zi_impl == 4 || zi_impl == 0) && blk_ready; }
     bool use_ui_dft() const { return twojmax >= 1 && twojmax <= kFullTileTwoJ && ui_impl != 1; }
     bool use_spec() const { return zi_impl == 2; }
     bool use_diag() const { return zi_impl == 3 || (zi_impl == 0 && !use_block()); }
@@ -232,6 +232,7 @@ int set_kernel_attributes(mala_snap *h) {
                                   (int)compute_zi_block_smem_bytes(uhalf_size(kFullTileTwoJ), triple_count(kFullTileTwoJ), kBlkMaxSlots)));
     CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_block_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   (int)compute_zi_block_smem_bytes(uhalf_size(kFullTileTwoJ), triple_count(kFullTileTwoJ), kBlkMaxSlots)));
+    CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_block_half_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kBlkHalfSmemMax));
     (void)h;
     return 0;
 }
@@ -392,7 +393,8 @@ int build_diag_schedule(mala_snap *h) {
 int build_block_schedule(mala_snap *h) {
     const SnapTables &T = h->tab;
     const int nt = T.ntriples, NW = kBlkWarps;
-    constexpr int RB = 32 * (int)sizeof(double2);
+    const bool half = h->half_tiles();   // 16-point items: the two half-warps take the items of a unit alternately
+    const int RB = (half ? 16 : 32) * (int)sizeof(double2);
     struct HostItem { int ex, ey; bool fx, fy; int mb1, mb2; double w; };   // element index of row 0 of each column as it is read
     struct HostUnit { int triple, items_first, nitems, a0, b0, bx, by, ub_elem; std::vector<double> coef; double cost; };
     std::vector<HostItem> items;
@@ -461,7 +463,7 @@ int build_block_schedule(mala_snap *h) {
                                                   ? cf(a_lo + a, b_lo + b) : 0.0);
                         }
                     // issue cycles: an FP64 instruction holds the port for two, anything else for one
-                    hu.cost = n * (2.0 * (4 * bx * by + 2 * by) + 3.0 * bx + 2.0 * by + 14.0) + 2.0 * (2 * bx * by + 2 * (bx + by - 1)) + 0.5 * bx * by +
+                    hu.cost = (half ? (n + 1) / 2 : n) * (2.0 * (4 * bx * by + 2 * by) + 3.0 * bx + 2.0 * by + 14.0) + 2.0 * (2 * bx * by + 2 * (bx + by - 1)) + 0.5 * bx * by +
                               bx + by + 2.0 * bx * by + 40.0;
                     tcost[t] += hu.cost;
                     tunits[t].push_back(std::move(hu));
@@ -507,7 +509,8 @@ int build_block_schedule(mala_snap *h) {
             if (pieces[i].triple == t) piece_slot[i] = nslots++;
     }
     tslot[nt] = nslots;
-    if (nslots > kBlkMaxSlots) return fail(MALA_SNAP_ECUDA, "internal: too many partial-sum slots");
+    if (half ? compute_zi_block_half_smem_bytes(h->sc.nelem, nslots) > (size_t)kBlkHalfSmemMax : nslots > kBlkMaxSlots)
+        return fail(MALA_SNAP_ECUDA, "internal: too many partial-sum slots");
     // one record stream per warp, units by decreasing shape (the order in which the kernel runs its shape loops)
     std::vector<int4> stream;
     std::vector<int> wrange((size_t)NW * (kBlkShapes + 2), 0);
@@ -532,7 +535,8 @@ int build_block_schedule(mala_snap *h) {
                         if (u.bx != bx || u.by != by) continue;
                         count++;
                         // a unit must not straddle the end of the ring: the unit before it skips the words up to the boundary
-                        const int words = 1 + 3 * u.nitems + (bx * by + 1) / 2;
+                        const int nit = half ? (u.nitems + 1) & ~1 : u.nitems;   // half tiles: an even count, the last item repeated at weight zero
+                        const int words = 1 + 3 * nit + (bx * by + 1) / 2;
                         const size_t pos = stream.size() - w0;
                         if (pos / kBlkRingWords != (pos + words - 1) / kBlkRingWords) {
                             const int skip = (int)(kBlkRingWords - pos % kBlkRingWords);
@@ -542,9 +546,10 @@ int build_block_schedule(mala_snap *h) {
                         }
                         last_header = stream.size();
                         have_header = true;
-                        stream.push_back(make_int4(u.nitems, u.ub_elem * RB, piece_slot[i], 0));
-                        for (int k = 0; k < u.nitems; k++) {
-                            const HostItem &it = items[u.items_first + k];
+                        stream.push_back(make_int4(nit, u.ub_elem * RB, piece_slot[i], 0));
+                        for (int k = 0; k < nit; k++) {
+                            HostItem it = items[u.items_first + std::min(k, u.nitems - 1)];
+                            if (k >= u.nitems) it.w = 0.0;
                             const int xe = it.fx ? it.ex - u.a0 : it.ex + u.a0, ye = it.fy ? it.ey - u.b0 : it.ey + u.b0;
                             // x = (-1)^(ma1 - mb1) conj(v) on a mirrored column: sign masks of the real part by the parity of the local row
                             const unsigned sgn = 0x80000000u;
@@ -589,7 +594,10 @@ void launch_ui_dft(mala_snap *h, const GridGeom &g, const DeviceTables &tb, cons
 int launch_zi(mala_snap *h, const ChunkBuffers &cb, double *out, cudaStream_t st) {
     const int grid = std::max(1, std::min(h->num_sms, h->half_tiles() ? 2 * cb.ntiles : cb.ntiles));
     TimedSpan span(h, st, kKindZi);
-    if (h->use_block()) {
+    if (h->use_block() && h->half_tiles())
+        compute_zi_bi_block_half_kernel<<<grid, kBlkWarps * 32, compute_zi_block_half_smem_bytes(h->sc.nelem, h->blk_nslots), st>>>(
+            h->geom, h->sc, h->tables(), h->blk_tables(), cb, out);
+    else if (h->use_block()) {
         const size_t smem = compute_zi_block_smem_bytes(h->sc.nelem, h->sc.ntriples, h->blk_nslots);
         if (h->twojmax >= 8) compute_zi_bi_block_kernel<true><<<grid, kBlkWarps * 32, smem, st>>>(h->geom, h->sc, h->tables(), h->blk_tables(), cb, out);
         else compute_zi_bi_block_kernel<false><<<grid, kBlkWarps * 32, smem, st>>>(h->geom, h->sc, h->tables(), h->blk_tables(), cb, out);
@@ -1613,7 +1621,7 @@ int mala_snap_create(mala_snap_t **handle, int twojmax, double rcutfac, double r
             CUDA_TRY(cudaMemcpyToSymbol(c_wlist, wlist, sizeof(wlist)));
         }
         if ((rc = build_diag_schedule(h))) return rc;
-        if (!h->half_tiles() && (rc = build_block_schedule(h))) return rc;
+        if ((rc = build_block_schedule(h))) return rc;
         if ((rc = set_kernel_attributes(h))) return rc;
         if (h->d_status.reserve(1)) return fail(MALA_SNAP_ENOMEM, "cudaMalloc (status) failed");
         CUDA_TRY(cudaMemset(h->d_status.p, 0, sizeof(int)));
@@ -1677,8 +1685,8 @@ int mala_snap_set_option(mala_snap_t *h, const char *name, long long value) {
     if (n == "zi_impl") {
         if (value < 0 || value > 4) return fail(MALA_SNAP_EINVAL, "zi_impl must be 0 .. 4");
         if (value == 2 && h->twojmax != kSpecTJ) return fail(MALA_SNAP_EINVAL, "the specialised kernel exists for twojmax = 10 only");
-        if (value != 0 && value != 3 && h->half_tiles())
-            return fail(MALA_SNAP_EINVAL, "twojmax > 10 runs on half tiles: only the anti-diagonal kernel (zi_impl 0 or 3) supports them");
+        if ((value == 1 || value == 2) && h->half_tiles())
+            return fail(MALA_SNAP_EINVAL, "twojmax > 10 runs on half tiles: only the anti-diagonal and the block kernel (zi_impl 0, 3, 4) support them");
         if (value == 4 && !h->blk_ready) return fail(MALA_SNAP_EINVAL, "the block kernel has no tables for this handle");
         h->zi_impl = (int)value;
         return compute_bconst(h);

@@ -1,4 +1,4 @@
-// snap_zi_block.cuh -- compute_zi / compute_bi as register-tiled outer products (rows a5 + a6 + a7), any twojmax <= 10.
+// snap_zi_block.cuh -- compute_zi / compute_bi as register-tiled outer products (rows a5 + a6 + a7), any twojmax (half tiles above 10).
 //
 // For a triple (J1,J2,J) and an output column mb, the Z column is
 //     z[ma] = sum_{ma1 + ma2 - sh = ma} CG(ma1, ma2) * T[ma1][ma2],     T[ma1][ma2] = sum_items w_i x_i[ma1] y_i[ma2],
@@ -168,9 +168,12 @@ __device__ __forceinline__ void blk_item(const unsigned char *Ulane, const uint3
 }
 
 // one unit: consumes its records from the reader and returns its contribution to B of its triple, per lane
-template <int BX, int BY, bool PEEL>
-__device__ __forceinline__ double blk_unit(const unsigned char *Ulane, BlkReader &rd, int &slot) {
-    constexpr int RB = 32 * (int)sizeof(double2);
+// HALF (twojmax 11..14: U_tot of 32 points does not fit shared memory): the tile is 16 points, lane = (point, half), and the
+// two half-warps take the items of the unit alternately (the host pads the item list to an even length with a zero-weight
+// item); T, z and the dot product are linear in the items, so each half finishes its own share and the two scalars are added.
+template <int BX, int BY, bool PEEL, bool HALF>
+__device__ __forceinline__ double blk_unit(const unsigned char *Ulane, BlkReader &rd, int &slot, const int h) {
+    constexpr int RB = (HALF ? 16 : 32) * (int)sizeof(double2);
     constexpr int NCW = (BX * BY + 1) / 2;
     double tr[BX][BY], ti[BX][BY];
     rd.ensure(rd.wpos + 1);
@@ -182,12 +185,14 @@ __device__ __forceinline__ double blk_unit(const unsigned char *Ulane, BlkReader
     const int wend = rd.wpos + 1 + 3 * nitems + NCW;
     rd.ensure(wend);
     rd.wpos = wend + hd.w;
-    base += 16;
+    base += 16 + (HALF ? 48 * h : 0);
+    constexpr int ISTEP = HALF ? 96 : 48;
+    const int ntrips = HALF ? (nitems >> 1) : nitems;
     // PEEL: the first item initialises the block (no zeroing pass, -4 % instructions) at the price of a second copy of the
     // item body; pays from twojmax 8 up, where a tile has enough work per fetched instruction
     if constexpr (PEEL) {
         blk_item<BX, BY, true>(Ulane, base, tr, ti);
-        base += 48;
+        base += ISTEP;
     } else {
 #pragma unroll
         for (int a = 0; a < BX; a++)
@@ -196,10 +201,11 @@ __device__ __forceinline__ double blk_unit(const unsigned char *Ulane, BlkReader
     }
     const int ifirst = PEEL ? 1 : 0;
 #pragma unroll 1
-    for (int i = ifirst; i < nitems; i++) {
+    for (int i = ifirst; i < ntrips; i++) {
         blk_item<BX, BY, false>(Ulane, base, tr, ti);
-        base += 48;
+        base += ISTEP;
     }
+    if constexpr (HALF) base -= 48 * h;   // both halves read the same coefficients
     // z on the anti-diagonals of the block (coefficients = CG x fold weight, read where they are used: T dies element by
     // element, so the registers never hold the block and its coefficients together), dotted with conj(U^J[:, mb]) at once
     const unsigned char *ub = Ulane + uboff;
@@ -227,7 +233,7 @@ __device__ __forceinline__ double blk_unit(const unsigned char *Ulane, BlkReader
     return bs0 + bs1;
 }
 
-template <int BX, int BY, bool PEEL>
+template <int BX, int BY, bool PEEL, bool HALF>
 __device__ __forceinline__ void blk_run_shape(const unsigned char *Ulane, const BlkTables &T, const int warp, const int lane, BlkReader &rd,
                                               double *P) {
     constexpr int shape = (BX - 1) * kBlkBY + (BY - 1);
@@ -235,16 +241,21 @@ __device__ __forceinline__ void blk_run_shape(const unsigned char *Ulane, const 
 #pragma unroll 1
     for (int k = 0; k < n; k++) {
         int slot;
-        const double b = blk_unit<BX, BY, PEEL>(Ulane, rd, slot);
-        P[slot * 32 + lane] += b;
+        double b = blk_unit<BX, BY, PEEL, HALF>(Ulane, rd, slot, lane >> 4);
+        if constexpr (HALF) {
+            b += __shfl_xor_sync(0xffffffffu, b, 16);
+            if (lane < 16) P[slot * 16 + lane] += b;
+        } else {
+            P[slot * 32 + lane] += b;
+        }
     }
 }
 
-template <int BX, int BY, bool PEEL>
+template <int BX, int BY, bool PEEL, bool HALF>
 __device__ __forceinline__ void blk_run_all(const unsigned char *Ulane, const BlkTables &T, const int warp, const int lane, BlkReader &rd, double *P) {
-    if constexpr (BX >= kBlkBXMin && BY >= kBlkBYMin) blk_run_shape<BX, BY, PEEL>(Ulane, T, warp, lane, rd, P);
-    if constexpr (BY > 1) blk_run_all<BX, BY - 1, PEEL>(Ulane, T, warp, lane, rd, P);
-    else if constexpr (BX > 1) blk_run_all<BX - 1, kBlkBY, PEEL>(Ulane, T, warp, lane, rd, P);
+    if constexpr (BX >= kBlkBXMin && BY >= kBlkBYMin) blk_run_shape<BX, BY, PEEL, HALF>(Ulane, T, warp, lane, rd, P);
+    if constexpr (BY > 1) blk_run_all<BX, BY - 1, PEEL, HALF>(Ulane, T, warp, lane, rd, P);
+    else if constexpr (BX > 1) blk_run_all<BX - 1, kBlkBY, PEEL, HALF>(Ulane, T, warp, lane, rd, P);
 }
 
 template <bool PEEL>
@@ -289,7 +300,7 @@ compute_zi_bi_block_kernel(GridGeom g, SnapConst sc, DeviceTables tb, BlkTables 
         parity ^= 1u;
         __syncthreads();  // P zeroed
         const unsigned char *Ulane = reinterpret_cast<const unsigned char *>(U + lane);
-        blk_run_all<kBlkBX, kBlkBY, PEEL>(Ulane, T, warp, lane, rd, P);   // shapes in decreasing size: the order of the stream
+        blk_run_all<kBlkBX, kBlkBY, PEEL, false>(Ulane, T, warp, lane, rd, P);   // shapes in decreasing size: the order of the stream
         __syncthreads();
         for (int t = warp; t < nt; t += NW) {   // fixed-order sum of the slots of triple t
             double s = 0.0;
@@ -299,6 +310,78 @@ compute_zi_bi_block_kernel(GridGeom g, SnapConst sc, DeviceTables tb, BlkTables 
         __syncthreads();
         write_tile(g, cb.tile_begin + wt, Bs, nt, out, NW, cb.compact_out, wt);
     }
+}
+
+// twojmax 11..14: half tiles (16 points).  U_tot of the half tile (up to 167 KB at twojmax 14), the partial-sum slots and the
+// rings fill the shared memory, so there is no staging of B: the sums of the slots go straight to global memory, a row of
+// ntriples doubles per grid point.
+__global__ void __launch_bounds__(kBlkWarps * 32, 1)
+compute_zi_bi_block_half_kernel(GridGeom g, SnapConst sc, DeviceTables tb, BlkTables T, ChunkBuffers cb, double *out) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int NW = kBlkWarps;
+    const int nelem = sc.nelem, nt = sc.ntriples;
+    double2 *U = reinterpret_cast<double2 *>(smem_raw + kBlkPadBytes);          // [nelem][16]
+    double *P = reinterpret_cast<double *>(U + (size_t)nelem * 16);              // [nslots][16]
+    int4 *rings = reinterpret_cast<int4 *>(P + (size_t)T.nslots * 16);           // [NW][kBlkRingWords]
+    __shared__ uint64_t bar;
+    __shared__ int s_item;
+    __shared__ long long s_dst[16];   // element offset of the output row of every point of the half tile, -1 = no such point
+    const int lane = threadIdx.x & 31, warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
+    if (threadIdx.x == 0) mbar_init(&bar, 1);
+    for (int i = threadIdx.x; i < kBlkPadBytes / 8; i += NW * 32) reinterpret_cast<double *>(smem_raw)[i] = 0.0;
+    uint32_t parity = 0;
+    const int nactive = cb.counters[0];
+    const size_t half_elems = (size_t)nelem * 16;
+    if (threadIdx.x == 0) s_item = atomicAdd(&cb.counters[2], 1);
+    for (;;) {
+        __syncthreads();  // previous half tile written out: P and U are free; s_item is visible
+        const int item = s_item;
+        const int slot = item >> 1, hh = item & 1;
+        if (slot >= nactive) break;
+        const int wt = cb.active[slot];
+        __syncthreads();  // everybody has read s_item
+        if (threadIdx.x == 0) {
+            tma_load_bytes(U, cb.utot + (size_t)item * half_elems, (uint32_t)(half_elems * sizeof(double2)), &bar);
+            s_item = atomicAdd(&cb.counters[2], 1);
+        }
+        if (threadIdx.x < 16) {
+            long long off = -1;
+            if (cb.compact_out) off = ((long long)wt * 32 + hh * 16 + threadIdx.x) * nt;
+            else {
+                int ix, iy, iz;
+                bool valid;
+                lane_point(g, cb.tile_begin + wt, hh * 16 + threadIdx.x, ix, iy, iz, valid);
+                if (valid) off = ((long long)((long long)(iz - g.z0) * g.ny + iy) * g.nx + ix) * nt;
+            }
+            s_dst[threadIdx.x] = off;
+        }
+        for (int i = threadIdx.x; i < T.nslots * 16; i += NW * 32) P[i] = 0.0;
+        BlkReader rd;
+        rd.src = T.stream + __ldg(T.wrange + warp * (kBlkShapes + 2) + kBlkShapes);
+        rd.wtotal = __ldg(T.wrange + warp * (kBlkShapes + 2) + kBlkShapes + 1);
+        rd.ring = smem_u32(rings + warp * kBlkRingWords);
+        rd.lane = lane; rd.wpos = 0; rd.wreq = 0; rd.wready = 0;
+        rd.fill();
+        mbar_wait(&bar, parity);
+        parity ^= 1u;
+        __syncthreads();  // P zeroed, s_dst written
+        const unsigned char *Ulane = reinterpret_cast<const unsigned char *>(U + (lane & 15));
+        blk_run_all<kBlkBX, kBlkBY, true, true>(Ulane, T, warp, lane, rd, P);
+        __syncthreads();
+        for (int i = threadIdx.x; i < 16 * nt; i += NW * 32) {   // fixed-order sum of the slots of triple t, point p
+            const int p = i / nt, t = i - p * nt;
+            const long long off = s_dst[p];
+            if (off < 0) continue;
+            double sum = 0.0;
+            for (int k = __ldg(T.tslot + t); k < __ldg(T.tslot + t + 1); k++) sum += P[k * 16 + p];
+            __stcs(out + off + t, sum);
+        }
+    }
+}
+
+constexpr int kBlkHalfSmemMax = 232448 - 256;   // the 227 KB of an SM less the kernel's static shared memory
+inline size_t compute_zi_block_half_smem_bytes(int nelem, int nslots) {
+    return (size_t)kBlkPadBytes + (size_t)nelem * 16 * sizeof(double2) + (size_t)nslots * 16 * sizeof(double) + (size_t)kBlkWarps * kBlkRingWords * 16 + 16;
 }
 
 inline size_t compute_zi_block_smem_bytes(int nelem, int nt, int nslots) {

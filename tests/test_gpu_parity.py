@@ -183,10 +183,12 @@ def test_small_cases_every_twojmax(twojmax):
         pos, types, box, origin, pbc, ngrid, params = _small_case(100 * twojmax + seed, twojmax, natoms, pbc, tri, two)
         ref = oracle.bispectrum_grid(pos, types, box, origin, pbc, ngrid, **params)
         with MalaSnap(**params) as snap:
-            got = snap.bispectrum_grid(pos, types, box, origin, pbc, ngrid)
-            torch.cuda.synchronize()
-            assert snap.ncomp == ref.shape[1]
-        assert_parity(got.cpu().numpy(), ref)
+            for zi in ([3, 4] if twojmax > 10 else [0]):   # half tiles: the anti-diagonal and the block kernel
+                snap.set_option("zi_impl", zi)
+                got = snap.bispectrum_grid(pos, types, box, origin, pbc, ngrid)
+                torch.cuda.synchronize()
+                assert snap.ncomp == ref.shape[1]
+                assert_parity(got.cpu().numpy(), ref)
 
 
 @pytest.mark.parametrize("ngrid,zr", [((1, 1, 1), (0, 1)), ((2, 3, 1), (0, 1)), ((9, 1, 5), (1, 4)), ((5, 13, 7), (0, 7)),
@@ -231,7 +233,7 @@ def test_random_small_systems_all_kernels():
         origin = tuple(rng.uniform(-0.3, 0.3, 3))
         ref = oracle.bispectrum_grid(pos, types, box, origin, pbc, ngrid, z0, z1, **params)
         with MalaSnap(**params) as snap:
-            for zi in ([3, 0] if tj > 10 else ([1, 3, 4] if tj != 10 else [1, 2, 3, 4])):
+            for zi in ([3, 4, 0] if tj > 10 else ([1, 3, 4] if tj != 10 else [1, 2, 3, 4])):
                 snap.set_option("zi_impl", zi)
                 if rng.random() < 0.3:
                     snap.set_option("workspace_mb", 1)
