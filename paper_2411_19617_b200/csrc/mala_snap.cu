@@ -21,6 +21,7 @@
 #include "snap_tables.h"
 #include "snap_ui.cuh"
 #include "snap_ui_dft.cuh"
+#include "snap_ui_pipe.cuh"
 #include "snap_zi.cuh"
 #include "snap_zi_coop.cuh"
 #include "snap_zi_diag.cuh"
@@ -103,7 +104,7 @@ struct mala_snap {
     int device = 0, num_sms = 0;
     // options
     int zi_impl = 0;
-    int ui_impl = 0;   // 0 automatic (sampling kernel when twojmax == 10), 1 column kernel, 2 sampling kernel
+    int ui_impl = 0;   // 0 automatic (sampling kernel for twojmax 1..10, pipelined from 8 up), 1 column kernel, 2 sampling kernel, 3 pipelined sampling kernel
     // tables of the anti-diagonal kernels (per handle, global memory)
     std::vector<double> k_dcg;
     std::vector<DiagTriple> k_dtriple;
@@ -196,6 +197,7 @@ struct mala_snap {
     // 0 = automatic: the block kernel (on half tiles above twojmax = 10)
     bool use_block() const { return (zi_impl == 4 || zi_impl == 0) && blk_ready; }
     bool use_ui_dft() const { return twojmax >= 1 && twojmax <= kFullTileTwoJ && ui_impl != 1; }
+    bool use_ui_pipe() const { return twojmax >= 8 && twojmax <= kFullTileTwoJ && (ui_impl == 0 || ui_impl == 3); }
     bool use_spec() const { return zi_impl == 2; }
     bool use_diag() const { return zi_impl == 3 || (zi_impl == 0 && !use_block()); }
 };
@@ -221,6 +223,9 @@ int set_kernel_attributes(mala_snap *h) {
     MALA_DFT_ATTR(1) MALA_DFT_ATTR(2) MALA_DFT_ATTR(3) MALA_DFT_ATTR(4) MALA_DFT_ATTR(5)
     MALA_DFT_ATTR(6) MALA_DFT_ATTR(7) MALA_DFT_ATTR(8) MALA_DFT_ATTR(9) MALA_DFT_ATTR(10)
 #undef MALA_DFT_ATTR
+    CUDA_TRY(cudaFuncSetAttribute(compute_ui_pipe_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)compute_ui_pipe_smem_bytes<8>()));
+    CUDA_TRY(cudaFuncSetAttribute(compute_ui_pipe_kernel<9>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)compute_ui_pipe_smem_bytes<9>()));
+    CUDA_TRY(cudaFuncSetAttribute(compute_ui_pipe_kernel<10>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)compute_ui_pipe_smem_bytes<10>()));
     const int zi_smem = (int)compute_zi_smem_bytes(uhalf_size(kFullTileTwoJ), triple_count(kFullTileTwoJ));
     CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, zi_smem));
     CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_coop_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)compute_zi_coop_smem_bytes()));
@@ -578,6 +583,17 @@ int build_block_schedule(mala_snap *h) {
 
 // enqueue the sampling compute_ui (snap_ui_dft.cuh) for one chunk: whole tiles, twojmax + 1 warps
 void launch_ui_dft(mala_snap *h, const GridGeom &g, const DeviceTables &tb, const ChunkBuffers &cb, cudaStream_t st) {
+    if (h->use_ui_pipe()) {   // twojmax 8..10: one CTA per SM, a producer warp ahead of the sample warps (snap_ui_pipe.cuh)
+        const int grid = std::max(1, std::min(h->num_sms, cb.ntiles));
+        switch (h->twojmax) {
+#define MALA_PIPE_CASE(TJ) \
+    case TJ: compute_ui_pipe_kernel<TJ><<<grid, (TJ + 2) * 32, compute_ui_pipe_smem_bytes<TJ>(), st>>>(g, h->sc, tb, cb); break;
+            MALA_PIPE_CASE(8) MALA_PIPE_CASE(9) MALA_PIPE_CASE(10)
+#undef MALA_PIPE_CASE
+            default: break;
+        }
+        return;
+    }
     switch (h->twojmax) {
 #define MALA_DFT_CASE(TJ) \
     case TJ: \
@@ -1677,7 +1693,8 @@ int mala_snap_set_option(mala_snap_t *h, const char *name, long long value) {
         return MALA_SNAP_OK;
     }
     if (n == "ui_impl") {
-        if (value < 0 || value > 2) return fail(MALA_SNAP_EINVAL, "ui_impl must be 0, 1 or 2");
+        if (value < 0 || value > 3) return fail(MALA_SNAP_EINVAL, "ui_impl must be 0 .. 3");
+        if (value == 3 && (h->twojmax < 8 || h->twojmax > kFullTileTwoJ)) return fail(MALA_SNAP_EINVAL, "the pipelined sampling compute_ui kernel covers twojmax 8..10");
         if (value == 2 && (h->twojmax < 1 || h->twojmax > kFullTileTwoJ)) return fail(MALA_SNAP_EINVAL, "the sampling compute_ui kernel covers twojmax 1..10");
         h->ui_impl = (int)value;
         return MALA_SNAP_OK;

@@ -59,20 +59,21 @@ def test_config1_tiny_al_full_grid(tiny_ref, zi_impl):
     assert_parity(got, ref)
 
 
-@pytest.mark.parametrize("ui_impl", [1, 2])
+@pytest.mark.parametrize("ui_impl", [1, 2, 3])
 def test_config1_both_compute_ui_kernels(tiny_ref, ui_impl):
-    """the column kernel (polynomial recursion) and the sampling kernel (roots of unity + inverse DFT) against the oracle"""
+    """the column kernel (polynomial recursion), the sampling kernel (roots of unity + inverse DFT) and its producer / consumer
+    form against the oracle"""
     w, ref = tiny_ref
     got = gpu_grid(w, ui_impl=ui_impl)
     assert_parity(got, ref)
 
 
-@pytest.mark.parametrize("twojmax", [1, 3, 6, 9])
+@pytest.mark.parametrize("twojmax", [1, 3, 6, 8, 9])
 def test_compute_ui_kernels_other_twojmax(twojmax):
     torch = _torch()
     pos, types, box, origin, pbc, ngrid, params = _small_case(7000 + twojmax, twojmax, 5, (1, 0, 1), True, True)
     ref = oracle.bispectrum_grid(pos, types, box, origin, pbc, ngrid, **params)
-    for ui in (1, 2):
+    for ui in ((1, 2, 3) if twojmax >= 8 else (1, 2)):
         with MalaSnap(**params) as snap:
             snap.set_option("ui_impl", ui)
             got = snap.bispectrum_grid(pos, types, box, origin, pbc, ngrid)
@@ -80,6 +81,26 @@ def test_compute_ui_kernels_other_twojmax(twojmax):
         assert_parity(got.cpu().numpy(), ref)
     with MalaSnap(twojmax=12) as snap, pytest.raises(MalaSnapError):
         snap.set_option("ui_impl", 2)
+
+
+@pytest.mark.parametrize("twojmax", [8, 10])
+def test_dense_system_several_candidate_windows(twojmax):
+    """70 atoms in a 6 A box: every grid point has far more neighbors than one window of candidates holds (48 in the sampling
+    kernel, 40 in the pipelined one, where several windows are also sent once per accumulation pass)"""
+    torch = _torch()
+    rng = np.random.default_rng(909 + twojmax)
+    box = np.eye(3) * 6.0
+    pos = rng.uniform(0.0, 6.0, size=(70, 3))
+    types = rng.integers(0, 2, 70).astype(np.int32)
+    params = dict(twojmax=twojmax, rcutfac=4.2, rfac0=0.99363, rmin0=0.0, wself=1.0, radelem=(0.5, 0.45), wj=(1.0, 0.8))
+    ngrid = (5, 6, 3)
+    ref = oracle.bispectrum_grid(pos, types, box, (0, 0, 0), (1, 1, 1), ngrid, **params)
+    for ui in (1, 2, 3):
+        with MalaSnap(**params) as snap:
+            snap.set_option("ui_impl", ui)
+            got = snap.bispectrum_grid(pos, types, box, (0, 0, 0), (1, 1, 1), ngrid)
+            torch.cuda.synchronize()
+        assert_parity(got.cpu().numpy(), ref)
 
 
 def test_triples_match_oracle_order():
