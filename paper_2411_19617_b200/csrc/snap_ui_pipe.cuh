@@ -42,7 +42,7 @@ struct PipeTask { unsigned short scol, e0, k0, k1; };   // column index inside i
 // then the binomial normalisation and the self term.  S holds the columns of one pass: [column][sample][lane].
 template <int TJ>
 __device__ __forceinline__ void pipe_dft(const double2 *S, const PipeTask *tasks, const int ntasks, const int lane, const double2 *s_tw,
-                                         double2 *dst, const DeviceTables &tb, const double wself) {
+                                         double2 *dst, const double2 *s_norm) {
     constexpr int NW = TJ + 1, NP = (NW - 1) / 2;
     for (int ti = 0; ti < ntasks; ti++) {
         const PipeTask t = tasks[ti];
@@ -69,8 +69,8 @@ __device__ __forceinline__ void pipe_dft(const double2 *S, const PipeTask *tasks
                 si = fma(pi_[sI - 1], w.x, si); si = fma(mr_[sI - 1], w.y, si);
             }
             const int e = t.e0 + k;
-            const double sN = tb.unorm[e] * (1.0 / (double)NW);
-            dst[(size_t)e * 32 + lane] = make_double2(sr * sN + (tb.udiag[e] ? wself : 0.0), si * sN);
+            const double2 nrm = s_norm[e];   // binomial normalisation / NW, self term of the diagonal elements
+            dst[(size_t)e * 32 + lane] = make_double2(fma(sr, nrm.x, nrm.y), si * nrm.x);
         }
     }
 }
@@ -91,6 +91,7 @@ compute_ui_pipe_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers c
     __shared__ int s_cnt[2][32];          // entries of every lane's queue in the buffer
     __shared__ int s_meta[2][2];          // slot of the tile the buffer belongs to (-1: no more tiles), windows of that tile
     __shared__ double2 s_tw[NW * NW];     // [k][s] = x_s^(-k) = e^{-2 pi i s k / NW}
+    __shared__ double2 s_norm[nelem];     // {unorm / NW, wself on the diagonal}
     __shared__ PipeTask s_task[2][NW][kPipeMaxTasks];
     __shared__ int s_ntask[2][NW];
     const int lane = threadIdx.x & 31, warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
@@ -99,6 +100,7 @@ compute_ui_pipe_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers c
         sincospi(2.0 * (double)(((threadIdx.x / NW) * (threadIdx.x % NW)) % NW) / (double)NW, &sn, &cs);
         s_tw[threadIdx.x] = make_double2(cs, -sn);
     }
+    for (int e = threadIdx.x; e < nelem; e += (NW + 1) * 32) s_norm[e] = make_double2(tb.unorm[e] * (1.0 / (double)NW), tb.udiag[e] ? sc.wself : 0.0);
     if (threadIdx.x == NW * 32) {
         mbar_init(&full[0], 32); mbar_init(&full[1], 32);
         mbar_init(&empty[0], NW); mbar_init(&empty[1], NW);
@@ -225,7 +227,7 @@ compute_ui_pipe_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers c
             for (int k = 0; k < KA; k++) S[((size_t)k * NW + warp) * 32 + lane] = make_double2(accr[k], acci[k]);
         }
         consumer_barrier<NW * 32>();
-        pipe_dft<TJ>(S, s_task[0][warp], s_ntask[0][warp], lane, s_tw, dst, tb, sc.wself);
+        pipe_dft<TJ>(S, s_task[0][warp], s_ntask[0][warp], lane, s_tw, dst, s_norm);
         if constexpr (KB > 0) {
             consumer_barrier<NW * 32>();   // S is free again
             double accr[NJM], acci[NJM];   // KB of them in use
@@ -245,7 +247,7 @@ compute_ui_pipe_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers c
 #pragma unroll
             for (int k = 0; k < KB; k++) S[((size_t)k * NW + warp) * 32 + lane] = make_double2(accr[k], acci[k]);
             consumer_barrier<NW * 32>();
-            pipe_dft<TJ>(S, s_task[1][warp], s_ntask[1][warp], lane, s_tw, dst, tb, sc.wself);
+            pipe_dft<TJ>(S, s_task[1][warp], s_ntask[1][warp], lane, s_tw, dst, s_norm);
         }
         consumer_barrier<NW * 32>();   // S is free for the next tile
     }
