@@ -196,8 +196,8 @@ struct mala_snap {
     bool half_tiles() const { return twojmax > kFullTileTwoJ; }
     // 0 = automatic: the block kernel (on half tiles above twojmax = 10)
     bool use_block() const { return (zi_impl == 4 || zi_impl == 0) && blk_ready; }
-    bool use_ui_dft() const { return twojmax >= 1 && twojmax <= kFullTileTwoJ && ui_impl != 1; }
-    bool use_ui_pipe() const { return twojmax >= 8 && twojmax <= kFullTileTwoJ && (ui_impl == 0 || ui_impl == 3); }
+    bool use_ui_pipe() const { return twojmax >= 8 && (ui_impl == 0 || ui_impl == 3); }
+    bool use_ui_dft() const { return (twojmax >= 1 && twojmax <= kFullTileTwoJ && ui_impl != 1) || use_ui_pipe(); }
     bool use_spec() const { return zi_impl == 2; }
     bool use_diag() const { return zi_impl == 3 || (zi_impl == 0 && !use_block()); }
 };
@@ -226,6 +226,10 @@ int set_kernel_attributes(mala_snap *h) {
     CUDA_TRY(cudaFuncSetAttribute(compute_ui_pipe_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)compute_ui_pipe_smem_bytes<8>()));
     CUDA_TRY(cudaFuncSetAttribute(compute_ui_pipe_kernel<9>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)compute_ui_pipe_smem_bytes<9>()));
     CUDA_TRY(cudaFuncSetAttribute(compute_ui_pipe_kernel<10>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)compute_ui_pipe_smem_bytes<10>()));
+    CUDA_TRY(cudaFuncSetAttribute(compute_ui_pipe_kernel<11>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)compute_ui_pipe_smem_bytes<11>()));
+    CUDA_TRY(cudaFuncSetAttribute(compute_ui_pipe_kernel<12>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)compute_ui_pipe_smem_bytes<12>()));
+    CUDA_TRY(cudaFuncSetAttribute(compute_ui_pipe_kernel<13>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)compute_ui_pipe_smem_bytes<13>()));
+    CUDA_TRY(cudaFuncSetAttribute(compute_ui_pipe_kernel<14>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)compute_ui_pipe_smem_bytes<14>()));
     const int zi_smem = (int)compute_zi_smem_bytes(uhalf_size(kFullTileTwoJ), triple_count(kFullTileTwoJ));
     CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, zi_smem));
     CUDA_TRY(cudaFuncSetAttribute(compute_zi_bi_coop_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)compute_zi_coop_smem_bytes()));
@@ -588,7 +592,7 @@ void launch_ui_dft(mala_snap *h, const GridGeom &g, const DeviceTables &tb, cons
         switch (h->twojmax) {
 #define MALA_PIPE_CASE(TJ) \
     case TJ: compute_ui_pipe_kernel<TJ><<<grid, (TJ + 2) * 32, compute_ui_pipe_smem_bytes<TJ>(), st>>>(g, h->sc, tb, cb); break;
-            MALA_PIPE_CASE(8) MALA_PIPE_CASE(9) MALA_PIPE_CASE(10)
+            MALA_PIPE_CASE(8) MALA_PIPE_CASE(9) MALA_PIPE_CASE(10) MALA_PIPE_CASE(11) MALA_PIPE_CASE(12) MALA_PIPE_CASE(13) MALA_PIPE_CASE(14)
 #undef MALA_PIPE_CASE
             default: break;
         }
@@ -1019,7 +1023,9 @@ int run_slab(mala_snap *h, int z0, int z1, double *out, double2 *u_out, cudaStre
         const int grid = std::max(1, std::min(h->num_sms, cb.ntiles));
         {
             TimedSpan span(h, st, kKindUi);
-            if (h->half_tiles()) {  // twojmax 11..14: eight column warps, one CTA per SM
+            if (h->half_tiles() && h->use_ui_pipe()) {  // twojmax 11..14: the pipelined sampling kernel, whole tiles stored as two halves
+                launch_ui_dft(h, g, tb, cb, st);
+            } else if (h->half_tiles()) {  // the column kernel: eight column warps, one CTA per SM
                 const int ui_grid = std::max(1, std::min(h->num_sms, 2 * cb.ntiles));
                 compute_ui_kernel<kMaxTwoJ, false><<<ui_grid, (kMaxTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kMaxTwoJ), st>>>(g, h->sc, tb, cb);
             } else {
@@ -1694,7 +1700,7 @@ int mala_snap_set_option(mala_snap_t *h, const char *name, long long value) {
     }
     if (n == "ui_impl") {
         if (value < 0 || value > 3) return fail(MALA_SNAP_EINVAL, "ui_impl must be 0 .. 3");
-        if (value == 3 && (h->twojmax < 8 || h->twojmax > kFullTileTwoJ)) return fail(MALA_SNAP_EINVAL, "the pipelined sampling compute_ui kernel covers twojmax 8..10");
+        if (value == 3 && h->twojmax < 8) return fail(MALA_SNAP_EINVAL, "the pipelined sampling compute_ui kernel covers twojmax 8..14");
         if (value == 2 && (h->twojmax < 1 || h->twojmax > kFullTileTwoJ)) return fail(MALA_SNAP_EINVAL, "the sampling compute_ui kernel covers twojmax 1..10");
         h->ui_impl = (int)value;
         return MALA_SNAP_OK;

@@ -21,12 +21,35 @@
 
 namespace mala {
 
-constexpr int kPipeCap = 40;     // candidates per window = entries of a queue buffer
-constexpr int kPipeMaxTasks = 6; // pieces of columns one warp transforms per pass
+constexpr int kPipeWin = 64;      // candidates per window of distance tests (hit masks are 64 bits)
+constexpr int kPipeMaxTasks = 6;  // pieces of columns one warp transforms per pass
+constexpr int kPipeMaxPass = 5;
 
-constexpr int pipe_split(int tj) { return 2; }
-constexpr int pipe_ka(int tj) { return dft_index(tj, pipe_split(tj), pipe_split(tj)); }                  // columns of the first pass
-constexpr int pipe_kmax(int tj) { return pipe_ka(tj) > dft_njm(tj) - pipe_ka(tj) ? pipe_ka(tj) : dft_njm(tj) - pipe_ka(tj); }
+// entries of a queue buffer per grid point (a window is cut short where a point would get more)
+constexpr int pipe_cap(int tj) { return tj >= 14 ? 32 : 40; }
+// columns whose sums a thread keeps in registers during one pass: whole chains (all n of one mb), as many as fit
+constexpr int pipe_klim(int tj) { return tj <= 10 ? 20 : (tj == 11 ? 18 : 16); }
+// first chain of pass p (p = number of passes: one past the last chain)
+constexpr int pipe_pass_mb(int tj, int p) {
+    int mb = 0;
+    for (int i = 0; i < p; i++) {
+        int cols = 0;
+        while (mb <= tj / 2 && (cols == 0 || cols + (tj - 2 * mb + 1) <= pipe_klim(tj))) { cols += tj - 2 * mb + 1; mb++; }
+    }
+    return mb;
+}
+constexpr int pipe_npass(int tj) {
+    int p = 0;
+    while (pipe_pass_mb(tj, p) <= tj / 2) p++;
+    return p;
+}
+constexpr int pipe_pass_col(int tj, int p) { return dft_index(tj, pipe_pass_mb(tj, p), pipe_pass_mb(tj, p)); }   // first column of pass p
+constexpr int pipe_kmax(int tj) {
+    int k = 0;
+    for (int p = 0; p < pipe_npass(tj); p++)
+        if (pipe_pass_col(tj, p + 1) - pipe_pass_col(tj, p) > k) k = pipe_pass_col(tj, p + 1) - pipe_pass_col(tj, p);
+    return k;
+}
 
 __device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
@@ -40,9 +63,10 @@ struct PipeTask { unsigned short scol, e0, k0, k1; };   // column index inside i
 
 // inverse DFT of this warp's pieces of columns: q_k = (1/NW) sum_s S_s x_s^(-k) over conjugate sample pairs (snap_ui_dft.cuh),
 // then the binomial normalisation and the self term.  S holds the columns of one pass: [column][sample][lane].
-template <int TJ>
+// dst points at this lane's word of element 0 of the tile (ESTRIDE words per element: 32, or 16 in the half-tile layout).
+template <int TJ, int ESTRIDE>
 __device__ __forceinline__ void pipe_dft(const double2 *S, const PipeTask *tasks, const int ntasks, const int lane, const double2 *s_tw,
-                                         double2 *dst, const double2 *s_norm) {
+                                         double2 *dst, const double2 *norm) {
     constexpr int NW = TJ + 1, NP = (NW - 1) / 2;
     for (int ti = 0; ti < ntasks; ti++) {
         const PipeTask t = tasks[ti];
@@ -69,9 +93,89 @@ __device__ __forceinline__ void pipe_dft(const double2 *S, const PipeTask *tasks
                 si = fma(pi_[sI - 1], w.x, si); si = fma(mr_[sI - 1], w.y, si);
             }
             const int e = t.e0 + k;
-            const double2 nrm = s_norm[e];   // binomial normalisation / NW, self term of the diagonal elements
-            dst[(size_t)e * 32 + lane] = make_double2(fma(sr, nrm.x, nrm.y), si * nrm.x);
+            const double2 nrm = norm[e];   // binomial normalisation / NW, self term of the diagonal elements
+            dst[(size_t)e * ESTRIDE] = make_double2(fma(sr, nrm.x, nrm.y), si * nrm.x);
         }
+    }
+}
+
+// most pieces a warp gets when the coefficients of a pass's columns are cut into twojmax + 1 runs of equal length (the deal
+// of the kernel's prologue, replayed at compile time)
+constexpr int pipe_max_tasks(int tj) {
+    int worst = 0;
+    for (int pass = 0; pass < pipe_npass(tj); pass++) {
+        const int mb0 = pipe_pass_mb(tj, pass), mb1 = pipe_pass_mb(tj, pass + 1), nw = tj + 1;
+        int total = 0;
+        for (int mb = mb0; mb < mb1; mb++)
+            for (int n = mb; n <= tj - mb; n++) total += mb + n + 1;
+        const int target = (total + nw - 1) / nw;
+        int room = target, count = 0;
+        for (int mb = mb0; mb < mb1; mb++)
+            for (int n = mb; n <= tj - mb; n++) {
+                int k = 0;
+                while (k <= mb + n) {
+                    const int take = room < mb + n + 1 - k ? room : mb + n + 1 - k;
+                    count++;
+                    if (count > worst) worst = count;
+                    k += take; room -= take;
+                    if (room == 0) { room = target; count = 0; }
+                }
+            }
+    }
+    return worst;
+}
+
+// what the consumer warps share between the passes of a tile
+template <int TJ>
+struct PipeCtx {
+    double2 *S;                 // [kmax][NW][32]
+    const double *geo;          // [2][cap][5][32]
+    uint64_t *full, *empty;     // [2] each
+    const int (*cnt)[32];       // [2][32]
+    const int (*meta)[2];       // [2]{slot, last window of its round}
+    const PipeTask (*task)[TJ + 1][kPipeMaxTasks];
+    const int (*ntask)[TJ + 1];
+    const double2 *tw, *norm;
+    double2 *dst;               // this lane's word of element 0 of the tile
+    double xsr, xsi;
+    uint32_t it;                // buffers taken so far
+    int buf, lane, warp;
+    bool single;                // the tile came in one window: its buffer serves every pass
+};
+
+// pass P of a tile and the passes behind it: sums of chains pipe_pass_mb(P) <= mb < pipe_pass_mb(P + 1) over every window,
+// then those columns through S and the inverse DFT
+template <int TJ, int P>
+__device__ __forceinline__ void pipe_passes(PipeCtx<TJ> &c) {
+    if constexpr (P < pipe_npass(TJ)) {
+        constexpr int NW = TJ + 1, NJM = dft_njm(TJ), GEO = pipe_cap(TJ) * 5 * 32;
+        constexpr int K = pipe_pass_col(TJ, P + 1) - pipe_pass_col(TJ, P);
+        constexpr bool LAST = (P + 1 == pipe_npass(TJ));
+        {
+            double accr[NJM], acci[NJM];   // K of them in use
+#pragma unroll
+            for (int k = 0; k < K; k++) { accr[k] = 0.0; acci[k] = 0.0; }
+            for (bool first = true;; first = false) {
+                if (!(first && (P == 0 || c.single))) {   // the first window of a tile is taken by the caller; a single one stays
+                    c.buf = c.it & 1;
+                    mbar_wait(&c.full[c.buf], (c.it >> 1) & 1);
+                }
+                dft_accumulate<TJ, pipe_pass_mb(TJ, P), pipe_pass_mb(TJ, P + 1)>(c.geo + (size_t)c.buf * GEO, c.lane, c.cnt[c.buf][c.lane], c.xsr,
+                                                                                  c.xsi, accr, acci);
+                if (c.single && !LAST) break;
+                const bool last = c.meta[c.buf][1] != 0;
+                __syncwarp();
+                if (c.lane == 0) mbar_arrive(&c.empty[c.buf]);
+                c.it++;
+                if (last) break;
+            }
+            consumer_barrier<NW * 32>();   // everybody is done with the inverse DFT of the previous pass: S is free
+#pragma unroll
+            for (int k = 0; k < K; k++) c.S[((size_t)k * NW + c.warp) * 32 + c.lane] = make_double2(accr[k], acci[k]);
+        }
+        consumer_barrier<NW * 32>();
+        pipe_dft<TJ, (TJ > kFullTileTwoJ ? 16 : 32)>(c.S, c.task[P][c.warp], c.ntask[P][c.warp], c.lane, c.tw, c.dst, c.norm);
+        pipe_passes<TJ, P + 1>(c);
     }
 }
 
@@ -79,21 +183,22 @@ template <int TJ>
 __global__ void __launch_bounds__((TJ + 2) * 32, 1)
 compute_ui_pipe_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers cb) {
     constexpr int NW = TJ + 1;          // consumer warps = sample points; warp NW is the producer
-    constexpr int NJM = dft_njm(TJ);
     constexpr int nelem = uhalf_size(TJ);
-    constexpr int SPLIT = pipe_split(TJ), KA = pipe_ka(TJ), KB = NJM - KA, KMAX = pipe_kmax(TJ);
-    constexpr int GEO = kPipeCap * 5 * 32;   // doubles per queue buffer
+    constexpr int NPASS = pipe_npass(TJ), KMAX = pipe_kmax(TJ), CAP = pipe_cap(TJ);
+    constexpr int GEO = CAP * 5 * 32;   // doubles per queue buffer
+    constexpr bool HALF = TJ > kFullTileTwoJ;   // U_tot is stored half tile by half tile
+    static_assert(NPASS <= kPipeMaxPass && pipe_max_tasks(TJ) <= kPipeMaxTasks, "pass tables");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double2 *S = reinterpret_cast<double2 *>(smem_raw);                       // [KMAX][NW][32]
-    double *geo = reinterpret_cast<double *>(S + (size_t)KMAX * NW * 32);     // [2][kPipeCap][5][32]
-    double *crec = geo + 2 * GEO;                                             // [kPipeCap][6], the producer's
+    double *geo = reinterpret_cast<double *>(S + (size_t)KMAX * NW * 32);     // [2][CAP][5][32]
+    double *crec = geo + 2 * GEO;                                             // [kPipeWin][6], the producer's
     __shared__ uint64_t full[2], empty[2];
     __shared__ int s_cnt[2][32];          // entries of every lane's queue in the buffer
-    __shared__ int s_meta[2][2];          // slot of the tile the buffer belongs to (-1: no more tiles), windows of that tile
+    __shared__ int s_meta[2][2];          // slot of the tile the buffer belongs to (-1: no more tiles); last window of its round
     __shared__ double2 s_tw[NW * NW];     // [k][s] = x_s^(-k) = e^{-2 pi i s k / NW}
     __shared__ double2 s_norm[nelem];     // {unorm / NW, wself on the diagonal}
-    __shared__ PipeTask s_task[2][NW][kPipeMaxTasks];
-    __shared__ int s_ntask[2][NW];
+    __shared__ PipeTask s_task[NPASS][NW][kPipeMaxTasks];
+    __shared__ int s_ntask[NPASS][NW];
     const int lane = threadIdx.x & 31, warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
     if (threadIdx.x < NW * NW) {
         double sn, cs;
@@ -107,8 +212,8 @@ compute_ui_pipe_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers c
     }
     if (threadIdx.x == 0) {
         // the coefficients of a pass's columns, cut into NW runs of equal length: every warp transforms the same number of them
-        for (int pass = 0; pass < 2; pass++) {
-            const int mb0 = pass ? SPLIT : 0, mb1 = pass ? TJ / 2 + 1 : SPLIT;
+        for (int pass = 0; pass < NPASS; pass++) {
+            const int mb0 = pipe_pass_mb(TJ, pass), mb1 = pipe_pass_mb(TJ, pass + 1);
             int total = 0;
             for (int mb = mb0; mb < mb1; mb++)
                 for (int n = mb; n <= TJ - mb; n++) total += mb + n + 1;
@@ -124,7 +229,7 @@ compute_ui_pipe_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers c
                         PipeTask t;
                         t.scol = (unsigned short)scol; t.e0 = (unsigned short)(uhalf_off(J) + mb * (J + 1));
                         t.k0 = (unsigned short)k; t.k1 = (unsigned short)(k + take);
-                        s_task[pass][w][s_ntask[pass][w]++] = t;
+                        s_task[pass][w][s_ntask[pass][w]++] = t;   // at most pipe_max_tasks(TJ) per warp
                         k += take; room -= take;
                         if (room == 0) { w++; room = target; }
                     }
@@ -157,12 +262,13 @@ compute_ui_pipe_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers c
             point_position(g, ix, iy, iz, px, py, pz);
             const int nc = cb.ncand[wt];
             const int *mycand = cb.cand + (size_t)wt * cb.cand_cap;
-            const int nwin = max(1, (nc + kPipeCap - 1) / kPipeCap);
-            const int rounds = (nwin > 1 && KB > 0) ? 2 : 1;   // several windows are sent once per pass
-            for (int round = 0; round < rounds; round++)
-                for (int win = 0; win < nwin; win++, it++) {
-                    const int wbase = win * kPipeCap, nw = min(kPipeCap, nc - wbase), buf = it & 1;
-                    __syncwarp();
+            int rounds = 1;   // a tile of several windows is sent once per pass
+            for (int round = 0; round < rounds; round++) {
+                int wbase = 0;
+                bool last;
+                do {
+                    int nw = min(kPipeWin, nc - wbase);
+                    __syncwarp();   // the geometry of the previous window has read crec
                     for (int k = lane; k < nw; k += 32) {
                         const Ghost gh = cb.ghosts[mycand[wbase + k]];
                         const double rc = tb.type_rcut[gh.type];
@@ -176,6 +282,14 @@ compute_ui_pipe_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers c
                         const double dx = q[0] - px, dy = q[1] - py, dz = q[2] - pz;
                         if (dx * dx + dy * dy + dz * dz < q[5]) hits |= 1ull << k;
                     }
+                    // the window ends where a point would get more entries than a buffer holds
+                    while (__reduce_max_sync(0xffffffffu, (unsigned)__popcll(hits)) > (unsigned)CAP) {
+                        nw--;
+                        hits &= (1ull << nw) - 1ull;
+                    }
+                    last = wbase + nw >= nc;
+                    if (round == 0 && wbase == 0 && !last) rounds = NPASS;
+                    const int buf = it & 1;
                     mbar_wait(&empty[buf], ((it >> 1) & 1) ^ 1);   // the consumers are done with this buffer
                     double *gq = geo + (size_t)buf * GEO + lane;
                     for (unsigned long long r = hits; r != 0ull; r &= r - 1ull, gq += 5 * 32) {
@@ -187,76 +301,40 @@ compute_ui_pipe_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers c
                         gq[0] = c; gq[32] = ar; gq[64] = ai; gq[96] = br; gq[128] = bi;
                     }
                     s_cnt[buf][lane] = __popcll(hits);
-                    if (lane == 0) { s_meta[buf][0] = slot; s_meta[buf][1] = nwin; }
+                    if (lane == 0) { s_meta[buf][0] = slot; s_meta[buf][1] = last ? 1 : 0; }
                     mbar_arrive(&full[buf]);
-                }
+                    it++;
+                    wbase += nw;
+                } while (!last);
+            }
         }
         return;
     }
 
     // -------------------------------------------------------------------- consumers: warp = sample point, lane = grid point
-    double xsr, xsi;                    // this warp's sample point x_s = e^{2 pi i s / NW}
-    {
+    PipeCtx<TJ> c;
+    c.S = S; c.geo = geo; c.full = full; c.empty = empty; c.cnt = s_cnt; c.meta = s_meta; c.task = s_task; c.ntask = s_ntask;
+    c.tw = s_tw; c.norm = s_norm; c.lane = lane; c.warp = warp; c.it = 0;
+    {   // this warp's sample point x_s = e^{2 pi i s / NW}
         double sn, cs;
         sincospi(2.0 * (double)warp / (double)NW, &sn, &cs);
-        xsr = cs; xsi = sn;
+        c.xsr = cs; c.xsi = sn;
     }
-    uint32_t it = 0;   // buffers taken so far
     for (;;) {
-        int buf = it & 1;
-        mbar_wait(&full[buf], (it >> 1) & 1);
-        const int slot = s_meta[buf][0];
+        c.buf = c.it & 1;
+        mbar_wait(&full[c.buf], (c.it >> 1) & 1);
+        const int slot = s_meta[c.buf][0];
         if (slot < 0) break;
-        const int nwin = s_meta[buf][1];
-        double2 *dst = cb.utot + (size_t)slot * nelem * 32;
-        {   // first pass: chains mb < SPLIT
-            double accr[NJM], acci[NJM];   // KA of them in use
-#pragma unroll
-            for (int k = 0; k < KA; k++) { accr[k] = 0.0; acci[k] = 0.0; }
-            for (int win = 0;;) {
-                dft_accumulate<TJ, 0, SPLIT>(geo + (size_t)buf * GEO, lane, s_cnt[buf][lane], xsr, xsi, accr, acci);
-                if (nwin == 1 && KB > 0) break;   // a single window stays for the second pass
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&empty[buf]);
-                it++;
-                if (++win == nwin) break;
-                buf = it & 1;
-                mbar_wait(&full[buf], (it >> 1) & 1);
-            }
-#pragma unroll
-            for (int k = 0; k < KA; k++) S[((size_t)k * NW + warp) * 32 + lane] = make_double2(accr[k], acci[k]);
-        }
-        consumer_barrier<NW * 32>();
-        pipe_dft<TJ>(S, s_task[0][warp], s_ntask[0][warp], lane, s_tw, dst, s_norm);
-        if constexpr (KB > 0) {
-            consumer_barrier<NW * 32>();   // S is free again
-            double accr[NJM], acci[NJM];   // KB of them in use
-#pragma unroll
-            for (int k = 0; k < KB; k++) { accr[k] = 0.0; acci[k] = 0.0; }
-            for (int win = 0;;) {
-                if (nwin > 1) {
-                    buf = it & 1;
-                    mbar_wait(&full[buf], (it >> 1) & 1);
-                }
-                dft_accumulate<TJ, SPLIT, TJ / 2 + 1>(geo + (size_t)buf * GEO, lane, s_cnt[buf][lane], xsr, xsi, accr, acci);
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&empty[buf]);
-                it++;
-                if (++win == nwin) break;
-            }
-#pragma unroll
-            for (int k = 0; k < KB; k++) S[((size_t)k * NW + warp) * 32 + lane] = make_double2(accr[k], acci[k]);
-            consumer_barrier<NW * 32>();
-            pipe_dft<TJ>(S, s_task[1][warp], s_ntask[1][warp], lane, s_tw, dst, s_norm);
-        }
-        consumer_barrier<NW * 32>();   // S is free for the next tile
+        c.single = s_meta[c.buf][1] != 0;
+        c.dst = HALF ? cb.utot + ((size_t)(2 * slot + (lane >> 4)) * nelem) * 16 + (lane & 15) : cb.utot + (size_t)slot * nelem * 32 + lane;
+        pipe_passes<TJ, 0>(c);
     }
 }
 
 template <int TJ>
 inline size_t compute_ui_pipe_smem_bytes() {
-    return (size_t)pipe_kmax(TJ) * (TJ + 1) * 32 * sizeof(double2) + (size_t)2 * kPipeCap * 5 * 32 * sizeof(double) +
-           (size_t)kPipeCap * 6 * sizeof(double) + 16;
+    return (size_t)pipe_kmax(TJ) * (TJ + 1) * 32 * sizeof(double2) + (size_t)2 * pipe_cap(TJ) * 5 * 32 * sizeof(double) +
+           (size_t)kPipeWin * 6 * sizeof(double) + 16;
 }
 
 }  // namespace mala
