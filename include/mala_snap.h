@@ -178,6 +178,28 @@ int mala_gaussian_grid(mala_snap_t *h, double sigma, int natoms, const double *p
                        void *cuda_stream);
 
 /*
+ * mala_gaussian_grid for callers that must not allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): same arguments, same result up to rounding, but the call makes no cudaMalloc /
+ * cudaMallocAsync / cudaFree and uses no allocating library routine.  Its scratch (ghost atoms, cell list, counters and the
+ * neighbor-candidate lists of tile_bin_kernel) is a file-scope static device array of MALA_SNAP_STATIC_SCRATCH_BYTES (16 MiB)
+ * that every GPU loading the library holds until exit; the handle resolves its device address once, in mala_snap_create.
+ *   limit    the ghost atoms of the slab (32 bytes each), the cell list (4 bytes per cell) and the candidate lists of one
+ *            tile per SM must fit the array; the grid is then walked in as many chunks as it takes.  Beyond that the call
+ *            returns MALA_SNAP_EINVAL with the byte counts in mala_last_error() and enqueues nothing: use
+ *            mala_gaussian_grid, or smaller z-slabs.  Config 2 (256 atoms, 90^3 points) needs about 3 % of the array.
+ *   sharing  ONE array per GPU (and process), shared by every handle and every call of this entry point, and it keeps the
+ *            last call's contents (the call clears the counters that must start at zero).  Calls on one handle are
+ *            serialised as everywhere else, but calls on DIFFERENT handles of one process that overlap on the GPU race on
+ *            the array: order them (one stream, or events).
+ * The device of the handle must be current (MALA_SNAP_EINVAL otherwise).  Host memory (the ghost list) is still taken from
+ * the C++ heap; positions are read from pageable host memory as in every other entry point.
+ */
+#define MALA_SNAP_STATIC_SCRATCH_BYTES (16u << 20)
+int mala_gaussian_grid_static(mala_snap_t *h, double sigma, int natoms, const double *pos, const int *types, const double box[9],
+                              const double origin[3], const int pbc[3], const int ngrid[3], int z_begin, int z_end, double *out,
+                              void *cuda_stream);
+
+/*
  * Tuning / test knobs.  Unknown names give MALA_SNAP_EINVAL.
  *   "zi_impl"          0 = automatic (register-tiled block kernel up to twojmax 10, anti-diagonal kernel on half tiles above),
  *                      1 = generic table-driven kernel (twojmax <= 10), 2 = per-triple specialised kernel (EINVAL if

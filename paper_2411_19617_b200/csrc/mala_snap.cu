@@ -43,6 +43,13 @@ namespace mala {
 int set_error(int code, const std::string &msg) { return fail(code, msg); }
 }  // namespace mala
 
+// Scratch of mala_gaussian_grid_static, the entry point that allocates nothing: ghost atoms, cell list, counters and the
+// candidate lists of tile_bin_kernel live here instead of in the handle's stream-ordered workspace.  Every GPU that loads the
+// library holds these bytes until exit.  In host code the name is a stand-in, not a device address: mala_snap_create resolves
+// it once per handle (= per device, with that device current) through cudaGetSymbolAddress.
+constexpr size_t kStaticScratchBytes = (size_t)16 << 20;
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+
 #define CUDA_TRY(call)                                                                              \
     do {                                                                                            \
         cudaError_t e_ = (call);                                                                    \
@@ -102,6 +109,7 @@ struct mala_snap {
     SnapTables tab;
     SnapConst sc{};
     int device = 0, num_sms = 0;
+    unsigned char *static_scratch = nullptr;   // device address of g_static_scratch on this handle's device
     // options
     int zi_impl = 0;
     int ui_impl = 0;   // 0 automatic (sampling kernel for twojmax 1..10, pipelined from 8 up), 1 column kernel, 2 sampling kernel, 3 pipelined sampling kernel
@@ -727,14 +735,14 @@ int validate(const mala_snap *h, const CallArgs &a, bool need_out, const void *o
     return 0;
 }
 
-// Ghost atoms + cell list for the slab [z_begin, z_end); fills h->geom (except the tile fields).
-int build_plan(mala_snap *h, const CallArgs &a, cudaStream_t st) {
+// Host half of build_plan: ghost atoms sorted by cell and the cell starts of the slab [z_begin, z_end); fills h->geom (except
+// the tile fields) and picks the buffer set of the call.
+int plan_host(mala_snap *h, const CallArgs &a, std::vector<Ghost> &sorted, std::vector<int> &start) {
     GridGeom &g = h->geom;
     h->spans.clear();
     h->ev_used = 0;
     h->cur = (int)(h->ncalls & 1ull);
     h->ncalls++;
-    const int cur = h->cur;
     std::memset(&g, 0, sizeof(g));
     for (int k = 0; k < 3; k++) {
         g.a1[k] = a.box[k]; g.a2[k] = a.box[3 + k]; g.a3[k] = a.box[6 + k]; g.origin[k] = a.origin[k];
@@ -823,7 +831,8 @@ int build_plan(mala_snap *h, const CallArgs &a, cudaStream_t st) {
     }
     g.ncx = nc[0]; g.ncy = nc[1]; g.ncz = nc[2];
     const size_t ncell = (size_t)nc[0] * nc[1] * nc[2];
-    std::vector<int> cell_of(ng), start(ncell + 1, 0);
+    std::vector<int> cell_of(ng);
+    start.assign(ncell + 1, 0);
     auto cidx = [&](double v, int d) {
         int i = (int)std::floor((v - g.cell_lo[d]) * g.cell_inv[d]);
         return std::min(std::max(i, 0), nc[d] - 1);
@@ -834,11 +843,22 @@ int build_plan(mala_snap *h, const CallArgs &a, cudaStream_t st) {
         start[c + 1]++;
     }
     for (size_t c = 0; c < ncell; c++) start[c + 1] += start[c];
-    std::vector<Ghost> sorted(ng);
+    sorted.resize(ng);
     {
         std::vector<int> fill(start.begin(), start.end() - 1);
         for (size_t i = 0; i < ng; i++) sorted[fill[cell_of[i]]++] = ghosts[i];
     }
+    return 0;
+}
+
+// Ghost atoms + cell list for the slab [z_begin, z_end) on the device; fills h->geom (except the tile fields).
+int build_plan(mala_snap *h, const CallArgs &a, cudaStream_t st) {
+    std::vector<Ghost> sorted;
+    std::vector<int> start;
+    int rc = plan_host(h, a, sorted, start);
+    if (rc) return rc;
+    const int cur = h->cur;
+    const size_t ng = sorted.size(), ncell = start.size() - 1;
     // The workspace (U_tot, candidate lists, counters) is one set per handle: a call on another stream must not start
     // before the previous call on this handle has drained (calls on one handle are serialised, whatever their streams).
     if (h->call_done_valid[cur ^ 1]) CUDA_TRY(cudaStreamWaitEvent(st, h->ev_call_done[cur ^ 1], 0));
@@ -1519,6 +1539,7 @@ int mala_snap_create(mala_snap_t **handle, int twojmax, double rcutfac, double r
         CUDA_TRY(cudaGetDeviceProperties(&prop, h->device));
         if (prop.major < 10) return fail(MALA_SNAP_ECUDA, "device is not sm_100 class (kernels are built for sm_100a only)");
         h->num_sms = prop.multiProcessorCount;
+        CUDA_TRY(cudaGetSymbolAddress((void **)&h->static_scratch, g_static_scratch));
         h->tab = build_tables(twojmax);
         h->sc.twojmax = twojmax; h->sc.ntriples = h->tab.ntriples; h->sc.nelem = h->tab.nelem; h->sc.ntypes = ntypes;
         h->sc.rfac0 = rfac0; h->sc.rmin0 = rmin0; h->sc.wself = wself;
@@ -1903,6 +1924,86 @@ int mala_gaussian_grid(mala_snap_t *h, double sigma, int natoms, const double *p
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if ((rc = build_plan(h, a, st))) return rc;
     if ((rc = run_slab_gauss(h, z_begin, z_end, sigma, out, st))) return rc;
+    return finish_call(h, st);
+}
+
+int mala_gaussian_grid_static(mala_snap_t *h, double sigma, int natoms, const double *pos, const int *types, const double box[9],
+                              const double origin[3], const int pbc[3], const int ngrid[3], int z_begin, int z_end, double *out,
+                              void *cuda_stream) {
+    const CallArgs a{natoms, pos, types, box, origin, pbc, ngrid, z_begin, z_end};
+    int rc = validate(h, a, true, out);
+    if (rc) return rc;
+    if ((rc = check_status(h, false))) return rc;
+    if (!(sigma > 0.0) || !std::isfinite(sigma)) return fail(MALA_SNAP_EINVAL, "sigma must be positive");
+    if (h->ntypes > kGaussMaxTypes) return fail(MALA_SNAP_EINVAL, "mala_gaussian_grid_static supports at most 4 atom types");
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev != h->device || !h->static_scratch) return fail(MALA_SNAP_EINVAL, "mala_gaussian_grid_static: the handle's device is not current");
+    std::fill(h->stats, h->stats + 8, 0LL);
+    if (z_end == z_begin) return MALA_SNAP_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    std::vector<Ghost> sorted;   // host memory only
+    std::vector<int> start;
+    if ((rc = plan_host(h, a, sorted, start))) return rc;
+    const size_t ng = sorted.size(), ncell1 = start.size();
+    h->h_cell_start.swap(start);   // candidate_bound reads the cell counts of this call
+    choose_tiles(h, z_begin, z_end);
+    const GridGeom &g = h->geom;
+    h->cand_cap = candidate_bound(h);
+    if (h->cand_cap < 0) return fail(MALA_SNAP_EINVAL, "more than 2^24 candidate atoms per tile; use a finer cell or smaller z-slabs");
+    const long long total_tiles = h->total_tiles;
+    if (total_tiles > 2000000000LL) return fail(MALA_SNAP_EINVAL, "slab has too many tiles; use smaller z-slabs");
+    // carve the static array: ghosts | cell starts | counters | per-tile lists of one chunk (every piece 256-byte aligned)
+    auto up = [](size_t n) { return (n + 255) & ~(size_t)255; };
+    const size_t off_cells = up(std::max<size_t>(ng, 1) * sizeof(Ghost)), off_counters = off_cells + up(ncell1 * sizeof(int));
+    const size_t off_tiles = off_counters + 256;
+    const size_t per_tile = (size_t)h->cand_cap * sizeof(int) + 2 * sizeof(int);
+    const long long want_tiles = std::min<long long>(total_tiles, h->num_sms);   // smallest chunk worth launching
+    if (off_tiles + 768 + (size_t)want_tiles * per_tile > kStaticScratchBytes) {
+        char msg[320];
+        std::snprintf(msg, sizeof msg, "mala_gaussian_grid_static: %zu ghost atoms, %zu cells and the candidate lists of %lld tiles (%d entries "
+                      "each) need %zu bytes, the static scratch holds %zu; use mala_gaussian_grid or smaller z-slabs",
+                      ng, ncell1 - 1, want_tiles, h->cand_cap, off_tiles + 768 + (size_t)want_tiles * per_tile, kStaticScratchBytes);
+        return fail(MALA_SNAP_EINVAL, msg);
+    }
+    const long long chunk_tiles = std::min<long long>(total_tiles, (long long)((kStaticScratchBytes - off_tiles - 768) / per_tile));
+    unsigned char *base = h->static_scratch;
+    Ghost *d_ghosts = reinterpret_cast<Ghost *>(base);
+    int *d_cells = reinterpret_cast<int *>(base + off_cells), *d_counters = reinterpret_cast<int *>(base + off_counters);
+    int *d_ncand = reinterpret_cast<int *>(base + off_tiles);
+    int *d_active = reinterpret_cast<int *>(base + off_tiles + up((size_t)chunk_tiles * sizeof(int)));
+    int *d_cand = reinterpret_cast<int *>(base + off_tiles + 2 * up((size_t)chunk_tiles * sizeof(int)));
+    // calls on one handle are serialised whatever their streams (status word, geometry); the scratch itself is shared by every
+    // handle of the device: calls that overlap on the GPU race (see include/mala_snap.h)
+    if (h->call_done_valid[h->cur ^ 1]) CUDA_TRY(cudaStreamWaitEvent(st, h->ev_call_done[h->cur ^ 1], 0));
+    if (h->call_done_valid[h->cur]) CUDA_TRY(cudaStreamWaitEvent(st, h->ev_call_done[h->cur], 0));
+    // pageable sources: cudaMemcpyAsync returns once they are staged, so the vectors may die with this scope
+    if (ng) CUDA_TRY(cudaMemcpyAsync(d_ghosts, sorted.data(), ng * sizeof(Ghost), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(d_cells, h->h_cell_start.data(), ncell1 * sizeof(int), cudaMemcpyHostToDevice, st));
+    h->stats[3] = (long long)ng;
+    const double pi = 3.14159265358979323846;
+    const double pref = 1.0 / (std::pow(2.0 * pi, 1.5) * sigma * sigma * sigma), inv2s2 = 1.0 / (2.0 * sigma * sigma);
+    const DeviceTables tb = h->tables();
+    for (long long t0 = 0; t0 < total_tiles; t0 += chunk_tiles) {
+        ChunkBuffers cb{};
+        cb.ghosts = d_ghosts; cb.cell_start = d_cells;
+        cb.cand = d_cand; cb.ncand = d_ncand; cb.active = d_active; cb.counters = d_counters;
+        cb.status = h->d_status.p;
+        cb.cand_cap = h->cand_cap;
+        cb.tile_begin = (int)t0;
+        cb.ntiles = (int)std::min(chunk_tiles, total_tiles - t0);
+        CUDA_TRY(cudaMemsetAsync(cb.counters, 0, 4 * sizeof(int), st));   // the array keeps the last call's contents
+        const int blocks = (cb.ntiles + 7) / 8;
+        tile_bin_kernel<<<blocks, 256, 0, st>>>(g, h->sc, tb, cb, nullptr);
+        CUDA_TRY(cudaGetLastError());
+        gaussian_grid_kernel<<<blocks, 256, 0, st>>>(g, h->sc, tb, cb, inv2s2, pref, out);
+        CUDA_TRY(cudaGetLastError());
+        h->stats[0] += 2;
+        h->stats[1]++;
+    }
+    h->stats[2] += total_tiles;
+    h->stats[4] = h->cand_cap;
+    h->stats[6] += (long long)g.nx * g.ny * (z_end - z_begin);
     return finish_call(h, st);
 }
 

@@ -20,7 +20,7 @@ MALA_SNAP_ECUDA = -2
 MALA_SNAP_ENOMEM = -3
 
 EXPORTS = ("mala_snap_create", "mala_snap_ncomp", "mala_snap_triples", "mala_bispectrum_grid", "mala_bispectrum_grid_host",
-           "mala_gaussian_grid", "mala_mlp_create", "mala_mlp_widths", "mala_mlp_forward", "mala_mlp_destroy", "mala_bispectrum_ldos_grid", "mala_bispectrum_force_adjoint",
+           "mala_gaussian_grid", "mala_gaussian_grid_static", "mala_mlp_create", "mala_mlp_widths", "mala_mlp_forward", "mala_mlp_destroy", "mala_bispectrum_ldos_grid", "mala_bispectrum_force_adjoint",
            "mala_snap_set_option", "mala_snap_last_stats", "mala_snap_kernel_times", "mala_snap_zi_kernel", "mala_snap_fp64_peak", "mala_snap_clebsch_gordan", "mala_snap_debug_utot",
            "mala_snap_destroy", "mala_last_error")
 
@@ -63,6 +63,8 @@ def load_library():
     lib.mala_bispectrum_grid_host.argtypes = grid_args
     lib.mala_gaussian_grid.restype = C.c_int
     lib.mala_gaussian_grid.argtypes = [vp, C.c_double] + grid_args[1:]
+    lib.mala_gaussian_grid_static.restype = C.c_int
+    lib.mala_gaussian_grid_static.argtypes = [vp, C.c_double] + grid_args[1:]
     lib.mala_mlp_create.restype = C.c_int
     lib.mala_mlp_create.argtypes = [C.POINTER(vp), C.c_int, ip, C.POINTER(dp), C.POINTER(dp), C.c_int, C.c_int, dp, dp]
     lib.mala_mlp_widths.restype = C.c_int
@@ -250,6 +252,20 @@ class MalaSnap:
         s = torch.cuda.current_stream() if stream is None else stream
         _check(self._lib.mala_gaussian_grid(self._h, C.c_double(float(sigma)), *args, C.c_void_p(out.data_ptr()),
                                             C.c_void_p(s.cuda_stream)))
+        return out
+
+    # -- mala_gaussian_grid_static: the same descriptors through the entry point that allocates no device memory
+    def gaussian_grid_static(self, sigma, pos, types, box, origin=(0, 0, 0), pbc=(1, 1, 1), ngrid=(1, 1, 1), z_begin=0, z_end=None,
+                             out=None, stream=None):
+        import torch
+        args, keep, npts = self._system(pos, types, box, origin, pbc, ngrid, z_begin, z_end)
+        if out is None:   # the caller of the C entry point owns the output; here torch allocates it before the call
+            out = torch.empty((npts, self.ntypes), dtype=torch.float64, device="cuda")
+        if (not out.is_cuda) or out.dtype != torch.float64 or (not out.is_contiguous()) or out.numel() < npts * self.ntypes:
+            raise ValueError("out must be a contiguous CUDA float64 tensor with at least npoints*ntypes elements")
+        s = torch.cuda.current_stream() if stream is None else stream
+        _check(self._lib.mala_gaussian_grid_static(self._h, C.c_double(float(sigma)), *args, C.c_void_p(out.data_ptr()),
+                                                   C.c_void_p(s.cuda_stream)))
         return out
 
     # -- mala_bispectrum_force_adjoint: g[atom, k] += sum_points sum_j beta[point, j] dB_j(point)/dR_{atom,k}
