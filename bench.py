@@ -93,6 +93,8 @@ def parse_args():
                    help="SURVEY 8(f) f3: the adjoint of the descriptor map (mala_bispectrum_force_adjoint), a separate metric line")
     p.add_argument("--zi-impl", type=int, default=0,
                    help="compute_zi kernel: 0 automatic, 1 table-driven, 2 per-triple (twojmax 10), 3 anti-diagonal, 4 register-tiled blocks")
+    p.add_argument("--ui-impl", type=int, default=0,
+                   help="compute_ui kernel: 0 automatic, 1 column, 2 sampling (twojmax 1..10), 3 pipelined sampling (twojmax 8..14)")
     p.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
     p.add_argument("--no-e2e", action="store_true", help="skip the host-output leg (profiling runs)")
     args = p.parse_args()
@@ -340,6 +342,8 @@ def run_native(args, w, rank, world, local):
     assert snap.ncomp == nt
     if args.zi_impl:
         snap.set_option("zi_impl", args.zi_impl)
+    if args.ui_impl:
+        snap.set_option("ui_impl", args.ui_impl)
     stream = torch.cuda.current_stream()
     out = torch.empty((max(npts, 1), nt), dtype=torch.float64, device=dev)
     call = lambda: snap.bispectrum_grid(w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, z0, z1, out=out, stream=stream)

@@ -595,7 +595,11 @@ int build_block_schedule(mala_snap *h) {
 
 // enqueue the sampling compute_ui (snap_ui_dft.cuh) for one chunk: whole tiles, twojmax + 1 warps
 void launch_ui_dft(mala_snap *h, const GridGeom &g, const DeviceTables &tb, const ChunkBuffers &cb, cudaStream_t st) {
-    if (h->use_ui_pipe()) {   // twojmax 8..10: one CTA per SM, a producer warp ahead of the sample warps (snap_ui_pipe.cuh)
+    // Dense systems (config 5: 46 neighbors per point) overflow the pipelined kernel's queue of 40 entries per point: every tile
+    // then comes in several windows, each prepared once per accumulation pass by the one producer warp, and the sampling kernel
+    // (all warps share that work) is faster.  The host sees the candidate bound, about seven times the neighbors per point.
+    const bool dense = !h->half_tiles() && h->ui_impl == 0 && h->cand_cap > 6 * pipe_cap(h->twojmax);
+    if (h->use_ui_pipe() && !dense) {   // twojmax 8..14: one CTA per SM, a producer warp ahead of the sample warps (snap_ui_pipe.cuh)
         const int grid = std::max(1, std::min(h->num_sms, cb.ntiles));
         switch (h->twojmax) {
 #define MALA_PIPE_CASE(TJ) \

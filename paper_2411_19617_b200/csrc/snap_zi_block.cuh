@@ -315,6 +315,9 @@ compute_zi_bi_block_kernel(GridGeom g, SnapConst sc, DeviceTables tb, BlkTables 
 // twojmax 11..14: half tiles (16 points).  U_tot of the half tile (up to 167 KB at twojmax 14), the partial-sum slots and the
 // rings fill the shared memory, so there is no staging of B: the sums of the slots go straight to global memory, a row of
 // ntriples doubles per grid point.
+#ifndef MALA_BLK_HALF_PEEL
+#define MALA_BLK_HALF_PEEL true
+#endif
 __global__ void __launch_bounds__(kBlkWarps * 32, 1)
 compute_zi_bi_block_half_kernel(GridGeom g, SnapConst sc, DeviceTables tb, BlkTables T, ChunkBuffers cb, double *out) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -366,7 +369,7 @@ compute_zi_bi_block_half_kernel(GridGeom g, SnapConst sc, DeviceTables tb, BlkTa
         parity ^= 1u;
         __syncthreads();  // P zeroed, s_dst written
         const unsigned char *Ulane = reinterpret_cast<const unsigned char *>(U + (lane & 15));
-        blk_run_all<kBlkBX, kBlkBY, true, true>(Ulane, T, warp, lane, rd, P);
+        blk_run_all<kBlkBX, kBlkBY, MALA_BLK_HALF_PEEL, true>(Ulane, T, warp, lane, rd, P);
         __syncthreads();
         for (int i = threadIdx.x; i < 16 * nt; i += NW * 32) {   // fixed-order sum of the slots of triple t, point p
             const int p = i / nt, t = i - p * nt;
