@@ -201,14 +201,17 @@ int mala_gaussian_grid_static(mala_snap_t *h, double sigma, int natoms, const do
 
 /*
  * Tuning / test knobs.  Unknown names give MALA_SNAP_EINVAL.
- *   "zi_impl"          0 = automatic (register-tiled block kernel up to twojmax 10, anti-diagonal kernel on half tiles above),
+ *   "zi_impl"          0 = automatic (register-tiled block kernel; on 16-point half tiles above twojmax 10),
  *                      1 = generic table-driven kernel (twojmax <= 10), 2 = per-triple specialised kernel (EINVAL if
  *                      twojmax != 10), 3 = anti-diagonal kernel (code specialised on j1 only, any twojmax), 4 = block kernel
- *                      (twojmax <= 10).  All tables but the per-triple kernel's are per-handle arrays in global memory, so
+ *                      (any twojmax).  All tables but the per-triple kernel's are per-handle arrays in global memory, so
  *                      handles of different twojmax coexist.  Every kernel gives the same B up to rounding (summation order).
- *   "ui_impl"          0 = automatic (sampling kernel for twojmax 1..10: column polynomials evaluated at the roots of unity,
- *                      sums in registers, inverse DFT per tile; column kernel otherwise), 1 = column kernel (polynomial
- *                      recursion, accumulators in shared memory; any twojmax), 2 = sampling kernel (EINVAL outside 1..10)
+ *   "ui_impl"          0 = automatic (twojmax 8..14: pipelined sampling kernel, except that at twojmax <= 10 a call whose
+ *                      candidate bound is large -- a dense system -- takes the sampling kernel; twojmax 1..7: sampling kernel;
+ *                      twojmax 0: column kernel), 1 = column kernel (polynomial recursion, accumulators in shared memory; any
+ *                      twojmax), 2 = sampling kernel (column polynomials evaluated at the roots of unity, sums in registers,
+ *                      inverse DFT per tile; EINVAL outside 1..10), 3 = pipelined sampling kernel (a producer warp prepares
+ *                      the neighbor queue of the next tile; EINVAL below 8)
  *   "yi_impl"          compute_yi of mala_bispectrum_force_adjoint: 0 = register-tiled block kernel (default), 1 = table-driven
  *                      kernel (element by element)
  *   "timing"           1 = record a CUDA-event pair on the caller's stream around every kernel launch of the
