@@ -206,8 +206,7 @@ int mala_gaussian_grid_static(mala_snap_t *h, double sigma, int natoms, const do
  *                      twojmax != 10), 3 = anti-diagonal kernel (code specialised on j1 only, any twojmax), 4 = block kernel
  *                      (any twojmax).  All tables but the per-triple kernel's are per-handle arrays in global memory, so
  *                      handles of different twojmax coexist.  Every kernel gives the same B up to rounding (summation order).
- *   "ui_impl"          0 = automatic (twojmax 8..14: pipelined sampling kernel, except that at twojmax <= 10 a call whose
- *                      candidate bound is large -- a dense system -- takes the sampling kernel; twojmax 1..7: sampling kernel;
+ *   "ui_impl"          0 = automatic (twojmax 8..14: pipelined sampling kernel; twojmax 1..7: sampling kernel;
  *                      twojmax 0: column kernel), 1 = column kernel (polynomial recursion, accumulators in shared memory; any
  *                      twojmax), 2 = sampling kernel (column polynomials evaluated at the roots of unity, sums in registers,
  *                      inverse DFT per tile; EINVAL outside 1..10), 3 = pipelined sampling kernel (a producer warp prepares

@@ -147,6 +147,7 @@ struct mala_snap {
     int cur = 0;  // buffer set of the current call
     std::vector<int> h_cell_start;
     DevBuf<int> d_cand, d_ncand, d_active, d_counters;
+    DevBuf<double> d_uispill;   // compute_ui_pipe_kernel: window geometry of multi-window tiles, per CTA
     DevBuf<int> d_status;          // kStatus* bits raised by the kernels; never cleared by a chunk
     int *h_status = nullptr;       // pinned mirror, refreshed at the end of every call
     int sticky_status = 0;         // bits seen so far (a raised bit makes every later call fail)
@@ -594,13 +595,21 @@ int build_block_schedule(mala_snap *h) {
 }
 
 // enqueue the sampling compute_ui (snap_ui_dft.cuh) for one chunk: whole tiles, twojmax + 1 warps
-void launch_ui_dft(mala_snap *h, const GridGeom &g, const DeviceTables &tb, const ChunkBuffers &cb, cudaStream_t st) {
-    // Dense systems (config 5: 46 neighbors per point) overflow the pipelined kernel's queue of 40 entries per point: every tile
-    // then comes in several windows, each prepared once per accumulation pass by the one producer warp, and the sampling kernel
-    // (all warps share that work) is faster.  The host sees the candidate bound, about seven times the neighbors per point.
-    const bool dense = !h->half_tiles() && h->ui_impl == 0 && h->cand_cap > 6 * pipe_cap(h->twojmax);
-    if (h->use_ui_pipe() && !dense) {   // twojmax 8..14: one CTA per SM, a producer warp ahead of the sample warps (snap_ui_pipe.cuh)
+int launch_ui_dft(mala_snap *h, const GridGeom &g, const DeviceTables &tb, const ChunkBuffers &cb_in, cudaStream_t st) {
+    ChunkBuffers cb = cb_in;
+    if (h->use_ui_pipe()) {   // twojmax 8..14: one CTA per SM, a producer warp ahead of the sample warps (snap_ui_pipe.cuh)
         const int grid = std::max(1, std::min(h->num_sms, cb.ntiles));
+        // A tile with more than 64 candidates, or a point with more neighbors than a queue buffer holds, comes in several windows
+        // and once per accumulation pass: the producer keeps the geometry of the first pass in global memory (per CTA, at most
+        // cand_cap / queue length windows; L2-resident) instead of preparing it again.
+        const int cap = pipe_cap(h->twojmax);
+        if (h->cand_cap > cap) {
+            const int windows = std::min(16, (h->cand_cap + cap - 1) / cap);
+            if (h->d_uispill.reserve((size_t)h->num_sms * windows * pipe_spill_record(h->twojmax), st, true))
+                return fail(MALA_SNAP_ENOMEM, "cudaMallocAsync (compute_ui window spill) failed");
+            cb.ui_spill = h->d_uispill.p;
+            cb.ui_spill_windows = windows;
+        }
         switch (h->twojmax) {
 #define MALA_PIPE_CASE(TJ) \
     case TJ: compute_ui_pipe_kernel<TJ><<<grid, (TJ + 2) * 32, compute_ui_pipe_smem_bytes<TJ>(), st>>>(g, h->sc, tb, cb); break;
@@ -608,7 +617,7 @@ void launch_ui_dft(mala_snap *h, const GridGeom &g, const DeviceTables &tb, cons
 #undef MALA_PIPE_CASE
             default: break;
         }
-        return;
+        return 0;
     }
     switch (h->twojmax) {
 #define MALA_DFT_CASE(TJ) \
@@ -620,6 +629,7 @@ void launch_ui_dft(mala_snap *h, const GridGeom &g, const DeviceTables &tb, cons
 #undef MALA_DFT_CASE
         default: break;
     }
+    return 0;
 }
 
 // enqueue compute_zi_bi for one chunk
@@ -1048,15 +1058,15 @@ int run_slab(mala_snap *h, int z0, int z1, double *out, double2 *u_out, cudaStre
         {
             TimedSpan span(h, st, kKindUi);
             if (h->half_tiles() && h->use_ui_pipe()) {  // twojmax 11..14: the pipelined sampling kernel, whole tiles stored as two halves
-                launch_ui_dft(h, g, tb, cb, st);
+                if (int rc = launch_ui_dft(h, g, tb, cb, st)) return rc;
             } else if (h->half_tiles()) {  // the column kernel: eight column warps, one CTA per SM
                 const int ui_grid = std::max(1, std::min(h->num_sms, 2 * cb.ntiles));
                 compute_ui_kernel<kMaxTwoJ, false><<<ui_grid, (kMaxTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kMaxTwoJ), st>>>(g, h->sc, tb, cb);
             } else {
                 const int ui_grid = std::max(1, std::min(2 * h->num_sms, 2 * cb.ntiles));  // half-tile items, two CTAs per SM
-                if (h->use_ui_dft())   // twojmax 1..10: column polynomials sampled at the roots of unity (snap_ui_dft.cuh), whole tiles
-                    launch_ui_dft(h, g, tb, cb, st);
-                else if (h->twojmax == kFullTileTwoJ)
+                if (h->use_ui_dft()) {   // twojmax 1..10: column polynomials sampled at the roots of unity (snap_ui_dft.cuh), whole tiles
+                    if (int rc = launch_ui_dft(h, g, tb, cb, st)) return rc;
+                } else if (h->twojmax == kFullTileTwoJ)
                     compute_ui_kernel<kFullTileTwoJ, true><<<ui_grid, (kFullTileTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kFullTileTwoJ), st>>>(g, h->sc, tb, cb);
                 else  // smaller twojmax: same code with run-time guards on the levels
                     compute_ui_kernel<kFullTileTwoJ, false><<<ui_grid, (kFullTileTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kFullTileTwoJ), st>>>(g, h->sc, tb, cb);
@@ -1416,9 +1426,9 @@ int run_slab_force(mala_snap *h, int z0, int z1, const double *beta, double *gou
         const int grid2 = std::max(1, std::min(2 * h->num_sms, 2 * cb.ntiles));
         {
             TimedSpan span(h, st, kKindUi);
-            if (h->use_ui_dft())
-                launch_ui_dft(h, g, tb, cb, st);
-            else if (h->twojmax == kFullTileTwoJ)
+            if (h->use_ui_dft()) {
+                if (int rc = launch_ui_dft(h, g, tb, cb, st)) return rc;
+            } else if (h->twojmax == kFullTileTwoJ)
                 compute_ui_kernel<kFullTileTwoJ, true><<<grid2, (kFullTileTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kFullTileTwoJ), st>>>(g, h->sc, tb, cb);
             else
                 compute_ui_kernel<kFullTileTwoJ, false><<<grid2, (kFullTileTwoJ / 2 + 1) * 32, compute_ui_smem_bytes(kFullTileTwoJ), st>>>(g, h->sc, tb, cb);
@@ -2041,7 +2051,7 @@ void mala_snap_destroy(mala_snap_t *h) {
         if (h->ev_done[i]) cudaEventDestroy(h->ev_done[i]);
         if (h->ev_copied[i]) cudaEventDestroy(h->ev_copied[i]);
     }
-    h->d_cand.release(); h->d_ncand.release(); h->d_active.release(); h->d_counters.release(); h->d_utot.release();
+    h->d_cand.release(); h->d_ncand.release(); h->d_active.release(); h->d_counters.release(); h->d_utot.release(); h->d_uispill.release();
     h->d_status.release(); h->d_bstage.release();
     h->d_yterms.release(); h->d_ylevel.release(); h->d_yorder.release(); h->d_ycg.release(); h->d_yweight.release(); h->d_ytot.release();
     h->d_dcg.release(); h->d_dtriple.release(); h->d_dsched.release(); h->d_ditems.release();

@@ -76,6 +76,8 @@ struct ChunkBuffers {
     int compact_out;         // 1: descriptors go to out[(local tile) * 32 + lane][ncomp] (staging for the fused network)
                              //    instead of out[grid point][ncomp]
     int cand_cap;
+    double *ui_spill;        // compute_ui_pipe_kernel: per CTA, the pair geometry of the first ui_spill_windows windows of a tile that
+    int ui_spill_windows;    // comes in several (kept for the later accumulation passes); nullptr / 0: every pass prepares them again
     int tile_begin;          // first global tile id of the chunk
     int ntiles;              // tiles in the chunk
 };

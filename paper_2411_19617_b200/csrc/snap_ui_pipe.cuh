@@ -27,6 +27,8 @@ constexpr int kPipeMaxPass = 5;
 
 // entries of a queue buffer per grid point (a window is cut short where a point would get more)
 constexpr int pipe_cap(int tj) { return tj >= 14 ? 32 : 40; }
+// doubles of one window kept in global memory for the later passes of a tile: its queue buffer, then the 32 entry counts
+constexpr int pipe_spill_record(int tj) { return pipe_cap(tj) * 5 * 32 + 32; }
 // columns whose sums a thread keeps in registers during one pass: whole chains (all n of one mb), as many as fit
 constexpr int pipe_klim(int tj) { return tj <= 10 ? 20 : (tj == 11 ? 18 : 16); }
 // first chain of pass p (p = number of passes: one past the last chain)
@@ -241,6 +243,9 @@ compute_ui_pipe_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers c
 
     if (warp == NW) {
         // ---------------------------------------------------------------- producer: lane = grid point
+        constexpr int REC = pipe_spill_record(TJ);
+        const int wmax = cb.ui_spill ? cb.ui_spill_windows : 0;
+        double *spill = wmax ? cb.ui_spill + (size_t)blockIdx.x * (size_t)wmax * REC : nullptr;
         uint32_t it = 0;   // buffers handed over so far
         for (;;) {
             int slot = 0;
@@ -263,9 +268,32 @@ compute_ui_pipe_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers c
             const int nc = cb.ncand[wt];
             const int *mycand = cb.cand + (size_t)wt * cb.cand_cap;
             int rounds = 1;   // a tile of several windows is sent once per pass
+            int nkept = 0, wbase_kept = 0;   // windows of this tile kept in global memory, the candidate they end at
+            bool kept_all = false;
             for (int round = 0; round < rounds; round++) {
-                int wbase = 0;
-                bool last;
+                int wbase = 0, win = 0;
+                bool last = false;
+                if (round > 0 && nkept > 0) {
+                    // later passes: the windows kept in round 0 come back from global memory (each lane reads what it wrote)
+                    for (; win < nkept; win++, it++) {
+                        const double *src = spill + (size_t)win * REC;
+                        const int cnt = reinterpret_cast<const int *>(src + GEO)[lane];
+                        const int buf = it & 1;
+                        mbar_wait(&empty[buf], ((it >> 1) & 1) ^ 1);
+                        double *gq = geo + (size_t)buf * GEO + lane;
+                        const double *sq = src + lane;
+                        for (int e = 0; e < cnt; e++, gq += 5 * 32, sq += 5 * 32) {
+                            const double c = sq[0], ar = sq[32], ai = sq[64], br = sq[96], bi = sq[128];
+                            gq[0] = c; gq[32] = ar; gq[64] = ai; gq[96] = br; gq[128] = bi;
+                        }
+                        s_cnt[buf][lane] = cnt;
+                        last = kept_all && win == nkept - 1;
+                        if (lane == 0) { s_meta[buf][0] = slot; s_meta[buf][1] = last ? 1 : 0; }
+                        mbar_arrive(&full[buf]);
+                    }
+                    if (kept_all) continue;
+                    wbase = wbase_kept;
+                }
                 do {
                     int nw = min(kPipeWin, nc - wbase);
                     __syncwarp();   // the geometry of the previous window has read crec
@@ -292,18 +320,26 @@ compute_ui_pipe_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers c
                     const int buf = it & 1;
                     mbar_wait(&empty[buf], ((it >> 1) & 1) ^ 1);   // the consumers are done with this buffer
                     double *gq = geo + (size_t)buf * GEO + lane;
-                    for (unsigned long long r = hits; r != 0ull; r &= r - 1ull, gq += 5 * 32) {
+                    const bool keep = round == 0 && rounds > 1 && win < wmax;
+                    double *kq = keep ? spill + (size_t)win * REC + lane : gq;
+                    for (unsigned long long r = hits; r != 0ull; r &= r - 1ull, gq += 5 * 32, kq += 5 * 32) {
                         const double *q = crec + (__ffsll((long long)r) - 1) * 6;
                         const double dx = q[0] - px, dy = q[1] - py, dz = q[2] - pz;
                         const double r2 = dx * dx + dy * dy + dz * dz;
                         double c, ar, ai, br, bi;
                         pair_geometry(dx, dy, dz, r2, q[3], q[4], sc.rfac0, sc.rmin0, c, ar, ai, br, bi);
                         gq[0] = c; gq[32] = ar; gq[64] = ai; gq[96] = br; gq[128] = bi;
+                        if (keep) { kq[0] = c; kq[32] = ar; kq[64] = ai; kq[96] = br; kq[128] = bi; }
                     }
                     s_cnt[buf][lane] = __popcll(hits);
+                    if (keep) {
+                        reinterpret_cast<int *>(spill + (size_t)win * REC + GEO)[lane] = __popcll(hits);
+                        nkept = win + 1; wbase_kept = wbase + nw; kept_all = last;
+                    }
                     if (lane == 0) { s_meta[buf][0] = slot; s_meta[buf][1] = last ? 1 : 0; }
                     mbar_arrive(&full[buf]);
                     it++;
+                    win++;
                     wbase += nw;
                 } while (!last);
             }
