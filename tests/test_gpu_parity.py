@@ -95,7 +95,7 @@ def test_dense_system_several_candidate_windows(twojmax):
     params = dict(twojmax=twojmax, rcutfac=4.2, rfac0=0.99363, rmin0=0.0, wself=1.0, radelem=(0.5, 0.45), wj=(1.0, 0.8))
     ngrid = (5, 6, 3)
     ref = oracle.bispectrum_grid(pos, types, box, (0, 0, 0), (1, 1, 1), ngrid, **params)
-    for ui in ((0, 1, 2, 3) if twojmax <= 10 else (0, 1, 3)):   # 0: automatic (the sampling kernel for a system this dense)
+    for ui in ((0, 1, 2, 3) if twojmax <= 10 else (0, 1, 3)):   # 0: automatic
         with MalaSnap(**params) as snap:
             snap.set_option("ui_impl", ui)
             got = snap.bispectrum_grid(pos, types, box, (0, 0, 0), (1, 1, 1), ngrid)
