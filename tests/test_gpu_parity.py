@@ -103,6 +103,26 @@ def test_dense_system_several_candidate_windows(twojmax):
         assert_parity(got.cpu().numpy(), ref)
 
 
+def test_very_dense_system_more_windows_than_the_spill_keeps():
+    """260 atoms in a 6 A box: about a thousand candidates per tile, i.e. more windows than the 16 whose pair geometry the
+    pipelined compute_ui keeps for its later passes -- the rest is prepared again in every pass"""
+    torch = _torch()
+    rng = np.random.default_rng(4242)
+    box = np.eye(3) * 6.0
+    pos = rng.uniform(0.0, 6.0, size=(260, 3))
+    types = np.zeros(260, np.int32)
+    params = dict(twojmax=8, rcutfac=4.2, rfac0=0.99363, rmin0=0.0, wself=1.0, radelem=(0.5,), wj=(1.0,))
+    ngrid = (4, 4, 2)
+    ref = oracle.bispectrum_grid(pos, types, box, (0, 0, 0), (1, 1, 1), ngrid, **params)
+    for ui in (2, 3):
+        with MalaSnap(**params) as snap:
+            snap.set_option("ui_impl", ui)
+            got = snap.bispectrum_grid(pos, types, box, (0, 0, 0), (1, 1, 1), ngrid)
+            torch.cuda.synchronize()
+            assert snap.last_stats()["cand_cap"] > 16 * 40
+        assert_parity(got.cpu().numpy(), ref)
+
+
 def test_triples_match_oracle_order():
     with MalaSnap(twojmax=10) as s:
         assert s.ncomp == 91
