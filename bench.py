@@ -665,7 +665,8 @@ def run_ldos(args, w, rank, world, local):
 def force_flop_model(twojmax):
     """Algorithmic flops of row f3 per non-empty grid point (compute_yi) and per (grid point, neighbor) pair (compute_dedr),
     counted from the index ranges.  Y^C[ma][mb] over half columns receives, for every bispectrum
-    component (j1, j2, j), the three Z-type contributions (j1, j2) -> j, (j, j2) -> j1 and (j, j1) -> j2: 10 flop per
+    component (j1, j2, j), the Z-type contributions (j1, j2) -> j, (j, j2) -> j1 and (j, j1) -> j2 (the distinct ones: with
+    equal entries two or all three coincide and are computed once): 10 flop per
     product term and 4 per outer step, as for compute_zi.  compute_dedr repeats the U recursion of the pair (F_PAIR) and
     dots every coefficient of levels 0 .. twojmax-1 with two Y columns for the four Cayley-Klein derivatives (4 complex
     multiply-adds = 32 flop) plus the weight sum (8 flop per element of U)."""
@@ -674,7 +675,7 @@ def force_flop_model(twojmax):
     triples = [(j1, j2, j) for j1 in range(tj + 1) for j2 in range(j1 + 1) for j in range(j1 - j2, min(tj, j1 + j2) + 1, 2) if j >= j1]
     terms = outer = 0
     for j1, j2, j in triples:
-        for A, B, C in ((j1, j2, j), (j, j2, j1), (j, j1, j2)):
+        for A, B, C in dict.fromkeys(((j1, j2, j), (j, j2, j1), (j, j1, j2))):   # equal entries: the same contraction once
             sh = (A + B - C) // 2
             for mb in range(C // 2 + 1):
                 mid = (C % 2 == 0) and (mb == C // 2)

@@ -1149,7 +1149,7 @@ int run_slab_gauss(mala_snap *h, int z0, int z1, double sigma, double *out, cuda
 struct YHostTerm { int A, B, C, index; double coef; int cgoff; };
 int build_yi_block_schedule(mala_snap *h, const std::vector<YHostTerm> &terms, const std::vector<double> &cg);
 
-// tables of compute_yi (snap_force.cuh): three Z-type contributions per bispectrum component, grouped by target level
+// tables of compute_yi (snap_force.cuh): the (up to three, distinct) Z-type contributions per bispectrum component, grouped by target level
 int build_force_tables(mala_snap *h) {
     if (h->force_ready) return 0;
     const SnapTables &T = h->tab;
@@ -1158,9 +1158,16 @@ int build_force_tables(mala_snap *h) {
     std::vector<Raw> raw;
     for (int t = 0; t < nt; t++) {
         const int j1 = T.triples[4 * t], j2 = T.triples[4 * t + 1], j = T.triples[4 * t + 2];
-        raw.push_back({j1, j2, j, t, 1.0});
-        raw.push_back({j, j2, j1, t, (double)(j + 1) / (double)(j1 + 1)});
-        raw.push_back({j, j1, j2, t, (double)(j + 1) / (double)(j2 + 1)});
+        // a triple with equal entries names the same contraction more than once (j1 == j2: the last two; j == j1: the first
+        // two): one term with the sum of the coefficients
+        const Raw three[3] = {{j1, j2, j, t, 1.0}, {j, j2, j1, t, (double)(j + 1) / (double)(j1 + 1)}, {j, j1, j2, t, (double)(j + 1) / (double)(j2 + 1)}};
+        const size_t first = raw.size();
+        for (const Raw &r : three) {
+            bool merged = false;
+            for (size_t k = first; k < raw.size() && !merged; k++)
+                if (raw[k].A == r.A && raw[k].B == r.B && raw[k].C == r.C) { raw[k].coef += r.coef; merged = true; }
+            if (!merged) raw.push_back(r);
+        }
     }
     std::stable_sort(raw.begin(), raw.end(), [](const Raw &a, const Raw &b) { return a.C < b.C; });
     std::vector<YTerm> terms;
