@@ -623,17 +623,34 @@ def run_ldos(args, w, rank, world, local):
     roofline["traffic"], roofline["traffic_source"] = ncu_traffic(f"config{w.extra.get('cfg')}/tj{w.twojmax}", "mlp_forward_kernel",
                                                                   mlp_ms / max(mlp_launches, 1))
     host = torch.empty((npts, sizes[-1]), dtype=torch.float32, pin_memory=True)
+    # e2e: the grid in z-slabs of eight planes through the z_begin / z_end arguments of the entry point, the device->host copy
+    # of one slab (a second stream) behind the kernels of the next; calls on one handle are serialised by the library
+    copy_stream = torch.cuda.Stream(device=dev)
+    plane_pts = w.ngrid[0] * w.ngrid[1]
+    slabs_z = [(za, min(za + 8, w.ngrid[2])) for za in range(0, w.ngrid[2], 8)]
+
+    def e2e_step():
+        for za, zb in slabs_z:
+            part = out[za * plane_pts:zb * plane_pts]
+            bispectrum_ldos_grid(snap, net, w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, za, zb, out=part, stream=stream)
+            done = torch.cuda.Event()
+            done.record(stream)
+            copy_stream.wait_event(done)
+            with torch.cuda.stream(copy_stream):
+                host[za * plane_pts:zb * plane_pts].copy_(part, non_blocking=True)
+        torch.cuda.synchronize()
+
+    e2e_step()   # slab-sized workspaces and the copy stream exist before the clock starts
     barrier()
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        call()
-        host.copy_(out, non_blocking=True)
-        torch.cuda.synchronize()
+        e2e_step()
     e2e_s = time.perf_counter() - t0
     e2e_s, e2e_pts = reduce_max_sum(e2e_s, npts * args.steps, world, dev)
     h2d = int(w.pos.nbytes + w.types.nbytes + 9 * 8 + 3 * 8 + 3 * 4 + 3 * 4)
     e2e = {"value": e2e_pts / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": int(npts * sizes[-1] * 4),
-           "ms_per_step": 1e3 * e2e_s / args.steps}
+           "ms_per_step": 1e3 * e2e_s / args.steps,
+           "note": "mala_bispectrum_ldos_grid per z-slab of eight planes: HOST atoms in, pinned HOST LDOS out; D2H of a slab behind the kernels of the next"}
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         import oracle
