@@ -29,6 +29,7 @@
 #include "snap_gauss.cuh"
 #include "snap_force.cuh"
 #include "snap_yi_block.cuh"
+#include "snap_dedr_dft.cuh"
 
 using namespace mala;
 
@@ -163,6 +164,7 @@ struct mala_snap {
     DevBuf<int> d_ybwrange, d_ybpass;
     int yb_npasses = 0, yb_yacc = 0;
     int yi_impl = 0;                  // 0 automatic (block kernel), 1 table-driven kernel
+    int dedr_impl = 0;                // 0 automatic (sampling kernel for twojmax 1..10), 1 column kernel
     YBlkTables yblk_tables() const {
         YBlkTables t;
         t.stream = d_ybstream.p; t.wrange = d_ybwrange.p; t.pass_elem = d_ybpass.p; t.yweight = d_yweight.p;
@@ -1214,6 +1216,11 @@ int build_force_tables(mala_snap *h) {
                                   (int)compute_yi_smem_bytes(uhalf_size(kFullTileTwoJ), triple_count(kFullTileTwoJ))));
     CUDA_TRY(cudaFuncSetAttribute(compute_dedr_kernel<kFullTileTwoJ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   (int)compute_dedr_smem_bytes(kFullTileTwoJ)));
+#define MALA_DD_ATTR(TJ) \
+    CUDA_TRY(cudaFuncSetAttribute(compute_dedr_dft_kernel<TJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)compute_dedr_dft_smem_bytes<TJ>()));
+    MALA_DD_ATTR(1) MALA_DD_ATTR(2) MALA_DD_ATTR(3) MALA_DD_ATTR(4) MALA_DD_ATTR(5)
+    MALA_DD_ATTR(6) MALA_DD_ATTR(7) MALA_DD_ATTR(8) MALA_DD_ATTR(9) MALA_DD_ATTR(10)
+#undef MALA_DD_ATTR
     {
         std::vector<YHostTerm> ht;
         for (const YTerm &y : terms) ht.push_back({y.A, y.B, y.C, y.index, y.coef, y.cgoff});
@@ -1454,8 +1461,21 @@ int run_slab_force(mala_snap *h, int z0, int z1, const double *beta, double *gou
         CUDA_TRY(cudaGetLastError());
         {
             TimedSpan span(h, st, kKindOther);
-            compute_dedr_kernel<kFullTileTwoJ><<<grid2, (kFullTileTwoJ / 2 + 1) * 32, compute_dedr_smem_bytes(kFullTileTwoJ), st>>>(g, h->sc, tb, cb,
-                                                                                                                                 h->d_ytot.p, gout);
+            if (h->dedr_impl == 0 && h->twojmax >= 1) {   // sampling form (snap_dedr_dft.cuh): whole tiles, twojmax + 1 warps
+                switch (h->twojmax) {
+#define MALA_DD_CASE(TJ) \
+    case TJ: \
+        compute_dedr_dft_kernel<TJ><<<std::max(1, std::min(dft_ctas(TJ) * h->num_sms, cb.ntiles)), (TJ + 1) * 32, compute_dedr_dft_smem_bytes<TJ>(), st>>>( \
+            g, h->sc, tb, cb, h->d_ytot.p, gout); \
+        break;
+                    MALA_DD_CASE(1) MALA_DD_CASE(2) MALA_DD_CASE(3) MALA_DD_CASE(4) MALA_DD_CASE(5)
+                    MALA_DD_CASE(6) MALA_DD_CASE(7) MALA_DD_CASE(8) MALA_DD_CASE(9) MALA_DD_CASE(10)
+#undef MALA_DD_CASE
+                    default: break;
+                }
+            } else
+                compute_dedr_kernel<kFullTileTwoJ><<<grid2, (kFullTileTwoJ / 2 + 1) * 32, compute_dedr_smem_bytes(kFullTileTwoJ), st>>>(g, h->sc, tb, cb,
+                                                                                                                                     h->d_ytot.p, gout);
         }
         CUDA_TRY(cudaGetLastError());
         h->stats[0] += 4;
@@ -1735,6 +1755,11 @@ int mala_snap_triples(const mala_snap_t *h, int *j1j2j) {
 int mala_snap_set_option(mala_snap_t *h, const char *name, long long value) {
     if (!h || !name) return fail(MALA_SNAP_EINVAL, "handle or name is NULL");
     const std::string n(name);
+    if (n == "dedr_impl") {
+        if (value < 0 || value > 1) return fail(MALA_SNAP_EINVAL, "dedr_impl must be 0 or 1");
+        h->dedr_impl = (int)value;
+        return MALA_SNAP_OK;
+    }
     if (n == "yi_impl") {
         if (value < 0 || value > 1) return fail(MALA_SNAP_EINVAL, "yi_impl must be 0 or 1");
         h->yi_impl = (int)value;
