@@ -74,7 +74,13 @@ compute_dedr_dft_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers 
         mbar_wait(&bar, parity);
         parity ^= 1u;
 
-        // W_{mb,n} = conj(Yhat_{mb+n,mb}(x_s)) / NW for this lane's grid point
+        // W_{mb,n} = conj(Yhat_{mb+n,mb}(x_s)) / NW for this lane's grid point.  36 complex W are 144 registers, more than a thread has
+        // at twelve warps: from twojmax 8 up the W of the longest chain (mb = 0) live in shared memory -- in the bytes of Y, which
+        // is dead once every warp has its W; until then they wait in the (still unused) queue and force buffers
+        constexpr bool W0_SHARED = TJ >= 8;
+        static_assert(!W0_SHARED || (size_t)NW * NW * 32 * sizeof(double2) <= (size_t)kDdCap * (kDdEntry + 3) * 32 * sizeof(double), "staging of W0");
+        double2 *W0 = reinterpret_cast<double2 *>(smem_raw) + (size_t)warp * NW * 32 + lane;      // [warp][n][lane]
+        double2 *W0stage = reinterpret_cast<double2 *>(geo) + (size_t)warp * NW * 32 + lane;
         double wr[NJM], wi[NJM];
 #pragma unroll
         for (int mb = 0; mb <= TJ / 2; mb++) {
@@ -91,9 +97,17 @@ compute_dedr_dft_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers 
                     m += warp;
                     if (m >= NW) m -= NW;
                 }
-                wr[dft_index(TJ, mb, n)] = sr * (1.0 / (double)NW);
-                wi[dft_index(TJ, mb, n)] = -si * (1.0 / (double)NW);
+                if (W0_SHARED && mb == 0) W0stage[n * 32] = make_double2(sr * (1.0 / (double)NW), -si * (1.0 / (double)NW));
+                else {
+                    wr[dft_index(TJ, mb, n)] = sr * (1.0 / (double)NW);
+                    wi[dft_index(TJ, mb, n)] = -si * (1.0 / (double)NW);
+                }
             }
+        }
+        if constexpr (W0_SHARED) {
+            __syncthreads();   // Y is dead
+#pragma unroll
+            for (int n = 0; n <= TJ; n++) W0[n * 32] = W0stage[n * 32];
         }
 
         const int nc = cb.ncand[wt];
@@ -179,11 +193,16 @@ compute_dedr_dft_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers 
                 double Ar = 0.0, Ai = 0.0, Awr = 0.0, Awi = 0.0, Bvr = 0.0, Bvi = 0.0;
 #pragma unroll
                 for (int mb = TJ / 2; mb >= 0; mb--) {
-                    double Pr = wr[dft_index(TJ, mb, TJ - mb)], Pi = wi[dft_index(TJ, mb, TJ - mb)], Dr = 0.0, Di = 0.0;
+                    double Pr, Pi, Dr = 0.0, Di = 0.0;
+                    if (W0_SHARED && mb == 0) { const double2 t = W0[TJ * 32]; Pr = t.x; Pi = t.y; }
+                    else { Pr = wr[dft_index(TJ, mb, TJ - mb)]; Pi = wi[dft_index(TJ, mb, TJ - mb)]; }
 #pragma unroll
                     for (int n = TJ - mb - 1; n >= mb; n--) {
+                        double cr, ci;
+                        if (W0_SHARED && mb == 0) { const double2 t = W0[n * 32]; cr = t.x; ci = t.y; }
+                        else { cr = wr[dft_index(TJ, mb, n)]; ci = wi[dft_index(TJ, mb, n)]; }
                         const double dr2 = fma(-Di, vi, fma(Dr, vr, Pr)), di2 = fma(Di, vr, fma(Dr, vi, Pi));
-                        const double pr2 = fma(-Pi, vi, fma(Pr, vr, wr[dft_index(TJ, mb, n)])), pi2 = fma(Pi, vr, fma(Pr, vi, wi[dft_index(TJ, mb, n)]));
+                        const double pr2 = fma(-Pi, vi, fma(Pr, vr, cr)), pi2 = fma(Pi, vr, fma(Pr, vi, ci));
                         Dr = dr2; Di = di2; Pr = pr2; Pi = pi2;
                     }
                     const double awr = fma(-Awi, pwi, fma(Awr, pwr, Ar)), awi = fma(Awi, pwr, fma(Awr, pwi, Ai));
