@@ -213,6 +213,8 @@ int mala_gaussian_grid_static(mala_snap_t *h, double sigma, int natoms, const do
  *                      the neighbor queue of the next tile; EINVAL below 8)
  *   "yi_impl"          compute_yi of mala_bispectrum_force_adjoint: 0 = register-tiled block kernel (default), 1 = table-driven
  *                      kernel (element by element)
+ *   "dedr_impl"        compute_dedr of mala_bispectrum_force_adjoint: 0 = sampling kernel (the DFT of Y's columns as the
+ *                      coefficients of a polynomial in the pair's sample values; twojmax 1..10, default), 1 = column kernel
  *   "timing"           1 = record a CUDA-event pair on the caller's stream around every kernel launch of the
  *                      following calls (read back with mala_snap_kernel_times); 0 = off (default)
  *   "workspace_mb"     cap, in MiB, of the U_tot + candidate workspace (default 4096)

@@ -23,7 +23,7 @@ def _grid_points(box, origin, ngrid, z0, z1):
     return frac @ np.asarray(box, float).reshape(3, 3) + np.asarray(origin, float)
 
 
-def _compare(pos, types, box, origin, pbc, ngrid, z0, z1, params, seed, tol=1e-9, yi_impl=0):
+def _compare(pos, types, box, origin, pbc, ngrid, z0, z1, params, seed, tol=1e-9, yi_impl=0, dedr_impl=0):
     torch = _torch()
     rng = np.random.default_rng(seed)
     pts = _grid_points(box, origin, ngrid, z0, z1)
@@ -32,6 +32,7 @@ def _compare(pos, types, box, origin, pbc, ngrid, z0, z1, params, seed, tol=1e-9
     ref = oracle.bispectrum_grad_points(pts, pos, types, box, origin, pbc, beta=beta, want_dB=False, **params)["g"]
     with MalaSnap(**params) as snap:
         snap.set_option("yi_impl", yi_impl)   # 0: register-tiled block kernel, 1: table-driven kernel
+        snap.set_option("dedr_impl", dedr_impl)   # 0: sampling kernel (DFT of Y as polynomial coefficients), 1: column kernel
         g = snap.force_adjoint(torch.as_tensor(beta, device="cuda"), pos, types, box, origin, pbc, ngrid, z0, z1)
         torch.cuda.synchronize()
         got = g.cpu().numpy()
@@ -46,6 +47,18 @@ def test_cluster_in_a_box_twojmax6(yi_impl):
     rng = np.random.default_rng(41)
     pos = rng.uniform(3.0, 7.0, size=(6, 3))
     _compare(pos, np.zeros(6, np.int32), np.eye(3) * 10.0, (0, 0, 0), (0, 0, 0), (9, 8, 7), 0, 7, dict(twojmax=6, rcutfac=3.0), 1, yi_impl=yi_impl)
+
+
+@pytest.mark.parametrize("dedr_impl", [0, 1])
+@pytest.mark.parametrize("tj", [4, 7, 8, 10])
+def test_both_compute_dedr_kernels_dense_periodic_system(tj, dedr_impl):
+    """40 atoms of two types in a periodic 5 A box, cutoff 3.4 A: every point has some eighty neighbors among several hundred
+    candidates (many windows of the sampling kernel, images of the same atom in one window)"""
+    rng = np.random.default_rng(90 + tj)
+    pos = rng.uniform(0.0, 5.0, size=(40, 3))
+    types = rng.integers(0, 2, 40).astype(np.int32)
+    params = dict(twojmax=tj, rcutfac=3.4, radelem=(0.5, 0.45), wj=(1.0, 0.8), rmin0=0.1 if tj == 7 else 0.0)
+    _compare(pos, types, np.eye(3) * 5.0, (0, 0, 0), (1, 1, 1), (5, 4, 3), 0, 3, params, 6, dedr_impl=dedr_impl)
 
 
 def test_periodic_triclinic_box_smaller_than_the_cutoff_two_types():
