@@ -230,8 +230,8 @@ compute_dedr_dft_kernel(GridGeom g, SnapConst sc, DeviceTables tb, ChunkBuffers 
             }
             __syncthreads();
             // per candidate: the sum over the points that have it as a neighbor (entry = its rank among the hits of the point)
-            if ((int)threadIdx.x < nw * 3) {
-                const int k = threadIdx.x / 3, d = threadIdx.x - 3 * k;
+            for (int t = threadIdx.x; t < nw * 3; t += NW * 32) {   // (twojmax 1 has 64 threads for up to 72 sums)
+                const int k = t / 3, d = t - 3 * k;
                 double v = 0.0;
                 for (int l = 0; l < 32; l++) {
                     const unsigned long long hl = hmask[NW * 32 + l];

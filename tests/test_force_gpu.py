@@ -50,10 +50,11 @@ def test_cluster_in_a_box_twojmax6(yi_impl):
 
 
 @pytest.mark.parametrize("dedr_impl", [0, 1])
-@pytest.mark.parametrize("tj", [4, 7, 8, 10])
+@pytest.mark.parametrize("tj", [1, 2, 4, 7, 8, 10])
 def test_both_compute_dedr_kernels_dense_periodic_system(tj, dedr_impl):
     """40 atoms of two types in a periodic 5 A box, cutoff 3.4 A: every point has some eighty neighbors among several hundred
-    candidates (many windows of the sampling kernel, images of the same atom in one window)"""
+    candidates (many full windows of the sampling kernel -- at twojmax 1 more sums per window than the CTA has threads --, images of
+    the same atom in one window)"""
     rng = np.random.default_rng(90 + tj)
     pos = rng.uniform(0.0, 5.0, size=(40, 3))
     types = rng.integers(0, 2, 40).astype(np.int32)
