@@ -161,13 +161,13 @@ struct mala_snap {
     DevBuf<double> d_ycg, d_yweight;
     DevBuf<double2> d_ytot;
     DevBuf<int4> d_ybstream;          // compute_yi on the block machinery (snap_yi_block.cuh)
-    DevBuf<int> d_ybwrange, d_ybpass;
+    DevBuf<int> d_ybwrange, d_ybpass, d_ybmirror;
     int yb_npasses = 0, yb_yacc = 0;
     int yi_impl = 0;                  // 0 automatic (block kernel), 1 table-driven kernel
     int dedr_impl = 0;                // 0 automatic (sampling kernel for twojmax 1..10), 1 column kernel
     YBlkTables yblk_tables() const {
         YBlkTables t;
-        t.stream = d_ybstream.p; t.wrange = d_ybwrange.p; t.pass_elem = d_ybpass.p; t.yweight = d_yweight.p;
+        t.stream = d_ybstream.p; t.wrange = d_ybwrange.p; t.pass_elem = d_ybpass.p; t.yweight = d_yweight.p; t.mirror = d_ybmirror.p;
         t.npasses = yb_npasses; t.yacc_elems = yb_yacc;
         return t;
     }
@@ -1281,9 +1281,11 @@ int build_yi_block_schedule(mala_snap *h, const std::vector<YHostTerm> &terms, c
                 items.push_back(it);
             }
             const int n = hi - lo + 1;
+            // the middle column of an even level is computed up to its centre row; the flush mirrors the rest (ma_hi rows)
+            const int ma_hi = (C % 2 == 0 && mb == C / 2) ? C / 2 : C;
             auto cf = [&](int m1, int m2) {
                 const int ma = m1 + m2 - sh;
-                return (ma < 0 || ma > C) ? 0.0 : cg[t.cgoff + m2 * (A + 1) + m1];
+                return (ma < 0 || ma > ma_hi) ? 0.0 : cg[t.cgoff + m2 * (A + 1) + m1];
             };
             for (auto cx : chunks(A + 1, kBlkBX))
                 for (auto cy : chunks(B + 1, kBlkBY)) {
@@ -1300,7 +1302,7 @@ int build_yi_block_schedule(mala_snap *h, const std::vector<YHostTerm> &terms, c
                     u.a0 = a_lo; u.b0 = b_lo; u.bx = bx; u.by = by;
                     const int ma0 = a_lo + b_lo - sh;
                     u.yelem = uhalf_off(C) + mb * (C + 1) + ma0 - e_pass;   // element of row ma0 in the pass's accumulator (may be negative)
-                    u.dlo = std::max(0, -ma0); u.dhi = std::min(bx + by - 2, C - ma0);
+                    u.dlo = std::max(0, -ma0); u.dhi = std::min(bx + by - 2, ma_hi - ma0);
                     for (int d = 0; d <= bx + by - 2; d++)   // in the order the kernel consumes them (blk_coef_index)
                         for (int a = 0; a < bx; a++) {
                             const int b = d - a;
@@ -1396,6 +1398,14 @@ int build_yi_block_schedule(mala_snap *h, const std::vector<YHostTerm> &terms, c
     if ((rc = upload(h->d_ybstream, stream))) return rc;
     if ((rc = upload(h->d_ybwrange, wrange))) return rc;
     if ((rc = upload(h->d_ybpass, pass_elem))) return rc;
+    // rows above the centre of a middle column: Y[C - ma][C/2] = (-1)^(ma - C/2) conj(Y[ma][C/2]); entry = mirror element << 1 | odd sign
+    std::vector<int> mirror(h->tab.nelem, -1);
+    for (int C = 0; C <= tj; C += 2)
+        for (int ma = C / 2 + 1; ma <= C; ma++) {
+            const int e = uhalf_off(C) + (C / 2) * (C + 1) + ma, me = uhalf_off(C) + (C / 2) * (C + 1) + (C - ma);
+            mirror[e] = (me << 1) | ((ma - C / 2) & 1);
+        }
+    if ((rc = upload(h->d_ybmirror, mirror))) return rc;
     h->yb_npasses = npasses;
     h->yb_yacc = yacc;
     CUDA_TRY(cudaFuncSetAttribute(compute_yi_block_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -2088,7 +2098,7 @@ void mala_snap_destroy(mala_snap_t *h) {
     h->d_yterms.release(); h->d_ylevel.release(); h->d_yorder.release(); h->d_ycg.release(); h->d_yweight.release(); h->d_ytot.release();
     h->d_dcg.release(); h->d_dtriple.release(); h->d_dsched.release(); h->d_ditems.release();
     h->d_bstream.release(); h->d_bwrange.release(); h->d_btslot.release();
-    h->d_ybstream.release(); h->d_ybwrange.release(); h->d_ybpass.release();
+    h->d_ybstream.release(); h->d_ybwrange.release(); h->d_ybpass.release(); h->d_ybmirror.release();
     if (h->h_status) cudaFreeHost(h->h_status);
     for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
     if (h->ev_upload) cudaEventDestroy(h->ev_upload);

@@ -8,7 +8,8 @@
 // accumulator holds the levels of one group (<= 34 KB), is flushed to global memory (with the weights of snap_force.cuh) and
 // cleared between passes.  Units of different warps may hit the same Y element at the same time: the additions are
 // shared-memory atomics (a compare-and-swap loop on sm_100a), so Y -- like the forces that follow -- is reproducible to
-// rounding, not bit for bit.
+// rounding, not bit for bit.  The middle column of an even level is computed up to its centre row only; the flush fills the
+// rows above it by Y[C - ma][C/2] = (-1)^(ma - C/2) conj(Y[ma][C/2]).
 #pragma once
 #include "snap_zi_block.cuh"
 
@@ -26,6 +27,7 @@ struct YBlkTables {
     const int *wrange;      // [warps][passes][kBlkShapes] units per shape, then per warp {first word, word count}: see yblk_wrange_*
     const int *pass_elem;   // [npasses][2] first and one-past-last element (uhalf order) of the levels of every pass
     const double *yweight;  // [nelem]
+    const int *mirror;      // [nelem] -1, or (element to mirror << 1 | odd sign) for the rows above the centre of a middle column
     int npasses, yacc_elems;
 };
 __host__ __device__ inline int yblk_wrange_count(int warp, int pass, int shape, int npasses) {
@@ -153,11 +155,18 @@ compute_yi_block_kernel(GridGeom g, SnapConst sc, YBlkTables T, ChunkBuffers cb,
             for (int i = threadIdx.x; i < (e1 - e0) * 32; i += NW * 32) {
                 const int e = e0 + (i >> 5);
                 const double yw = __ldg(T.yweight + e);
-                const int at = (i >> 5) * 64 + (i & 31);
-                Yt[(size_t)e * 32 + (i & 31)] = make_double2(yw * Yacc[at], yw * Yacc[at + 32]);
-                Yacc[at] = 0.0;
-                Yacc[at + 32] = 0.0;
+                const int mm = __ldg(T.mirror + e);
+                if (mm < 0) {
+                    const int at = (i >> 5) * 64 + (i & 31);
+                    Yt[(size_t)e * 32 + (i & 31)] = make_double2(yw * Yacc[at], yw * Yacc[at + 32]);
+                } else {   // a row above the centre of a middle column: the conjugate of its mirror row, with the sign of the symmetry
+                    const int at = ((mm >> 1) - e0) * 64 + (i & 31);
+                    const double sg = (mm & 1) ? -yw : yw;
+                    Yt[(size_t)e * 32 + (i & 31)] = make_double2(sg * Yacc[at], -sg * Yacc[at + 32]);
+                }
             }
+            __syncthreads();   // the mirror rows have read their sources
+            for (int i = threadIdx.x; i < (e1 - e0) * 64; i += NW * 32) Yacc[i] = 0.0;
             __syncthreads();
         }
     }
