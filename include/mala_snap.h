@@ -222,7 +222,9 @@ int mala_gaussian_grid_static(mala_snap_t *h, double sigma, int natoms, const do
  *                      the true bound makes tile_bin_kernel overflow, which must surface as MALA_SNAP_ECUDA (see
  *                      mala_snap_last_stats); never set it in production
  *   "host_chunk_mb"    cap, in MiB, of each of the two staging buffers of mala_bispectrum_grid_host (default 256;
- *                      outputs above 96 MiB are split into about ten chunks of at least eight planes so the copies overlap the kernels)
+ *                      outputs above 96 MiB go in chunks that shrink -- a third of what is left, whole tile layers, at least
+ *                      eight planes -- so that the copy of one chunk overlaps the kernels of the next and the last, exposed
+ *                      copy is short)
  */
 int mala_snap_set_option(mala_snap_t *h, const char *name, long long value);
 

@@ -1901,20 +1901,26 @@ int mala_bispectrum_grid_host(mala_snap_t *h, int natoms, const double *pos, con
     if ((rc = build_plan(h, a, st))) return rc;
     const size_t plane = (size_t)ngrid[0] * ngrid[1] * h->sc.ntriples;  // doubles per z-plane
     const size_t budget = ((size_t)h->host_chunk_mb << 20) / sizeof(double);
-    int planes = (int)std::max<size_t>(1, std::min<size_t>(budget / std::max<size_t>(plane, 1), (size_t)(z_end - z_begin)));
-    // about ten chunks once the output is large enough for the copy to matter: the device->host copy of a chunk overlaps
-    // the kernels of the next one, so only the last chunk's copy is exposed (config 2: 25.9 ms with 4 chunks, 25.2 with 12;
-    // 18 chunks of 5 planes: 26.3 -- the persistent kernels want a dozen tiles per SM)
+    const int planes_max = (int)std::max<size_t>(1, std::min<size_t>(budget / std::max<size_t>(plane, 1), (size_t)(z_end - z_begin)));
+    // The device->host copy of a chunk overlaps the kernels of the next one, so only the last chunk's copy is exposed, and
+    // every chunk costs the tails of its three persistent kernels.  Hence chunks that shrink: a third of what is left, in whole
+    // tile layers (multiples of eight planes), at least eight planes, at most what a staging buffer holds -- config 2: 24, 16,
+    // 16, 8, 8, 8, 8, 2 planes (equal chunks of 8 planes: 23.5 ms end to end).  Small outputs go in one piece.
     const size_t total = plane * (size_t)(z_end - z_begin);
-    if (total * sizeof(double) > ((size_t)96 << 20)) planes = std::min(planes, std::max(8, (z_end - z_begin + 9) / 10));
-    if (planes >= 8) planes = planes / 8 * 8;  // whole tiles for every tile shape
+    const bool split = total * sizeof(double) > ((size_t)96 << 20);
+    auto next_planes = [&](int left) {
+        int p = planes_max;
+        if (split) p = std::min(p, std::max(8, left / 3));
+        if (p >= 8) p = p / 8 * 8;  // whole tiles for every tile shape
+        return std::min(p, left);
+    };
     for (int b = 0; b < 2; b++)
-        if (h->d_stage[b].reserve(plane * planes, st, true)) return fail(MALA_SNAP_ENOMEM, "cudaMallocAsync (staging) failed");
+        if (h->d_stage[b].reserve(plane * (size_t)next_planes(z_end - z_begin), st, true)) return fail(MALA_SNAP_ENOMEM, "cudaMallocAsync (staging) failed");
     bool used[2] = {false, false};
     int i = 0;
-    for (int z = z_begin; z < z_end; z += planes, i++) {
+    for (int z = z_begin; z < z_end; i++) {
         const int b = i & 1;
-        const int ze = std::min(z + planes, z_end);
+        const int ze = z + next_planes(z_end - z);
         if (used[b]) CUDA_TRY(cudaStreamWaitEvent(st, h->ev_copied[b], 0));
         if ((rc = run_slab(h, z, ze, h->d_stage[b].p, nullptr, st))) return rc;
         CUDA_TRY(cudaEventRecord(h->ev_done[b], st));
@@ -1923,6 +1929,7 @@ int mala_bispectrum_grid_host(mala_snap_t *h, int natoms, const double *pos, con
                                  cudaMemcpyDeviceToHost, h->copy_stream));
         CUDA_TRY(cudaEventRecord(h->ev_copied[b], h->copy_stream));
         used[b] = true;
+        z = ze;
     }
     if ((rc = finish_call(h, st))) return rc;
     CUDA_TRY(cudaStreamSynchronize(h->copy_stream));
