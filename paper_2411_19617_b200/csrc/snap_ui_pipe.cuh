@@ -1,20 +1,25 @@
-// snap_ui_pipe.cuh -- the sampling compute_ui of snap_ui_dft.cuh as a producer / consumer pipeline (rows a3 + a4), twojmax 8..10.
+// snap_ui_pipe.cuh -- the sampling compute_ui of snap_ui_dft.cuh as a producer / consumer pipeline (rows a3 + a4), twojmax 8..14.
 //
 // At these twojmax the sums of a sample fill the registers, one CTA of twojmax + 1 warps owns an SM, and everything in front of
 // the accumulation -- claiming a tile, four dependent global loads for its candidates, distance tests, the pair geometry (a
 // square root, two divisions, three trigonometric values per pair) -- is latency-bound work between barriers during which the
-// FP64 pipe idles: about a third of the kernel.  twojmax + 1 = 9..11 warps also leave one of the four schedulers a warp short.
-// Here that slot goes to a PRODUCER warp (lane = grid point) which prepares the neighbor queue of the NEXT tile while the
-// twojmax + 1 CONSUMER warps (warp = sample point, as before) accumulate and transform the current one:
+// FP64 pipe idles: about a third of the kernel.  Here one more warp, the PRODUCER (lane = grid point), prepares the neighbor
+// queue of the NEXT tile while the twojmax + 1 CONSUMER warps (warp = sample point, as before) accumulate and transform the
+// current one:
 //
 //   producer   claim tile -> candidates -> distance tests -> pair geometry -> geo[buf][entry][c, ar, ai, br, bi][lane]   -> full[buf]
-//   consumers  full[buf] -> sums of chains mb < SPLIT -> S -> inverse DFT of those columns -> sums of the other chains
-//              -> empty[buf] -> S -> inverse DFT of those columns
+//   consumers  per pass (a group of whole chains sized to the registers, pipe_klim):
+//              full[buf] -> sums of the pass's columns over the queue -> empty[buf] -> S -> inverse DFT of those columns
 //
-// Two queue buffers (mbarriers full / empty, the usual parities), consumer-only named barriers around the two uses of S.  The
-// inverse DFT runs in two parts so that S holds the columns of one pass only: S (113 KB at twojmax 10) and two queues of
-// kPipeCap entries (2 x 51 KB) fit the 227 KB of an SM.  A tile with more candidates than kPipeCap is sent window by window,
-// once per pass.  The arithmetic of a sample is that of compute_ui_dft_kernel (dft_accumulate); summation order is fixed.
+// Two queue buffers (mbarriers full / empty, the usual parities), consumer-only named barriers around the uses of S.  The
+// inverse DFT runs pass by pass so that S holds the columns of one pass only: S (113 KB at twojmax 10) and two queues of
+// pipe_cap entries per point (2 x 51 KB) fit the 227 KB of an SM.  A window takes up to 64 candidates and ends early where a
+// point would get more neighbors than a queue holds.  A tile of one window stays in its buffer for every pass; a tile of
+// several windows is sent once per pass -- from the second pass on out of global memory (ChunkBuffers::ui_spill), where the
+// producer kept the geometry of the first pass.  Above twojmax 10 U_tot is written half tile by half tile (the layout the
+// half-tile contraction kernels read).  The arithmetic of a sample is that of compute_ui_dft_kernel (dft_accumulate); the
+// summation order is fixed, results are bit-reproducible.  Below twojmax 8 the one producer warp cannot feed the consumers
+// (measured), so compute_ui_dft_kernel stays there.
 #pragma once
 #include "snap_ui_dft.cuh"
 #include "snap_zi.cuh"
