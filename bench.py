@@ -93,6 +93,7 @@ def parse_args():
                    help="SURVEY 8(f) f3: the adjoint of the descriptor map (mala_bispectrum_force_adjoint), a separate metric line")
     p.add_argument("--zi-impl", type=int, default=0,
                    help="compute_zi kernel: 0 automatic, 1 table-driven, 2 per-triple (twojmax 10), 3 anti-diagonal, 4 register-tiled blocks")
+    p.add_argument("--yi-impl", type=int, default=0, help="compute_yi kernel of --force: 0 automatic, 1 table-driven, 2 fixed-point block kernel")
     p.add_argument("--ui-impl", type=int, default=0,
                    help="compute_ui kernel: 0 automatic, 1 column, 2 sampling (twojmax 1..10), 3 pipelined sampling (twojmax 8..14)")
     p.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
@@ -735,6 +736,8 @@ def run_force(args, w, rank, world, local):
         g.zero_()
         snap.force_adjoint(beta, w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, out=g, stream=stream)
 
+    if args.yi_impl:
+        snap.set_option("yi_impl", args.yi_impl)
     snap.set_option("timing", 1)
     for _ in range(args.warmup):
         call()

@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmala_snap.so")
 SOURCES = ["mala_snap.cu", "mala_mlp.cu"]
-DEPS = ["mala_snap.cu", "mala_mlp.cu", "snap_common.cuh", "snap_internal.h", "snap_tables.h", "snap_ui.cuh", "snap_ui_dft.cuh", "snap_ui_pipe.cuh", "snap_dedr_dft.cuh", "snap_zi.cuh", "snap_zi_coop.cuh",
+DEPS = ["mala_snap.cu", "mala_mlp.cu", "snap_common.cuh", "snap_internal.h", "snap_tables.h", "snap_ui.cuh", "snap_ui_dft.cuh", "snap_ui_pipe.cuh", "snap_dedr_dft.cuh", "snap_yi_fix.cuh", "snap_zi.cuh", "snap_zi_coop.cuh",
         "snap_zi_diag.cuh", "snap_zi_block.cuh", "snap_gauss.cuh", "snap_force.cuh", "snap_yi_block.cuh", os.path.join("..", "..", "include", "mala_snap.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "--expt-relaxed-constexpr", "-std=c++17",
               "-Xcompiler", "-fPIC", "-diag-suppress", "177"]

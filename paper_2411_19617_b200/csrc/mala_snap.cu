@@ -29,6 +29,7 @@
 #include "snap_gauss.cuh"
 #include "snap_force.cuh"
 #include "snap_yi_block.cuh"
+#include "snap_yi_fix.cuh"
 #include "snap_dedr_dft.cuh"
 
 using namespace mala;
@@ -1408,6 +1409,8 @@ int build_yi_block_schedule(mala_snap *h, const std::vector<YHostTerm> &terms, c
     if ((rc = upload(h->d_ybmirror, mirror))) return rc;
     h->yb_npasses = npasses;
     h->yb_yacc = yacc;
+    CUDA_TRY(cudaFuncSetAttribute(compute_yi_fix_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)compute_yi_fix_smem_bytes(uhalf_size(kFullTileTwoJ), std::max(64, uhalf_off(kFullTileTwoJ + 1) - uhalf_off(kFullTileTwoJ)))));
     CUDA_TRY(cudaFuncSetAttribute(compute_yi_block_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   (int)compute_yi_block_smem_bytes(uhalf_size(kFullTileTwoJ), triple_count(kFullTileTwoJ), std::max(64, uhalf_off(kFullTileTwoJ + 1) - uhalf_off(kFullTileTwoJ)))));
     return 0;
@@ -1461,7 +1464,13 @@ int run_slab_force(mala_snap *h, int z0, int z1, const double *beta, double *gou
         {
             TimedSpan span(h, st, kKindZi);   // reported in the compute_zi_bi slot: the same kind of contraction
             const int grid = std::max(1, std::min(h->num_sms, cb.ntiles));
-            if (h->yi_impl == 1)
+            if (h->yi_impl == 2) {   // the block kernel with Y in fixed point (snap_yi_fix.cuh)
+                // |Z^C_AB component| <= (sum |CG|)^2 * 2 max|U component|^2 with sum |CG| <= sqrt(twojmax + 1); at most three terms per
+                // bispectrum component, coefficients <= twojmax + 1
+                const double bound = 2.0 * (h->twojmax + 1) * 3.0 * (h->twojmax + 1);
+                compute_yi_fix_kernel<<<grid, kBlkWarps * 32, compute_yi_fix_smem_bytes(h->sc.nelem, h->yb_yacc), st>>>(g, h->sc, h->yblk_tables(), cb, beta,
+                                                                                                                     h->d_ytot.p, bound);
+            } else if (h->yi_impl == 1)
                 compute_yi_kernel<<<grid, kYiWarps * 32, compute_yi_smem_bytes(h->sc.nelem, h->sc.ntriples), st>>>(g, h->sc, h->force_tables(), cb, beta,
                                                                                                                     h->d_ytot.p);
             else   // the same contraction on the register-tiled block machinery (snap_yi_block.cuh)
@@ -1771,7 +1780,7 @@ int mala_snap_set_option(mala_snap_t *h, const char *name, long long value) {
         return MALA_SNAP_OK;
     }
     if (n == "yi_impl") {
-        if (value < 0 || value > 1) return fail(MALA_SNAP_EINVAL, "yi_impl must be 0 or 1");
+        if (value < 0 || value > 2) return fail(MALA_SNAP_EINVAL, "yi_impl must be 0, 1 or 2");
         h->yi_impl = (int)value;
         return MALA_SNAP_OK;
     }

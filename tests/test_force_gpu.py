@@ -42,7 +42,7 @@ def _compare(pos, types, box, origin, pbc, ngrid, z0, z1, params, seed, tol=1e-9
     return got, beta
 
 
-@pytest.mark.parametrize("yi_impl", [0, 1])
+@pytest.mark.parametrize("yi_impl", [0, 1, 2])
 def test_cluster_in_a_box_twojmax6(yi_impl):
     rng = np.random.default_rng(41)
     pos = rng.uniform(3.0, 7.0, size=(6, 3))
