@@ -93,7 +93,7 @@ def parse_args():
                    help="SURVEY 8(f) f3: the adjoint of the descriptor map (mala_bispectrum_force_adjoint), a separate metric line")
     p.add_argument("--zi-impl", type=int, default=0,
                    help="compute_zi kernel: 0 automatic, 1 table-driven, 2 per-triple (twojmax 10), 3 anti-diagonal, 4 register-tiled blocks")
-    p.add_argument("--yi-impl", type=int, default=0, help="compute_yi kernel of --force: 0 automatic, 1 table-driven, 2 fixed-point block kernel")
+    p.add_argument("--yi-impl", type=int, default=0, help="compute_yi kernel of --force: 0 automatic (2), 1 table-driven, 2 block kernel with Y in fixed point, 3 block kernel with fp64 atomics")
     p.add_argument("--ui-impl", type=int, default=0,
                    help="compute_ui kernel: 0 automatic, 1 column, 2 sampling (twojmax 1..10), 3 pipelined sampling (twojmax 8..14)")
     p.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
@@ -768,7 +768,7 @@ def run_force(args, w, rank, world, local):
     achieved = yi_flop / (kms["compute_yi"] * 1e-3) / 1e12 if kms["compute_yi"] > 0 else 0.0
     peak_meas, mhz_eff = mala_snap_fp64_peak(stream)
     step_flop = yi_flop + pairs * (fm["F_PAIR"] + ffm["F_DEDR_PAIR"])
-    roofline = {"bound": "alu", "kernel": "compute_yi_block_kernel", "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS, "unit": "TFLOP/s",
+    roofline = {"bound": "alu", "kernel": "compute_yi_fix_kernel" if args.yi_impl in (0, 2) else "compute_yi_block_kernel", "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS, "unit": "TFLOP/s",
                 "frac": achieved / FP64_NOMINAL_TFLOPS,
                 "peak_source": "nominal FP64 FMA pipe: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md 'FP64 roofline')",
                 "peak_measured_dfma": peak_meas, "frac_of_measured_dfma": achieved / peak_meas if peak_meas > 0 else None, "traffic": None,
@@ -777,7 +777,7 @@ def run_force(args, w, rank, world, local):
                 "ms_per_launch": kms["compute_yi"] / max(yi_launches, 1), "kernel_ms_per_step": kms,
                 "compute_dedr_tflops": pairs * ffm["F_DEDR_PAIR"] / (kms["compute_dedr"] * 1e-3) / 1e12 if kms["compute_dedr"] > 0 else None,
                 "step_model_tflops": step_flop / (total_ms / args.steps * 1e-3) / 1e12 if world == 1 else None}
-    roofline["traffic"], roofline["traffic_source"] = ncu_traffic(f"config{w.extra.get('cfg')}/tj{w.twojmax}", "compute_yi_block_kernel",
+    roofline["traffic"], roofline["traffic_source"] = ncu_traffic(f"config{w.extra.get('cfg')}/tj{w.twojmax}", roofline["kernel"],
                                                                   kms["compute_yi"] / max(yi_launches, 1))
     # end to end: beta from pinned host memory, g back to the host, every step
     g_host = torch.empty((natoms, 3), dtype=torch.float64, pin_memory=True)

@@ -211,8 +211,11 @@ int mala_gaussian_grid_static(mala_snap_t *h, double sigma, int natoms, const do
  *                      twojmax), 2 = sampling kernel (column polynomials evaluated at the roots of unity, sums in registers,
  *                      inverse DFT per tile; EINVAL outside 1..10), 3 = pipelined sampling kernel (a producer warp prepares
  *                      the neighbor queue of the next tile; EINVAL below 8)
- *   "yi_impl"          compute_yi of mala_bispectrum_force_adjoint: 0 = register-tiled block kernel (default), 1 = table-driven
- *                      kernel (element by element)
+ *   "yi_impl"          compute_yi of mala_bispectrum_force_adjoint: 0 = automatic (2), 1 = table-driven kernel (element by
+ *                      element), 2 = register-tiled block kernel with Y accumulated in 60-bit fixed point by native 32-bit
+ *                      shared-memory atomics (a power-of-two scale per grid point; Y does not depend on the order of the warps;
+ *                      rounding about 1e-12 of the largest |Y| of a grid point), 3 = the same kernel with fp64 atomics (compare-and-
+ *                      swap loops on sm_100a; rounding 1e-14, order-dependent)
  *   "dedr_impl"        compute_dedr of mala_bispectrum_force_adjoint: 0 = sampling kernel (the DFT of Y's columns as the
  *                      coefficients of a polynomial in the pair's sample values; twojmax 1..10, default), 1 = column kernel
  *   "timing"           1 = record a CUDA-event pair on the caller's stream around every kernel launch of the

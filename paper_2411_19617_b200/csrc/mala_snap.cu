@@ -164,7 +164,7 @@ struct mala_snap {
     DevBuf<int4> d_ybstream;          // compute_yi on the block machinery (snap_yi_block.cuh)
     DevBuf<int> d_ybwrange, d_ybpass, d_ybmirror;
     int yb_npasses = 0, yb_yacc = 0;
-    int yi_impl = 0;                  // 0 automatic (block kernel), 1 table-driven kernel
+    int yi_impl = 0;                  // 0 automatic (2), 1 table-driven kernel, 2 block kernel with Y in fixed point, 3 block kernel with fp64 atomics
     int dedr_impl = 0;                // 0 automatic (sampling kernel for twojmax 1..10), 1 column kernel
     YBlkTables yblk_tables() const {
         YBlkTables t;
@@ -1464,7 +1464,7 @@ int run_slab_force(mala_snap *h, int z0, int z1, const double *beta, double *gou
         {
             TimedSpan span(h, st, kKindZi);   // reported in the compute_zi_bi slot: the same kind of contraction
             const int grid = std::max(1, std::min(h->num_sms, cb.ntiles));
-            if (h->yi_impl == 2) {   // the block kernel with Y in fixed point (snap_yi_fix.cuh)
+            if (h->yi_impl == 0 || h->yi_impl == 2) {   // the block kernel with Y in fixed point (snap_yi_fix.cuh)
                 // |Z^C_AB component| <= (sum |CG|)^2 * 2 max|U component|^2 with sum |CG| <= sqrt(twojmax + 1); at most three terms per
                 // bispectrum component, coefficients <= twojmax + 1
                 const double bound = 2.0 * (h->twojmax + 1) * 3.0 * (h->twojmax + 1);
@@ -1780,7 +1780,7 @@ int mala_snap_set_option(mala_snap_t *h, const char *name, long long value) {
         return MALA_SNAP_OK;
     }
     if (n == "yi_impl") {
-        if (value < 0 || value > 2) return fail(MALA_SNAP_EINVAL, "yi_impl must be 0, 1 or 2");
+        if (value < 0 || value > 3) return fail(MALA_SNAP_EINVAL, "yi_impl must be 0 .. 3");
         h->yi_impl = (int)value;
         return MALA_SNAP_OK;
     }

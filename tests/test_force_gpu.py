@@ -31,7 +31,7 @@ def _compare(pos, types, box, origin, pbc, ngrid, z0, z1, params, seed, tol=1e-9
     beta = rng.normal(size=(pts.shape[0], nt))
     ref = oracle.bispectrum_grad_points(pts, pos, types, box, origin, pbc, beta=beta, want_dB=False, **params)["g"]
     with MalaSnap(**params) as snap:
-        snap.set_option("yi_impl", yi_impl)   # 0: register-tiled block kernel, 1: table-driven kernel
+        snap.set_option("yi_impl", yi_impl)   # 0 / 2: block kernel, Y in fixed point; 1: table-driven kernel; 3: block kernel, fp64 atomics
         snap.set_option("dedr_impl", dedr_impl)   # 0: sampling kernel (DFT of Y as polynomial coefficients), 1: column kernel
         g = snap.force_adjoint(torch.as_tensor(beta, device="cuda"), pos, types, box, origin, pbc, ngrid, z0, z1)
         torch.cuda.synchronize()
@@ -42,7 +42,7 @@ def _compare(pos, types, box, origin, pbc, ngrid, z0, z1, params, seed, tol=1e-9
     return got, beta
 
 
-@pytest.mark.parametrize("yi_impl", [0, 1, 2])
+@pytest.mark.parametrize("yi_impl", [0, 1, 2, 3])
 def test_cluster_in_a_box_twojmax6(yi_impl):
     rng = np.random.default_rng(41)
     pos = rng.uniform(3.0, 7.0, size=(6, 3))
@@ -59,7 +59,7 @@ def test_both_compute_dedr_kernels_dense_periodic_system(tj, dedr_impl):
     pos = rng.uniform(0.0, 5.0, size=(40, 3))
     types = rng.integers(0, 2, 40).astype(np.int32)
     params = dict(twojmax=tj, rcutfac=3.4, radelem=(0.5, 0.45), wj=(1.0, 0.8), rmin0=0.1 if tj == 7 else 0.0)
-    _compare(pos, types, np.eye(3) * 5.0, (0, 0, 0), (1, 1, 1), (5, 4, 3), 0, 3, params, 6, dedr_impl=dedr_impl)
+    _compare(pos, types, np.eye(3) * 5.0, (0, 0, 0), (1, 1, 1), (5, 4, 3), 0, 3, params, 6, dedr_impl=dedr_impl, yi_impl=3 if dedr_impl else 0)
 
 
 def test_periodic_triclinic_box_smaller_than_the_cutoff_two_types():
