@@ -155,8 +155,8 @@ int mala_bispectrum_ldos_grid(mala_snap_t *h, mala_mlp_t *net, int natoms, const
  *   beta   DEVICE [(z_end-z_begin)*ny*nx][ncomp] fp64, ix fastest (the layout of mala_bispectrum_grid's out)
  *   g      DEVICE [natoms*3] fp64; the call ADDS the slab's contribution (zero it before the first slab; slabs and GPUs sum)
  * All other arguments as mala_bispectrum_grid.  twojmax <= 10 (MALA_SNAP_EINVAL above).  Enqueued on cuda_stream; does not
- * synchronise.  The per-atom sums (and the accumulation of Y in shared memory) use floating-point atomics: results are
- * reproducible to rounding, not bit for bit.
+ * synchronise.  The per-atom sums use floating-point atomics: results are reproducible to rounding, not bit for bit (Y itself is
+ * accumulated in fixed point and does not depend on the order of the additions; see "yi_impl").
  * mala_snap_kernel_times reports compute_yi under ms[2] and compute_dedr under ms[3].
  */
 int mala_bispectrum_force_adjoint(mala_snap_t *h, int natoms, const double *pos, const int *types, const double box[9],
