@@ -1,7 +1,7 @@
 """GPU parity of row f3, mala_bispectrum_force_adjoint (Eqs. (44)-(45)): the Y contraction + dU recursion of
 the CUDA path against the oracle's forward-mode derivative (oracle_bispectrum_grad_points, pinned in test_force_oracle.py by
 finite differences and closed forms) on the same seeded inputs.  Both sides are exact up to rounding: tolerance 1e-9 of the
-largest |g| (the atomics of the CUDA path change the summation order, nothing else)."""
+largest |g| (the CUDA path sums in another order, and its default compute_yi accumulates Y in 60-bit fixed point: about 1e-12)."""
 import numpy as np
 import pytest
 
