@@ -122,6 +122,32 @@ def test_config2_full_grid_sparse_beta_in_bench_configuration():
     assert np.abs(got - ref).max() <= 1e-9 * scale, f"max |dg| / max |g| = {np.abs(got - ref).max() / scale:.3e}"
 
 
+@pytest.mark.parametrize("case", ["one huge component", "tiny", "sixteen decades"])
+def test_beta_ranges_through_the_fixed_point_and_the_fp64_accumulator(case):
+    """the fixed-point Y of the default compute_yi takes its scale from the beta of each grid point: a single component a
+    million times the others, betas of 1e-12, and betas spread over sixteen decades all stay at 1e-10 of the largest |g|
+    (the fp64 accumulator at 1e-12)"""
+    torch = _torch()
+    w = workloads.make(1)
+    rng = np.random.default_rng(5)
+    nt, z0, z1 = 91, 4, 6
+    pts = _grid_points(w.box, w.origin, w.ngrid, z0, z1)
+    beta = rng.normal(size=(pts.shape[0], nt))
+    if case == "one huge component":
+        beta[:, 37] *= 1e6
+    elif case == "tiny":
+        beta *= 1e-12
+    else:
+        beta *= 10.0 ** rng.uniform(-8, 8, size=beta.shape)
+    ref = oracle.bispectrum_grad_points(pts, w.pos, w.types, w.box, w.origin, w.pbc, beta=beta, want_dB=False, **w.snap_params())["g"]
+    with MalaSnap(**w.snap_params()) as snap:
+        for yi, tol in ((2, 1e-10), (3, 1e-12)):
+            snap.set_option("yi_impl", yi)
+            g = snap.force_adjoint(torch.as_tensor(beta, device="cuda"), w.pos, w.types, w.box, w.origin, w.pbc, w.ngrid, z0, z1).cpu().numpy()
+            assert np.isfinite(g).all()
+            assert np.abs(g - ref).max() <= tol * np.abs(ref).max(), f"yi_impl {yi}: {np.abs(g - ref).max() / np.abs(ref).max():.3e}"
+
+
 def test_uniform_beta_on_a_full_periodic_grid_gives_a_small_net_translation_force():
     """moving all atoms together equals moving the grid the other way: with the same beta at every point of a full periodic grid
     the sum over atoms of g is the beta-weighted grid sum of -dB/dr, which converges to zero as the grid resolves B (a sanity
